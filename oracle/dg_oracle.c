@@ -1,0 +1,522 @@
+/*
+ * dg_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.  See dg_oracle.h.
+ *
+ * Plain CPU oracle of the hot path named in BASELINE.json `north_star`, written from the
+ * paper (arXiv 2006.15698, /root/reference/PAPER.md) and the readings listed in DESIGN.md.
+ * It follows the algorithm step by step in the paper's order:
+ *
+ *   step 0  operators of the collocated Gauss-Legendre Lagrange basis   PAPER.md:72-80, eq (6)-(7)
+ *   step 1  volume term: pointwise Euler flux + sum-factorised          PAPER.md:45-50 eq (2)-(3),
+ *           differentiation, weak form                                  63-68 eq (5) 2nd term, 220-237
+ *   step 2  face traces of the conserved variables                      PAPER.md:67 (psi_s(x|Gamma))
+ *   step 3  local Lax-Friedrichs interface flux
+ *   step 4  lift + inverse (diagonal) mass: dQ/dt = V - S               PAPER.md:63-68 eq (5)
+ *   step 5  five-stage 2N-storage Runge-Kutta update (LSERK45)
+ *   step 6  max wavespeed for the CFL time step                         not in the paper; R10
+ *
+ * No blocking, fusion or reordering: whole-mesh arrays for traces and interface fluxes, one
+ * loop nest per step.  Pins (tests/test_oracle_*.py, -m "not gpu"): Gauss-Legendre closed
+ * forms and numpy's leggauss; exact differentiation/interpolation of monomials; the
+ * summation-by-parts identity; brute-force dense (Kronecker) evaluation of eq (5) written
+ * out with explicit quadrature in numpy, in weak AND strong form; free-stream preservation;
+ * discrete conservation; rotation symmetry; Runge-Kutta order conditions and a Butcher-form
+ * re-evaluation of the step; p+1 convergence on two exact Euler solutions.
+ *
+ * Parity unpinned BY THE PAPER (fixed by DESIGN.md readings, pinned only by consistency,
+ * conservation and convergence): the exact Lax-Friedrichs variant (R3), the CFL rule (R10),
+ * the element ordering (R13).
+ *
+ * Floating-point form: products and sums are evaluated in the
+ * order written below, q ascending; build with -ffp-contract=off so the compiler fuses nothing.
+ */
+#include "dg_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#ifndef ORACLE_REAL
+#define ORACLE_REAL double
+#endif
+typedef ORACLE_REAL real;
+typedef long double xreal; /* operator construction is always done in long double */
+
+#define R_SQRT(x) _Generic((real)0, long double: sqrtl, default: sqrt)(x)
+#define R_FABS(x) _Generic((real)0, long double: fabsl, default: fabs)(x)
+
+#define NV 5     /* rho, rho u, rho v, rho w, rho E        PAPER.md:45 eq (2) */
+#define NMAX 16  /* largest N = p+1 this file accepts */
+
+int oracle_real_bytes(void) { return (int)sizeof(real); }
+
+int oracle_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------------------------------
+ * step 0: operators
+ * ---------------------------------------------------------------------------------------- */
+
+/* Legendre P_N(x) and P_N'(x) by the three-term recurrence
+ * (n+1) P_{n+1} = (2n+1) x P_n - n P_{n-1};  (x^2-1) P_N' = N (x P_N - P_{N-1}). */
+static void legendre(int N, xreal x, xreal *P, xreal *dP) {
+    xreal p0 = 1.0L, p1 = x;
+    for (int n = 1; n < N; ++n) {
+        xreal p2 = ((2 * n + 1) * x * p1 - n * p0) / (n + 1);
+        p0 = p1;
+        p1 = p2;
+    }
+    *P = p1;
+    *dP = N * (x * p1 - p0) / (x * x - 1.0L);
+}
+
+/* Roots of P_N by Newton iteration, weights w = 2 / ((1-x^2) P_N'(x)^2). Ascending order. */
+static void gauss_legendre_x(int N, xreal *xi, xreal *w) {
+    const xreal pi = 3.14159265358979323846264338327950288L;
+    for (int m = 0; m < N; ++m) {
+        xreal x = cosl(pi * (m + 0.75L) / (N + 0.5L)); /* m-th root from the right */
+        xreal P, dP;
+        for (int it = 0; it < 100; ++it) {
+            legendre(N, x, &P, &dP);
+            xreal dx = P / dP;
+            x -= dx;
+            if (fabsl(dx) < 1e-19L) break;
+        }
+        if (N % 2 == 1 && m == N / 2) x = 0.0L; /* middle root of an odd rule */
+        legendre(N, x, &P, &dP);
+        xi[N - 1 - m] = x;
+        w[N - 1 - m] = 2.0L / ((1.0L - x * x) * dP * dP);
+    }
+}
+
+/* Lagrange basis eq (7) (product over i != s; R2):
+ *   barycentric weights  b_i = 1 / prod_{j!=i} (xi_i - xi_j)
+ *   D_{qi} = l_i'(xi_q) = (b_i / b_q) / (xi_q - xi_i)  (q != i),  D_{qq} = -sum_{i!=q} D_{qi}
+ *   l_i(+-1) = prod_{j!=i} (+-1 - xi_j) / (xi_i - xi_j)                                      */
+static void operators_x(int N, xreal *xi, xreal *w, xreal *D, xreal *lp, xreal *lm) {
+    xreal b[NMAX];
+    gauss_legendre_x(N, xi, w);
+    for (int i = 0; i < N; ++i) {
+        xreal prod = 1.0L;
+        for (int j = 0; j < N; ++j)
+            if (j != i) prod *= (xi[i] - xi[j]);
+        b[i] = 1.0L / prod;
+    }
+    for (int q = 0; q < N; ++q) {
+        xreal diag = 0.0L;
+        for (int i = 0; i < N; ++i) {
+            if (i == q) continue;
+            D[q * N + i] = (b[i] / b[q]) / (xi[q] - xi[i]);
+            diag -= D[q * N + i];
+        }
+        D[q * N + q] = diag;
+    }
+    for (int i = 0; i < N; ++i) {
+        xreal pp = 1.0L, pm = 1.0L;
+        for (int j = 0; j < N; ++j) {
+            if (j == i) continue;
+            pp *= (1.0L - xi[j]) / (xi[i] - xi[j]);
+            pm *= (-1.0L - xi[j]) / (xi[i] - xi[j]);
+        }
+        lp[i] = pp;
+        lm[i] = pm;
+    }
+}
+
+int oracle_gauss_legendre(int N, double *xi, double *w) {
+    if (N < 1 || N > NMAX || !xi || !w) return 1;
+    xreal x[NMAX], ww[NMAX];
+    gauss_legendre_x(N, x, ww);
+    for (int i = 0; i < N; ++i) {
+        xi[i] = (double)x[i];
+        w[i] = (double)ww[i];
+    }
+    return 0;
+}
+
+int oracle_operators(int N, double *xi, double *w, double *D, double *lp, double *lm,
+                     double *Dhat) {
+    if (N < 1 || N > NMAX) return 1;
+    xreal x[NMAX], ww[NMAX], DD[NMAX * NMAX], p[NMAX], m[NMAX];
+    operators_x(N, x, ww, DD, p, m);
+    for (int i = 0; i < N; ++i) {
+        if (xi) xi[i] = (double)x[i];
+        if (w) w[i] = (double)ww[i];
+        if (lp) lp[i] = (double)p[i];
+        if (lm) lm[i] = (double)m[i];
+        for (int q = 0; q < N; ++q) {
+            if (D) D[q * N + i] = (double)DD[q * N + i];
+            if (Dhat) Dhat[i * N + q] = (double)(ww[q] * DD[q * N + i] / ww[i]);
+        }
+    }
+    return 0;
+}
+
+/* The discretisation: mesh, gas, and the 1-D operators rounded to `real`. */
+typedef struct {
+    int nx, ny, nz, N;
+    size_t nelem, nnode; /* elements; nodes per element N^3 */
+    real gamma, gm1;
+    real g[3];              /* 2/h_a: constant geometric factor per axis  PAPER.md:31, 143 (`vgeo`) */
+    real Dhat[NMAX * NMAX]; /* Dhat[i*N+q] = w_q l_i'(xi_q) / w_i */
+    real lp[NMAX], lm[NMAX], w[NMAX];
+} disc;
+
+static int disc_init(disc *d, int nx, int ny, int nz, int p, double gamma,
+                     const double extent[3]) {
+    if (nx < 1 || ny < 1 || nz < 1 || p < 0 || p + 1 > NMAX || !(gamma > 1.0) || !extent)
+        return 1;
+    if (!(extent[0] > 0.0) || !(extent[1] > 0.0) || !(extent[2] > 0.0)) return 1;
+    const int N = p + 1;
+    xreal x[NMAX], w[NMAX], D[NMAX * NMAX], lp[NMAX], lm[NMAX];
+    operators_x(N, x, w, D, lp, lm);
+    d->nx = nx; d->ny = ny; d->nz = nz; d->N = N;
+    d->nelem = (size_t)nx * ny * nz;
+    d->nnode = (size_t)N * N * N;
+    d->gamma = (real)gamma;
+    d->gm1 = (real)gamma - (real)1;
+    d->g[0] = (real)2 / ((real)extent[0] / (real)nx);
+    d->g[1] = (real)2 / ((real)extent[1] / (real)ny);
+    d->g[2] = (real)2 / ((real)extent[2] / (real)nz);
+    for (int i = 0; i < N; ++i) {
+        d->lp[i] = (real)lp[i];
+        d->lm[i] = (real)lm[i];
+        d->w[i] = (real)w[i];
+        for (int q = 0; q < N; ++q) d->Dhat[i * N + q] = (real)(w[q] * D[q * N + i] / w[i]);
+    }
+    return 0;
+}
+
+/* canonical index of variable 0 at node (i,j,k) of element e */
+static size_t qidx(const disc *d, size_t e, int i, int j, int k) {
+    const size_t N = (size_t)d->N;
+    return ((((e * N + (size_t)k) * N + (size_t)j) * N + (size_t)i) * NV);
+}
+
+static size_t eidx(const disc *d, int ex, int ey, int ez) {
+    return (size_t)ex + (size_t)d->nx * ((size_t)ey + (size_t)d->ny * (size_t)ez);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * pointwise Euler flux along one axis                        PAPER.md:45-50, eq (2)-(3); 186-217
+ *   1/rho, u,v,w, p = (gamma-1)(rho E - rho/2 (u^2+v^2+w^2)), rho E + p, then column `axis`
+ *   of the flux matrix F.  Also returns the normal velocity and the sound speed
+ *   c = sqrt(gamma p / rho) (needed by the interface flux).
+ * ---------------------------------------------------------------------------------------- */
+static void euler_flux(const disc *d, const real Q[NV], int axis, real F[NV], real *un,
+                       real *c) {
+    const real oneOrho = (real)1 / Q[0];
+    const real u = Q[1] * oneOrho;
+    const real v = Q[2] * oneOrho;
+    const real w = Q[3] * oneOrho;
+    const real p = d->gm1 * (Q[4] - (real)0.5 * Q[0] * (u * u + v * v + w * w));
+    const real Ep = Q[4] + p; /* rho H */
+    const real vel = (axis == 0) ? u : (axis == 1) ? v : w;
+    F[0] = Q[0] * vel;
+    F[1] = Q[1] * vel;
+    F[2] = Q[2] * vel;
+    F[3] = Q[3] * vel;
+    F[4] = Ep * vel;
+    F[1 + axis] = F[1 + axis] + p;
+    if (un) *un = vel;
+    if (c) *c = R_SQRT(d->gamma * p * oneOrho);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * step 1: volume term                                   PAPER.md:63-68 eq (5) 2nd term; 220-237
+ *   V_ijk = (2/hx) sum_q Dhat_iq F1_qjk + (2/hy) sum_q Dhat_jq F2_iqk + (2/hz) sum_q Dhat_kq F3_ijq
+ * ---------------------------------------------------------------------------------------- */
+static void volume_term(const disc *d, const real *q, real *V) {
+    const int N = d->N;
+    const size_t nn = d->nnode;
+#ifdef _OPENMP
+#pragma omp parallel
+#endif
+    {
+        real *F = (real *)malloc(sizeof(real) * 3 * nn * NV); /* F[axis][k][j][i][n] */
+#ifdef _OPENMP
+#pragma omp for
+#endif
+        for (long long el = 0; el < (long long)d->nelem; ++el) {
+            const size_t e = (size_t)el;
+            for (int k = 0; k < N; ++k)
+                for (int j = 0; j < N; ++j)
+                    for (int i = 0; i < N; ++i) {
+                        const size_t ln = ((size_t)k * N + j) * N + i;
+                        const real *Qn = q + qidx(d, e, i, j, k);
+                        for (int a = 0; a < 3; ++a)
+                            euler_flux(d, Qn, a, F + (a * nn + ln) * NV, 0, 0);
+                    }
+            for (int k = 0; k < N; ++k)
+                for (int j = 0; j < N; ++j)
+                    for (int i = 0; i < N; ++i) {
+                        real *Vn = V + qidx(d, e, i, j, k);
+                        for (int n = 0; n < NV; ++n) {
+                            real sx = 0, sy = 0, sz = 0;
+                            for (int qp = 0; qp < N; ++qp) {
+                                const size_t lx = ((size_t)k * N + j) * N + qp;
+                                const size_t ly = ((size_t)k * N + qp) * N + i;
+                                const size_t lz = ((size_t)qp * N + j) * N + i;
+                                sx += d->Dhat[i * N + qp] * F[(0 * nn + lx) * NV + n];
+                                sy += d->Dhat[j * N + qp] * F[(1 * nn + ly) * NV + n];
+                                sz += d->Dhat[k * N + qp] * F[(2 * nn + lz) * NV + n];
+                            }
+                            Vn[n] = d->g[0] * sx + d->g[1] * sy + d->g[2] * sz;
+                        }
+                    }
+        }
+        free(F);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * steps 2-4: surface term                               PAPER.md:63-70 eq (5) 3rd term
+ *   traces        T+-_a(t1,t2) = sum_i l_i(+-1) Q along axis a           (conserved variables, R4)
+ *   interface     F*_a at the + face of every element: left state = own T+, right state = T- of
+ *                 the neighbour (index+1 mod n_a): local Lax-Friedrichs (R3)
+ *                   F* = 1/2 (F_a(QL) + F_a(QR)) - 1/2 lam (QR - QL),
+ *                   lam = max(|u_a^L| + c_L, |u_a^R| + c_R)
+ *   lift          S_ijk = sum_a (2/h_a) ( l_i(+1) F*_{a+} - l_i(-1) F*_{a-} ) / w_i   (index of
+ *                 l, w along axis a; F*_{a-} is the + face value of the neighbour below)
+ * transverse face coordinates: axis x: (t1,t2) = (j,k);  y: (i,k);  z: (i,j).
+ * ---------------------------------------------------------------------------------------- */
+static void node_of_line(int axis, int s, int t1, int t2, int *i, int *j, int *k) {
+    if (axis == 0) { *i = s;  *j = t1; *k = t2; }
+    if (axis == 1) { *i = t1; *j = s;  *k = t2; }
+    if (axis == 2) { *i = t1; *j = t2; *k = s;  }
+}
+
+static void surface_term(const disc *d, const real *q, real *S) {
+    const int N = d->N;
+    const size_t nf = (size_t)N * N;              /* nodes per face */
+    const size_t per_elem = 3 * nf * NV;          /* [axis][t2][t1][n] */
+    real *Tp = (real *)malloc(sizeof(real) * d->nelem * per_elem);
+    real *Tm = (real *)malloc(sizeof(real) * d->nelem * per_elem);
+    real *Fs = (real *)malloc(sizeof(real) * d->nelem * per_elem);
+
+    /* step 2: traces */
+#ifdef _OPENMP
+#pragma omp parallel for
+#endif
+    for (long long el = 0; el < (long long)d->nelem; ++el) {
+        const size_t e = (size_t)el;
+        for (int a = 0; a < 3; ++a)
+            for (int t2 = 0; t2 < N; ++t2)
+                for (int t1 = 0; t1 < N; ++t1) {
+                    real *tp = Tp + e * per_elem + ((a * nf) + (size_t)t2 * N + t1) * NV;
+                    real *tm = Tm + e * per_elem + ((a * nf) + (size_t)t2 * N + t1) * NV;
+                    for (int n = 0; n < NV; ++n) {
+                        real sp = 0, sm = 0;
+                        for (int s = 0; s < N; ++s) {
+                            int i, j, k;
+                            node_of_line(a, s, t1, t2, &i, &j, &k);
+                            const real Qv = q[qidx(d, e, i, j, k) + n];
+                            sp += d->lp[s] * Qv;
+                            sm += d->lm[s] * Qv;
+                        }
+                        tp[n] = sp;
+                        tm[n] = sm;
+                    }
+                }
+    }
+
+    /* step 3: interface flux at the + face of every element along every axis */
+#ifdef _OPENMP
+#pragma omp parallel for
+#endif
+    for (long long el = 0; el < (long long)d->nelem; ++el) {
+        const size_t e = (size_t)el;
+        const int ex = (int)(e % (size_t)d->nx);
+        const int ey = (int)((e / (size_t)d->nx) % (size_t)d->ny);
+        const int ez = (int)(e / ((size_t)d->nx * d->ny));
+        for (int a = 0; a < 3; ++a) {
+            const size_t en = (a == 0)   ? eidx(d, (ex + 1) % d->nx, ey, ez)
+                              : (a == 1) ? eidx(d, ex, (ey + 1) % d->ny, ez)
+                                         : eidx(d, ex, ey, (ez + 1) % d->nz);
+            for (size_t f = 0; f < nf; ++f) {
+                const real *QL = Tp + e * per_elem + (a * nf + f) * NV;
+                const real *QR = Tm + en * per_elem + (a * nf + f) * NV;
+                real *Fst = Fs + e * per_elem + (a * nf + f) * NV;
+                real FL[NV], FR[NV], uL, uR, cL, cR;
+                euler_flux(d, QL, a, FL, &uL, &cL);
+                euler_flux(d, QR, a, FR, &uR, &cR);
+                const real lamL = R_FABS(uL) + cL;
+                const real lamR = R_FABS(uR) + cR;
+                const real lam = (lamL > lamR) ? lamL : lamR;
+                for (int n = 0; n < NV; ++n)
+                    Fst[n] = (real)0.5 * (FL[n] + FR[n]) - (real)0.5 * lam * (QR[n] - QL[n]);
+            }
+        }
+    }
+
+    /* step 4: lift, divided by the diagonal mass matrix */
+#ifdef _OPENMP
+#pragma omp parallel for
+#endif
+    for (long long el = 0; el < (long long)d->nelem; ++el) {
+        const size_t e = (size_t)el;
+        const int ex = (int)(e % (size_t)d->nx);
+        const int ey = (int)((e / (size_t)d->nx) % (size_t)d->ny);
+        const int ez = (int)(e / ((size_t)d->nx * d->ny));
+        const size_t em[3] = {eidx(d, (ex + d->nx - 1) % d->nx, ey, ez),
+                              eidx(d, ex, (ey + d->ny - 1) % d->ny, ez),
+                              eidx(d, ex, ey, (ez + d->nz - 1) % d->nz)};
+        for (int k = 0; k < N; ++k)
+            for (int j = 0; j < N; ++j)
+                for (int i = 0; i < N; ++i) {
+                    real *Sn = S + qidx(d, e, i, j, k);
+                    const int s[3] = {i, j, k};
+                    const size_t f[3] = {(size_t)k * N + j, (size_t)k * N + i, (size_t)j * N + i};
+                    for (int n = 0; n < NV; ++n) {
+                        real acc = 0;
+                        for (int a = 0; a < 3; ++a) {
+                            const real Fplus = Fs[e * per_elem + (a * nf + f[a]) * NV + n];
+                            const real Fminus = Fs[em[a] * per_elem + (a * nf + f[a]) * NV + n];
+                            acc += d->g[a] *
+                                   ((d->lp[s[a]] * Fplus - d->lm[s[a]] * Fminus) / d->w[s[a]]);
+                        }
+                        Sn[n] = acc;
+                    }
+                }
+    }
+    free(Tp);
+    free(Tm);
+    free(Fs);
+}
+
+/* dQ/dt = V - S in `real`, whole mesh. */
+static void residual_real(const disc *d, const real *q, real *r, real *tmp) {
+    const size_t len = d->nelem * d->nnode * NV;
+    volume_term(d, q, r);
+    surface_term(d, q, tmp);
+    for (size_t m = 0; m < len; ++m) r[m] = r[m] - tmp[m];
+}
+
+/* ---- double <-> real marshalling ---- */
+static real *to_real(const double *x, size_t len) {
+    real *y = (real *)malloc(sizeof(real) * len);
+    for (size_t m = 0; m < len; ++m) y[m] = (real)x[m];
+    return y;
+}
+static void to_double(const real *y, double *x, size_t len) {
+    for (size_t m = 0; m < len; ++m) x[m] = (double)y[m];
+}
+
+static int run_term(int which, int nx, int ny, int nz, int p, double gamma,
+                    const double extent[3], const double *q, double *r) {
+    disc d;
+    if (!q || !r || disc_init(&d, nx, ny, nz, p, gamma, extent)) return 1;
+    const size_t len = d.nelem * d.nnode * NV;
+    real *qq = to_real(q, len);
+    real *rr = (real *)malloc(sizeof(real) * len);
+    if (which == 0) volume_term(&d, qq, rr);
+    if (which == 1) surface_term(&d, qq, rr);
+    if (which == 2) {
+        real *tmp = (real *)malloc(sizeof(real) * len);
+        residual_real(&d, qq, rr, tmp);
+        free(tmp);
+    }
+    to_double(rr, r, len);
+    free(qq);
+    free(rr);
+    return 0;
+}
+
+int oracle_volume_term(int nx, int ny, int nz, int p, double gamma, const double extent[3],
+                       const double *q, double *r) {
+    return run_term(0, nx, ny, nz, p, gamma, extent, q, r);
+}
+int oracle_surface_term(int nx, int ny, int nz, int p, double gamma, const double extent[3],
+                        const double *q, double *r) {
+    return run_term(1, nx, ny, nz, p, gamma, extent, q, r);
+}
+int oracle_residual(int nx, int ny, int nz, int p, double gamma, const double extent[3],
+                    const double *q, double *r) {
+    return run_term(2, nx, ny, nz, p, gamma, extent, q, r);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * step 5: LSERK45
+ *   K = 0; for s = 1..5:  K = A_s K + dt L(Q);  Q = Q + B_s K
+ * Carpenter & Kennedy (1994) 2N-storage (5,4) coefficients as rationals (R9); the
+ * system is autonomous so the C_s abscissae are not needed.
+ * ---------------------------------------------------------------------------------------- */
+static const xreal RK_A[5] = {
+    0.0L,
+    -567301805773.0L / 1357537059087.0L,
+    -2404267990393.0L / 2016746695238.0L,
+    -3550918686646.0L / 2091501179385.0L,
+    -1275806237668.0L / 842570457699.0L};
+static const xreal RK_B[5] = {
+    1432997174477.0L / 9575080441755.0L,
+    5161836677717.0L / 13612068292357.0L,
+    1720146321549.0L / 2090206949498.0L,
+    3134564353537.0L / 4481467310338.0L,
+    2277821191437.0L / 14882151754819.0L};
+
+void oracle_lserk45(double A[5], double B[5]) {
+    for (int s = 0; s < 5; ++s) {
+        A[s] = (double)RK_A[s];
+        B[s] = (double)RK_B[s];
+    }
+}
+
+int oracle_rk_step(int nx, int ny, int nz, int p, double gamma, const double extent[3],
+                   double *q, double dt, int nsteps) {
+    disc d;
+    if (!q || nsteps < 0 || disc_init(&d, nx, ny, nz, p, gamma, extent)) return 1;
+    const size_t len = d.nelem * d.nnode * NV;
+    real *Q = to_real(q, len);
+    real *K = (real *)malloc(sizeof(real) * len);
+    real *R = (real *)malloc(sizeof(real) * len);
+    real *tmp = (real *)malloc(sizeof(real) * len);
+    const real h = (real)dt;
+    for (int step = 0; step < nsteps; ++step) {
+        for (size_t m = 0; m < len; ++m) K[m] = 0;
+        for (int s = 0; s < 5; ++s) {
+            const real A = (real)RK_A[s], B = (real)RK_B[s];
+            residual_real(&d, Q, R, tmp);
+            for (size_t m = 0; m < len; ++m) {
+                K[m] = A * K[m] + h * R[m];
+                Q[m] = Q[m] + B * K[m];
+            }
+        }
+    }
+    to_double(Q, q, len);
+    free(Q);
+    free(K);
+    free(R);
+    free(tmp);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * step 6: max wavespeed  lam = max_nodes ( sqrt(u^2+v^2+w^2) + sqrt(gamma p / rho) )
+ * (not in the paper; R10.  dt = CFL min(h_a) / ((2p+1) lam) is formed by the caller.)
+ * ---------------------------------------------------------------------------------------- */
+int oracle_max_wavespeed(int nx, int ny, int nz, int p, double gamma, const double *q,
+                         double *lam) {
+    const double unit[3] = {1.0, 1.0, 1.0};
+    disc d;
+    if (!q || !lam || disc_init(&d, nx, ny, nz, p, gamma, unit)) return 1;
+    const size_t nodes = d.nelem * d.nnode;
+    real best = 0;
+    for (size_t m = 0; m < nodes; ++m) {
+        const real Q0 = (real)q[m * NV + 0], Q1 = (real)q[m * NV + 1], Q2 = (real)q[m * NV + 2],
+                   Q3 = (real)q[m * NV + 3], Q4 = (real)q[m * NV + 4];
+        const real oneOrho = (real)1 / Q0;
+        const real u = Q1 * oneOrho, v = Q2 * oneOrho, w = Q3 * oneOrho;
+        const real pr = d.gm1 * (Q4 - (real)0.5 * Q0 * (u * u + v * v + w * w));
+        const real s = R_SQRT(u * u + v * v + w * w) + R_SQRT(d.gamma * pr * oneOrho);
+        if (s > best) best = s;
+    }
+    *lam = (double)best;
+    return 0;
+}
