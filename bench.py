@@ -1,0 +1,323 @@
+#!/usr/bin/env python
+"""bench.py -- DOF-updates/s per Runge-Kutta stage of the fused DG Euler time step (fp64, B200).
+
+One "step" = one LSERK45 time step = 5 passes of the whole hot path (flux, differentiation, traces,
+Lax-Friedrichs flux, lift, 2/h scaling, stage update) over the whole mesh.  Default workload:
+BASELINE.json config 3 (Taylor-Green vortex, 64^3 elements, p = 4, 32.8 M nodes), the configuration
+the metric asks DOF-updates/s and HBM GB/s for; `--workload cfg5` runs the largest single-GPU case,
+`--workload cfg4_p<k>` one point of the order sweep, and the default line also carries the whole
+p = 1..7 sweep of config 4 ("p_sweep", skip with --no-sweep).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl ours|reference]
+    python -m torch.distributed.run --nproc-per-node N ... bench.py --gpus N ...   (N replicas)
+
+Prints ONE JSON line (rank 0).  Timing: CUDA events on the stream the kernels are launched on,
+after W >= 3 warm-up steps, barrier + synchronize on both sides, max over ranks.  The working set
+(>= 2.6 GB per stage) is far larger than the 126 MB L2, so no flush is needed between iterations.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "DOF-updates/s per RK stage"
+UNIT = "DOF-updates/s"
+STAGES = 5
+ALGO_BYTES_PER_DOF_STAGE = 152.0   # read Q,K + write Q,K = 4 x 40 B, stage 1 does not read K
+GAMMA = 1.4
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(workload):
+    """Per-launch DRAM bytes of the stage kernel from the committed ncu --set full capture, or None."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f).get(workload)
+    return None
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": nv.nvmlClocksThrottleReasonHwSlowdown,
+                 "hw_thermal_slowdown": nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksThrottleReasonSwThermalSlowdown,
+                 "sw_power_cap": nv.nvmlClocksThrottleReasonSwPowerCap}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                bits = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, v in names.items():
+                    if bits & v:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(0.02)
+
+    def __enter__(self):
+        if self.nv:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thread:
+            self._thread.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+def physical_gpu_index(local_rank):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+# ----------------------------------------------------------------------------------------------
+# the oracle on the host cores: cpu_baseline leg and --impl reference
+# ----------------------------------------------------------------------------------------------
+def oracle_sample(workload, target_seconds=10.0, fixed_steps=None):
+    """Time the CPU oracle (as it stands) on a bounded sub-box of the workload's field."""
+    from oracle import Oracle
+    from paper_2006_15698_b200 import inputs as I
+    c = I.CONFIGS[workload]
+    p, ext = c["p"], c["extent"]
+    ne = max(2, min(c["nx"], int(round((4.0e5 / (p + 1) ** 3) ** (1.0 / 3.0)))))   # ~4e5 nodes, out of cache
+    box = ((0, ne), (0, ne), (0, ne))
+    q = I.make_field(workload, box=box)
+    sub_ext = tuple(ext[a] * ne / (c["nx"], c["ny"], c["nz"])[a] for a in range(3))
+    orc = Oracle("omp")
+    dt = I.cfl_dt(orc.max_wavespeed(q, p, GAMMA), p, sub_ext, (ne, ne, ne), 0.1)
+    dof = ne ** 3 * (p + 1) ** 3
+    t0 = time.perf_counter()
+    orc.rk_step(q, p, GAMMA, sub_ext, dt, 1)
+    t1 = time.perf_counter() - t0
+    steps = fixed_steps if fixed_steps is not None else max(1, min(50, int(round(target_seconds / max(t1, 1e-6)))))
+    t0 = time.perf_counter()
+    orc.rk_step(q, p, GAMMA, sub_ext, dt, steps)
+    t = time.perf_counter() - t0
+    return {"value": dof * STAGES * steps / t, "unit": UNIT, "cores": orc.threads, "kind": "oracle",
+            "sample": f"{ne}^3-element sub-box of {workload} (p={p}, {dof} nodes), {steps} LSERK45 steps, "
+                      f"oracle/dg_oracle.c OpenMP-over-elements build, {t:.1f} s",
+            "seconds_per_step": t / steps, "dof": dof}
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    K, W = args.steps, args.warmup
+    samp = oracle_sample(args.workload, fixed_steps=max(1, W))     # warm-up
+    samp = oracle_sample(args.workload, fixed_steps=K)
+    line = {"impl": "reference", "metric": METRIC, "value": samp["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": K, "warmup": W, "ms_per_step": 1e3 * samp["seconds_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{args.workload} (bounded sample: {samp['sample']})"},
+            "cpu_baseline": {k: samp[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": samp["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------------
+# the CUDA path
+# ----------------------------------------------------------------------------------------------
+def time_workload(workload, K, W, device, dist, sampler_index=None, want_e2e=False):
+    import torch
+    from paper_2006_15698_b200 import DG
+    from paper_2006_15698_b200 import inputs as I
+    c = I.CONFIGS[workload]
+    p, ext, n = c["p"], c["extent"], (c["nx"], c["ny"], c["nz"])
+    q = I.make_field(workload, xp=torch, device=device)
+    dg = DG(*n, p, GAMMA, ext, device=device)
+    dg.set_state(q)
+    dt = I.cfl_dt(dg.max_wavespeed(), p, ext, n, 0.1)
+    dof = n[0] * n[1] * n[2] * (p + 1) ** 3
+    stream = torch.cuda.current_stream(device)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(device)
+
+    dg.rk_step(dt, W)
+    barrier()
+    l0 = dg.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(sampler_index) if sampler_index is not None else None
+    if sampler:
+        sampler.__enter__()
+    e0.record(stream)
+    dg.rk_step(dt, K)
+    e1.record(stream)
+    barrier()
+    if sampler:
+        sampler.__exit__()
+    ms = e0.elapsed_time(e1)
+    launches = dg.launch_count - l0
+    finite = bool(torch.isfinite(dg.get_state(q)).all().item())
+    out = {"workload": workload, "p": p, "elements": list(n), "dof": dof, "ms": ms, "launches": launches,
+           "dt": dt, "finite": finite, "kernel": dg.kernel_info(),
+           "clocks": sampler.summary() if sampler else None}
+
+    if want_e2e:
+        # end to end through the public API with HOST buffers: every step copies the state in from
+        # pinned host memory, advances one LSERK45 step and copies the result back.
+        steps = min(K, 10)
+        host_in = torch.empty(q.shape, dtype=torch.float64, pin_memory=True)
+        host_out = torch.empty(q.shape, dtype=torch.float64, pin_memory=True)
+        dg.get_state(host_in)
+        for _ in range(2):
+            dg.set_state(host_in)
+            dg.rk_step(dt, 1)
+            dg.get_state(host_out)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            dg.set_state(host_in)
+            dg.rk_step(dt, 1)
+            dg.get_state(host_out)            # synchronises
+        torch.cuda.synchronize(device)
+        t = time.perf_counter() - t0
+        out["e2e"] = {"seconds": t, "steps": steps, "bytes_each_way": q.numel() * 8}
+        del host_in, host_out
+    dg.close()
+    del q
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    dist = None
+    if world > 1:
+        import torch.distributed as td
+        td.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        dist = td
+    device = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(device)
+    K, W = args.steps, max(3, args.warmup)
+    main = time_workload(args.workload, K, W, device, dist, physical_gpu_index(local_rank), want_e2e=True)
+
+    def reduce_max(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    ms = reduce_max(main["ms"])
+    e2e_s = reduce_max(main["e2e"]["seconds"])
+    sweep = []
+    if not args.no_sweep and world == 1:
+        for p in range(1, 8):
+            s = time_workload(f"cfg4_p{p}", 20, 3, device, None)
+            rate = s["dof"] * STAGES * 20 / (s["ms"] * 1e-3)
+            sweep.append({"p": p, "elements_per_side": s["elements"][0], "dof": s["dof"], "value": rate,
+                          "ms_per_step": s["ms"] / 20, "brick": [s["kernel"][k] for k in ("bx", "by", "bz")],
+                          "finite": s["finite"]})
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    peak, peak_src = measured_peaks()
+    dof = main["dof"]
+    value = world * dof * STAGES * K / (ms * 1e-3)
+    launch_s = ms * 1e-3 / main["launches"]                       # the step IS 5 stage-kernel launches
+    achieved = ALGO_BYTES_PER_DOF_STAGE * dof / launch_s / 1e9
+    for s in sweep:
+        s["roofline_frac"] = s["value"] * ALGO_BYTES_PER_DOF_STAGE / 1e9 / peak
+    e2e = main["e2e"]
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: {main['elements']} periodic elements, p={main['p']}, "
+                               f"{dof} nodes ({5 * dof} unknowns), fixed dt, one step = one LSERK45 step (5 stages)",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "l2": "working set per stage (Q+K, >= 2.6 GB) >> 126 MB L2; no flush needed",
+                   "brick": main["kernel"]},
+        "unknown_updates_per_s": 5 * value,
+        "finite": main["finite"],
+        "gpu_launches": main["launches"],
+        "clocks": main["clocks"],
+        "roofline": {"bound": "hbm", "kernel": "dg_stage_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": ALGO_BYTES_PER_DOF_STAGE * dof,
+                     "avg_launch_ms": launch_s * 1e3, "frac_of_8TBs_nominal": achieved / 8000.0,
+                     "traffic": ncu_traffic(args.workload)},
+        "e2e": {"value": world * dof * STAGES * e2e["steps"] / e2e_s, "unit": UNIT,
+                "h2d_bytes_per_step": e2e["bytes_each_way"], "d2h_bytes_per_step": e2e["bytes_each_way"],
+                "steps": e2e["steps"], "api": "DG.set_state(pinned host) -> DG.rk_step(dt,1) -> DG.get_state(pinned host)"},
+        "p_sweep": sweep,
+        "context": "paper: 1.13e9 DOF-updates/s per V100 (kernels only, derived from Table II, PAPER.md:264-269); "
+                   "another machine, not a target",
+    }
+    if not args.no_cpu and world == 1:
+        cb = oracle_sample(args.workload, target_seconds=10.0)
+        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

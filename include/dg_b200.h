@@ -1,0 +1,119 @@
+/*
+ * dg_b200.h -- C ABI of the B200-native (sm_100a, fp64) explicit time step of the nodal
+ * discontinuous Galerkin discretisation of the 3-D compressible Euler equations on a uniform
+ * periodic Cartesian hex mesh with collocated Gauss-Legendre points
+ * (Kirby & Mavriplis, arXiv 2006.15698; citations are PAPER.md:<line>).
+ *
+ * One context = one mesh + one state vector resident in GPU memory.  The hot path is
+ *     dg_rk_step : 5 x [ pointwise flux -> sum-factorised differentiation -> face traces ->
+ *                        Lax-Friedrichs interface flux -> lift -> 2/h scaling -> LSERK45 stage ]
+ * every step of which runs in this library's CUDA kernels (no CPU fallback, no other library).
+ *
+ * Memory ownership: the CALLER allocates all device memory (one workspace of
+ * dg_workspace_bytes(), e.g. a torch uint8 tensor) and owns the CUDA stream; the library borrows
+ * both from dg_bind() until dg_destroy().  The context itself (host struct + small operator
+ * tables in __constant__ memory) is owned by the library.
+ *
+ * Canonical array layout of every state-sized argument (`q`, `r`), N = p+1:
+ *     a[ ((((e*N + k)*N + j)*N + i)*5 + n ],   n = rho, rho u, rho v, rho w, rho E   (eq (2))
+ *     e = ex + nx*(ey + ny*ez)                 (element order: DESIGN.md reading R13)
+ * Node (i,j,k) of element (ex,ey,ez) is at x = (ex + (xi_i+1)/2) Lx/nx, ... with xi the
+ * N Gauss-Legendre points on [-1,1], ascending.  The library keeps the state in its
+ * own brick-major, variable-planar layout; dg_set_state/dg_get_state
+ * convert on the device.
+ *
+ * Pointers flagged `on_device` are device pointers (same device as the workspace) when
+ * on_device != 0, host pointers otherwise (pinned memory makes the copies asynchronous).
+ *
+ * Errors: every int-returning call returns DG_OK or one of the codes below and never throws or
+ * aborts; dg_last_error() gives the text.  Invalid arguments leave the context unchanged.  CUDA
+ * errors of asynchronous work surface at the next synchronising call.  Non-physical states
+ * (rho <= 0, p <= 0) are not trapped: the paper has no limiter; NaNs propagate (reading R15).
+ *
+ * Thread safety: calls on one context must be serialised by the caller.
+ */
+#ifndef DG_B200_H
+#define DG_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dg_ctx dg_ctx; /* opaque */
+
+enum {
+    DG_OK = 0,
+    DG_EINVAL = 1,       /* bad argument */
+    DG_EUNSUPPORTED = 2, /* p outside 1..7 */
+    DG_ENOMEM = 3,       /* workspace too small / host allocation failed */
+    DG_ECUDA = 4,        /* CUDA runtime error (text in dg_last_error) */
+    DG_ESTATE = 5        /* call out of order: not bound, or no state set */
+};
+
+/* Create a context for nx*ny*nz periodic elements on [0,Lx]x[0,Ly]x[0,Lz], extent = {Lx,Ly,Lz},
+ * polynomial degree p (N = p+1 Gauss-Legendre points per direction) and ratio of
+ * specific heats gamma.  nx,ny,nz >= 1; 1 <= p <= 7 else DG_EUNSUPPORTED;
+ * gamma > 1; extents > 0.  Touches no GPU.  *out is set only on DG_OK. */
+int dg_create(dg_ctx **out, int nx, int ny, int nz, int p, double gamma, const double extent[3]);
+
+/* Optional tuning knob, before dg_bind: elements per thread-block "brick" along each axis.  Only
+ * the shapes compiled into the library for this p are accepted (DG_EUNSUPPORTED otherwise);
+ * bx=by=bz=0 restores the default.  Changes layout sizes, so it is refused after dg_bind. */
+int dg_set_brick(dg_ctx *ctx, int bx, int by, int bz);
+
+/* 5*(p+1)^3*nx*ny*nz: number of doubles in a canonical state vector (size_t: config 5 > 2^31). */
+size_t dg_state_len(const dg_ctx *ctx);
+
+/* Device bytes the caller must provide to dg_bind: state Q, Runge-Kutta register K, one
+ * canonical staging vector, two face-trace buffers, scalars. */
+size_t dg_workspace_bytes(const dg_ctx *ctx);
+
+/* Borrow `bytes` (>= dg_workspace_bytes) of device memory, 256-byte aligned, and a CUDA stream
+ * (cudaStream_t passed as void*; NULL = legacy default stream).  All later work of this context
+ * is enqueued on that stream.  Uploads the operator tables (first CUDA call). */
+int dg_bind(dg_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream);
+
+/* Copy a canonical state vector in (host or device), convert it to the internal layout and
+ * compute its face traces.  Asynchronous for device / pinned-host sources. */
+int dg_set_state(dg_ctx *ctx, const double *q, int on_device);
+
+/* r_out = dQ/dt = L(Q) of the current state, canonical layout: eq (5) solved
+ * for the time derivative, with the local Lax-Friedrichs flux (reading R3).  Does
+ * not change the state.  Synchronises the stream when r_out is a host pointer. */
+int dg_residual(dg_ctx *ctx, double *r_out, int on_device);
+
+/* *lam_host = max over nodes of sqrt(u^2+v^2+w^2) + sqrt(gamma p/rho) of the current state
+ * (for the caller's CFL time step, reading R10).  Synchronises the stream. */
+int dg_max_wavespeed(dg_ctx *ctx, double *lam_host);
+
+/* Advance nsteps >= 0 LSERK45 steps of fixed dt:
+ * K = 0; for s = 1..5: K = A_s K + dt L(Q); Q = Q + B_s K.  One fused kernel per stage,
+ * enqueued on the stream, no host synchronisation. */
+int dg_rk_step(dg_ctx *ctx, double dt, int nsteps);
+
+/* Copy the current state out in canonical layout.  Synchronises when q_out is a host pointer. */
+int dg_get_state(dg_ctx *ctx, double *q_out, int on_device);
+
+/* The library's own N Gauss-Legendre nodes and weights (host arrays of p+1 doubles). */
+int dg_nodes(const dg_ctx *ctx, double *xi, double *w);
+
+/* Number of CUDA kernels this context has launched so far (bench.py's `gpu_launches`). */
+unsigned long long dg_launch_count(const dg_ctx *ctx);
+
+/* Launch geometry of the fused stage kernel, for reports: out[0..7] = brick elements bx,by,bz,
+ * threads per block, dynamic shared bytes per block, grid size (blocks), internal (padded)
+ * state length in doubles / 2^20 rounded up, face-trace doubles per brick. */
+int dg_kernel_info(const dg_ctx *ctx, long long out[8]);
+
+/* Release the context (never the borrowed workspace).  NULL is accepted. */
+int dg_destroy(dg_ctx *ctx);
+
+/* Text of the last error on this context ("" if none).  Valid until the next call on ctx. */
+const char *dg_last_error(const dg_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DG_B200_H */

@@ -1,0 +1,199 @@
+"""Thin ctypes binding of include/dg_b200.h: argument marshalling only.
+
+PyTorch is used for what the boundary leaves to the caller: device memory (one uint8 workspace
+tensor) and the CUDA stream.  Every step of the method runs in the library's CUDA kernels; there
+is no fallback of any kind: if libdg_b200.so is missing or a call fails, this raises.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+_DP = ctypes.POINTER(ctypes.c_double)
+_LIB = None
+
+# every symbol include/dg_b200.h declares (tests check the header against this and the .so)
+SYMBOLS = {
+    "dg_create": (ctypes.c_int, [ctypes.POINTER(ctypes.c_void_p), ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                 ctypes.c_int, ctypes.c_double, _DP]),
+    "dg_set_brick": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
+    "dg_state_len": (ctypes.c_size_t, [ctypes.c_void_p]),
+    "dg_workspace_bytes": (ctypes.c_size_t, [ctypes.c_void_p]),
+    "dg_bind": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]),
+    "dg_set_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
+    "dg_residual": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
+    "dg_max_wavespeed": (ctypes.c_int, [ctypes.c_void_p, _DP]),
+    "dg_rk_step": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int]),
+    "dg_get_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
+    "dg_nodes": (ctypes.c_int, [ctypes.c_void_p, _DP, _DP]),
+    "dg_launch_count": (ctypes.c_ulonglong, [ctypes.c_void_p]),
+    "dg_kernel_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_longlong)]),
+    "dg_destroy": (ctypes.c_int, [ctypes.c_void_p]),
+    "dg_last_error": (ctypes.c_char_p, [ctypes.c_void_p]),
+}
+ERRORS = {1: "DG_EINVAL", 2: "DG_EUNSUPPORTED", 3: "DG_ENOMEM", 4: "DG_ECUDA", 5: "DG_ESTATE"}
+
+
+class DGError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__(f"{ERRORS.get(code, code)}: {text}")
+        self.code = code
+
+
+def lib_path():
+    return os.path.join(HERE, "libdg_b200.so")
+
+
+def load_library(build_if_missing=True):
+    """dlopen libdg_b200.so (building it in-tree with nvcc if it is not there). No fallback."""
+    global _LIB
+    if _LIB is None:
+        path = lib_path()
+        if not os.path.exists(path):
+            if not build_if_missing:
+                raise FileNotFoundError(path)
+            from . import build
+            build.build()
+        lib = ctypes.CDLL(path)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(lib, name)      # AttributeError if the library does not export it
+            fn.restype = res
+            fn.argtypes = args
+        _LIB = lib
+    return _LIB
+
+
+def exported_symbols():
+    return sorted(SYMBOLS)
+
+
+class DG:
+    """One mesh + one state vector on the GPU.  Arrays are float64, shape (nz,ny,nx,N,N,N,5)."""
+
+    def __init__(self, nx, ny, nz, p, gamma=1.4, extent=(1.0, 1.0, 1.0), device="cuda:0", brick=None, bind=True):
+        self.lib = load_library()
+        self.nx, self.ny, self.nz, self.p, self.N = nx, ny, nz, p, p + 1
+        self.gamma, self.extent = float(gamma), tuple(float(e) for e in extent)
+        self.shape = (nz, ny, nx, self.N, self.N, self.N, 5)
+        self._h = ctypes.c_void_p()
+        ext = (ctypes.c_double * 3)(*self.extent)
+        rc = self.lib.dg_create(ctypes.byref(self._h), nx, ny, nz, p, self.gamma, ext)
+        if rc != 0:
+            self._h = None
+            raise DGError(rc, f"dg_create({nx},{ny},{nz},p={p},gamma={gamma},extent={extent})")
+        if brick is not None:
+            self._check(self.lib.dg_set_brick(self._h, *brick))
+        self.workspace = None
+        self.device = None
+        self._torch = None
+        if bind:
+            self.bind(device)
+
+    # -- plumbing -------------------------------------------------------------------------------
+    def _check(self, rc):
+        if rc != 0:
+            raise DGError(rc, self.lib.dg_last_error(self._h).decode())
+
+    def bind(self, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2006_15698_b200 needs a CUDA device; there is no CPU fallback")
+        self.device = torch.device(device)
+        self._torch = torch
+        nbytes = self.lib.dg_workspace_bytes(self._h)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self._check(self.lib.dg_bind(self._h, self.workspace.data_ptr(), nbytes, self.stream.cuda_stream))
+
+    @property
+    def state_len(self):
+        return self.lib.dg_state_len(self._h)
+
+    @property
+    def workspace_bytes(self):
+        return self.lib.dg_workspace_bytes(self._h)
+
+    @property
+    def launch_count(self):
+        return self.lib.dg_launch_count(self._h)
+
+    def kernel_info(self):
+        out = (ctypes.c_longlong * 8)()
+        self._check(self.lib.dg_kernel_info(self._h, out))
+        keys = ("bx", "by", "bz", "threads", "smem_bytes", "grid", "internal_mdoubles", "trace_doubles_per_brick")
+        return dict(zip(keys, [int(v) for v in out]))
+
+    def nodes(self):
+        xi = np.empty(self.N)
+        w = np.empty(self.N)
+        self._check(self.lib.dg_nodes(self._h, xi.ctypes.data_as(_DP), w.ctypes.data_as(_DP)))
+        return xi, w
+
+    def _ptr(self, a, writable):
+        """(pointer, on_device, keepalive) for a numpy array or a torch tensor of the state's size."""
+        torch = self._torch
+        if isinstance(a, torch.Tensor):
+            if a.dtype != torch.float64 or not a.is_contiguous() or a.numel() != self.state_len:
+                raise ValueError("state tensors must be contiguous float64 with dg_state_len elements")
+            if a.is_cuda and a.device != self.device:
+                raise ValueError("tensor is on another device")
+            return ctypes.c_void_p(a.data_ptr()), int(a.is_cuda), a
+        a = np.asarray(a)
+        if a.dtype != np.float64 or not a.flags.c_contiguous or a.size != self.state_len:
+            raise ValueError("state arrays must be C-contiguous float64 with dg_state_len elements")
+        if writable and not a.flags.writeable:
+            raise ValueError("output array is read-only")
+        return ctypes.c_void_p(a.ctypes.data), 0, a
+
+    # -- the six calls of north_star (+ max wavespeed) ---------------------------------------------
+    def set_state(self, q):
+        ptr, dev, keep = self._ptr(q, False)
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.dg_set_state(self._h, ptr, dev))
+        if dev == 0 and isinstance(keep, self._torch.Tensor) and keep.is_pinned():
+            self.stream.synchronize()     # the async copy reads the caller's pinned buffer
+        return self
+
+    def residual(self, out=None):
+        """dQ/dt of the current state; `out` may be a numpy array, a host or a cuda tensor."""
+        if out is None:
+            out = np.empty(self.shape)
+        ptr, dev, _ = self._ptr(out, True)
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.dg_residual(self._h, ptr, dev))
+        return out
+
+    def rk_step(self, dt, nsteps=1):
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.dg_rk_step(self._h, float(dt), int(nsteps)))
+        return self
+
+    def get_state(self, out=None):
+        if out is None:
+            out = np.empty(self.shape)
+        ptr, dev, _ = self._ptr(out, True)
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.dg_get_state(self._h, ptr, dev))
+        return out
+
+    def max_wavespeed(self):
+        lam = ctypes.c_double(0.0)
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.dg_max_wavespeed(self._h, ctypes.byref(lam)))
+        return lam.value
+
+    def close(self):
+        if getattr(self, "_h", None):
+            if self.workspace is not None:
+                self._torch.cuda.synchronize(self.device)
+            self.lib.dg_destroy(self._h)
+            self._h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

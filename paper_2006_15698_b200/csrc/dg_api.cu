@@ -1,0 +1,411 @@
+// dg_api.cu -- the C-ABI boundary (include/dg_b200.h): argument checking, workspace carving, operator
+// tables and kernel launches.  No arithmetic of the method runs here; it all runs in dg_kernels.cu.
+// Shares nothing with oracle/ (the operator construction below is written independently).
+#include "../../include/dg_b200.h"
+#include "dg_internal.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------
+// 1-D operators of the N-point Gauss-Legendre collocation basis, long double.
+// ------------------------------------------------------------------------------------------------
+struct HostOps {
+    long double xi[DG_NMAX], w[DG_NMAX];
+    long double D[DG_NMAX][DG_NMAX];   // D[q][i] = l_i'(xi_q)
+    long double lp[DG_NMAX], lm[DG_NMAX];
+};
+
+// Legendre polynomial by Bonnet's recurrence; derivative from P_N' = N (P_{N-1} - x P_N) / (1 - x^2).
+void legendre_pair(int N, long double x, long double &PN, long double &dPN) {
+    long double Pm = 1.0L, P = x;
+    if (N == 0) { PN = 1.0L; dPN = 0.0L; return; }
+    for (int k = 2; k <= N; ++k) {
+        const long double Pk = ((2 * k - 1) * x * P - (k - 1) * Pm) / k;
+        Pm = P;
+        P = Pk;
+    }
+    PN = P;
+    dPN = N * (Pm - x * P) / (1.0L - x * x);
+}
+
+void build_host_ops(int N, HostOps &o) {
+    const long double pi = acosl(-1.0L);
+    // nodes: Newton from the Chebyshev-like guess, left half then mirrored (ascending order)
+    for (int i = 0; i < (N + 1) / 2; ++i) {
+        long double x = -cosl(pi * (4 * i + 3) / (4 * N + 2));
+        for (int it = 0; it < 60; ++it) {
+            long double P, dP;
+            legendre_pair(N, x, P, dP);
+            const long double step = P / dP;
+            x -= step;
+            if (fabsl(step) <= 4e-20L) break;
+        }
+        if (2 * i + 1 == N) x = 0.0L;
+        long double P, dP;
+        legendre_pair(N, x, P, dP);
+        const long double wi = 2.0L / ((1.0L - x * x) * dP * dP);
+        o.xi[i] = x;          o.w[i] = wi;
+        o.xi[N - 1 - i] = -x; o.w[N - 1 - i] = wi;
+    }
+    // l_i'(xi_q) by the product formula: q != i: prod_{m != i,q} (xi_q - xi_m) / prod_{m != i} (xi_i - xi_m);
+    // q == i: sum_{m != i} 1 / (xi_i - xi_m).  l_i(+-1) = prod_{m != i} (+-1 - xi_m) / (xi_i - xi_m).
+    for (int i = 0; i < N; ++i) {
+        long double den = 1.0L, ep = 1.0L, em = 1.0L;
+        for (int m = 0; m < N; ++m) {
+            if (m == i) continue;
+            den *= (o.xi[i] - o.xi[m]);
+            ep *= (1.0L - o.xi[m]);
+            em *= (-1.0L - o.xi[m]);
+        }
+        o.lp[i] = ep / den;
+        o.lm[i] = em / den;
+        for (int q = 0; q < N; ++q) {
+            if (q == i) {
+                long double s = 0.0L;
+                for (int m = 0; m < N; ++m)
+                    if (m != i) s += 1.0L / (o.xi[i] - o.xi[m]);
+                o.D[q][i] = s;
+            } else {
+                long double num = 1.0L;
+                for (int m = 0; m < N; ++m)
+                    if (m != i && m != q) num *= (o.xi[q] - o.xi[m]);
+                o.D[q][i] = num / den;
+            }
+        }
+    }
+}
+
+void build_device_ops(int N, DgOps &d) {
+    HostOps o;
+    build_host_ops(N, o);
+    std::memset(&d, 0, sizeof(d));
+    for (int i = 0; i < N; ++i) {
+        d.lp[i] = (double)o.lp[i];
+        d.lm[i] = (double)o.lm[i];
+        d.lpw[i] = (double)(o.lp[i] / o.w[i]);
+        d.lmw[i] = (double)(o.lm[i] / o.w[i]);
+        for (int q = 0; q < N; ++q) d.Dhat[i * N + q] = (double)(o.w[q] * o.D[q][i] / o.w[i]);
+    }
+}
+
+// Carpenter-Kennedy (5,4) 2N-storage Runge-Kutta, "LSERK45" (reading R9).
+const long double kRkA[5] = {0.0L, -567301805773.0L / 1357537059087.0L, -2404267990393.0L / 2016746695238.0L,
+                             -3550918686646.0L / 2091501179385.0L, -1275806237668.0L / 842570457699.0L};
+const long double kRkB[5] = {1432997174477.0L / 9575080441755.0L, 5161836677717.0L / 13612068292357.0L,
+                             1720146321549.0L / 2090206949498.0L, 3134564353537.0L / 4481467310338.0L,
+                             2277821191437.0L / 14882151754819.0L};
+
+const DgKernelTable *variants_for(int N, int *count) {
+    switch (N) {
+        case 2: return dg_variants_N2(count);
+        case 3: return dg_variants_N3(count);
+        case 4: return dg_variants_N4(count);
+        case 5: return dg_variants_N5(count);
+        case 6: return dg_variants_N6(count);
+        case 7: return dg_variants_N7(count);
+        case 8: return dg_variants_N8(count);
+    }
+    *count = 0;
+    return nullptr;
+}
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+}  // namespace
+
+struct dg_ctx {
+    int nx, ny, nz, p, N;
+    double gamma;
+    double extent[3];
+    const DgKernelTable *kt;
+    int nbx, nby, nbz;
+    size_t nbricks;
+    size_t state_len;   // canonical doubles
+    size_t int_len;     // internal (brick-padded) doubles
+    size_t trace_len;   // doubles per trace buffer
+    // borrowed workspace
+    double *Q, *K, *S, *T[2];
+    unsigned long long *scal;
+    int tcur;           // T[tcur] holds the traces of the current Q
+    bool bound, has_state;
+    cudaStream_t stream;
+    unsigned long long launches;
+    char err[256];
+};
+
+namespace {
+
+int fail(dg_ctx *c, int code, const char *fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+int cuda_fail(dg_ctx *c, cudaError_t e, const char *what) {
+    return fail(c, DG_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+void set_layout(dg_ctx *c, const DgKernelTable *kt) {
+    c->kt = kt;
+    c->nbx = (c->nx + kt->bx - 1) / kt->bx;
+    c->nby = (c->ny + kt->by - 1) / kt->by;
+    c->nbz = (c->nz + kt->bz - 1) / kt->bz;
+    c->nbricks = (size_t)c->nbx * c->nby * c->nbz;
+    c->int_len = c->nbricks * (size_t)kt->slot;
+    c->trace_len = c->nbricks * (size_t)kt->tslot;
+}
+
+struct Carve {
+    size_t q, k, s, t0, t1, scal, total;
+};
+Carve carve(const dg_ctx *c) {
+    Carve v;
+    size_t off = 0;
+    v.q = off;    off += align_up(c->int_len * 8, 256);
+    v.k = off;    off += align_up(c->int_len * 8, 256);
+    v.s = off;    off += align_up(c->state_len * 8, 256);
+    v.t0 = off;   off += align_up(c->trace_len * 8, 256);
+    v.t1 = off;   off += align_up(c->trace_len * 8, 256);
+    v.scal = off; off += 256;
+    v.total = off;
+    return v;
+}
+
+DgStageArgs stage_args(const dg_ctx *c, int mode) {
+    DgStageArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.Q = c->Q;
+    a.K = c->K;
+    a.Rout = c->K;   // the Runge-Kutta register is dead between steps: residual output lands there
+    a.Told = c->T[c->tcur];
+    a.Tnew = c->T[1 - c->tcur];
+    a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
+    a.nbx = c->nbx; a.nby = c->nby; a.nbz = c->nbz;
+    a.g[0] = 2.0 / (c->extent[0] / c->nx);
+    a.g[1] = 2.0 / (c->extent[1] / c->ny);
+    a.g[2] = 2.0 / (c->extent[2] / c->nz);
+    a.gamma = c->gamma;
+    a.gm1 = c->gamma - 1.0;
+    a.mode = mode;
+    return a;
+}
+
+int launch_layout(dg_ctx *c, double *internal, double *canonical, int to_internal) {
+    DgLayoutArgs a;
+    a.internal = internal;
+    a.canonical = canonical;
+    a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
+    a.nbx = c->nbx; a.nby = c->nby; a.nbz = c->nbz;
+    a.to_internal = to_internal;
+    cudaError_t e = c->kt->launch_layout(a, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "layout kernel");
+    c->launches++;
+    return DG_OK;
+}
+
+// internal vector -> caller's canonical array (device: directly; host: through the staging vector)
+int export_vector(dg_ctx *c, double *internal, double *out, int on_device, const char *what) {
+    if (on_device) return launch_layout(c, internal, out, 0);
+    int rc = launch_layout(c, internal, c->S, 0);
+    if (rc != DG_OK) return rc;
+    cudaError_t e = cudaMemcpyAsync(out, c->S, c->state_len * 8, cudaMemcpyDeviceToHost, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, what);
+    e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, what);
+    return DG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int dg_create(dg_ctx **out, int nx, int ny, int nz, int p, double gamma, const double extent[3]) {
+    if (!out || !extent) return DG_EINVAL;
+    if (nx < 1 || ny < 1 || nz < 1) return DG_EINVAL;
+    if (!(gamma > 1.0) || !std::isfinite(gamma)) return DG_EINVAL;
+    for (int a = 0; a < 3; ++a)
+        if (!(extent[a] > 0.0) || !std::isfinite(extent[a])) return DG_EINVAL;
+    if (p < 1 || p > 7) return DG_EUNSUPPORTED;
+    int count = 0;
+    const DgKernelTable *kt = variants_for(p + 1, &count);
+    if (!kt || count < 1) return DG_EUNSUPPORTED;
+    dg_ctx *c = new (std::nothrow) dg_ctx;
+    if (!c) return DG_ENOMEM;
+    std::memset(c, 0, sizeof(*c));
+    c->nx = nx; c->ny = ny; c->nz = nz; c->p = p; c->N = p + 1;
+    c->gamma = gamma;
+    for (int a = 0; a < 3; ++a) c->extent[a] = extent[a];
+    c->state_len = (size_t)nx * ny * nz * (size_t)(c->N * c->N * c->N) * DG_NV;
+    set_layout(c, &kt[0]);
+    *out = c;
+    return DG_OK;
+}
+
+int dg_set_brick(dg_ctx *c, int bx, int by, int bz) {
+    if (!c) return DG_EINVAL;
+    if (c->bound) return fail(c, DG_ESTATE, "dg_set_brick after dg_bind");
+    int count = 0;
+    const DgKernelTable *kt = variants_for(c->N, &count);
+    if (bx == 0 && by == 0 && bz == 0) {
+        set_layout(c, &kt[0]);
+        return DG_OK;
+    }
+    for (int v = 0; v < count; ++v)
+        if (kt[v].bx == bx && kt[v].by == by && kt[v].bz == bz) {
+            set_layout(c, &kt[v]);
+            return DG_OK;
+        }
+    return fail(c, DG_EUNSUPPORTED, "brick %dx%dx%d is not compiled for p=%d", bx, by, bz, c->p);
+}
+
+size_t dg_state_len(const dg_ctx *c) { return c ? c->state_len : 0; }
+
+size_t dg_workspace_bytes(const dg_ctx *c) { return c ? carve(c).total : 0; }
+
+int dg_bind(dg_ctx *c, void *ws, size_t bytes, void *stream) {
+    if (!c) return DG_EINVAL;
+    if (!ws || ((size_t)ws & 255u)) return fail(c, DG_EINVAL, "workspace must be a 256-byte aligned device pointer");
+    const Carve v = carve(c);
+    if (bytes < v.total) return fail(c, DG_ENOMEM, "workspace %zu bytes < required %zu", bytes, v.total);
+    if (c->nbricks > 2147483647ull) return fail(c, DG_EUNSUPPORTED, "more than 2^31-1 bricks");
+    char *base = (char *)ws;
+    c->Q = (double *)(base + v.q);
+    c->K = (double *)(base + v.k);
+    c->S = (double *)(base + v.s);
+    c->T[0] = (double *)(base + v.t0);
+    c->T[1] = (double *)(base + v.t1);
+    c->scal = (unsigned long long *)(base + v.scal);
+    c->stream = (cudaStream_t)stream;
+    c->tcur = 0;
+    c->has_state = false;
+    DgOps ops;
+    build_device_ops(c->N, ops);
+    cudaError_t e = c->kt->upload_ops(&ops, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "operator upload");
+    c->bound = true;
+    c->err[0] = 0;
+    return DG_OK;
+}
+
+int dg_set_state(dg_ctx *c, const double *q, int on_device) {
+    if (!c || !q) return c ? fail(c, DG_EINVAL, "null state pointer") : DG_EINVAL;
+    if (!c->bound) return fail(c, DG_ESTATE, "dg_set_state before dg_bind");
+    const double *src = q;
+    if (!on_device) {
+        cudaError_t e = cudaMemcpyAsync(c->S, q, c->state_len * 8, cudaMemcpyHostToDevice, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "host->device copy of the state");
+        src = c->S;
+    }
+    int rc = launch_layout(c, c->Q, const_cast<double *>(src), 1);
+    if (rc != DG_OK) return rc;
+    // traces of the new state into T[tcur]
+    c->tcur = 0;
+    DgStageArgs a = stage_args(c, DG_MODE_TRACES);
+    a.Tnew = c->T[0];
+    a.Told = c->T[1];
+    cudaError_t e = c->kt->launch_stage(a, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "trace kernel");
+    c->launches++;
+    c->has_state = true;
+    return DG_OK;
+}
+
+int dg_residual(dg_ctx *c, double *r_out, int on_device) {
+    if (!c || !r_out) return c ? fail(c, DG_EINVAL, "null residual pointer") : DG_EINVAL;
+    if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_residual needs dg_bind and dg_set_state first");
+    DgStageArgs a = stage_args(c, DG_MODE_RESIDUAL);
+    cudaError_t e = c->kt->launch_stage(a, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "residual kernel");
+    c->launches++;
+    return export_vector(c, c->K, r_out, on_device, "device->host copy of the residual");
+}
+
+int dg_max_wavespeed(dg_ctx *c, double *lam_host) {
+    if (!c || !lam_host) return c ? fail(c, DG_EINVAL, "null pointer") : DG_EINVAL;
+    if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_max_wavespeed needs dg_bind and dg_set_state first");
+    cudaError_t e = cudaMemsetAsync(c->scal, 0, 8, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "memset");
+    DgWaveArgs a;
+    a.Q = c->Q;
+    a.lam_bits = c->scal;
+    a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
+    a.nbx = c->nbx; a.nby = c->nby; a.nbz = c->nbz;
+    a.gamma = c->gamma;
+    a.gm1 = c->gamma - 1.0;
+    e = c->kt->launch_wavespeed(a, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "wavespeed kernel");
+    c->launches++;
+    e = cudaMemcpyAsync(lam_host, c->scal, 8, cudaMemcpyDeviceToHost, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "device->host copy");
+    e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "synchronise");
+    return DG_OK;
+}
+
+int dg_rk_step(dg_ctx *c, double dt, int nsteps) {
+    if (!c) return DG_EINVAL;
+    if (nsteps < 0 || !std::isfinite(dt)) return fail(c, DG_EINVAL, "nsteps < 0 or dt not finite");
+    if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_rk_step needs dg_bind and dg_set_state first");
+    for (int step = 0; step < nsteps; ++step) {
+        for (int s = 0; s < 5; ++s) {
+            DgStageArgs a = stage_args(c, DG_MODE_STAGE);
+            a.rkA = (double)kRkA[s];
+            a.rkB = (double)kRkB[s];
+            a.dt = dt;
+            cudaError_t e = c->kt->launch_stage(a, c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e, "stage kernel");
+            c->launches++;
+            c->tcur = 1 - c->tcur;
+        }
+    }
+    return DG_OK;
+}
+
+int dg_get_state(dg_ctx *c, double *q_out, int on_device) {
+    if (!c || !q_out) return c ? fail(c, DG_EINVAL, "null state pointer") : DG_EINVAL;
+    if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_get_state needs dg_bind and dg_set_state first");
+    return export_vector(c, c->Q, q_out, on_device, "device->host copy of the state");
+}
+
+int dg_nodes(const dg_ctx *c, double *xi, double *w) {
+    if (!c || !xi || !w) return DG_EINVAL;
+    HostOps o;
+    build_host_ops(c->N, o);
+    for (int i = 0; i < c->N; ++i) {
+        xi[i] = (double)o.xi[i];
+        w[i] = (double)o.w[i];
+    }
+    return DG_OK;
+}
+
+unsigned long long dg_launch_count(const dg_ctx *c) { return c ? c->launches : 0; }
+
+int dg_kernel_info(const dg_ctx *c, long long out[8]) {
+    if (!c || !out) return DG_EINVAL;
+    out[0] = c->kt->bx; out[1] = c->kt->by; out[2] = c->kt->bz;
+    out[3] = c->kt->threads;
+    out[4] = c->kt->smem_bytes;
+    out[5] = (long long)c->nbricks;
+    out[6] = (long long)((c->int_len + (1u << 20) - 1) >> 20);
+    out[7] = c->kt->tslot;
+    return DG_OK;
+}
+
+int dg_destroy(dg_ctx *c) {
+    delete c;
+    return DG_OK;
+}
+
+const char *dg_last_error(const dg_ctx *c) { return c ? c->err : "null context"; }
+
+}  // extern "C"

@@ -1,0 +1,76 @@
+// dg_internal.h -- shared between the C-ABI translation unit (dg_api.cu) and the per-degree
+// kernel translation units (dg_kernels.cu compiled once per N = p+1 with -DDG_N=<N>).
+// Not part of the public boundary (include/dg_b200.h is).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+
+#define DG_NV 5      // rho, rho u, rho v, rho w, rho E       (eq (2))
+#define DG_NMAX 8    // largest N = p+1 compiled
+
+// 1-D operators of the collocated Gauss-Legendre Lagrange basis, built on the
+// host in long double (dg_api.cu) and placed in __constant__ memory of each kernel TU so that
+// fully unrolled loops read them as immediate constant-bank operands of DFMA.
+struct DgOps {
+    double Dhat[DG_NMAX * DG_NMAX];  // Dhat[i*N+q] = w_q l_i'(xi_q) / w_i   (eq (5) 2nd term / mass)
+    double lp[DG_NMAX], lm[DG_NMAX]; // l_i(+1), l_i(-1)                     (face traces)
+    double lpw[DG_NMAX], lmw[DG_NMAX]; // l_i(+-1) / w_i                     (lift / mass)
+};
+
+enum DgMode {
+    DG_MODE_STAGE = 0,     // full Runge-Kutta stage: residual + K,Q update + new traces
+    DG_MODE_RESIDUAL = 1,  // residual only, written to Rout (internal layout)
+    DG_MODE_TRACES = 2     // face traces of Q only (after dg_set_state)
+};
+
+// Arguments of the fused stage kernel (passed by value, lives in the constant bank).
+struct DgStageArgs {
+    double *Q;            // state, internal layout [brick][n][gz][gy][gx]
+    double *K;            // Runge-Kutta register, same layout
+    double *Rout;         // residual output (mode RESIDUAL)
+    const double *Told;   // brick-boundary face traces of the current Q
+    double *Tnew;         // ... of the updated Q (mode STAGE / TRACES)
+    int nx, ny, nz;       // elements per axis
+    int nbx, nby, nbz;    // bricks per axis
+    double g[3];          // 2/h_a: constant geometric factor per axis
+    double gamma, gm1;
+    double rkA, rkB, dt;  // stage coefficients; rkA == 0 means "do not read K" (stage 1)
+    int mode;
+};
+
+struct DgLayoutArgs {
+    double *internal;       // [brick][n][gz][gy][gx]
+    double *canonical;      // [e][k][j][i][n]
+    int nx, ny, nz, nbx, nby, nbz;
+    int to_internal;        // 1: canonical -> internal, 0: internal -> canonical
+};
+
+struct DgWaveArgs {
+    const double *Q;
+    unsigned long long *lam_bits;  // max reduced on the bit pattern (non-negative doubles order as integers)
+    int nx, ny, nz, nbx, nby, nbz;
+    double gamma, gm1;
+};
+
+// One compiled (N, brick shape) variant.
+struct DgKernelTable {
+    int N, bx, by, bz;
+    int threads;             // threads per block of the stage kernel
+    int smem_bytes;          // dynamic shared memory of the stage kernel
+    long long slot;          // doubles per brick in Q/K/R (5 * nodes per brick)
+    long long tslot;         // face-trace doubles per brick
+    cudaError_t (*upload_ops)(const DgOps *ops, cudaStream_t s);
+    cudaError_t (*launch_stage)(const DgStageArgs &a, cudaStream_t s);
+    cudaError_t (*launch_layout)(const DgLayoutArgs &a, cudaStream_t s);
+    cudaError_t (*launch_wavespeed)(const DgWaveArgs &a, cudaStream_t s);
+};
+
+// Each kernel TU exports its variants: dg_variants_N<N>(&count) -> array of tables, default first.
+#define DG_DECLARE_VARIANTS(NN) const DgKernelTable *dg_variants_N##NN(int *count);
+DG_DECLARE_VARIANTS(2)
+DG_DECLARE_VARIANTS(3)
+DG_DECLARE_VARIANTS(4)
+DG_DECLARE_VARIANTS(5)
+DG_DECLARE_VARIANTS(6)
+DG_DECLARE_VARIANTS(7)
+DG_DECLARE_VARIANTS(8)

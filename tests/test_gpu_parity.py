@@ -1,0 +1,163 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the CPU oracle, element by element.
+
+Error norm: e = max over the 5 variables of
+|gpu_n - oracle_n|_inf / |oracle_n|_inf  (absolute where the oracle's variable is identically 0).
+Tolerances are north_star's: 1e-11 per residual evaluation, 1e-9 after 100 Runge-Kutta steps.
+The oracle's OpenMP build is used for speed; tests/test_oracle_residual.py checks it is
+bit-identical to the single-threaded fp64 build.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import Oracle                                    # noqa: E402
+from paper_2006_15698_b200 import DG, DGError                # noqa: E402
+from paper_2006_15698_b200 import inputs as I                # noqa: E402
+import dg_bruteforce as bf                                   # noqa: E402
+
+G = 1.4
+TOL_RES = 1e-11
+TOL_RK100 = 1e-9
+ORC = Oracle("omp")
+
+VARIANTS = {1: [(4, 4, 2), (2, 2, 2), (4, 4, 4)], 2: [(2, 2, 2), (1, 1, 1), (4, 2, 2)], 3: [(2, 2, 1), (1, 1, 1), (2, 2, 2)],
+            4: [(2, 1, 1), (1, 1, 1), (2, 2, 1)], 5: [(1, 1, 1), (2, 1, 1), (2, 2, 1)], 6: [(1, 1, 1), (2, 1, 1)],
+            7: [(1, 1, 1), (2, 1, 1)]}
+
+
+def relerr(a, b):
+    out = 0.0
+    for n in range(5):
+        d = np.abs(a[..., n] - b[..., n]).max()
+        s = np.abs(b[..., n]).max()
+        out = max(out, d / s if s > 0 else d)
+    return out
+
+
+def rough_field(nx, ny, nz, p, extent, seed=11):
+    return I.density_wave(nx, ny, nz, p, extent, vel=(0.5, -0.3, 0.2), noise=5e-2, seed=seed, waves=(1, 2, 1))
+
+
+def test_library_is_the_cuda_one_and_fails_loudly_without_state():
+    dg = DG(2, 2, 2, 1)
+    with pytest.raises(DGError):
+        dg.rk_step(1e-3, 1)                      # DG_ESTATE: no state yet
+    with pytest.raises(DGError):
+        DG(2, 2, 2, 9)
+    assert dg.launch_count == 0
+    dg.close()
+
+
+@pytest.mark.parametrize("p", range(1, 8))
+def test_layout_roundtrip_and_wavespeed_all_variants(p):
+    nx, ny, nz, ext = 5, 3, 2, (1.0, 0.6, 0.4)                # ragged against every brick shape
+    q = rough_field(nx, ny, nz, p, ext)
+    for brick in [None] + VARIANTS[p]:
+        dg = DG(nx, ny, nz, p, G, ext, brick=brick)
+        dg.set_state(q)
+        assert np.array_equal(dg.get_state(), q)
+        qd = torch.empty(q.shape, dtype=torch.float64, device="cuda")
+        dg.get_state(qd)
+        assert np.array_equal(qd.cpu().numpy(), q)
+        lam = dg.max_wavespeed()
+        assert abs(lam - ORC.max_wavespeed(q, p, G)) <= 4e-16 * lam
+        dg.close()
+
+
+@pytest.mark.parametrize("p", range(1, 8))
+def test_residual_parity_ragged_mesh_all_variants(p):
+    nx, ny, nz, ext = 5, 3, 2, (1.0, 0.6, 0.4)
+    q = rough_field(nx, ny, nz, p, ext)
+    r_orc = ORC.residual(q, p, G, ext)
+    for brick in [None] + VARIANTS[p]:
+        dg = DG(nx, ny, nz, p, G, ext, brick=brick)
+        r = dg.set_state(q).residual()
+        assert relerr(r, r_orc) < TOL_RES, (p, brick, relerr(r, r_orc))
+        assert np.array_equal(dg.get_state(), q)              # residual leaves the state alone
+        r2 = dg.residual(torch.empty(q.shape, dtype=torch.float64, device="cuda")).cpu().numpy()
+        assert np.array_equal(r2, r)                          # device output == host output, repeatable
+        dg.close()
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 1), (1, 4, 2), (7, 1, 3), (9, 9, 9)])
+def test_residual_parity_degenerate_meshes(shape):
+    """n_a = 1 (the element is its own neighbour), meshes smaller than a brick, odd sizes."""
+    nx, ny, nz = shape
+    for p in (1, 2, 3, 4):
+        ext = (1.0, 1.3, 0.7)
+        q = rough_field(nx, ny, nz, p, ext, seed=3)
+        dg = DG(nx, ny, nz, p, G, ext)
+        e = relerr(dg.set_state(q).residual(), ORC.residual(q, p, G, ext))
+        assert e < TOL_RES, (shape, p, e)
+        dg.close()
+
+
+def test_cfg1_residual_freestream_conservation_and_ten_steps():
+    c = I.CONFIGS["cfg1"]
+    p, ext, n = c["p"], c["extent"], (c["nx"], c["ny"], c["nz"])
+    q0 = I.make_field("cfg1")
+    dg = DG(*n, p, G, ext)
+    dg.set_state(q0)
+    r = dg.residual()
+    assert relerr(r, ORC.residual(q0, p, G, ext)) < TOL_RES
+    tot = bf.integrals(r, p, ext)                              # discrete conservation on the GPU result
+    assert np.all(np.abs(tot) < 1e-14 * np.maximum(bf.integrals(np.abs(r), p, ext), 1.0))
+    dt = I.cfl_dt(ORC.max_wavespeed(q0, p, G), p, ext, n, 0.1)
+    q10 = dg.rk_step(dt, 10).get_state()
+    q10_orc = ORC.rk_step(q0, p, G, ext, dt, 10)
+    assert relerr(q10, q10_orc) < 1e-12
+    assert np.all(np.abs(bf.integrals(q10, p, ext) - bf.integrals(q0, p, ext)) < 5e-15)
+    # free stream: uniform state gives a zero residual to roundoff
+    qu = I.uniform_state(*n, p, rho=1.0, vel=(0.5, 0.5, 0.5), pres=1.0)
+    assert np.abs(dg.set_state(qu).residual()).max() < 2e-13
+    dg.close()
+
+
+def test_cfg2_vortex_residual_and_100_steps():
+    c = I.CONFIGS["cfg2"]
+    p, ext, n = c["p"], c["extent"], (c["nx"], c["ny"], c["nz"])
+    q0 = I.make_field("cfg2")
+    dg = DG(*n, p, G, ext)
+    dg.set_state(q0)
+    assert relerr(dg.residual(), ORC.residual(q0, p, G, ext)) < TOL_RES
+    dt = I.cfl_dt(ORC.max_wavespeed(q0, p, G), p, ext, n, 0.1)
+    q = dg.rk_step(dt, 100).get_state()
+    e = relerr(q, ORC.rk_step(q0, p, G, ext, dt, 100))
+    assert e < TOL_RK100, e
+    # and the solution is the translated vortex to discretisation accuracy
+    exact = I.isentropic_vortex(*n, p, ext, t=100 * dt)
+    assert np.abs(q[..., 0] - exact[..., 0]).max() < 5e-3
+    dg.close()
+
+
+@pytest.mark.parametrize("p", range(1, 8))
+def test_100_steps_reduced_grids_of_cfg3_cfg4_cfg5(p):
+    """The 1e-9 / 100-step check for every p of configs 3-5 on reduced grids, same field formulas."""
+    n = 8 if p < 6 else 6
+    fields = [("fourier_modes", (1.0, 1.0, 1.0))]
+    if p in (4, 7):
+        fields.append(("taylor_green", (2 * np.pi,) * 3))
+    for field, ext in fields:
+        cfg = dict(nx=n, ny=n, nz=n, p=p, extent=ext, field=field)
+        q0 = I.make_field(cfg)
+        dt = I.cfl_dt(ORC.max_wavespeed(q0, p, G), p, ext, (n, n, n), 0.1)
+        dg = DG(n, n, n, p, G, ext)
+        q = dg.set_state(q0).rk_step(dt, 100).get_state()
+        e = relerr(q, ORC.rk_step(q0, p, G, ext, dt, 100))
+        assert e < TOL_RK100, (p, field, e)
+        dg.close()
+
+
+def test_rk_step_composes_and_zero_steps_is_identity():
+    nx, ny, nz, p, ext = 6, 4, 3, 2, (1.0, 1.0, 0.5)
+    q0 = rough_field(nx, ny, nz, p, ext)
+    dg = DG(nx, ny, nz, p, G, ext)
+    a = dg.set_state(q0).rk_step(1e-3, 0).get_state()
+    assert np.array_equal(a, q0)
+    b = dg.set_state(q0).rk_step(1e-3, 3).get_state()
+    c = dg.set_state(q0).rk_step(1e-3, 1).rk_step(1e-3, 2).get_state()
+    assert np.array_equal(b, c)
+    assert dg.launch_count > 0
+    dg.close()
