@@ -17,7 +17,8 @@ _LIBS = {}
 
 
 def _load(variant):
-    name = {"fp64": "libdg_oracle.so", "ld": "libdg_oracle_ld.so", "omp": "libdg_oracle_omp.so"}[variant]
+    name = {"fp64": "libdg_oracle.so", "ld": "libdg_oracle_ld.so", "omp": "libdg_oracle_omp.so",
+            "ld_omp": "libdg_oracle_ld_omp.so"}[variant]
     if name not in _LIBS:
         paths = _build.build()
         lib = ctypes.CDLL(paths[name])
@@ -44,7 +45,7 @@ def _check(rc, what):
 
 
 class Oracle:
-    """One build variant of the oracle: 'fp64' (parity), 'ld' (long-double arbiter), 'omp'."""
+    """One build variant of the oracle: 'fp64' (parity), 'ld' (long-double arbiter), 'omp', 'ld_omp'."""
 
     def __init__(self, variant="fp64"):
         self.variant = variant

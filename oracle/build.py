@@ -5,6 +5,8 @@ Three shared objects from the one source dg_oracle.c:
   libdg_oracle_ld.so   x87 long double arbiter build, same source (-DORACLE_REAL="long double")
   libdg_oracle_omp.so  fp64 with `#pragma omp parallel for` over elements (timing baseline;
                        bit-identical to the single-threaded build, tests check that)
+  libdg_oracle_ld_omp.so  the long double arbiter with the same OpenMP loops (bit-identical to
+                       the single-threaded arbiter; used where the arbiter runs 100 steps)
 
 Usage:  python oracle/build.py [--force]
 """
@@ -20,6 +22,7 @@ VARIANTS = {
     "libdg_oracle.so": [],
     "libdg_oracle_ld.so": ['-DORACLE_REAL=long double'],
     "libdg_oracle_omp.so": ["-fopenmp"],
+    "libdg_oracle_ld_omp.so": ['-DORACLE_REAL=long double', "-fopenmp"],
 }
 CFLAGS = ["-std=c11", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared",
           "-Wall", "-Wextra"]
