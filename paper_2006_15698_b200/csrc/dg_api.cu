@@ -288,9 +288,12 @@ int dg_bind(dg_ctx *c, void *ws, size_t bytes, void *stream) {
     c->stream = (cudaStream_t)stream;
     c->tcur = 0;
     c->has_state = false;
+    // bricks of a ragged mesh carry padding nodes that are staged but never used: give them a defined value
+    cudaError_t e = cudaMemsetAsync(base, 0, v.total, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "workspace memset");
     DgOps ops;
     build_device_ops(c->N, ops);
-    cudaError_t e = c->kt->upload_ops(&ops, c->stream);
+    e = c->kt->upload_ops(&ops, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "operator upload");
     c->bound = true;
     c->err[0] = 0;

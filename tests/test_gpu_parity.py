@@ -25,9 +25,9 @@ TOL_RK100 = 1e-9
 ORC = Oracle("omp")
 ARB = Oracle("ld_omp")
 
-VARIANTS = {1: [(4, 4, 2), (2, 2, 2), (4, 4, 4)], 2: [(2, 2, 2), (1, 1, 1), (4, 2, 2)], 3: [(2, 2, 1), (1, 1, 1), (2, 2, 2)],
-            4: [(2, 1, 1), (1, 1, 1), (2, 2, 1)], 5: [(1, 1, 1), (2, 1, 1), (2, 2, 1)], 6: [(1, 1, 1), (2, 1, 1)],
-            7: [(1, 1, 1), (2, 1, 1)]}
+VARIANTS = {1: [(4, 4, 4), (2, 2, 2), (4, 4, 2)], 2: [(3, 3, 2), (1, 1, 1), (2, 2, 2)], 3: [(2, 2, 2), (1, 1, 1), (2, 2, 1)],
+            4: [(1, 2, 2), (1, 1, 1), (2, 2, 1)], 5: [(1, 1, 2), (1, 1, 1), (2, 2, 1)], 6: [(1, 1, 1), (2, 1, 1), (1, 1, 2)],
+            7: [(1, 1, 1), (2, 1, 1), (1, 1, 2)]}
 
 
 def relerr(a, b):
