@@ -63,6 +63,14 @@ int dg_create(dg_ctx **out, int nx, int ny, int nz, int p, double gamma, const d
  * bx=by=bz=0 restores the default.  Changes layout sizes, so it is refused after dg_bind. */
 int dg_set_brick(dg_ctx *ctx, int bx, int by, int bz);
 
+/* Number of stage-kernel variants (brick shape x buffering depth x residency) compiled into the
+ * library for degree p; 0 when p is outside 1..7.  Variant 0 is the default. */
+int dg_variant_count(int p);
+
+/* Tuning knob, before dg_bind: select variant 0 <= index < dg_variant_count(p) (DG_EINVAL otherwise).
+ * The environment variable DG_VARIANT=<index> sets the default picked by dg_create. */
+int dg_set_variant(dg_ctx *ctx, int index);
+
 /* 5*(p+1)^3*nx*ny*nz: number of doubles in a canonical state vector (size_t: config 5 > 2^31). */
 size_t dg_state_len(const dg_ctx *ctx);
 
@@ -103,7 +111,7 @@ int dg_nodes(const dg_ctx *ctx, double *xi, double *w);
 unsigned long long dg_launch_count(const dg_ctx *ctx);
 
 /* Launch geometry of the fused stage kernel, for reports: out[0..7] = brick elements bx,by,bz,
- * threads per block, dynamic shared bytes per block, grid size (blocks), internal (padded)
+ * threads per block, dynamic shared bytes per block, grid size (persistent blocks once bound, bricks before), internal (padded)
  * state length in doubles / 2^20 rounded up, face-trace doubles per brick. */
 int dg_kernel_info(const dg_ctx *ctx, long long out[8]);
 

@@ -18,6 +18,8 @@ SYMBOLS = {
     "dg_create": (ctypes.c_int, [ctypes.POINTER(ctypes.c_void_p), ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                  ctypes.c_int, ctypes.c_double, _DP]),
     "dg_set_brick": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
+    "dg_variant_count": (ctypes.c_int, [ctypes.c_int]),
+    "dg_set_variant": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
     "dg_state_len": (ctypes.c_size_t, [ctypes.c_void_p]),
     "dg_workspace_bytes": (ctypes.c_size_t, [ctypes.c_void_p]),
     "dg_bind": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]),
@@ -71,7 +73,8 @@ def exported_symbols():
 class DG:
     """One mesh + one state vector on the GPU.  Arrays are float64, shape (nz,ny,nx,N,N,N,5)."""
 
-    def __init__(self, nx, ny, nz, p, gamma=1.4, extent=(1.0, 1.0, 1.0), device="cuda:0", brick=None, bind=True):
+    def __init__(self, nx, ny, nz, p, gamma=1.4, extent=(1.0, 1.0, 1.0), device="cuda:0", brick=None, bind=True,
+                 variant=None):
         self.lib = load_library()
         self.nx, self.ny, self.nz, self.p, self.N = nx, ny, nz, p, p + 1
         self.gamma, self.extent = float(gamma), tuple(float(e) for e in extent)
@@ -84,6 +87,8 @@ class DG:
             raise DGError(rc, f"dg_create({nx},{ny},{nz},p={p},gamma={gamma},extent={extent})")
         if brick is not None:
             self._check(self.lib.dg_set_brick(self._h, *brick))
+        if variant is not None:
+            self._check(self.lib.dg_set_variant(self._h, int(variant)))
         self.workspace = None
         self.device = None
         self._torch = None

@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -81,16 +82,21 @@ void build_host_ops(int N, HostOps &o) {
     }
 }
 
-void build_device_ops(int N, DgOps &d) {
+// Device tables: the weak-form volume operator and the lift weights with the inverse (diagonal) mass and
+// the constant geometric factor g_a = 2/h_a of each axis folded in.
+void build_device_ops(int N, const double g[3], DgOps &d) {
     HostOps o;
     build_host_ops(N, o);
     std::memset(&d, 0, sizeof(d));
     for (int i = 0; i < N; ++i) {
         d.lp[i] = (double)o.lp[i];
         d.lm[i] = (double)o.lm[i];
-        d.lpw[i] = (double)(o.lp[i] / o.w[i]);
-        d.lmw[i] = (double)(o.lm[i] / o.w[i]);
-        for (int q = 0; q < N; ++q) d.Dhat[i * N + q] = (double)(o.w[q] * o.D[q][i] / o.w[i]);
+        for (int a = 0; a < 3; ++a) {
+            const long double ga = (long double)g[a];
+            d.lpg[a][i] = (double)(ga * o.lp[i] / o.w[i]);
+            d.lmg[a][i] = (double)(ga * o.lm[i] / o.w[i]);
+            for (int q = 0; q < N; ++q) d.Dg[a][q][i] = (double)(ga * o.w[q] * o.D[q][i] / o.w[i]);
+        }
     }
 }
 
@@ -133,6 +139,8 @@ struct dg_ctx {
     double *Q, *K, *S, *T[2];
     unsigned long long *scal;
     int tcur;           // T[tcur] holds the traces of the current Q
+    int grid;           // persistent stage kernel: resident blocks per SM x SMs, capped by the brick count
+    DgOps ops;          // device operator tables of this mesh (travel in the kernel arguments)
     bool bound, has_state;
     cudaStream_t stream;
     unsigned long long launches;
@@ -171,8 +179,8 @@ struct Carve {
 Carve carve(const dg_ctx *c) {
     Carve v;
     size_t off = 0;
-    v.q = off;    off += align_up(c->int_len * 8, 256);
-    v.k = off;    off += align_up(c->int_len * 8, 256);
+    v.q = off;    off += align_up(c->int_len * 8 + 16, 256);   // +16: the L2 prefetch rounds out to 16-byte granules
+    v.k = off;    off += align_up(c->int_len * 8 + 16, 256);
     v.s = off;    off += align_up(c->state_len * 8, 256);
     v.t0 = off;   off += align_up(c->trace_len * 8, 256);
     v.t1 = off;   off += align_up(c->trace_len * 8, 256);
@@ -191,12 +199,11 @@ DgStageArgs stage_args(const dg_ctx *c, int mode) {
     a.Tnew = c->T[1 - c->tcur];
     a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
     a.nbx = c->nbx; a.nby = c->nby; a.nbz = c->nbz;
-    a.g[0] = 2.0 / (c->extent[0] / c->nx);
-    a.g[1] = 2.0 / (c->extent[1] / c->ny);
-    a.g[2] = 2.0 / (c->extent[2] / c->nz);
     a.gamma = c->gamma;
     a.gm1 = c->gamma - 1.0;
     a.mode = mode;
+    a.grid = c->grid;
+    a.ops = c->ops;
     return a;
 }
 
@@ -246,7 +253,12 @@ int dg_create(dg_ctx **out, int nx, int ny, int nz, int p, double gamma, const d
     c->gamma = gamma;
     for (int a = 0; a < 3; ++a) c->extent[a] = extent[a];
     c->state_len = (size_t)nx * ny * nz * (size_t)(c->N * c->N * c->N) * DG_NV;
-    set_layout(c, &kt[0]);
+    int pick = 0;
+    if (const char *ev = std::getenv("DG_VARIANT")) {   // tuning knob: index into this p's compiled variants
+        const int v = std::atoi(ev);
+        if (v >= 0 && v < count) pick = v;
+    }
+    set_layout(c, &kt[pick]);
     *out = c;
     return DG_OK;
 }
@@ -266,6 +278,23 @@ int dg_set_brick(dg_ctx *c, int bx, int by, int bz) {
             return DG_OK;
         }
     return fail(c, DG_EUNSUPPORTED, "brick %dx%dx%d is not compiled for p=%d", bx, by, bz, c->p);
+}
+
+int dg_variant_count(int p) {
+    int count = 0;
+    if (p < 1 || p > 7) return 0;
+    variants_for(p + 1, &count);
+    return count;
+}
+
+int dg_set_variant(dg_ctx *c, int index) {
+    if (!c) return DG_EINVAL;
+    if (c->bound) return fail(c, DG_ESTATE, "dg_set_variant after dg_bind");
+    int count = 0;
+    const DgKernelTable *kt = variants_for(c->N, &count);
+    if (index < 0 || index >= count) return fail(c, DG_EINVAL, "variant %d outside 0..%d", index, count - 1);
+    set_layout(c, &kt[index]);
+    return DG_OK;
 }
 
 size_t dg_state_len(const dg_ctx *c) { return c ? c->state_len : 0; }
@@ -291,10 +320,16 @@ int dg_bind(dg_ctx *c, void *ws, size_t bytes, void *stream) {
     // bricks of a ragged mesh carry padding nodes that are staged but never used: give them a defined value
     cudaError_t e = cudaMemsetAsync(base, 0, v.total, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "workspace memset");
-    DgOps ops;
-    build_device_ops(c->N, ops);
-    e = c->kt->upload_ops(&ops, c->stream);
-    if (e != cudaSuccess) return cuda_fail(c, e, "operator upload");
+    const double g[3] = {2.0 / (c->extent[0] / c->nx), 2.0 / (c->extent[1] / c->ny), 2.0 / (c->extent[2] / c->nz)};
+    build_device_ops(c->N, g, c->ops);
+    int dev = 0, sms = 0, per_sm = 0;
+    e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = c->kt->prepare(&per_sm);
+    if (e != cudaSuccess) return cuda_fail(c, e, "stage kernel setup");
+    if (per_sm < 1 || sms < 1) return fail(c, DG_ECUDA, "stage kernel does not fit on an SM");
+    const size_t resident = (size_t)per_sm * (size_t)sms;
+    c->grid = (int)(c->nbricks < resident ? c->nbricks : resident);
     c->bound = true;
     c->err[0] = 0;
     return DG_OK;
@@ -398,7 +433,7 @@ int dg_kernel_info(const dg_ctx *c, long long out[8]) {
     out[0] = c->kt->bx; out[1] = c->kt->by; out[2] = c->kt->bz;
     out[3] = c->kt->threads;
     out[4] = c->kt->smem_bytes;
-    out[5] = (long long)c->nbricks;
+    out[5] = c->bound ? (long long)c->grid : (long long)c->nbricks;
     out[6] = (long long)((c->int_len + (1u << 20) - 1) >> 20);
     out[7] = c->kt->tslot;
     return DG_OK;

@@ -9,12 +9,14 @@
 #define DG_NMAX 8    // largest N = p+1 compiled
 
 // 1-D operators of the collocated Gauss-Legendre Lagrange basis, built on the
-// host in long double (dg_api.cu) and placed in __constant__ memory of each kernel TU so that
-// fully unrolled loops read them as immediate constant-bank operands of DFMA.
+// host in long double (dg_api.cu) with the constant geometric factor 2/h_a of each axis
+// folded in, rounded to double once.  They travel inside the kernel
+// arguments (constant bank; per context, so contexts with different meshes can coexist).
 struct DgOps {
-    double Dhat[DG_NMAX * DG_NMAX];  // Dhat[i*N+q] = w_q l_i'(xi_q) / w_i   (eq (5) 2nd term / mass)
-    double lp[DG_NMAX], lm[DG_NMAX]; // l_i(+1), l_i(-1)                     (face traces)
-    double lpw[DG_NMAX], lmw[DG_NMAX]; // l_i(+-1) / w_i                     (lift / mass)
+    double Dg[3][DG_NMAX][DG_NMAX];     // Dg[a][q][i] = (2/h_a) w_q l_i'(xi_q) / w_i   (eq (5) 2nd term / mass)
+    double lpg[3][DG_NMAX];             // (2/h_a) l_i(+1) / w_i                        (lift / mass)
+    double lmg[3][DG_NMAX];             // (2/h_a) l_i(-1) / w_i
+    double lp[DG_NMAX], lm[DG_NMAX];    // l_i(+1), l_i(-1)                             (face traces)
 };
 
 enum DgMode {
@@ -32,10 +34,11 @@ struct DgStageArgs {
     double *Tnew;         // ... of the updated Q (mode STAGE / TRACES)
     int nx, ny, nz;       // elements per axis
     int nbx, nby, nbz;    // bricks per axis
-    double g[3];          // 2/h_a: constant geometric factor per axis
     double gamma, gm1;
     double rkA, rkB, dt;  // stage coefficients; rkA == 0 means "do not read K" (stage 1)
     int mode;
+    int grid;             // blocks to launch (persistent: blocks stride over the bricks)
+    DgOps ops;
 };
 
 struct DgLayoutArgs {
@@ -59,7 +62,7 @@ struct DgKernelTable {
     int smem_bytes;          // dynamic shared memory of the stage kernel
     long long slot;          // doubles per brick in Q/K/R (5 * nodes per brick)
     long long tslot;         // face-trace doubles per brick
-    cudaError_t (*upload_ops)(const DgOps *ops, cudaStream_t s);
+    cudaError_t (*prepare)(int *blocks_per_sm);   // opt in to the shared memory size; resident blocks per SM
     cudaError_t (*launch_stage)(const DgStageArgs &a, cudaStream_t s);
     cudaError_t (*launch_layout)(const DgLayoutArgs &a, cudaStream_t s);
     cudaError_t (*launch_wavespeed)(const DgWaveArgs &a, cudaStream_t s);

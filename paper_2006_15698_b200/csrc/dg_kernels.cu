@@ -1,17 +1,18 @@
 // dg_kernels.cu -- CUDA kernels of the DG Euler time step for one N = p+1 (compile with -DDG_N=<N>,
 // -gencode arch=compute_100a,code=sm_100a).  Hand-written for B200; fp64 throughout.
 //
-// The fused stage kernel does, for one "brick" of BX x BY x BZ elements per thread block and in one
-// sweep over HBM:
-//   P0  asynchronous copies (cp.async, no registers): the brick's Q (5 x nodes) and the 6 neighbour
-//       bricks' face traces into shared memory
-//   then, one thread per node LINE, for the axes x, y, z in turn:
+// The fused stage kernel is PERSISTENT: each thread block strides over "bricks" of BX x BY x BZ elements
+// and, for every brick, in one sweep over HBM:
+//   P0  asynchronous copies (cp.async, no registers) of the NEXT brick's Q (5 x nodes) and of its 6
+//       neighbour bricks' face traces into the other half of a double buffer in shared memory, plus an
+//       L2 prefetch of its K, all of which land while the current brick is being computed
+//   then, one thread per node LINE, for the axes x, y, z in turn (one rolled loop, small code):
 //   PA  pointwise Euler flux (eq (2)-(3)) at the line's N nodes,
 //       V_i = sum_q Dhat_iq F_q in registers (eq (5) 2nd term, the contraction of
 //       listing lines 220-237), and the two face traces T+- = sum_q l_q(+-1) Q_q
 //   PB  local Lax-Friedrichs interface flux at the + end of the line, and at the - end of
 //       the lines that start on the brick boundary (neighbour traces come from the trace buffer)
-//   PC  lift and 2/h scaling: r_i = (2/h_a) (V_i - (l_i(+1) F*_+ - l_i(-1) F*_-)/w_i)  (eq (5) 3rd term),
+//   PC  lift with 2/h folded in: r_i = V_i - (l_i(+1) F*_+ - l_i(-1) F*_-) (2/h_a)/w_i  (eq (5) 3rd term),
 //       accumulated over the axes in shared memory
 //   PD  (with the z lines, whose global accesses coalesce) LSERK45 stage  K = A K + dt R, Q = Q + B K
 //       (PAPER.md:80, 254): K read and K, Q written straight from/to HBM; or R itself in residual mode
@@ -22,20 +23,20 @@
 // Nothing here is shared with oracle/ (separate source, separate operator construction).
 #include "dg_internal.h"
 
+#include <stdint.h>
+
 #ifndef DG_N
 #error "compile with -DDG_N=<p+1>"
 #endif
 
 namespace {
 
-__constant__ DgOps c_ops;
-
 // ------------------------------------------------------------------------------------------------
 // compile-time geometry of one variant
 // ------------------------------------------------------------------------------------------------
-template <int N_, int BX_, int BY_, int BZ_, int MINB_>
+template <int N_, int BX_, int BY_, int BZ_, int MINB_, int NBUF_>
 struct Cfg {
-    static constexpr int N = N_, BX = BX_, BY = BY_, BZ = BZ_, MINB = MINB_;
+    static constexpr int N = N_, BX = BX_, BY = BY_, BZ = BZ_, MINB = MINB_, NBUF = NBUF_;
     static constexpr int GX = BX * N, GY = BY * N, GZ = BZ * N;   // nodes of the brick per axis
     static constexpr int NODES = GX * GY * GZ;
     static constexpr int SLOT = DG_NV * NODES;                     // doubles per brick in Q, K, R
@@ -48,7 +49,7 @@ struct Cfg {
     static constexpr int TSLOT = 2 * DG_NV * (CX + CY + CZ);       // trace doubles per brick
     static constexpr bool MULTI = (BX > 1) || (BY > 1) || (BZ > 1);
     static constexpr int LINEBUF = MULTI ? DG_NV * L : 0;          // T- / F* hand-over between elements of a brick
-    static constexpr int SMEM_DOUBLES = 2 * DG_NV * PLANE + TSLOT + 2 * LINEBUF;
+    static constexpr int SMEM_DOUBLES = (NBUF + 1) * DG_NV * PLANE + TSLOT + 2 * LINEBUF;
     static constexpr int SMEM_BYTES = SMEM_DOUBLES * 8;
 };
 
@@ -56,164 +57,167 @@ __device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) 
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gsrc) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit_wait_all() {
-    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int PENDING>
+__device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;" ::"n"(PENDING) : "memory");
+}
+// Ask L2 to fetch [ptr, ptr + bytes) (rounded out to 16-byte granules): one instruction per brick of K.
+__device__ __forceinline__ void l2_prefetch(const void *ptr, unsigned bytes) {
+    const uintptr_t lo = (uintptr_t)ptr & ~(uintptr_t)15;
+    const uintptr_t hi = ((uintptr_t)ptr + bytes + 15) & ~(uintptr_t)15;
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(lo), "r"((unsigned)(hi - lo)) : "memory");
 }
 
-// Column AX of the Euler flux matrix, eq (2)-(3) (listing lines 186-217).
-// Same expression tree as DESIGN.md "arithmetic form".
-template <int AX>
-__device__ __forceinline__ void euler_flux(const double (&Q)[DG_NV], double gm1, double (&F)[DG_NV], double &vel,
-                                           double &pres, double &oneOrho) {
+// Euler flux along the face/line normal, eq (2)-(3) (listing lines 186-217), for a state
+// whose momentum components have been ROTATED so that slot 1 is the normal one:
+//   slots = (rho, rho u_a, rho u_b, rho u_c, rho E),  (a,b,c) = (x,y,z), (y,z,x) or (z,x,y).
+// One copy of the code then serves the three axes with no run-time selection.
+__device__ __forceinline__ void euler_flux_normal(const double (&Q)[DG_NV], double gm1, double (&F)[DG_NV],
+                                                  double &vel, double &pres, double &oneOrho) {
     oneOrho = 1.0 / Q[0];
-    const double u = Q[1] * oneOrho, v = Q[2] * oneOrho, w = Q[3] * oneOrho;
-    pres = gm1 * (Q[4] - 0.5 * Q[0] * (u * u + v * v + w * w));
-    const double Ep = Q[4] + pres;
-    vel = (AX == 0) ? u : (AX == 1) ? v : w;
+    vel = Q[1] * oneOrho;
+    const double ub = Q[2] * oneOrho, uc = Q[3] * oneOrho;
+    pres = gm1 * (Q[4] - 0.5 * Q[0] * (vel * vel + ub * ub + uc * uc));
     F[0] = Q[0] * vel;
-    F[1] = Q[1] * vel + ((AX == 0) ? pres : 0.0);
-    F[2] = Q[2] * vel + ((AX == 1) ? pres : 0.0);
-    F[3] = Q[3] * vel + ((AX == 2) ? pres : 0.0);
-    F[4] = Ep * vel;
+    F[1] = Q[1] * vel + pres;
+    F[2] = Q[2] * vel;
+    F[3] = Q[3] * vel;
+    F[4] = (Q[4] + pres) * vel;
 }
 
-// Local Lax-Friedrichs flux (reading R3):
+// Local Lax-Friedrichs flux (reading R3), rotated slots as above:
 //   F* = 1/2 (F(QL) + F(QR)) - 1/2 lam (QR - QL),  lam = max(|u_a^L| + c_L, |u_a^R| + c_R)
-template <int AX>
-__device__ __forceinline__ void lax_friedrichs(const double (&QL)[DG_NV], const double (&QR)[DG_NV], double gamma,
-                                               double gm1, double (&Fs)[DG_NV]) {
-    double FL[DG_NV], FR[DG_NV], uL, uR, pL, pR, rL, rR;
-    euler_flux<AX>(QL, gm1, FL, uL, pL, rL);
-    euler_flux<AX>(QR, gm1, FR, uR, pR, rR);
-    const double lamL = fabs(uL) + sqrt(gamma * pL * rL);
-    const double lamR = fabs(uR) + sqrt(gamma * pR * rR);
-    const double lam = (lamL > lamR) ? lamL : lamR;
+// written for (own, other) with sgn = +1 when own is the left state, -1 when it is the right one.
+__device__ __forceinline__ void lax_friedrichs(const double (&Qown)[DG_NV], const double (&Qoth)[DG_NV], double sgn,
+                                               double gamma, double gm1, double (&Fs)[DG_NV]) {
+    double Fa[DG_NV], Fb[DG_NV], ua, ub, pa, pb, ra, rb;
+    euler_flux_normal(Qown, gm1, Fa, ua, pa, ra);
+    euler_flux_normal(Qoth, gm1, Fb, ub, pb, rb);
+    const double lama = fabs(ua) + sqrt(gamma * pa * ra);
+    const double lamb = fabs(ub) + sqrt(gamma * pb * rb);
+    const double hl = 0.5 * sgn * ((lama > lamb) ? lama : lamb);
 #pragma unroll
-    for (int n = 0; n < DG_NV; ++n) Fs[n] = 0.5 * (FL[n] + FR[n]) - 0.5 * lam * (QR[n] - QL[n]);
+    for (int n = 0; n < DG_NV; ++n) Fs[n] = 0.5 * (Fa[n] + Fb[n]) - hl * (Qoth[n] - Qown[n]);
 }
 
 // ------------------------------------------------------------------------------------------------
-// geometry of one node line along axis AX inside the brick, for thread `l`
+// geometry of the node line of thread `l` along axis `ax` inside the brick
 //   l = e * Ca + c,  e = element along the axis, c = face node = t2 * T1 + t1
 //   axis x: (t1,t2) = (gy,gz);  y: (gx,gz);  z: (gx,gy)
 // ------------------------------------------------------------------------------------------------
-template <class C, int AX>
 struct Line {
-    static constexpr int Ca = (AX == 0) ? C::CX : (AX == 1) ? C::CY : C::CZ;
-    static constexpr int T1 = (AX == 0) ? C::GY : C::GX;
-    static constexpr int Ba = (AX == 0) ? C::BX : (AX == 1) ? C::BY : C::BZ;
-    static constexpr int STRIDE = (AX == 0) ? 1 : (AX == 1) ? C::P : C::GY * C::P;   // shared-memory node stride
-    static constexpr int TBASE = (AX == 0) ? 0 : (AX == 1) ? 2 * DG_NV * C::CX : 2 * DG_NV * (C::CX + C::CY);
-    int e, c, t1, t2, base, exta;
-    bool active;
-    __device__ __forceinline__ Line(int l, int nodx, int nody, int nodz, int ext0, int ext1, int ext2) {
-        e = (Ba == 1) ? 0 : l / Ca;
-        c = l - e * Ca;
-        t2 = c / T1;
-        t1 = c - t2 * T1;
-        if (AX == 0) {
-            base = (t2 * C::GY + t1) * C::P + e * C::N;
-            exta = ext0;
-            active = t1 < nody && t2 < nodz;
-        } else if (AX == 1) {
-            base = (t2 * C::GY + e * C::N) * C::P + t1;
-            exta = ext1;
-            active = t1 < nodx && t2 < nodz;
-        } else {
-            base = (e * C::N * C::GY + t2) * C::P + t1;
-            exta = ext2;
-            active = t1 < nodx && t2 < nody;
-        }
-        active = active && l < C::L && e < exta;
-    }
+    int e, c, base, stride, Ca, tbase, exta;
+    bool active, multi;
 };
 
-// PA..PC for one axis: returns r[n][i] = (2/h_a) (V - lift) of this thread's line.
-template <class C, int AX>
-__device__ __forceinline__ void axis_residual(const Line<C, AX> &ln, int l, const double *Qs, const double *Hs,
-                                              double *Tms, double *Fss, const DgStageArgs &a,
-                                              double (&V)[DG_NV][C::N]) {
-    constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE, L = C::L;
-    using LN = Line<C, AX>;
-    constexpr int Ca = LN::Ca, STRIDE = LN::STRIDE, Ba = LN::Ba;
-    double Tp[NV], Tm[NV];
-    // ------------- PA: flux, sum-factorised derivative, traces -------------------------------------
-    if (ln.active) {
+template <class C>
+__device__ __forceinline__ Line make_line(int ax, int l, int ext0, int ext1, int ext2) {
+    constexpr int N = C::N;
+    Line ln;
+    int t1, t2;
+    if (ax == 0) {
+        ln.Ca = C::CX;
+        ln.e = (C::BX == 1) ? 0 : l / C::CX;
+        ln.c = l - ln.e * C::CX;
+        t2 = ln.c / C::GY;
+        t1 = ln.c - t2 * C::GY;
+        ln.base = (t2 * C::GY + t1) * C::P + ln.e * N;
+        ln.stride = 1;
+        ln.tbase = 0;
+        ln.exta = ext0;
+        ln.multi = C::BX > 1;
+        ln.active = t1 < ext1 * N && t2 < ext2 * N;
+    } else if (ax == 1) {
+        ln.Ca = C::CY;
+        ln.e = (C::BY == 1) ? 0 : l / C::CY;
+        ln.c = l - ln.e * C::CY;
+        t2 = ln.c / C::GX;
+        t1 = ln.c - t2 * C::GX;
+        ln.base = (t2 * C::GY + ln.e * N) * C::P + t1;
+        ln.stride = C::P;
+        ln.tbase = 2 * DG_NV * C::CX;
+        ln.exta = ext1;
+        ln.multi = C::BY > 1;
+        ln.active = t1 < ext0 * N && t2 < ext2 * N;
+    } else {
+        ln.Ca = C::CZ;
+        ln.e = (C::BZ == 1) ? 0 : l / C::CZ;
+        ln.c = l - ln.e * C::CZ;
+        t2 = ln.c / C::GX;
+        t1 = ln.c - t2 * C::GX;
+        ln.base = (ln.e * N * C::GY + t2) * C::P + t1;
+        ln.stride = C::GY * C::P;
+        ln.tbase = 2 * DG_NV * (C::CX + C::CY);
+        ln.exta = ext2;
+        ln.multi = C::BZ > 1;
+        ln.active = t1 < ext0 * N && t2 < ext1 * N;
+    }
+    ln.active = ln.active && l < C::L && ln.e < ln.exta;
+    return ln;
+}
+
+// P0a: enqueue the asynchronous copy of one brick's Q, and ask L2 for its K and its neighbours' traces.
+template <class C>
+__device__ __forceinline__ void issue_q_loads(const DgStageArgs &a, int brick, double *Qd, int tid, bool want_k) {
+    constexpr int NV = DG_NV, GX = C::GX, P = C::P, THREADS = C::THREADS;
+    const double *src = a.Q + (size_t)brick * C::SLOT;
+    constexpr int TOTAL = NV * C::NODES;
+#pragma unroll 4
+    for (int idx = tid; idx < TOTAL; idx += THREADS) {
+        const int row = idx / GX;                         // row over all 5 variables: PLANE = ROWS * P
+        cp_async8(Qd + idx + row * (P - GX), src + idx);
+    }
+    if (want_k && tid == 0) l2_prefetch(a.K + (size_t)brick * C::SLOT, C::SLOT * 8);
+}
+
+// Neighbour brick and offset of the trace block a brick needs for (axis, side): side 0 = T+ of the brick
+// below (stored as that brick's side 1), side 1 = T- of the brick above (its side 0).
+template <class C>
+__device__ __forceinline__ const double *halo_source(const DgStageArgs &a, int bxi, int byi, int bzi, int ax, int side) {
+    const int Ca = (ax == 0) ? C::CX : (ax == 1) ? C::CY : C::CZ;
+    const int tbase = (ax == 0) ? 0 : (ax == 1) ? 2 * DG_NV * C::CX : 2 * DG_NV * (C::CX + C::CY);
+    int bx = bxi, by = byi, bz = bzi;   // (no run-time indexed local array: it would live in local memory)
+    if (ax == 0) bx = (side == 0) ? ((bx == 0) ? a.nbx - 1 : bx - 1) : ((bx + 1 == a.nbx) ? 0 : bx + 1);
+    else if (ax == 1) by = (side == 0) ? ((by == 0) ? a.nby - 1 : by - 1) : ((by + 1 == a.nby) ? 0 : by + 1);
+    else bz = (side == 0) ? ((bz == 0) ? a.nbz - 1 : bz - 1) : ((bz + 1 == a.nbz) ? 0 : bz + 1);
+    const size_t nbr = (size_t)bx + (size_t)a.nbx * ((size_t)by + (size_t)a.nby * bz);
+    return a.Told + nbr * C::TSLOT + tbase + (side == 0 ? DG_NV * Ca : 0);
+}
+
+// P0b: enqueue the asynchronous copies of the 6 neighbour trace blocks of this brick.
+template <class C>
+__device__ __forceinline__ void issue_halo_loads(const DgStageArgs &a, int bxi, int byi, int bzi, double *Hd, int tid) {
+    constexpr int NV = DG_NV, THREADS = C::THREADS;
 #pragma unroll
-        for (int n = 0; n < NV; ++n) {
-            Tp[n] = 0.0;
-            Tm[n] = 0.0;
-#pragma unroll
-            for (int i = 0; i < N; ++i) V[n][i] = 0.0;
-        }
-#pragma unroll
-        for (int q = 0; q < N; ++q) {
-            double Qn[NV], F[NV], vel, pres, rinv;
-#pragma unroll
-            for (int n = 0; n < NV; ++n) Qn[n] = Qs[n * PLANE + ln.base + q * STRIDE];
-            euler_flux<AX>(Qn, a.gm1, F, vel, pres, rinv);
-#pragma unroll
-            for (int n = 0; n < NV; ++n) {
-#pragma unroll
-                for (int i = 0; i < N; ++i) V[n][i] = fma(c_ops.Dhat[i * N + q], F[n], V[n][i]);
-                Tp[n] = fma(c_ops.lp[q], Qn[n], Tp[n]);
-                Tm[n] = fma(c_ops.lm[q], Qn[n], Tm[n]);
-            }
-        }
-        if (Ba > 1) {
-#pragma unroll
-            for (int n = 0; n < NV; ++n) Tms[n * L + l] = Tm[n];
+    for (int ax = 0; ax < 3; ++ax) {
+        const int Ca = (ax == 0) ? C::CX : (ax == 1) ? C::CY : C::CZ;
+        const int tbase = (ax == 0) ? 0 : (ax == 1) ? 2 * NV * C::CX : 2 * NV * (C::CX + C::CY);
+        const double *srcm = halo_source<C>(a, bxi, byi, bzi, ax, 0);
+        const double *srcp = halo_source<C>(a, bxi, byi, bzi, ax, 1);
+        for (int r = tid; r < NV * Ca; r += THREADS) {
+            cp_async8(Hd + tbase + r, srcm + r);
+            cp_async8(Hd + tbase + NV * Ca + r, srcp + r);
         }
     }
-    if (Ba > 1) __syncthreads();
+}
 
-    // ------------- PB: interface fluxes ------------------------------------------------------------
-    double Fp[NV], Fm[NV];
-    if (ln.active) {
-        double Qo[NV];
-        if (Ba > 1 && ln.e + 1 < ln.exta) {
-#pragma unroll
-            for (int n = 0; n < NV; ++n) Qo[n] = Tms[n * L + l + Ca];
-        } else {
-#pragma unroll
-            for (int n = 0; n < NV; ++n) Qo[n] = Hs[LN::TBASE + (NV + n) * Ca + ln.c];
-        }
-        lax_friedrichs<AX>(Tp, Qo, a.gamma, a.gm1, Fp);
-        if (Ba > 1) {
-#pragma unroll
-            for (int n = 0; n < NV; ++n) Fss[n * L + l] = Fp[n];
-        }
-        if (ln.e == 0) {
-#pragma unroll
-            for (int n = 0; n < NV; ++n) Qo[n] = Hs[LN::TBASE + n * Ca + ln.c];
-            lax_friedrichs<AX>(Qo, Tm, a.gamma, a.gm1, Fm);
-        }
-    }
-    if (Ba > 1) __syncthreads();
-
-    // ------------- PC: lift, scale -----------------------------------------------------------------
-    if (ln.active) {
-        if (Ba > 1 && ln.e > 0) {
-#pragma unroll
-            for (int n = 0; n < NV; ++n) Fm[n] = Fss[n * L + l - Ca];
-        }
-        const double g = a.g[AX];
-#pragma unroll
-        for (int n = 0; n < NV; ++n) {
-#pragma unroll
-            for (int i = 0; i < N; ++i) {
-                const double lift = c_ops.lpw[i] * Fp[n] - c_ops.lmw[i] * Fm[n];
-                V[n][i] = g * (V[n][i] - lift);
-            }
-        }
+// ... and the L2 prefetch of the same 6 blocks for the NEXT brick (6 threads, one instruction each).
+template <class C>
+__device__ __forceinline__ void prefetch_halo(const DgStageArgs &a, int brick, int tid) {
+    if (tid < 6) {
+        const int bxi = brick % a.nbx, byi = (brick / a.nbx) % a.nby, bzi = brick / (a.nbx * a.nby);
+        const int ax = tid >> 1, side = tid & 1;
+        const int Ca = (ax == 0) ? C::CX : (ax == 1) ? C::CY : C::CZ;
+        l2_prefetch(halo_source<C>(a, bxi, byi, bzi, ax, side), DG_NV * Ca * 8);
     }
 }
 
 // PE for one axis: traces of the (updated) Q in shared memory on the brick boundary -> Tnew.
-template <class C, int AX>
-__device__ __forceinline__ void boundary_traces(const Line<C, AX> &ln, const double *Qs, double *Tbrick) {
+template <class C>
+__device__ __forceinline__ void boundary_traces(const Line &ln, const double *Qs, double *Tbrick,
+                                                const DgStageArgs &a) {
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE;
-    using LN = Line<C, AX>;
     if (ln.active && (ln.e == 0 || ln.e == ln.exta - 1)) {
         double Tp[NV], Tm[NV];
 #pragma unroll
@@ -223,184 +227,281 @@ __device__ __forceinline__ void boundary_traces(const Line<C, AX> &ln, const dou
         }
 #pragma unroll
         for (int q = 0; q < N; ++q) {
+            const double lpq = a.ops.lp[q], lmq = a.ops.lm[q];
 #pragma unroll
             for (int n = 0; n < NV; ++n) {
-                const double Qv = Qs[n * PLANE + ln.base + q * LN::STRIDE];
-                Tp[n] = fma(c_ops.lp[q], Qv, Tp[n]);
-                Tm[n] = fma(c_ops.lm[q], Qv, Tm[n]);
+                const double Qv = Qs[n * PLANE + ln.base + q * ln.stride];
+                Tp[n] = fma(lpq, Qv, Tp[n]);
+                Tm[n] = fma(lmq, Qv, Tm[n]);
             }
         }
-        double *dst = Tbrick + LN::TBASE + ln.c;
+        double *dst = Tbrick + ln.tbase + ln.c;
         if (ln.e == 0) {
 #pragma unroll
-            for (int n = 0; n < NV; ++n) dst[n * LN::Ca] = Tm[n];
+            for (int n = 0; n < NV; ++n) dst[n * ln.Ca] = Tm[n];
         }
         if (ln.e == ln.exta - 1) {
 #pragma unroll
-            for (int n = 0; n < NV; ++n) dst[(NV + n) * LN::Ca] = Tp[n];
+            for (int n = 0; n < NV; ++n) dst[(NV + n) * ln.Ca] = Tp[n];
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// the fused stage kernel
+// the fused, persistent stage kernel
 // ------------------------------------------------------------------------------------------------
-template <class C>
+template <class C, int MODE>
 __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __grid_constant__ DgStageArgs a) {
-    constexpr int N = C::N, GX = C::GX, GY = C::GY, P = C::P;
-    constexpr int NODES = C::NODES, PLANE = C::PLANE, L = C::L, THREADS = C::THREADS;
-    constexpr int NV = DG_NV;
+    constexpr int N = C::N, GX = C::GX, GY = C::GY;
+    constexpr int NODES = C::NODES, PLANE = C::PLANE, L = C::L;
+    constexpr int NV = DG_NV, NBUF = C::NBUF;
+    constexpr int mode = MODE;   // one kernel per mode: the hot stage kernel carries no residual/trace-only code
 
     extern __shared__ __align__(16) double smem[];
-    double *Qs = smem;                  // [5][PLANE]  nodal values of the brick (old, then updated)
-    double *Rs = Qs + NV * PLANE;       // [5][PLANE]  x (+ y) contribution to R
-    double *Hs = Rs + NV * PLANE;       // [TSLOT]     neighbour bricks' traces, laid out like a brick's own slot:
-                                        //             [axis][side][5][Ca]; side 0 = T+ of the brick below,
-                                        //             side 1 = T- of the brick above
-    double *Tms = Hs + C::TSLOT;        // [5][L]      T- of every line (right state of the line below)
-    double *Fss = Tms + C::LINEBUF;     // [5][L]      F* at the + end of every line
+    double *Qbuf = smem;                       // [NBUF][5][PLANE] nodal values of a brick (old, then updated)
+    double *Rs = Qbuf + NBUF * NV * PLANE;     // [5][PLANE]       x (+ y) contribution to R
+    double *Hs = Rs + NV * PLANE;              // [TSLOT]          neighbour bricks' traces, laid out like a brick's
+                                               //                  own slot: [axis][side][5][Ca]; side 0 = T+ of the
+                                               //                  brick below, side 1 = T- of the brick above
+    double *Tms = Hs + C::TSLOT;               // [5][L]           T- of every line (right state of the line below)
+    double *Fss = Tms + C::LINEBUF;            // [5][L]           F* at the + end of every line
 
-    const int tid = threadIdx.x;
-    const long long brick = blockIdx.x;
-    const int bxi = (int)(brick % a.nbx);
-    const int byi = (int)((brick / a.nbx) % a.nby);
-    const int bzi = (int)(brick / ((long long)a.nbx * a.nby));
-    const int ext0 = min(C::BX, a.nx - bxi * C::BX);   // elements of this brick per axis (ragged last brick)
-    const int ext1 = min(C::BY, a.ny - byi * C::BY);
-    const int ext2 = min(C::BZ, a.nz - bzi * C::BZ);
-    const int nodx = ext0 * N, nody = ext1 * N, nodz = ext2 * N;
-    const size_t qbase = (size_t)brick * C::SLOT;
-    const int mode = a.mode;
+    const int tid = threadIdx.x, l = tid;
+    const int nbricks = a.nbx * a.nby * a.nbz;
+    const bool readK = (mode == DG_MODE_STAGE) && (a.rkA != 0.0);
+    constexpr bool want_halo = (mode != DG_MODE_TRACES);
 
-    // ---------------- P0: asynchronous staging of Q and of the neighbour traces ----------------------
-    {
-        const double *src = a.Q + qbase;
-        constexpr int TOTAL = NV * NODES;
-#pragma unroll 4
-        for (int idx = tid; idx < TOTAL; idx += THREADS) {
-            const int row = idx / GX;                         // row over all 5 variables: PLANE = ROWS * P
-            cp_async8(Qs + idx + row * (P - GX), src + idx);
-        }
+    int brick = blockIdx.x;
+    int buf = 0;
+    if (NBUF == 2) {
+        if (brick < nbricks) issue_q_loads<C>(a, brick, Qbuf, tid, readK);
+        cp_async_commit();
     }
-    if (mode != DG_MODE_TRACES) {
-#pragma unroll
-        for (int ax = 0; ax < 3; ++ax) {
-            const int Ca = (ax == 0) ? C::CX : (ax == 1) ? C::CY : C::CZ;
-            const int tbase = (ax == 0) ? 0 : (ax == 1) ? 2 * NV * C::CX : 2 * NV * (C::CX + C::CY);
-            int bm[3] = {bxi, byi, bzi}, bp[3] = {bxi, byi, bzi};
-            const int nb = (ax == 0) ? a.nbx : (ax == 1) ? a.nby : a.nbz;
-            bm[ax] = (bm[ax] == 0) ? nb - 1 : bm[ax] - 1;
-            bp[ax] = (bp[ax] + 1 == nb) ? 0 : bp[ax] + 1;
-            const size_t brm = (size_t)bm[0] + (size_t)a.nbx * ((size_t)bm[1] + (size_t)a.nby * bm[2]);
-            const size_t brp = (size_t)bp[0] + (size_t)a.nbx * ((size_t)bp[1] + (size_t)a.nby * bp[2]);
-            const double *srcm = a.Told + brm * C::TSLOT + tbase + NV * Ca;   // T+ (side 1) of the brick below
-            const double *srcp = a.Told + brp * C::TSLOT + tbase;             // T- (side 0) of the brick above
-            for (int r = tid; r < NV * Ca; r += THREADS) {
-                cp_async8(Hs + tbase + r, srcm + r);
-                cp_async8(Hs + tbase + NV * Ca + r, srcp + r);
+    for (; brick < nbricks; brick += gridDim.x) {
+        const int bxi = brick % a.nbx, byi = (brick / a.nbx) % a.nby, bzi = brick / (a.nbx * a.nby);
+        // ---------------- P0: this brick's neighbour traces and the next brick's Q go out ---------------
+        double *Qs;
+        if (NBUF == 2) {
+            if (want_halo) issue_halo_loads<C>(a, bxi, byi, bzi, Hs, tid);
+            cp_async_commit();
+            const int next = brick + gridDim.x;
+            if (next < nbricks) {
+                issue_q_loads<C>(a, next, Qbuf + (buf ^ 1) * NV * PLANE, tid, readK);
+                if (want_halo) prefetch_halo<C>(a, next, tid);
             }
-        }
-    }
-    cp_async_commit_wait_all();
-    __syncthreads();
-
-    const int l = tid;
-    const Line<C, 2> lz(l, nodx, nody, nodz, ext0, ext1, ext2);
-    double *Tbrick = a.Tnew + (size_t)brick * C::TSLOT;
-
-    if (mode != DG_MODE_TRACES) {
-        double V[NV][N];
-        // ---------------- x lines --------------------------------------------------------------------
-        {
-            const Line<C, 0> lx(l, nodx, nody, nodz, ext0, ext1, ext2);
-            axis_residual<C, 0>(lx, l, Qs, Hs, Tms, Fss, a, V);
-            if (lx.active) {
-#pragma unroll
-                for (int n = 0; n < NV; ++n)
-#pragma unroll
-                    for (int i = 0; i < N; ++i) Rs[n * PLANE + lx.base + i] = V[n][i];
-            }
+            cp_async_commit();
+            cp_async_wait<2>();                    // this brick's Q (asked for one brick ago) has landed
+            Qs = Qbuf + buf * NV * PLANE;
+            buf ^= 1;
+        } else {
+            issue_q_loads<C>(a, brick, Qbuf, tid, readK);
+            cp_async_commit();
+            if (want_halo) issue_halo_loads<C>(a, bxi, byi, bzi, Hs, tid);
+            cp_async_commit();
+            cp_async_wait<1>();
+            Qs = Qbuf;
         }
         __syncthreads();
-        // ---------------- y lines --------------------------------------------------------------------
-        {
-            const Line<C, 1> ly(l, nodx, nody, nodz, ext0, ext1, ext2);
-            axis_residual<C, 1>(ly, l, Qs, Hs, Tms, Fss, a, V);
-            if (ly.active) {
-#pragma unroll
-                for (int n = 0; n < NV; ++n)
-#pragma unroll
-                    for (int i = 0; i < N; ++i) {
-                        const int sa = n * PLANE + ly.base + i * P;
-                        Rs[sa] = Rs[sa] + V[n][i];
-                    }
-            }
-        }
-        __syncthreads();
-        // ---------------- z lines: residual, Runge-Kutta stage, write back ---------------------------
-        constexpr int ZS = Line<C, 2>::STRIDE;
-        const size_t g0 = qbase + (size_t)(lz.e * N) * (GY * GX) + lz.c;   // node q=0 of this z-line, n=0
-        const bool readK = (mode == DG_MODE_STAGE) && (a.rkA != 0.0);
-        double Kold[NV][N];
-        if (lz.active && readK) {   // issued before the z contraction: the loads land while it runs
-#pragma unroll
-            for (int n = 0; n < NV; ++n)
-#pragma unroll
-                for (int q = 0; q < N; ++q) Kold[n][q] = __ldcs(a.K + g0 + (size_t)n * NODES + (size_t)q * (GY * GX));
-        }
-        axis_residual<C, 2>(lz, l, Qs, Hs, Tms, Fss, a, V);
-        if (lz.active) {
-            if (mode == DG_MODE_RESIDUAL) {
-#pragma unroll
-                for (int n = 0; n < NV; ++n)
-#pragma unroll
-                    for (int q = 0; q < N; ++q)
-                        a.Rout[g0 + (size_t)n * NODES + (size_t)q * (GY * GX)] = Rs[n * PLANE + lz.base + q * ZS] + V[n][q];
-            } else {
-                const double A = a.rkA, B = a.rkB, dt = a.dt;
+
+        const int ext0 = min(C::BX, a.nx - bxi * C::BX);   // elements of this brick per axis (ragged last brick)
+        const int ext1 = min(C::BY, a.ny - byi * C::BY);
+        const int ext2 = min(C::BZ, a.nz - bzi * C::BZ);
+        const size_t qbase = (size_t)brick * C::SLOT;
+        double *Tbrick = a.Tnew + (size_t)brick * C::TSLOT;
+
+        if (mode != DG_MODE_TRACES) {
+            double V[NV][N];
+#pragma unroll 1
+            for (int ax = 0; ax < 3; ++ax) {
+                const Line ln = make_line<C>(ax, l, ext0, ext1, ext2);
+                // momentum slots rotated so that slot 1 is the component along this axis
+                const int m1 = 1 + ax, m2 = (ax == 2) ? 1 : 2 + ax, m3 = (ax == 0) ? 3 : ax;
+                const int po1 = m1 * PLANE, po2 = m2 * PLANE, po3 = m3 * PLANE;
                 double Tp[NV], Tm[NV];
+                // ------------- PA: flux, sum-factorised derivative, traces ---------------------------
+                if (ln.active) {
 #pragma unroll
-                for (int n = 0; n < NV; ++n) {
-                    Tp[n] = 0.0;
-                    Tm[n] = 0.0;
+                    for (int n = 0; n < NV; ++n) {
+                        Tp[n] = 0.0;
+                        Tm[n] = 0.0;
+#pragma unroll
+                        for (int i = 0; i < N; ++i) V[n][i] = 0.0;
+                    }
+                    const double *Q0p = Qs + ln.base;
 #pragma unroll
                     for (int q = 0; q < N; ++q) {
-                        const int sa = n * PLANE + lz.base + q * ZS;
-                        const size_t go = g0 + (size_t)n * NODES + (size_t)q * (GY * GX);
-                        const double R = Rs[sa] + V[n][q];
-                        const double Kn = readK ? fma(A, Kold[n][q], dt * R) : dt * R;
-                        const double Qn = fma(B, Kn, Qs[sa]);
-                        a.K[go] = Kn;
-                        a.Q[go] = Qn;
-                        Qs[sa] = Qn;
-                        Tp[n] = fma(c_ops.lp[q], Qn, Tp[n]);
-                        Tm[n] = fma(c_ops.lm[q], Qn, Tm[n]);
+                        double Qn[NV], F[NV], vel, pres, rinv;
+                        const double *Qq = Q0p + q * ln.stride;
+                        Qn[0] = Qq[0];
+                        Qn[1] = Qq[po1];
+                        Qn[2] = Qq[po2];
+                        Qn[3] = Qq[po3];
+                        Qn[4] = Qq[4 * PLANE];
+                        euler_flux_normal(Qn, a.gm1, F, vel, pres, rinv);
+                        const double *Dq = a.ops.Dg[ax][q];
+                        const double lpq = a.ops.lp[q], lmq = a.ops.lm[q];
+#pragma unroll
+                        for (int n = 0; n < NV; ++n) {
+#pragma unroll
+                            for (int i = 0; i < N; ++i) V[n][i] = fma(Dq[i], F[n], V[n][i]);
+                            Tp[n] = fma(lpq, Qn[n], Tp[n]);
+                            Tm[n] = fma(lmq, Qn[n], Tm[n]);
+                        }
+                    }
+                    if (ln.multi) {
+#pragma unroll
+                        for (int n = 0; n < NV; ++n) Tms[n * L + l] = Tm[n];
                     }
                 }
-                // z traces of the updated Q straight from registers
-                double *dst = Tbrick + Line<C, 2>::TBASE + lz.c;
-                if (lz.e == 0) {
-#pragma unroll
-                    for (int n = 0; n < NV; ++n) dst[n * C::CZ] = Tm[n];
+                if (ax == 0) {
+                    cp_async_wait<(NBUF == 2) ? 1 : 0>();   // the neighbour traces have landed
+                    __syncthreads();
+                } else if (ln.multi) {
+                    __syncthreads();
                 }
-                if (lz.e == lz.exta - 1) {
+
+                // ------------- PB: interface fluxes ----------------------------------------------------
+                double Fp[NV], Fm[NV];
+                if (ln.active) {
+                    double Qown[NV];
 #pragma unroll
-                    for (int n = 0; n < NV; ++n) dst[(NV + n) * C::CZ] = Tp[n];
+                    for (int n = 0; n < NV; ++n) Qown[n] = Tp[n];
+#pragma unroll 1
+                    for (int s = 0; s < 2; ++s) {
+                        // s = 0: + face (own state is the left one); s = 1: - face, only for the lines that
+                        // start on the brick boundary (own state is the right one)
+                        double Qo[NV], Fs[NV];
+                        const double *src;
+                        int sstride;
+                        if (s == 0 && ln.multi && ln.e + 1 < ln.exta) {
+                            src = Tms + l + ln.Ca;        // T- of the next element of this brick (rotated slots)
+                            sstride = L;
+                            Qo[1] = src[1 * sstride];
+                            Qo[2] = src[2 * sstride];
+                            Qo[3] = src[3 * sstride];
+                        } else {
+                            src = Hs + ln.tbase + ((s == 0) ? NV * ln.Ca : 0) + ln.c;
+                            sstride = ln.Ca;
+                            Qo[1] = src[m1 * sstride];
+                            Qo[2] = src[m2 * sstride];
+                            Qo[3] = src[m3 * sstride];
+                        }
+                        Qo[0] = src[0];
+                        Qo[4] = src[4 * sstride];
+                        lax_friedrichs(Qown, Qo, (s == 0) ? 1.0 : -1.0, a.gamma, a.gm1, Fs);
+                        if (s == 0) {
+#pragma unroll
+                            for (int n = 0; n < NV; ++n) {
+                                Fp[n] = Fs[n];
+                                Qown[n] = Tm[n];
+                            }
+                            if (ln.e != 0) break;
+                        } else {
+#pragma unroll
+                            for (int n = 0; n < NV; ++n) Fm[n] = Fs[n];
+                        }
+                    }
+                    if (ln.multi) {
+#pragma unroll
+                        for (int n = 0; n < NV; ++n) Fss[n * L + l] = Fp[n];
+                    }
                 }
+                if (ln.multi) __syncthreads();
+
+                // ------------- PC: lift (2/h and 1/w folded into the tables) ---------------------------
+                if (ln.active) {
+                    if (ln.multi && ln.e > 0) {
+#pragma unroll
+                        for (int n = 0; n < NV; ++n) Fm[n] = Fss[n * L + l - ln.Ca];
+                    }
+                    // K of this z line: asked for now (an L2 hit: prefetched a brick ago), used after the lift
+                    const size_t g0 = qbase + (size_t)(ln.e * N) * (GY * GX) + ln.c;   // node q=0 of a z-line, n=0
+                    double Kold[NV][N];
+                    if (ax == 2 && readK) {
+#pragma unroll
+                        for (int n = 0; n < NV; ++n)
+#pragma unroll
+                            for (int q = 0; q < N; ++q)
+                                Kold[n][q] = __ldcs(a.K + g0 + (size_t)n * NODES + (size_t)q * (GY * GX));
+                    }
+                    const double *lpg = a.ops.lpg[ax], *lmg = a.ops.lmg[ax];
+#pragma unroll
+                    for (int i = 0; i < N; ++i) {
+                        const double cp = lpg[i], cm = lmg[i];
+#pragma unroll
+                        for (int n = 0; n < NV; ++n) V[n][i] = fma(cm, Fm[n], fma(-cp, Fp[n], V[n][i]));
+                    }
+                    if (ax < 2) {
+                        // x: R = r_x;  y: R += r_y   (slot s holds variable 0, m1, m2, m3, 4)
+                        double *R0p = Rs + ln.base;
+#pragma unroll
+                        for (int i = 0; i < N; ++i) {
+                            double *Rq = R0p + i * ln.stride;
+                            if (ax == 0) {
+                                Rq[0] = V[0][i];
+                                Rq[po1] = V[1][i];
+                                Rq[po2] = V[2][i];
+                                Rq[po3] = V[3][i];
+                                Rq[4 * PLANE] = V[4][i];
+                            } else {
+                                Rq[0] += V[0][i];
+                                Rq[po1] += V[1][i];
+                                Rq[po2] += V[2][i];
+                                Rq[po3] += V[3][i];
+                                Rq[4 * PLANE] += V[4][i];
+                            }
+                        }
+                    } else {
+                        // z: slots (0,1,2,3,4) hold variables (0,3,1,2,4)
+                        constexpr int var_of_slot[NV] = {0, 3, 1, 2, 4};
+                        if (mode == DG_MODE_RESIDUAL) {
+#pragma unroll
+                            for (int s = 0; s < NV; ++s)
+#pragma unroll
+                                for (int q = 0; q < N; ++q) {
+                                    const int n = var_of_slot[s];
+                                    a.Rout[g0 + (size_t)n * NODES + (size_t)q * (GY * GX)] =
+                                        Rs[n * PLANE + ln.base + q * ln.stride] + V[s][q];
+                                }
+                        } else {
+                            // ------------- PD: LSERK45 stage, write back, z traces of the updated Q -----
+                            const double A = a.rkA, B = a.rkB, dt = a.dt;
+                            double *dst = Tbrick + ln.tbase + ln.c;
+#pragma unroll
+                            for (int s = 0; s < NV; ++s) {
+                                const int n = var_of_slot[s];
+                                double tp = 0.0, tm = 0.0;
+#pragma unroll
+                                for (int q = 0; q < N; ++q) {
+                                    const int sa = n * PLANE + ln.base + q * ln.stride;
+                                    const size_t go = g0 + (size_t)n * NODES + (size_t)q * (GY * GX);
+                                    const double R = Rs[sa] + V[s][q];
+                                    const double Kn = readK ? fma(A, Kold[n][q], dt * R) : dt * R;
+                                    const double Qn = fma(B, Kn, Qs[sa]);
+                                    a.K[go] = Kn;
+                                    a.Q[go] = Qn;
+                                    Qs[sa] = Qn;
+                                    tp = fma(a.ops.lp[q], Qn, tp);
+                                    tm = fma(a.ops.lm[q], Qn, tm);
+                                }
+                                if (ln.e == 0) dst[n * C::CZ] = tm;
+                                if (ln.e == ln.exta - 1) dst[(NV + n) * C::CZ] = tp;
+                            }
+                        }
+                    }
+                }
+                if (ax < 2) __syncthreads();
             }
         }
-        if (mode == DG_MODE_RESIDUAL) return;
-        __syncthreads();
-    } else {
-        boundary_traces<C, 2>(lz, Qs, Tbrick);
-    }
 
-    // ---------------- PE: x and y traces of the updated Q on the brick boundary -----------------------
-    {
-        const Line<C, 0> lx(l, nodx, nody, nodz, ext0, ext1, ext2);
-        boundary_traces<C, 0>(lx, Qs, Tbrick);
-        const Line<C, 1> ly(l, nodx, nody, nodz, ext0, ext1, ext2);
-        boundary_traces<C, 1>(ly, Qs, Tbrick);
+        // ---------------- PE: traces of the updated Q on the brick boundary (z came from registers) ----
+        if (mode != DG_MODE_RESIDUAL) {
+            if (mode == DG_MODE_STAGE) __syncthreads();
+            const int nax = (mode == DG_MODE_TRACES) ? 3 : 2;
+#pragma unroll 1
+            for (int ax = 0; ax < nax; ++ax) boundary_traces<C>(make_line<C>(ax, l, ext0, ext1, ext2), Qs, Tbrick, a);
+        }
+        __syncthreads();   // everyone is done with this brick's buffers before they are refilled
     }
 }
 
@@ -473,19 +574,29 @@ __global__ void __launch_bounds__(256) dg_wavespeed_kernel(const DgWaveArgs a) {
 // host-side launchers, one table per variant
 // ------------------------------------------------------------------------------------------------
 template <class C>
-cudaError_t upload_ops(const DgOps *ops, cudaStream_t s) {
-    cudaError_t err = cudaMemcpyToSymbolAsync(c_ops, ops, sizeof(DgOps), 0, cudaMemcpyHostToDevice, s);
+cudaError_t prepare(int *blocks_per_sm) {
+    cudaError_t err = cudaFuncSetAttribute(dg_stage_kernel<C, DG_MODE_STAGE>,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    if (err == cudaSuccess)
+        err = cudaFuncSetAttribute(dg_stage_kernel<C, DG_MODE_RESIDUAL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   C::SMEM_BYTES);
+    if (err == cudaSuccess)
+        err = cudaFuncSetAttribute(dg_stage_kernel<C, DG_MODE_TRACES>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   C::SMEM_BYTES);
     if (err != cudaSuccess) return err;
-    err = cudaStreamSynchronize(s);   // ops lives on the caller's stack
-    if (err != cudaSuccess) return err;
-    return cudaFuncSetAttribute(dg_stage_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, dg_stage_kernel<C, DG_MODE_STAGE>,
+                                                         C::THREADS, C::SMEM_BYTES);
 }
 
 template <class C>
 cudaError_t launch_stage(const DgStageArgs &a, cudaStream_t s) {
-    const long long bricks = (long long)a.nbx * a.nby * a.nbz;
-    if (bricks <= 0 || bricks > 2147483647LL) return cudaErrorInvalidConfiguration;
-    dg_stage_kernel<C><<<(unsigned)bricks, C::THREADS, C::SMEM_BYTES, s>>>(a);
+    if (a.grid <= 0) return cudaErrorInvalidConfiguration;
+    if (a.mode == DG_MODE_STAGE)
+        dg_stage_kernel<C, DG_MODE_STAGE><<<(unsigned)a.grid, C::THREADS, C::SMEM_BYTES, s>>>(a);
+    else if (a.mode == DG_MODE_RESIDUAL)
+        dg_stage_kernel<C, DG_MODE_RESIDUAL><<<(unsigned)a.grid, C::THREADS, C::SMEM_BYTES, s>>>(a);
+    else
+        dg_stage_kernel<C, DG_MODE_TRACES><<<(unsigned)a.grid, C::THREADS, C::SMEM_BYTES, s>>>(a);
     return cudaGetLastError();
 }
 
@@ -513,46 +624,51 @@ template <class C>
 constexpr DgKernelTable make_table() {
     return DgKernelTable{C::N,       C::BX,          C::BY,           C::BZ,
                          C::THREADS, C::SMEM_BYTES,  C::SLOT,         C::TSLOT,
-                         &upload_ops<C>, &launch_stage<C>, &launch_layout<C>, &launch_wavespeed<C>};
+                         &prepare<C>, &launch_stage<C>, &launch_layout<C>, &launch_wavespeed<C>};
 }
 
-// Brick shapes per N (default first).  DESIGN.md "brick shapes" explains the choice: about 350-650 nodes
-// per brick keeps Q + R + halo under ~70 KB of shared memory (3+ blocks per SM overlap each other's load,
-// compute and store phases) while the brick-boundary trace traffic 160/(B_a N) bytes per node and axis
-// stays at 53-69 B per node.
+// Brick shapes per N (default first): Cfg<N, BX, BY, BZ, min blocks per SM, Q buffers>.
+// DESIGN.md "brick shapes" explains the choice.
 #if DG_N == 2
-using V0 = Cfg<2, 4, 4, 4, 3>;
-using V1 = Cfg<2, 2, 2, 2, 4>;
-using V2 = Cfg<2, 4, 4, 2, 4>;
+using V0 = Cfg<2, 4, 4, 4, 2, 2>;
+using V1 = Cfg<2, 4, 4, 4, 3, 1>;
+using V2 = Cfg<2, 4, 4, 2, 4, 2>;
+using V3 = Cfg<2, 2, 2, 2, 4, 1>;
 #elif DG_N == 3
-using V0 = Cfg<3, 3, 3, 2, 3>;
-using V1 = Cfg<3, 1, 1, 1, 8>;
-using V2 = Cfg<3, 2, 2, 2, 4>;
+using V0 = Cfg<3, 4, 4, 2, 2, 2>;
+using V1 = Cfg<3, 4, 4, 2, 2, 1>;
+using V2 = Cfg<3, 2, 2, 2, 4, 2>;
+using V3 = Cfg<3, 1, 1, 1, 8, 1>;
 #elif DG_N == 4
-using V0 = Cfg<4, 2, 2, 2, 3>;
-using V1 = Cfg<4, 1, 1, 1, 8>;
-using V2 = Cfg<4, 2, 2, 1, 4>;
+using V0 = Cfg<4, 2, 2, 2, 2, 2>;
+using V1 = Cfg<4, 2, 2, 2, 3, 1>;
+using V2 = Cfg<4, 2, 2, 1, 4, 2>;
+using V3 = Cfg<4, 1, 1, 1, 8, 1>;
 #elif DG_N == 5
-using V0 = Cfg<5, 1, 2, 2, 3>;
-using V1 = Cfg<5, 1, 1, 1, 8>;
-using V2 = Cfg<5, 2, 2, 1, 3>;
+using V0 = Cfg<5, 1, 2, 2, 2, 2>;
+using V1 = Cfg<5, 1, 2, 2, 3, 1>;
+using V2 = Cfg<5, 2, 2, 2, 1, 2>;
+using V3 = Cfg<5, 1, 1, 1, 6, 2>;
 #elif DG_N == 6
-using V0 = Cfg<6, 1, 1, 2, 4>;
-using V1 = Cfg<6, 1, 1, 1, 6>;
-using V2 = Cfg<6, 2, 2, 1, 2>;
+using V0 = Cfg<6, 1, 2, 2, 1, 2>;
+using V1 = Cfg<6, 1, 2, 2, 1, 1>;
+using V2 = Cfg<6, 1, 1, 2, 2, 2>;
+using V3 = Cfg<6, 1, 1, 1, 5, 2>;
 #elif DG_N == 7
-using V0 = Cfg<7, 1, 1, 1, 5>;
-using V1 = Cfg<7, 2, 1, 1, 3>;
-using V2 = Cfg<7, 1, 1, 2, 3>;
+using V0 = Cfg<7, 1, 1, 2, 2, 2>;
+using V1 = Cfg<7, 1, 1, 2, 2, 1>;
+using V2 = Cfg<7, 1, 2, 2, 1, 2>;
+using V3 = Cfg<7, 1, 1, 1, 4, 2>;
 #elif DG_N == 8
-using V0 = Cfg<8, 1, 1, 1, 4>;
-using V1 = Cfg<8, 2, 1, 1, 2>;
-using V2 = Cfg<8, 1, 1, 2, 2>;
+using V0 = Cfg<8, 1, 1, 2, 1, 2>;
+using V1 = Cfg<8, 1, 1, 2, 2, 1>;
+using V2 = Cfg<8, 1, 1, 1, 3, 2>;
+using V3 = Cfg<8, 1, 1, 1, 4, 1>;
 #else
 #error "DG_N must be 2..8"
 #endif
 
-const DgKernelTable k_tables[] = {make_table<V0>(), make_table<V1>(), make_table<V2>()};
+const DgKernelTable k_tables[] = {make_table<V0>(), make_table<V1>(), make_table<V2>(), make_table<V3>()};
 
 }  // namespace
 

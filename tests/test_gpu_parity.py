@@ -25,9 +25,12 @@ TOL_RK100 = 1e-9
 ORC = Oracle("omp")
 ARB = Oracle("ld_omp")
 
-VARIANTS = {1: [(4, 4, 4), (2, 2, 2), (4, 4, 2)], 2: [(3, 3, 2), (1, 1, 1), (2, 2, 2)], 3: [(2, 2, 2), (1, 1, 1), (2, 2, 1)],
-            4: [(1, 2, 2), (1, 1, 1), (2, 2, 1)], 5: [(1, 1, 2), (1, 1, 1), (2, 2, 1)], 6: [(1, 1, 1), (2, 1, 1), (1, 1, 2)],
-            7: [(1, 1, 1), (2, 1, 1), (1, 1, 2)]}
+
+
+def variants(p):
+    """Every stage-kernel variant compiled for degree p (brick shape x buffering), default first."""
+    from paper_2006_15698_b200 import load_library
+    return list(range(load_library().dg_variant_count(p)))
 
 
 def relerr(a, b):
@@ -57,8 +60,8 @@ def test_library_is_the_cuda_one_and_fails_loudly_without_state():
 def test_layout_roundtrip_and_wavespeed_all_variants(p):
     nx, ny, nz, ext = 5, 3, 2, (1.0, 0.6, 0.4)                # ragged against every brick shape
     q = rough_field(nx, ny, nz, p, ext)
-    for brick in [None] + VARIANTS[p]:
-        dg = DG(nx, ny, nz, p, G, ext, brick=brick)
+    for brick in variants(p):
+        dg = DG(nx, ny, nz, p, G, ext, variant=brick)
         dg.set_state(q)
         assert np.array_equal(dg.get_state(), q)
         qd = torch.empty(q.shape, dtype=torch.float64, device="cuda")
@@ -74,13 +77,21 @@ def test_residual_parity_ragged_mesh_all_variants(p):
     nx, ny, nz, ext = 5, 3, 2, (1.0, 0.6, 0.4)
     q = rough_field(nx, ny, nz, p, ext)
     r_orc = ORC.residual(q, p, G, ext)
-    for brick in [None] + VARIANTS[p]:
-        dg = DG(nx, ny, nz, p, G, ext, brick=brick)
+    for brick in variants(p):
+        dg = DG(nx, ny, nz, p, G, ext, variant=brick)
         r = dg.set_state(q).residual()
         assert relerr(r, r_orc) < TOL_RES, (p, brick, relerr(r, r_orc))      # strict: no cancellation here
         assert np.array_equal(dg.get_state(), q)              # residual leaves the state alone
         r2 = dg.residual(torch.empty(q.shape, dtype=torch.float64, device="cuda")).cpu().numpy()
         assert np.array_equal(r2, r)                          # device output == host output, repeatable
+        dg.close()
+    # three full LSERK45 steps through every variant (stage mode: K, both trace buffers, ragged bricks)
+    dt = I.cfl_dt(ORC.max_wavespeed(q, p, G), p, ext, (nx, ny, nz), 0.1)
+    q_orc = ORC.rk_step(q, p, G, ext, dt, 3)
+    for brick in variants(p):
+        dg = DG(nx, ny, nz, p, G, ext, variant=brick)
+        q3 = dg.set_state(q).rk_step(dt, 3).get_state()
+        assert relerr(q3, q_orc) < 1e-12, (p, brick, relerr(q3, q_orc))
         dg.close()
 
 
