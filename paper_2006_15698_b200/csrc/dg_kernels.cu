@@ -1,21 +1,23 @@
 // dg_kernels.cu -- CUDA kernels of the DG Euler time step for one N = p+1 (compile with -DDG_N=<N>,
 // -gencode arch=compute_100a,code=sm_100a).  Hand-written for B200; fp64 throughout.
 //
-// The fused stage kernel is PERSISTENT: each thread block strides over "bricks" of BX x BY x BZ elements
-// and, for every brick, in one sweep over HBM:
-//   P0  asynchronous copies (cp.async, no registers) of the NEXT brick's Q (5 x nodes) and of its 6
-//       neighbour bricks' face traces into the other half of a double buffer in shared memory, plus an
-//       L2 prefetch of its K, all of which land while the current brick is being computed
-//   then, one thread per node LINE, for the axes x, y, z in turn (one rolled loop, small code):
+// The fused stage kernel (v4) is PERSISTENT: a thread block strides over "bricks" of BX x BY x BZ elements.
+// The geometry of a thread's three node lines (one per axis) does not depend on the brick, so it is computed
+// once per kernel; every shared-memory stride below is a compile-time constant.  Per brick, in ONE sweep
+// over HBM:
+//   P0  cp.async (no registers) of the brick's Q and K (5 x nodes each) into shared memory; one L2 prefetch
+//       instruction each for the NEXT brick's Q, K and 6 neighbour trace blocks
+//   then, one thread per node LINE, for the axes x, y, z in turn (three instances of one template):
+//   PH  the neighbour bricks' face traces this line touches go straight from HBM/L2 into registers
 //   PA  pointwise Euler flux (eq (2)-(3)) at the line's N nodes,
 //       V_i = sum_q Dhat_iq F_q in registers (eq (5) 2nd term, the contraction of
 //       listing lines 220-237), and the two face traces T+- = sum_q l_q(+-1) Q_q
 //   PB  local Lax-Friedrichs interface flux at the + end of the line, and at the - end of
-//       the lines that start on the brick boundary (neighbour traces come from the trace buffer)
-//   PC  lift with 2/h folded in: r_i = V_i - (l_i(+1) F*_+ - l_i(-1) F*_-) (2/h_a)/w_i  (eq (5) 3rd term),
-//       accumulated over the axes in shared memory
-//   PD  (with the z lines, whose global accesses coalesce) LSERK45 stage  K = A K + dt R, Q = Q + B K
-//       (PAPER.md:80, 254): K read and K, Q written straight from/to HBM; or R itself in residual mode
+//       the lines that start on the brick boundary
+//   PC  lift with 2/h folded in: r_i = V_i - (l_i(+1) F*_+ - l_i(-1) F*_-) (2/h_a)/w_i  (eq (5) 3rd term)
+//   PD  LSERK45 accumulated in place on the staged K:  x: K = A K + dt r_x,
+//       y: K += dt r_y,  z: K += dt r_z, Q += B K, both written straight to HBM from the z lines
+//       (coalesced); or R itself in residual mode
 //   PE  face traces of the UPDATED Q on the brick boundary, written to the other trace buffer
 // so that Q and K are read once and written once per stage and no element ever needs another
 // element's nodal values: neighbours meet only through the double-buffered brick-boundary traces.
@@ -34,13 +36,31 @@ namespace {
 // ------------------------------------------------------------------------------------------------
 // compile-time geometry of one variant
 // ------------------------------------------------------------------------------------------------
-template <int N_, int BX_, int BY_, int BZ_, int MINB_, int NBUF_>
+// Shared-memory row pitch (doubles) and cp.async width (doubles) for a brick GX nodes wide.
+//   GX odd : rows stay dense (x lines, one per thread at stride GX doubles, are already conflict-free)
+//   GX even: rows are padded.  16-byte copies need an even pitch; an even pitch with pitch/2 odd leaves
+//            a 2-way conflict on the x lines only.  If that padding would cost more than a third of the
+//            plane, pad by one double (conflict-free) and copy 8 bytes at a time instead.
+constexpr int pitch_even16(int gx) {
+    int p = gx + 2;
+    while ((p / 2) % 2 == 0) p += 2;
+    return p;
+}
+constexpr bool use_vec2(int gx) { return gx % 2 == 0 && 3 * pitch_even16(gx) <= 4 * gx; }
+constexpr int smem_pitch(int gx) { return gx % 2 ? gx : (use_vec2(gx) ? pitch_even16(gx) : gx + 1); }
+
+template <int N_, int BX_, int BY_, int BZ_, int MINB_, int RELOAD_ = 0>
 struct Cfg {
-    static constexpr int N = N_, BX = BX_, BY = BY_, BZ = BZ_, MINB = MINB_, NBUF = NBUF_;
+    static constexpr int N = N_, BX = BX_, BY = BY_, BZ = BZ_, MINB = MINB_;
+    // RELOAD = 1: the volume term reads the line's Q from shared memory a second time instead of keeping
+    // it in 10 N registers across the interface fluxes (fewer registers, more blocks per SM, 15 more
+    // shared loads per node)
+    static constexpr bool RELOAD = RELOAD_ != 0;
     static constexpr int GX = BX * N, GY = BY * N, GZ = BZ * N;   // nodes of the brick per axis
     static constexpr int NODES = GX * GY * GZ;
-    static constexpr int SLOT = DG_NV * NODES;                     // doubles per brick in Q, K, R
-    static constexpr int P = GX | 1;                               // odd shared-memory row pitch: x-lines conflict-free
+    static constexpr int SLOT = DG_NV * NODES;                     // doubles per brick in Q, K, R (HBM, dense)
+    static constexpr int P = smem_pitch(GX);                       // shared-memory row pitch
+    static constexpr int VEC = use_vec2(GX) ? 2 : 1;               // doubles per cp.async
     static constexpr int ROWS = GZ * GY;                           // rows per variable
     static constexpr int PLANE = ROWS * P;                         // shared doubles per variable
     static constexpr int L = NODES / N;                            // node lines per axis = threads that work
@@ -49,24 +69,51 @@ struct Cfg {
     static constexpr int TSLOT = 2 * DG_NV * (CX + CY + CZ);       // trace doubles per brick
     static constexpr bool MULTI = (BX > 1) || (BY > 1) || (BZ > 1);
     static constexpr int LINEBUF = MULTI ? DG_NV * L : 0;          // T- / F* hand-over between elements of a brick
-    static constexpr int SMEM_DOUBLES = (NBUF + 1) * DG_NV * PLANE + TSLOT + 2 * LINEBUF;
+    static constexpr int SMEM_DOUBLES = 2 * DG_NV * PLANE + 2 * LINEBUF;
     static constexpr int SMEM_BYTES = SMEM_DOUBLES * 8;
 };
 
-__device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) {
+template <int VEC>
+__device__ __forceinline__ void cp_async(double *smem_dst, const double *gsrc) {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gsrc) : "memory");
+    if (VEC == 2)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gsrc) : "memory");
+    else
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gsrc) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int PENDING>
 __device__ __forceinline__ void cp_async_wait() {
     asm volatile("cp.async.wait_group %0;" ::"n"(PENDING) : "memory");
 }
-// Ask L2 to fetch [ptr, ptr + bytes) (rounded out to 16-byte granules): one instruction per brick of K.
+// Ask L2 to fetch [ptr, ptr + bytes) (rounded out to 16-byte granules): one instruction per block of data.
 __device__ __forceinline__ void l2_prefetch(const void *ptr, unsigned bytes) {
     const uintptr_t lo = (uintptr_t)ptr & ~(uintptr_t)15;
     const uintptr_t hi = ((uintptr_t)ptr + bytes + 15) & ~(uintptr_t)15;
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(lo), "r"((unsigned)(hi - lo)) : "memory");
+}
+
+// Compiler-level fence on memory operations: bounds how far loads are hoisted (register pressure).
+__device__ __forceinline__ void sched_fence() { asm volatile("" ::: "memory"); }
+
+// Branch-free reciprocal and square root for positive, normal arguments (densities, gamma p / rho):
+// hardware seed (MUFU.RCP64H / MUFU.RSQ64H), one cubic and one quadratic correction; the result is within
+// about one unit in the last place (tests/test_gpu_parity.py::test_fast_math measures it), with none of
+// the slow-path branches of the IEEE-rounded library routines.
+__device__ __forceinline__ double rcp_pos(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    const double e = fma(-x, r, 1.0);
+    r = fma(r, fma(e, e, e), r);                    // r (1 + e + e^2)
+    return fma(r, fma(-x, r, 1.0), r);
+}
+__device__ __forceinline__ double sqrt_pos(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-(x * y), y, 1.0);         // 1 - x y^2
+    y = fma(y, e * fma(0.375, e, 0.5), y);          // y (1 + e/2 + 3 e^2/8)
+    const double s = x * y;
+    return fma(fma(-s, s, x), 0.5 * y, s);          // s + (x - s^2) / (2 sqrt x)
 }
 
 // Euler flux along the face/line normal, eq (2)-(3) (listing lines 186-217), for a state
@@ -75,7 +122,7 @@ __device__ __forceinline__ void l2_prefetch(const void *ptr, unsigned bytes) {
 // One copy of the code then serves the three axes with no run-time selection.
 __device__ __forceinline__ void euler_flux_normal(const double (&Q)[DG_NV], double gm1, double (&F)[DG_NV],
                                                   double &vel, double &pres, double &oneOrho) {
-    oneOrho = 1.0 / Q[0];
+    oneOrho = rcp_pos(Q[0]);
     vel = Q[1] * oneOrho;
     const double ub = Q[2] * oneOrho, uc = Q[3] * oneOrho;
     pres = gm1 * (Q[4] - 0.5 * Q[0] * (vel * vel + ub * ub + uc * uc));
@@ -94,417 +141,383 @@ __device__ __forceinline__ void lax_friedrichs(const double (&Qown)[DG_NV], cons
     double Fa[DG_NV], Fb[DG_NV], ua, ub, pa, pb, ra, rb;
     euler_flux_normal(Qown, gm1, Fa, ua, pa, ra);
     euler_flux_normal(Qoth, gm1, Fb, ub, pb, rb);
-    const double lama = fabs(ua) + sqrt(gamma * pa * ra);
-    const double lamb = fabs(ub) + sqrt(gamma * pb * rb);
+    const double lama = fabs(ua) + sqrt_pos(gamma * pa * ra);
+    const double lamb = fabs(ub) + sqrt_pos(gamma * pb * rb);
     const double hl = 0.5 * sgn * ((lama > lamb) ? lama : lamb);
 #pragma unroll
     for (int n = 0; n < DG_NV; ++n) Fs[n] = 0.5 * (Fa[n] + Fb[n]) - hl * (Qoth[n] - Qown[n]);
 }
 
 // ------------------------------------------------------------------------------------------------
-// geometry of the node line of thread `l` along axis `ax` inside the brick
-//   l = e * Ca + c,  e = element along the axis, c = face node = t2 * T1 + t1
+// per-axis compile-time traits and the (brick-independent) geometry of a thread's node line
+//   line l = e * Ca + c,  e = element along the axis, c = face node = t2 * T1 + t1
 //   axis x: (t1,t2) = (gy,gz);  y: (gx,gz);  z: (gx,gy)
 // ------------------------------------------------------------------------------------------------
-struct Line {
-    int e, c, base, stride, Ca, tbase, exta;
-    bool active, multi;
+template <class C, int AX>
+struct Axis {
+    static constexpr int S = (AX == 0) ? 1 : (AX == 1) ? C::P : C::GY * C::P;          // shared stride along the line
+    static constexpr int Ca = (AX == 0) ? C::CX : (AX == 1) ? C::CY : C::CZ;           // face nodes of a brick side
+    static constexpr int T1 = (AX == 0) ? C::GY : C::GX;
+    static constexpr int B = (AX == 0) ? C::BX : (AX == 1) ? C::BY : C::BZ;            // elements along the axis
+    static constexpr int TBASE = (AX == 0) ? 0 : (AX == 1) ? 2 * DG_NV * C::CX : 2 * DG_NV * (C::CX + C::CY);
+    static constexpr bool MULTI = B > 1;
+    // momentum slots rotated so that slot 1 is the component along this axis: slot s holds variable VAR[s]
+    static constexpr int M1 = 1 + AX, M2 = (AX == 2) ? 1 : 2 + AX, M3 = (AX == 0) ? 3 : AX;
+};
+template <class C, int AX>
+__device__ __forceinline__ constexpr int var_of_slot(int s) {
+    return s == 0 ? 0 : s == 1 ? Axis<C, AX>::M1 : s == 2 ? Axis<C, AX>::M2 : s == 3 ? Axis<C, AX>::M3 : 4;
+}
+
+struct Geo {
+    int base;   // shared-memory offset (doubles, inside one variable plane) of node 0 of the line
+    int c;      // face-node index of the line on the brick side
+    int e;      // element along the axis
 };
 
-template <class C>
-__device__ __forceinline__ Line make_line(int ax, int l, int ext0, int ext1, int ext2) {
+template <class C, int AX>
+__device__ __forceinline__ Geo make_geo(int l) {
+    using A = Axis<C, AX>;
     constexpr int N = C::N;
-    Line ln;
-    int t1, t2;
-    if (ax == 0) {
-        ln.Ca = C::CX;
-        ln.e = (C::BX == 1) ? 0 : l / C::CX;
-        ln.c = l - ln.e * C::CX;
-        t2 = ln.c / C::GY;
-        t1 = ln.c - t2 * C::GY;
-        ln.base = (t2 * C::GY + t1) * C::P + ln.e * N;
-        ln.stride = 1;
-        ln.tbase = 0;
-        ln.exta = ext0;
-        ln.multi = C::BX > 1;
-        ln.active = t1 < ext1 * N && t2 < ext2 * N;
-    } else if (ax == 1) {
-        ln.Ca = C::CY;
-        ln.e = (C::BY == 1) ? 0 : l / C::CY;
-        ln.c = l - ln.e * C::CY;
-        t2 = ln.c / C::GX;
-        t1 = ln.c - t2 * C::GX;
-        ln.base = (t2 * C::GY + ln.e * N) * C::P + t1;
-        ln.stride = C::P;
-        ln.tbase = 2 * DG_NV * C::CX;
-        ln.exta = ext1;
-        ln.multi = C::BY > 1;
-        ln.active = t1 < ext0 * N && t2 < ext2 * N;
-    } else {
-        ln.Ca = C::CZ;
-        ln.e = (C::BZ == 1) ? 0 : l / C::CZ;
-        ln.c = l - ln.e * C::CZ;
-        t2 = ln.c / C::GX;
-        t1 = ln.c - t2 * C::GX;
-        ln.base = (ln.e * N * C::GY + t2) * C::P + t1;
-        ln.stride = C::GY * C::P;
-        ln.tbase = 2 * DG_NV * (C::CX + C::CY);
-        ln.exta = ext2;
-        ln.multi = C::BZ > 1;
-        ln.active = t1 < ext0 * N && t2 < ext1 * N;
-    }
-    ln.active = ln.active && l < C::L && ln.e < ln.exta;
-    return ln;
+    Geo g;
+    g.e = (A::B == 1) ? 0 : l / A::Ca;
+    g.c = l - g.e * A::Ca;
+    const int t2 = g.c / A::T1, t1 = g.c - t2 * A::T1;
+    if (AX == 0) g.base = (t2 * C::GY + t1) * C::P + g.e * N;
+    else if (AX == 1) g.base = (t2 * C::GY + g.e * N) * C::P + t1;
+    else g.base = (g.e * N * C::GY + t2) * C::P + t1;
+    return g;
 }
 
-// P0a: enqueue the asynchronous copy of one brick's Q, and ask L2 for its K and its neighbours' traces.
-template <class C>
-__device__ __forceinline__ void issue_q_loads(const DgStageArgs &a, int brick, double *Qd, int tid, bool want_k) {
-    constexpr int NV = DG_NV, GX = C::GX, P = C::P, THREADS = C::THREADS;
-    const double *src = a.Q + (size_t)brick * C::SLOT;
-    constexpr int TOTAL = NV * C::NODES;
-#pragma unroll 4
-    for (int idx = tid; idx < TOTAL; idx += THREADS) {
-        const int row = idx / GX;                         // row over all 5 variables: PLANE = ROWS * P
-        cp_async8(Qd + idx + row * (P - GX), src + idx);
-    }
-    if (want_k && tid == 0) l2_prefetch(a.K + (size_t)brick * C::SLOT, C::SLOT * 8);
+// Is the line inside a ragged (last) brick of ext0 x ext1 x ext2 elements?
+template <class C, int AX>
+__device__ __forceinline__ bool line_inside(const Geo &g, int ext0, int ext1, int ext2) {
+    using A = Axis<C, AX>;
+    const int t2 = g.c / A::T1, t1 = g.c - t2 * A::T1;
+    const int lim1 = ((AX == 0) ? ext1 : ext0) * C::N, lim2 = ((AX == 2) ? ext1 : ext2) * C::N;
+    const int exta = (AX == 0) ? ext0 : (AX == 1) ? ext1 : ext2;
+    return t1 < lim1 && t2 < lim2 && g.e < exta;
 }
 
-// Neighbour brick and offset of the trace block a brick needs for (axis, side): side 0 = T+ of the brick
-// below (stored as that brick's side 1), side 1 = T- of the brick above (its side 0).
+// P0: enqueue the asynchronous copy of one dense HBM slot [5][GZ][GY][GX] into the pitched shared planes.
 template <class C>
-__device__ __forceinline__ const double *halo_source(const DgStageArgs &a, int bxi, int byi, int bzi, int ax, int side) {
-    const int Ca = (ax == 0) ? C::CX : (ax == 1) ? C::CY : C::CZ;
-    const int tbase = (ax == 0) ? 0 : (ax == 1) ? 2 * DG_NV * C::CX : 2 * DG_NV * (C::CX + C::CY);
-    int bx = bxi, by = byi, bz = bzi;   // (no run-time indexed local array: it would live in local memory)
-    if (ax == 0) bx = (side == 0) ? ((bx == 0) ? a.nbx - 1 : bx - 1) : ((bx + 1 == a.nbx) ? 0 : bx + 1);
-    else if (ax == 1) by = (side == 0) ? ((by == 0) ? a.nby - 1 : by - 1) : ((by + 1 == a.nby) ? 0 : by + 1);
-    else bz = (side == 0) ? ((bz == 0) ? a.nbz - 1 : bz - 1) : ((bz + 1 == a.nbz) ? 0 : bz + 1);
-    const size_t nbr = (size_t)bx + (size_t)a.nbx * ((size_t)by + (size_t)a.nby * bz);
-    return a.Told + nbr * C::TSLOT + tbase + (side == 0 ? DG_NV * Ca : 0);
-}
-
-// P0b: enqueue the asynchronous copies of the 6 neighbour trace blocks of this brick.
-template <class C>
-__device__ __forceinline__ void issue_halo_loads(const DgStageArgs &a, int bxi, int byi, int bzi, double *Hd, int tid) {
-    constexpr int NV = DG_NV, THREADS = C::THREADS;
-#pragma unroll
-    for (int ax = 0; ax < 3; ++ax) {
-        const int Ca = (ax == 0) ? C::CX : (ax == 1) ? C::CY : C::CZ;
-        const int tbase = (ax == 0) ? 0 : (ax == 1) ? 2 * NV * C::CX : 2 * NV * (C::CX + C::CY);
-        const double *srcm = halo_source<C>(a, bxi, byi, bzi, ax, 0);
-        const double *srcp = halo_source<C>(a, bxi, byi, bzi, ax, 1);
-        for (int r = tid; r < NV * Ca; r += THREADS) {
-            cp_async8(Hd + tbase + r, srcm + r);
-            cp_async8(Hd + tbase + NV * Ca + r, srcp + r);
+__device__ __forceinline__ void stage_in(double *dst, const double *src, int tid) {
+    constexpr int CPR = C::GX / C::VEC;                    // chunks per row
+    constexpr int TOTAL = DG_NV * C::ROWS * CPR;
+#pragma unroll 1
+    for (int k = tid; k < TOTAL; k += C::THREADS) {
+        if (C::P == C::GX) {
+            cp_async<C::VEC>(dst + k * C::VEC, src + k * C::VEC);
+        } else {
+            const int row = k / CPR;
+            cp_async<C::VEC>(dst + k * C::VEC + row * (C::P - C::GX), src + k * C::VEC);
         }
     }
 }
 
-// ... and the L2 prefetch of the same 6 blocks for the NEXT brick (6 threads, one instruction each).
+// Trace block [5][Ca] a brick needs for (axis, side): side 0 = T+ of the brick below (stored as that brick's
+// side 1), side 1 = T- of the brick above (its side 0).  Periodic in every direction.
+template <class C, int AX>
+__device__ __forceinline__ const double *halo_source(const DgStageArgs &a, int bx, int by, int bz, int side) {
+    using A = Axis<C, AX>;
+    if (AX == 0) bx = (side == 0) ? ((bx == 0) ? a.nbx - 1 : bx - 1) : ((bx + 1 == a.nbx) ? 0 : bx + 1);
+    else if (AX == 1) by = (side == 0) ? ((by == 0) ? a.nby - 1 : by - 1) : ((by + 1 == a.nby) ? 0 : by + 1);
+    else bz = (side == 0) ? ((bz == 0) ? a.nbz - 1 : bz - 1) : ((bz + 1 == a.nbz) ? 0 : bz + 1);
+    const size_t nbr = (size_t)bx + (size_t)a.nbx * ((size_t)by + (size_t)a.nby * bz);
+    return a.Told + nbr * C::TSLOT + A::TBASE + (side == 0 ? DG_NV * A::Ca : 0);
+}
+
+// L2 prefetch of everything the block's NEXT brick will read: 8 threads, one instruction each.
 template <class C>
-__device__ __forceinline__ void prefetch_halo(const DgStageArgs &a, int brick, int tid) {
-    if (tid < 6) {
-        const int bxi = brick % a.nbx, byi = (brick / a.nbx) % a.nby, bzi = brick / (a.nbx * a.nby);
-        const int ax = tid >> 1, side = tid & 1;
-        const int Ca = (ax == 0) ? C::CX : (ax == 1) ? C::CY : C::CZ;
-        l2_prefetch(halo_source<C>(a, bxi, byi, bzi, ax, side), DG_NV * Ca * 8);
+__device__ __forceinline__ void prefetch_brick(const DgStageArgs &a, int brick, int tid, bool want_k, bool want_halo) {
+    if (tid == 0) l2_prefetch(a.Q + (size_t)brick * C::SLOT, C::SLOT * 8);
+    if (tid == 1 && want_k) l2_prefetch(a.K + (size_t)brick * C::SLOT, C::SLOT * 8);
+    if (tid >= 2 && tid < 8 && want_halo) {
+        const int bx = brick % a.nbx, by = (brick / a.nbx) % a.nby, bz = brick / (a.nbx * a.nby);
+        const int side = tid & 1;
+        if (tid < 4) l2_prefetch(halo_source<C, 0>(a, bx, by, bz, side), DG_NV * C::CX * 8);
+        else if (tid < 6) l2_prefetch(halo_source<C, 1>(a, bx, by, bz, side), DG_NV * C::CY * 8);
+        else l2_prefetch(halo_source<C, 2>(a, bx, by, bz, side), DG_NV * C::CZ * 8);
     }
 }
 
 // PE for one axis: traces of the (updated) Q in shared memory on the brick boundary -> Tnew.
-template <class C>
-__device__ __forceinline__ void boundary_traces(const Line &ln, const double *Qs, double *Tbrick,
+template <class C, int AX>
+__device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta, const double *Qs, double *Tbrick,
                                                 const DgStageArgs &a) {
+    using A = Axis<C, AX>;
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE;
-    if (ln.active && (ln.e == 0 || ln.e == ln.exta - 1)) {
+    const bool first = g.e == 0, last = g.e == exta - 1;
+    if (!act || !(first || last)) return;
+    double *dst = Tbrick + A::TBASE + g.c;
+    const double *Q0 = Qs + g.base;
+    if (first && last) {
         double Tp[NV], Tm[NV];
 #pragma unroll
-        for (int n = 0; n < NV; ++n) {
-            Tp[n] = 0.0;
-            Tm[n] = 0.0;
-        }
+        for (int n = 0; n < NV; ++n) Tp[n] = Tm[n] = 0.0;
 #pragma unroll
-        for (int q = 0; q < N; ++q) {
-            const double lpq = a.ops.lp[q], lmq = a.ops.lm[q];
+        for (int q = 0; q < N; ++q)
 #pragma unroll
             for (int n = 0; n < NV; ++n) {
-                const double Qv = Qs[n * PLANE + ln.base + q * ln.stride];
-                Tp[n] = fma(lpq, Qv, Tp[n]);
-                Tm[n] = fma(lmq, Qv, Tm[n]);
+                const double Qv = Q0[n * PLANE + q * A::S];
+                Tp[n] = fma(a.ops.lp[q], Qv, Tp[n]);
+                Tm[n] = fma(a.ops.lm[q], Qv, Tm[n]);
+            }
+#pragma unroll
+        for (int n = 0; n < NV; ++n) {
+            dst[n * A::Ca] = Tm[n];
+            dst[(NV + n) * A::Ca] = Tp[n];
+        }
+    } else {
+        // one end only: the interpolation weights of the - end are those of the + end reversed
+        double T[NV];
+#pragma unroll
+        for (int n = 0; n < NV; ++n) T[n] = 0.0;
+#pragma unroll
+        for (int q = 0; q < N; ++q) {
+            const double w = first ? a.ops.lm[q] : a.ops.lp[q];
+#pragma unroll
+            for (int n = 0; n < NV; ++n) T[n] = fma(w, Q0[n * PLANE + q * A::S], T[n]);
+        }
+        if (!first) dst += NV * A::Ca;
+#pragma unroll
+        for (int n = 0; n < NV; ++n) dst[n * A::Ca] = T[n];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// one axis of the residual for one brick
+// ------------------------------------------------------------------------------------------------
+// PH: the neighbour bricks' traces this line touches, momentum slots rotated, HBM/L2 -> registers.
+template <class C, int AX>
+__device__ __forceinline__ void load_halo(const Geo &g, bool act, int exta, const double *halo_lo,
+                                          const double *halo_hi, double (&Hlo)[DG_NV], double (&Hhi)[DG_NV]) {
+    constexpr int Ca = Axis<C, AX>::Ca;
+    if (act && g.e == 0) {
+#pragma unroll
+        for (int s = 0; s < DG_NV; ++s) Hlo[s] = __ldg(halo_lo + var_of_slot<C, AX>(s) * Ca + g.c);
+    }
+    if (act && g.e == exta - 1) {
+#pragma unroll
+        for (int s = 0; s < DG_NV; ++s) Hhi[s] = __ldg(halo_hi + var_of_slot<C, AX>(s) * Ca + g.c);
+    }
+}
+
+// PA..PD for one axis.  Order chosen for register pressure: the line's Q goes into registers once; the
+// face traces and the two interface fluxes come first (no accumulators alive yet); the accumulators then
+// START from the lift term and the volume term is added node by node.
+//   r_i = sum_q Dhat_iq F_q - (l_i(+1) F*_+ - l_i(-1) F*_-) (2/h_a)/w_i
+template <class C, int AX, int MODE>
+__device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, int l, bool act, int exta,
+                                          const double *halo_lo, const double *halo_hi, double *Qs, double *Ks,
+                                          double *Tms, double *Fss, bool readK, double cR, size_t qbase,
+                                          double *Tbrick) {
+    using A = Axis<C, AX>;
+    constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE, L = C::L, S = A::S, Ca = A::Ca;
+    const bool first = g.e == 0, last = g.e == exta - 1;
+    double Hlo[NV], Hhi[NV];
+    load_halo<C, AX>(g, act, exta, halo_lo, halo_hi, Hlo, Hhi);
+
+    double QL[C::RELOAD ? 1 : NV][C::RELOAD ? 1 : N], Tp[NV], Tm[NV];
+    if (act) {
+        // ------------- the line's nodal values (slot s holds variable var_of_slot(s)) and its traces ----
+        const double *Q0 = Qs + g.base;
+#pragma unroll
+        for (int s = 0; s < NV; ++s) {
+            Tp[s] = 0.0;
+            Tm[s] = 0.0;
+#pragma unroll
+            for (int q = 0; q < N; ++q) {
+                const double Qv = Q0[var_of_slot<C, AX>(s) * PLANE + q * S];
+                if (!C::RELOAD) QL[s][q] = Qv;
+                Tp[s] = fma(a.ops.lp[q], Qv, Tp[s]);
+                Tm[s] = fma(a.ops.lm[q], Qv, Tm[s]);
             }
         }
-        double *dst = Tbrick + ln.tbase + ln.c;
-        if (ln.e == 0) {
+        if (A::MULTI) {
 #pragma unroll
-            for (int n = 0; n < NV; ++n) dst[n * ln.Ca] = Tm[n];
+            for (int n = 0; n < NV; ++n) Tms[n * L + l] = Tm[n];
         }
-        if (ln.e == ln.exta - 1) {
+    }
+    if (A::MULTI) __syncthreads();
+
+    // ------------- PB: interface fluxes ----------------------------------------------------------------
+    double Fp[NV], Fm[NV];
+    if (act) {
+        if (A::MULTI && !last) {
 #pragma unroll
-            for (int n = 0; n < NV; ++n) dst[(NV + n) * ln.Ca] = Tp[n];
+            for (int n = 0; n < NV; ++n) Hhi[n] = Tms[n * L + l + Ca];   // T- of the next element of this brick
+        }
+        lax_friedrichs(Tp, Hhi, 1.0, a.gamma, a.gm1, Fp);
+        if (A::MULTI) {
+#pragma unroll
+            for (int n = 0; n < NV; ++n) Fss[n * L + l] = Fp[n];
+        }
+        if (first) lax_friedrichs(Tm, Hlo, -1.0, a.gamma, a.gm1, Fm);
+    }
+    if (A::MULTI) __syncthreads();
+
+    if (act) {
+        if (A::MULTI && !first) {
+#pragma unroll
+            for (int n = 0; n < NV; ++n) Fm[n] = Fss[n * L + l - Ca];
+        }
+        // ------------- PC: lift (2/h and 1/w folded into the tables) starts the accumulators -----------
+        double V[NV][N];
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            const double cp = a.ops.lpg[AX][i], cm = a.ops.lmg[AX][i];
+#pragma unroll
+            for (int n = 0; n < NV; ++n) V[n][i] = fma(cm, Fm[n], -cp * Fp[n]);
+        }
+        // ------------- PA: pointwise flux and sum-factorised derivative --------------------------------
+#pragma unroll
+        for (int q = 0; q < N; ++q) {
+            double Qn[NV], F[NV], vel, pres, rinv;
+#pragma unroll
+            for (int s = 0; s < NV; ++s)
+                Qn[s] = C::RELOAD ? Qs[g.base + var_of_slot<C, AX>(s) * PLANE + q * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : q];
+            euler_flux_normal(Qn, a.gm1, F, vel, pres, rinv);
+#pragma unroll
+            for (int n = 0; n < NV; ++n)
+#pragma unroll
+                for (int i = 0; i < N; ++i) V[n][i] = fma(a.ops.Dg[AX][q][i], F[n], V[n][i]);
+        }
+        // ------------- PD: Runge-Kutta accumulation on the staged K ------------------------------------
+        double *K0 = Ks + g.base;
+        if (AX == 0) {
+            if (readK) {
+                const double rkA = a.rkA;
+#pragma unroll
+                for (int s = 0; s < NV; ++s)
+#pragma unroll
+                    for (int i = 0; i < N; ++i) {
+                        double *p = K0 + var_of_slot<C, AX>(s) * PLANE + i * S;
+                        *p = fma(rkA, *p, cR * V[s][i]);
+                    }
+            } else {
+#pragma unroll
+                for (int s = 0; s < NV; ++s)
+#pragma unroll
+                    for (int i = 0; i < N; ++i) K0[var_of_slot<C, AX>(s) * PLANE + i * S] = cR * V[s][i];
+            }
+        } else if (AX == 1) {
+#pragma unroll
+            for (int s = 0; s < NV; ++s)
+#pragma unroll
+                for (int i = 0; i < N; ++i) {
+                    double *p = K0 + var_of_slot<C, AX>(s) * PLANE + i * S;
+                    *p = fma(cR, V[s][i], *p);
+                }
+        } else {
+            // z lines: consecutive threads hold consecutive (gx, gy), so HBM accesses coalesce
+            const size_t g0 = qbase + (size_t)(g.e * N) * (C::GY * C::GX) + g.c;   // node 0 of the line, variable 0
+            if (MODE == DG_MODE_RESIDUAL) {
+#pragma unroll
+                for (int s = 0; s < NV; ++s)
+#pragma unroll
+                    for (int i = 0; i < N; ++i) {
+                        const int n = var_of_slot<C, AX>(s);
+                        a.Rout[g0 + (size_t)n * C::NODES + (size_t)i * (C::GY * C::GX)] =
+                            fma(cR, V[s][i], K0[n * PLANE + i * S]);
+                    }
+            } else {
+                const double rkB = a.rkB;
+                double *Q0w = Qs + g.base;
+                double *dst = Tbrick + A::TBASE + g.c;
+#pragma unroll
+                for (int s = 0; s < NV; ++s) {
+                    const int n = var_of_slot<C, AX>(s);
+                    double tp = 0.0, tm = 0.0;
+#pragma unroll
+                    for (int i = 0; i < N; ++i) {
+                        const size_t go = g0 + (size_t)n * C::NODES + (size_t)i * (C::GY * C::GX);
+                        const double Kn = fma(cR, V[s][i], K0[n * PLANE + i * S]);
+                        const double Qn = fma(rkB, Kn, Q0w[n * PLANE + i * S]);
+                        a.K[go] = Kn;
+                        a.Q[go] = Qn;
+                        Q0w[n * PLANE + i * S] = Qn;
+                        tp = fma(a.ops.lp[i], Qn, tp);
+                        tm = fma(a.ops.lm[i], Qn, tm);
+                    }
+                    if (first) dst[n * Ca] = tm;
+                    if (last) dst[(NV + n) * Ca] = tp;
+                }
+            }
         }
     }
 }
 
+// ------------------------------------------------------------------------------------------------
 // ------------------------------------------------------------------------------------------------
 // the fused, persistent stage kernel
 // ------------------------------------------------------------------------------------------------
 template <class C, int MODE>
 __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __grid_constant__ DgStageArgs a) {
-    constexpr int N = C::N, GX = C::GX, GY = C::GY;
-    constexpr int NODES = C::NODES, PLANE = C::PLANE, L = C::L;
-    constexpr int NV = DG_NV, NBUF = C::NBUF;
-    constexpr int mode = MODE;   // one kernel per mode: the hot stage kernel carries no residual/trace-only code
-
+    constexpr int NV = DG_NV, PLANE = C::PLANE, L = C::L;
     extern __shared__ __align__(16) double smem[];
-    double *Qbuf = smem;                       // [NBUF][5][PLANE] nodal values of a brick (old, then updated)
-    double *Rs = Qbuf + NBUF * NV * PLANE;     // [5][PLANE]       x (+ y) contribution to R
-    double *Hs = Rs + NV * PLANE;              // [TSLOT]          neighbour bricks' traces, laid out like a brick's
-                                               //                  own slot: [axis][side][5][Ca]; side 0 = T+ of the
-                                               //                  brick below, side 1 = T- of the brick above
-    double *Tms = Hs + C::TSLOT;               // [5][L]           T- of every line (right state of the line below)
-    double *Fss = Tms + C::LINEBUF;            // [5][L]           F* at the + end of every line
+    double *Qs = smem;                     // [5][PLANE] nodal values of the brick (old, then updated)
+    double *Ks = Qs + NV * PLANE;          // [5][PLANE] Runge-Kutta register of the brick, accumulated in place
+    double *Tms = Ks + NV * PLANE;         // [5][L]     T- of every line (right state of the line below)
+    double *Fss = Tms + C::LINEBUF;        // [5][L]     F* at the + end of every line
 
     const int tid = threadIdx.x, l = tid;
     const int nbricks = a.nbx * a.nby * a.nbz;
-    const bool readK = (mode == DG_MODE_STAGE) && (a.rkA != 0.0);
-    constexpr bool want_halo = (mode != DG_MODE_TRACES);
+    const bool readK = (MODE == DG_MODE_STAGE) && (a.rkA != 0.0);
+    const double cR = (MODE == DG_MODE_STAGE) ? a.dt : 1.0;
+    const Geo gx = make_geo<C, 0>(l), gy = make_geo<C, 1>(l), gz = make_geo<C, 2>(l);
+    const bool inL = l < L;
 
-    int brick = blockIdx.x;
-    int buf = 0;
-    if (NBUF == 2) {
-        if (brick < nbricks) issue_q_loads<C>(a, brick, Qbuf, tid, readK);
-        cp_async_commit();
-    }
-    for (; brick < nbricks; brick += gridDim.x) {
+    // One brick per block (no persistent loop: a loop over bricks makes the compiler hoist the operator
+    // tables out of it into registers).  Blocks are dispatched in index order, so the brick that is
+    // `a.grid` (= resident blocks of the whole GPU) ahead is the one that starts when this one ends.
+    {
+        const int brick = blockIdx.x;
         const int bxi = brick % a.nbx, byi = (brick / a.nbx) % a.nby, bzi = brick / (a.nbx * a.nby);
-        // ---------------- P0: this brick's neighbour traces and the next brick's Q go out ---------------
-        double *Qs;
-        if (NBUF == 2) {
-            if (want_halo) issue_halo_loads<C>(a, bxi, byi, bzi, Hs, tid);
-            cp_async_commit();
-            const int next = brick + gridDim.x;
-            if (next < nbricks) {
-                issue_q_loads<C>(a, next, Qbuf + (buf ^ 1) * NV * PLANE, tid, readK);
-                if (want_halo) prefetch_halo<C>(a, next, tid);
-            }
-            cp_async_commit();
-            cp_async_wait<2>();                    // this brick's Q (asked for one brick ago) has landed
-            Qs = Qbuf + buf * NV * PLANE;
-            buf ^= 1;
-        } else {
-            issue_q_loads<C>(a, brick, Qbuf, tid, readK);
-            cp_async_commit();
-            if (want_halo) issue_halo_loads<C>(a, bxi, byi, bzi, Hs, tid);
-            cp_async_commit();
-            cp_async_wait<1>();
-            Qs = Qbuf;
-        }
-        __syncthreads();
+        const size_t qbase = (size_t)brick * C::SLOT;
+        // ---------------- P0: this brick's Q and K come in; the next brick's data is asked into L2 ------
+        stage_in<C>(Qs, a.Q + qbase, tid);
+        if (readK) stage_in<C>(Ks, a.K + qbase, tid);
+        cp_async_commit();
+        const int next = brick + a.grid;
+        if (next < nbricks) prefetch_brick<C>(a, next, tid, readK, MODE != DG_MODE_TRACES);
 
         const int ext0 = min(C::BX, a.nx - bxi * C::BX);   // elements of this brick per axis (ragged last brick)
         const int ext1 = min(C::BY, a.ny - byi * C::BY);
         const int ext2 = min(C::BZ, a.nz - bzi * C::BZ);
-        const size_t qbase = (size_t)brick * C::SLOT;
+        const bool full = (ext0 == C::BX) && (ext1 == C::BY) && (ext2 == C::BZ);
+        bool actx = inL, acty = inL, actz = inL;
+        if (!full) {
+            actx = inL && line_inside<C, 0>(gx, ext0, ext1, ext2);
+            acty = inL && line_inside<C, 1>(gy, ext0, ext1, ext2);
+            actz = inL && line_inside<C, 2>(gz, ext0, ext1, ext2);
+        }
         double *Tbrick = a.Tnew + (size_t)brick * C::TSLOT;
 
-        if (mode != DG_MODE_TRACES) {
-            double V[NV][N];
-#pragma unroll 1
-            for (int ax = 0; ax < 3; ++ax) {
-                const Line ln = make_line<C>(ax, l, ext0, ext1, ext2);
-                // momentum slots rotated so that slot 1 is the component along this axis
-                const int m1 = 1 + ax, m2 = (ax == 2) ? 1 : 2 + ax, m3 = (ax == 0) ? 3 : ax;
-                const int po1 = m1 * PLANE, po2 = m2 * PLANE, po3 = m3 * PLANE;
-                double Tp[NV], Tm[NV];
-                // ------------- PA: flux, sum-factorised derivative, traces ---------------------------
-                if (ln.active) {
-#pragma unroll
-                    for (int n = 0; n < NV; ++n) {
-                        Tp[n] = 0.0;
-                        Tm[n] = 0.0;
-#pragma unroll
-                        for (int i = 0; i < N; ++i) V[n][i] = 0.0;
-                    }
-                    const double *Q0p = Qs + ln.base;
-#pragma unroll
-                    for (int q = 0; q < N; ++q) {
-                        double Qn[NV], F[NV], vel, pres, rinv;
-                        const double *Qq = Q0p + q * ln.stride;
-                        Qn[0] = Qq[0];
-                        Qn[1] = Qq[po1];
-                        Qn[2] = Qq[po2];
-                        Qn[3] = Qq[po3];
-                        Qn[4] = Qq[4 * PLANE];
-                        euler_flux_normal(Qn, a.gm1, F, vel, pres, rinv);
-                        const double *Dq = a.ops.Dg[ax][q];
-                        const double lpq = a.ops.lp[q], lmq = a.ops.lm[q];
-#pragma unroll
-                        for (int n = 0; n < NV; ++n) {
-#pragma unroll
-                            for (int i = 0; i < N; ++i) V[n][i] = fma(Dq[i], F[n], V[n][i]);
-                            Tp[n] = fma(lpq, Qn[n], Tp[n]);
-                            Tm[n] = fma(lmq, Qn[n], Tm[n]);
-                        }
-                    }
-                    if (ln.multi) {
-#pragma unroll
-                        for (int n = 0; n < NV; ++n) Tms[n * L + l] = Tm[n];
-                    }
-                }
-                if (ax == 0) {
-                    cp_async_wait<(NBUF == 2) ? 1 : 0>();   // the neighbour traces have landed
-                    __syncthreads();
-                } else if (ln.multi) {
-                    __syncthreads();
-                }
-
-                // ------------- PB: interface fluxes ----------------------------------------------------
-                double Fp[NV], Fm[NV];
-                if (ln.active) {
-                    double Qown[NV];
-#pragma unroll
-                    for (int n = 0; n < NV; ++n) Qown[n] = Tp[n];
-#pragma unroll 1
-                    for (int s = 0; s < 2; ++s) {
-                        // s = 0: + face (own state is the left one); s = 1: - face, only for the lines that
-                        // start on the brick boundary (own state is the right one)
-                        double Qo[NV], Fs[NV];
-                        const double *src;
-                        int sstride;
-                        if (s == 0 && ln.multi && ln.e + 1 < ln.exta) {
-                            src = Tms + l + ln.Ca;        // T- of the next element of this brick (rotated slots)
-                            sstride = L;
-                            Qo[1] = src[1 * sstride];
-                            Qo[2] = src[2 * sstride];
-                            Qo[3] = src[3 * sstride];
-                        } else {
-                            src = Hs + ln.tbase + ((s == 0) ? NV * ln.Ca : 0) + ln.c;
-                            sstride = ln.Ca;
-                            Qo[1] = src[m1 * sstride];
-                            Qo[2] = src[m2 * sstride];
-                            Qo[3] = src[m3 * sstride];
-                        }
-                        Qo[0] = src[0];
-                        Qo[4] = src[4 * sstride];
-                        lax_friedrichs(Qown, Qo, (s == 0) ? 1.0 : -1.0, a.gamma, a.gm1, Fs);
-                        if (s == 0) {
-#pragma unroll
-                            for (int n = 0; n < NV; ++n) {
-                                Fp[n] = Fs[n];
-                                Qown[n] = Tm[n];
-                            }
-                            if (ln.e != 0) break;
-                        } else {
-#pragma unroll
-                            for (int n = 0; n < NV; ++n) Fm[n] = Fs[n];
-                        }
-                    }
-                    if (ln.multi) {
-#pragma unroll
-                        for (int n = 0; n < NV; ++n) Fss[n * L + l] = Fp[n];
-                    }
-                }
-                if (ln.multi) __syncthreads();
-
-                // ------------- PC: lift (2/h and 1/w folded into the tables) ---------------------------
-                if (ln.active) {
-                    if (ln.multi && ln.e > 0) {
-#pragma unroll
-                        for (int n = 0; n < NV; ++n) Fm[n] = Fss[n * L + l - ln.Ca];
-                    }
-                    // K of this z line: asked for now (an L2 hit: prefetched a brick ago), used after the lift
-                    const size_t g0 = qbase + (size_t)(ln.e * N) * (GY * GX) + ln.c;   // node q=0 of a z-line, n=0
-                    double Kold[NV][N];
-                    if (ax == 2 && readK) {
-#pragma unroll
-                        for (int n = 0; n < NV; ++n)
-#pragma unroll
-                            for (int q = 0; q < N; ++q)
-                                Kold[n][q] = __ldcs(a.K + g0 + (size_t)n * NODES + (size_t)q * (GY * GX));
-                    }
-                    const double *lpg = a.ops.lpg[ax], *lmg = a.ops.lmg[ax];
-#pragma unroll
-                    for (int i = 0; i < N; ++i) {
-                        const double cp = lpg[i], cm = lmg[i];
-#pragma unroll
-                        for (int n = 0; n < NV; ++n) V[n][i] = fma(cm, Fm[n], fma(-cp, Fp[n], V[n][i]));
-                    }
-                    if (ax < 2) {
-                        // x: R = r_x;  y: R += r_y   (slot s holds variable 0, m1, m2, m3, 4)
-                        double *R0p = Rs + ln.base;
-#pragma unroll
-                        for (int i = 0; i < N; ++i) {
-                            double *Rq = R0p + i * ln.stride;
-                            if (ax == 0) {
-                                Rq[0] = V[0][i];
-                                Rq[po1] = V[1][i];
-                                Rq[po2] = V[2][i];
-                                Rq[po3] = V[3][i];
-                                Rq[4 * PLANE] = V[4][i];
-                            } else {
-                                Rq[0] += V[0][i];
-                                Rq[po1] += V[1][i];
-                                Rq[po2] += V[2][i];
-                                Rq[po3] += V[3][i];
-                                Rq[4 * PLANE] += V[4][i];
-                            }
-                        }
-                    } else {
-                        // z: slots (0,1,2,3,4) hold variables (0,3,1,2,4)
-                        constexpr int var_of_slot[NV] = {0, 3, 1, 2, 4};
-                        if (mode == DG_MODE_RESIDUAL) {
-#pragma unroll
-                            for (int s = 0; s < NV; ++s)
-#pragma unroll
-                                for (int q = 0; q < N; ++q) {
-                                    const int n = var_of_slot[s];
-                                    a.Rout[g0 + (size_t)n * NODES + (size_t)q * (GY * GX)] =
-                                        Rs[n * PLANE + ln.base + q * ln.stride] + V[s][q];
-                                }
-                        } else {
-                            // ------------- PD: LSERK45 stage, write back, z traces of the updated Q -----
-                            const double A = a.rkA, B = a.rkB, dt = a.dt;
-                            double *dst = Tbrick + ln.tbase + ln.c;
-#pragma unroll
-                            for (int s = 0; s < NV; ++s) {
-                                const int n = var_of_slot[s];
-                                double tp = 0.0, tm = 0.0;
-#pragma unroll
-                                for (int q = 0; q < N; ++q) {
-                                    const int sa = n * PLANE + ln.base + q * ln.stride;
-                                    const size_t go = g0 + (size_t)n * NODES + (size_t)q * (GY * GX);
-                                    const double R = Rs[sa] + V[s][q];
-                                    const double Kn = readK ? fma(A, Kold[n][q], dt * R) : dt * R;
-                                    const double Qn = fma(B, Kn, Qs[sa]);
-                                    a.K[go] = Kn;
-                                    a.Q[go] = Qn;
-                                    Qs[sa] = Qn;
-                                    tp = fma(a.ops.lp[q], Qn, tp);
-                                    tm = fma(a.ops.lm[q], Qn, tm);
-                                }
-                                if (ln.e == 0) dst[n * C::CZ] = tm;
-                                if (ln.e == ln.exta - 1) dst[(NV + n) * C::CZ] = tp;
-                            }
-                        }
-                    }
-                }
-                if (ax < 2) __syncthreads();
-            }
+        if (MODE != DG_MODE_TRACES) {
+            cp_async_wait<0>();
+            __syncthreads();
+            axis_pass<C, 0, MODE>(a, gx, l, actx, ext0, halo_source<C, 0>(a, bxi, byi, bzi, 0),
+                                  halo_source<C, 0>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, cR, qbase, Tbrick);
+            __syncthreads();
+            axis_pass<C, 1, MODE>(a, gy, l, acty, ext1, halo_source<C, 1>(a, bxi, byi, bzi, 0),
+                                  halo_source<C, 1>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, cR, qbase, Tbrick);
+            __syncthreads();
+            axis_pass<C, 2, MODE>(a, gz, l, actz, ext2, halo_source<C, 2>(a, bxi, byi, bzi, 0),
+                                  halo_source<C, 2>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, cR, qbase, Tbrick);
+        } else {
+            cp_async_wait<0>();
+            __syncthreads();
         }
-
         // ---------------- PE: traces of the updated Q on the brick boundary (z came from registers) ----
-        if (mode != DG_MODE_RESIDUAL) {
-            if (mode == DG_MODE_STAGE) __syncthreads();
-            const int nax = (mode == DG_MODE_TRACES) ? 3 : 2;
-#pragma unroll 1
-            for (int ax = 0; ax < nax; ++ax) boundary_traces<C>(make_line<C>(ax, l, ext0, ext1, ext2), Qs, Tbrick, a);
+        if (MODE != DG_MODE_RESIDUAL) {
+            if (MODE == DG_MODE_STAGE) __syncthreads();
+            boundary_traces<C, 0>(gx, actx, ext0, Qs, Tbrick, a);
+            boundary_traces<C, 1>(gy, acty, ext1, Qs, Tbrick, a);
+            if (MODE == DG_MODE_TRACES) boundary_traces<C, 2>(gz, actz, ext2, Qs, Tbrick, a);
         }
-        __syncthreads();   // everyone is done with this brick's buffers before they are refilled
     }
 }
-
 // ------------------------------------------------------------------------------------------------
 // layout conversion canonical [e][k][j][i][n] <-> internal [brick][n][gz][gy][gx]
 // one thread per node; canonical side reads/writes 40 contiguous bytes per thread
@@ -591,12 +604,13 @@ cudaError_t prepare(int *blocks_per_sm) {
 template <class C>
 cudaError_t launch_stage(const DgStageArgs &a, cudaStream_t s) {
     if (a.grid <= 0) return cudaErrorInvalidConfiguration;
+    const unsigned blocks = (unsigned)(a.nbx * a.nby * a.nbz);   // one block per brick
     if (a.mode == DG_MODE_STAGE)
-        dg_stage_kernel<C, DG_MODE_STAGE><<<(unsigned)a.grid, C::THREADS, C::SMEM_BYTES, s>>>(a);
+        dg_stage_kernel<C, DG_MODE_STAGE><<<blocks, C::THREADS, C::SMEM_BYTES, s>>>(a);
     else if (a.mode == DG_MODE_RESIDUAL)
-        dg_stage_kernel<C, DG_MODE_RESIDUAL><<<(unsigned)a.grid, C::THREADS, C::SMEM_BYTES, s>>>(a);
+        dg_stage_kernel<C, DG_MODE_RESIDUAL><<<blocks, C::THREADS, C::SMEM_BYTES, s>>>(a);
     else
-        dg_stage_kernel<C, DG_MODE_TRACES><<<(unsigned)a.grid, C::THREADS, C::SMEM_BYTES, s>>>(a);
+        dg_stage_kernel<C, DG_MODE_TRACES><<<blocks, C::THREADS, C::SMEM_BYTES, s>>>(a);
     return cudaGetLastError();
 }
 
@@ -627,48 +641,51 @@ constexpr DgKernelTable make_table() {
                          &prepare<C>, &launch_stage<C>, &launch_layout<C>, &launch_wavespeed<C>};
 }
 
-// Brick shapes per N (default first): Cfg<N, BX, BY, BZ, min blocks per SM, Q buffers>.
+// Brick shapes per N (default first): Cfg<N, BX, BY, BZ, min blocks per SM>.
 // DESIGN.md "brick shapes" explains the choice.
 #if DG_N == 2
-using V0 = Cfg<2, 4, 4, 4, 2, 2>;
+using V0 = Cfg<2, 4, 4, 4, 2, 0>;
 using V1 = Cfg<2, 4, 4, 4, 3, 1>;
-using V2 = Cfg<2, 4, 4, 2, 4, 2>;
-using V3 = Cfg<2, 2, 2, 2, 4, 1>;
+using V2 = Cfg<2, 4, 4, 2, 4, 0>;
+using V3 = Cfg<2, 4, 4, 2, 6, 1>;
 #elif DG_N == 3
-using V0 = Cfg<3, 4, 4, 2, 2, 2>;
-using V1 = Cfg<3, 4, 4, 2, 2, 1>;
-using V2 = Cfg<3, 2, 2, 2, 4, 2>;
-using V3 = Cfg<3, 1, 1, 1, 8, 1>;
+using V0 = Cfg<3, 4, 4, 2, 2, 1>;
+using V1 = Cfg<3, 4, 4, 2, 1, 0>;
+using V2 = Cfg<3, 2, 2, 2, 5, 0>;
+using V3 = Cfg<3, 2, 2, 2, 7, 1>;
 #elif DG_N == 4
-using V0 = Cfg<4, 2, 2, 2, 2, 2>;
-using V1 = Cfg<4, 2, 2, 2, 3, 1>;
-using V2 = Cfg<4, 2, 2, 1, 4, 2>;
-using V3 = Cfg<4, 1, 1, 1, 8, 1>;
+using V0 = Cfg<4, 2, 2, 2, 3, 1>;
+using V1 = Cfg<4, 2, 2, 2, 2, 0>;
+using V2 = Cfg<4, 2, 2, 1, 4, 0>;
+using V3 = Cfg<4, 2, 2, 1, 6, 1>;
 #elif DG_N == 5
-using V0 = Cfg<5, 1, 2, 2, 2, 2>;
+using V0 = Cfg<5, 1, 2, 2, 4, 1>;
 using V1 = Cfg<5, 1, 2, 2, 3, 1>;
-using V2 = Cfg<5, 2, 2, 2, 1, 2>;
-using V3 = Cfg<5, 1, 1, 1, 6, 2>;
+using V2 = Cfg<5, 1, 2, 2, 2, 0>;
+using V3 = Cfg<5, 1, 2, 3, 3, 1>;
 #elif DG_N == 6
-using V0 = Cfg<6, 1, 2, 2, 1, 2>;
-using V1 = Cfg<6, 1, 2, 2, 1, 1>;
-using V2 = Cfg<6, 1, 1, 2, 2, 2>;
-using V3 = Cfg<6, 1, 1, 1, 5, 2>;
+using V0 = Cfg<6, 1, 1, 2, 4, 1>;
+using V1 = Cfg<6, 1, 1, 2, 3, 0>;
+using V2 = Cfg<6, 1, 2, 2, 2, 1>;
+using V3 = Cfg<6, 1, 1, 1, 8, 1>;
 #elif DG_N == 7
-using V0 = Cfg<7, 1, 1, 2, 2, 2>;
-using V1 = Cfg<7, 1, 1, 2, 2, 1>;
-using V2 = Cfg<7, 1, 2, 2, 1, 2>;
-using V3 = Cfg<7, 1, 1, 1, 4, 2>;
+using V0 = Cfg<7, 1, 1, 2, 3, 1>;
+using V1 = Cfg<7, 1, 1, 2, 2, 0>;
+using V2 = Cfg<7, 1, 2, 2, 1, 0>;
+using V3 = Cfg<7, 1, 1, 1, 6, 1>;
 #elif DG_N == 8
-using V0 = Cfg<8, 1, 1, 2, 1, 2>;
-using V1 = Cfg<8, 1, 1, 2, 2, 1>;
-using V2 = Cfg<8, 1, 1, 1, 3, 2>;
-using V3 = Cfg<8, 1, 1, 1, 4, 1>;
+using V0 = Cfg<8, 1, 1, 2, 2, 1>;
+using V1 = Cfg<8, 1, 1, 2, 2, 0>;
+using V2 = Cfg<8, 1, 1, 1, 4, 1>;
+using V3 = Cfg<8, 1, 1, 1, 4, 0>;
 #else
 #error "DG_N must be 2..8"
 #endif
 
-const DgKernelTable k_tables[] = {make_table<V0>(), make_table<V1>(), make_table<V2>(), make_table<V3>()};
+using VE = Cfg<DG_N, 1, 1, 1, 4, 1>;   // one element per block: always there (tiny and ragged meshes, tests)
+
+const DgKernelTable k_tables[] = {make_table<V0>(), make_table<V1>(), make_table<V2>(), make_table<V3>(),
+                                  make_table<VE>()};
 
 }  // namespace
 
