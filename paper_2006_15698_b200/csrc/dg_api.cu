@@ -139,7 +139,8 @@ struct dg_ctx {
     double *Q, *K, *S, *T[2];
     unsigned long long *scal;
     int tcur;           // T[tcur] holds the traces of the current Q
-    int grid;           // persistent stage kernel: resident blocks per SM x SMs, capped by the brick count
+    int grid;           // resident blocks per SM x SMs, capped by the brick count (L2 prefetch distance)
+    int flags;          // DG_FLAGS tuning knobs, see DgStageArgs
     DgOps ops;          // device operator tables of this mesh (travel in the kernel arguments)
     bool bound, has_state;
     cudaStream_t stream;
@@ -203,6 +204,7 @@ DgStageArgs stage_args(const dg_ctx *c, int mode) {
     a.gm1 = c->gamma - 1.0;
     a.mode = mode;
     a.grid = c->grid;
+    a.flags = c->flags;
     a.ops = c->ops;
     return a;
 }
@@ -258,6 +260,7 @@ int dg_create(dg_ctx **out, int nx, int ny, int nz, int p, double gamma, const d
         const int v = std::atoi(ev);
         if (v >= 0 && v < count) pick = v;
     }
+    if (const char *ev = std::getenv("DG_FLAGS")) c->flags = std::atoi(ev);
     set_layout(c, &kt[pick]);
     *out = c;
     return DG_OK;

@@ -37,7 +37,8 @@ struct DgStageArgs {
     double gamma, gm1;
     double rkA, rkB, dt;  // stage coefficients; rkA == 0 means "do not read K" (stage 1)
     int mode;
-    int grid;             // blocks to launch (persistent: blocks stride over the bricks)
+    int grid;             // resident blocks of the whole GPU = how far ahead (in bricks) the L2 prefetch looks
+    int flags;            // tuning knobs (DG_FLAGS): 1 = no L2 prefetch, 2 = prefetch at block start
     DgOps ops;
 };
 

@@ -36,20 +36,16 @@ namespace {
 // ------------------------------------------------------------------------------------------------
 // compile-time geometry of one variant
 // ------------------------------------------------------------------------------------------------
-// Shared-memory row pitch (doubles) and cp.async width (doubles) for a brick GX nodes wide.
-//   GX odd : rows stay dense (x lines, one per thread at stride GX doubles, are already conflict-free)
-//   GX even: rows are padded.  16-byte copies need an even pitch; an even pitch with pitch/2 odd leaves
-//            a 2-way conflict on the x lines only.  If that padding would cost more than a third of the
-//            plane, pad by one double (conflict-free) and copy 8 bytes at a time instead.
-constexpr int pitch_even16(int gx) {
-    int p = gx + 2;
-    while ((p / 2) % 2 == 0) p += 2;
-    return p;
-}
-constexpr bool use_vec2(int gx) { return gx % 2 == 0 && 3 * pitch_even16(gx) <= 4 * gx; }
-constexpr int smem_pitch(int gx) { return gx % 2 ? gx : (use_vec2(gx) ? pitch_even16(gx) : gx + 1); }
-
-template <int N_, int BX_, int BY_, int BZ_, int MINB_, int RELOAD_ = 0>
+// Shared-memory layout of a brick: [5][GZ] planes of pitch PP doubles, rows of pitch P doubles inside a
+// plane, and, per axis, the order in which a warp's lanes walk the node lines (ORD):
+//   0: t1 fastest, then t2, then the element e along the axis      1: t2, t1, e
+//   2: t1, e, t2                                                   3: t2, e, t1
+// (t1,t2) = (gy,gz) for x lines, (gx,gz) for y lines, (gx,gy) for z lines.  P, PP and the orders are picked
+// per brick shape so that the 16 lanes of a half-warp hit 16 different 8-byte bank pairs in all three
+// passes (0 = dense).  z lines keep t1 = gx fastest: their lanes also
+// address HBM.
+template <int N_, int BX_, int BY_, int BZ_, int MINB_, int RELOAD_ = 0, int P_ = 0, int PP_ = 0, int OX_ = 0,
+          int OY_ = 0, int OZ_ = 0>
 struct Cfg {
     static constexpr int N = N_, BX = BX_, BY = BY_, BZ = BZ_, MINB = MINB_;
     // RELOAD = 1: the volume term reads the line's Q from shared memory a second time instead of keeping
@@ -59,10 +55,10 @@ struct Cfg {
     static constexpr int GX = BX * N, GY = BY * N, GZ = BZ * N;   // nodes of the brick per axis
     static constexpr int NODES = GX * GY * GZ;
     static constexpr int SLOT = DG_NV * NODES;                     // doubles per brick in Q, K, R (HBM, dense)
-    static constexpr int P = smem_pitch(GX);                       // shared-memory row pitch
-    static constexpr int VEC = use_vec2(GX) ? 2 : 1;               // doubles per cp.async
-    static constexpr int ROWS = GZ * GY;                           // rows per variable
-    static constexpr int PLANE = ROWS * P;                         // shared doubles per variable
+    static constexpr int P = P_ ? P_ : GX;                         // shared-memory row pitch
+    static constexpr int PP = PP_ ? PP_ : GY * P;                  // shared-memory plane pitch
+    static constexpr int PLANE = GZ * PP;                          // shared doubles per variable
+    static constexpr int OX = OX_, OY = OY_, OZ = OZ_;
     static constexpr int L = NODES / N;                            // node lines per axis = threads that work
     static constexpr int THREADS = (L + 31) / 32 * 32;
     static constexpr int CX = GY * GZ, CY = GX * GZ, CZ = GX * GY; // face nodes of a brick side per axis
@@ -71,15 +67,13 @@ struct Cfg {
     static constexpr int LINEBUF = MULTI ? DG_NV * L : 0;          // T- / F* hand-over between elements of a brick
     static constexpr int SMEM_DOUBLES = 2 * DG_NV * PLANE + 2 * LINEBUF;
     static constexpr int SMEM_BYTES = SMEM_DOUBLES * 8;
+    static_assert(P >= GX && PP >= GY * P, "pitches too small");
+    static_assert(OZ == 0 || OZ == 2, "z lines must keep gx fastest across lanes");
 };
 
-template <int VEC>
-__device__ __forceinline__ void cp_async(double *smem_dst, const double *gsrc) {
+__device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-    if (VEC == 2)
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gsrc) : "memory");
-    else
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gsrc) : "memory");
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gsrc) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int PENDING>
@@ -155,9 +149,11 @@ __device__ __forceinline__ void lax_friedrichs(const double (&Qown)[DG_NV], cons
 // ------------------------------------------------------------------------------------------------
 template <class C, int AX>
 struct Axis {
-    static constexpr int S = (AX == 0) ? 1 : (AX == 1) ? C::P : C::GY * C::P;          // shared stride along the line
+    static constexpr int S = (AX == 0) ? 1 : (AX == 1) ? C::P : C::PP;                 // shared stride along the line
     static constexpr int Ca = (AX == 0) ? C::CX : (AX == 1) ? C::CY : C::CZ;           // face nodes of a brick side
     static constexpr int T1 = (AX == 0) ? C::GY : C::GX;
+    static constexpr int T2 = (AX == 2) ? C::GY : C::GZ;
+    static constexpr int ORD = (AX == 0) ? C::OX : (AX == 1) ? C::OY : C::OZ;
     static constexpr int B = (AX == 0) ? C::BX : (AX == 1) ? C::BY : C::BZ;            // elements along the axis
     static constexpr int TBASE = (AX == 0) ? 0 : (AX == 1) ? 2 * DG_NV * C::CX : 2 * DG_NV * (C::CX + C::CY);
     static constexpr bool MULTI = B > 1;
@@ -171,47 +167,64 @@ __device__ __forceinline__ constexpr int var_of_slot(int s) {
 
 struct Geo {
     int base;   // shared-memory offset (doubles, inside one variable plane) of node 0 of the line
-    int c;      // face-node index of the line on the brick side
+    int c;      // face-node index of the line on the brick side (lane order: this is how the traces are stored)
     int e;      // element along the axis
+    int t1, t2; // transverse node indices
 };
 
 template <class C, int AX>
 __device__ __forceinline__ Geo make_geo(int l) {
     using A = Axis<C, AX>;
-    constexpr int N = C::N;
+    constexpr int N = C::N, T1 = A::T1, T2 = A::T2, B = A::B;
     Geo g;
-    g.e = (A::B == 1) ? 0 : l / A::Ca;
-    g.c = l - g.e * A::Ca;
-    const int t2 = g.c / A::T1, t1 = g.c - t2 * A::T1;
-    if (AX == 0) g.base = (t2 * C::GY + t1) * C::P + g.e * N;
-    else if (AX == 1) g.base = (t2 * C::GY + g.e * N) * C::P + t1;
-    else g.base = (g.e * N * C::GY + t2) * C::P + t1;
+    if (A::ORD == 0) {
+        g.t1 = l % T1;
+        g.t2 = (l / T1) % T2;
+        g.e = l / (T1 * T2);
+        g.c = g.t2 * T1 + g.t1;
+    } else if (A::ORD == 1) {
+        g.t2 = l % T2;
+        g.t1 = (l / T2) % T1;
+        g.e = l / (T1 * T2);
+        g.c = g.t1 * T2 + g.t2;
+    } else if (A::ORD == 2) {
+        g.t1 = l % T1;
+        g.e = (l / T1) % B;
+        g.t2 = l / (T1 * B);
+        g.c = g.t2 * T1 + g.t1;
+    } else {
+        g.t2 = l % T2;
+        g.e = (l / T2) % B;
+        g.t1 = l / (T2 * B);
+        g.c = g.t1 * T2 + g.t2;
+    }
+    if (AX == 0) g.base = g.t2 * C::PP + g.t1 * C::P + g.e * N;
+    else if (AX == 1) g.base = g.t2 * C::PP + g.e * N * C::P + g.t1;
+    else g.base = g.e * N * C::PP + g.t2 * C::P + g.t1;
     return g;
 }
 
 // Is the line inside a ragged (last) brick of ext0 x ext1 x ext2 elements?
 template <class C, int AX>
 __device__ __forceinline__ bool line_inside(const Geo &g, int ext0, int ext1, int ext2) {
-    using A = Axis<C, AX>;
-    const int t2 = g.c / A::T1, t1 = g.c - t2 * A::T1;
     const int lim1 = ((AX == 0) ? ext1 : ext0) * C::N, lim2 = ((AX == 2) ? ext1 : ext2) * C::N;
     const int exta = (AX == 0) ? ext0 : (AX == 1) ? ext1 : ext2;
-    return t1 < lim1 && t2 < lim2 && g.e < exta;
+    return g.t1 < lim1 && g.t2 < lim2 && g.e < exta;
 }
 
 // P0: enqueue the asynchronous copy of one dense HBM slot [5][GZ][GY][GX] into the pitched shared planes.
+// Thread tid < L = BZ * GX * GY owns one node of a group of BZ consecutive z planes; the 5 N groups of the
+// slot are then a fixed stride apart on both sides, so the whole copy is 5 N instructions per thread with
+// immediate offsets (consecutive lanes read consecutive doubles of HBM).
 template <class C>
 __device__ __forceinline__ void stage_in(double *dst, const double *src, int tid) {
-    constexpr int CPR = C::GX / C::VEC;                    // chunks per row
-    constexpr int TOTAL = DG_NV * C::ROWS * CPR;
-#pragma unroll 1
-    for (int k = tid; k < TOTAL; k += C::THREADS) {
-        if (C::P == C::GX) {
-            cp_async<C::VEC>(dst + k * C::VEC, src + k * C::VEC);
-        } else {
-            const int row = k / CPR;
-            cp_async<C::VEC>(dst + k * C::VEC + row * (C::P - C::GX), src + k * C::VEC);
-        }
+    if (tid < C::L) {
+        const int pz = tid / (C::GX * C::GY), k = tid - pz * (C::GX * C::GY);
+        const int gy = k / C::GX, gx = k - gy * C::GX;
+        double *d = dst + pz * C::PP + gy * C::P + gx;
+        const double *g = src + tid;
+#pragma unroll
+        for (int j = 0; j < DG_NV * C::N; ++j) cp_async8(d + j * (C::BZ * C::PP), g + j * C::L);
     }
 }
 
@@ -315,6 +328,7 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
     using A = Axis<C, AX>;
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE, L = C::L, S = A::S, Ca = A::Ca;
     const bool first = g.e == 0, last = g.e == exta - 1;
+    const int lb = g.e * Ca + g.c;   // slot of this line in the hand-over buffers
     double Hlo[NV], Hhi[NV];
     load_halo<C, AX>(g, act, exta, halo_lo, halo_hi, Hlo, Hhi);
 
@@ -336,7 +350,7 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
         }
         if (A::MULTI) {
 #pragma unroll
-            for (int n = 0; n < NV; ++n) Tms[n * L + l] = Tm[n];
+            for (int n = 0; n < NV; ++n) Tms[n * L + lb] = Tm[n];
         }
     }
     if (A::MULTI) __syncthreads();
@@ -346,12 +360,12 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
     if (act) {
         if (A::MULTI && !last) {
 #pragma unroll
-            for (int n = 0; n < NV; ++n) Hhi[n] = Tms[n * L + l + Ca];   // T- of the next element of this brick
+            for (int n = 0; n < NV; ++n) Hhi[n] = Tms[n * L + lb + Ca];   // T- of the next element of this brick
         }
         lax_friedrichs(Tp, Hhi, 1.0, a.gamma, a.gm1, Fp);
         if (A::MULTI) {
 #pragma unroll
-            for (int n = 0; n < NV; ++n) Fss[n * L + l] = Fp[n];
+            for (int n = 0; n < NV; ++n) Fss[n * L + lb] = Fp[n];
         }
         if (first) lax_friedrichs(Tm, Hlo, -1.0, a.gamma, a.gm1, Fm);
     }
@@ -360,7 +374,7 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
     if (act) {
         if (A::MULTI && !first) {
 #pragma unroll
-            for (int n = 0; n < NV; ++n) Fm[n] = Fss[n * L + l - Ca];
+            for (int n = 0; n < NV; ++n) Fm[n] = Fss[n * L + lb - Ca];
         }
         // ------------- PC: lift (2/h and 1/w folded into the tables) starts the accumulators -----------
         double V[NV][N];
@@ -411,7 +425,7 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
                 }
         } else {
             // z lines: consecutive threads hold consecutive (gx, gy), so HBM accesses coalesce
-            const size_t g0 = qbase + (size_t)(g.e * N) * (C::GY * C::GX) + g.c;   // node 0 of the line, variable 0
+            const size_t g0 = qbase + (size_t)(g.e * N) * (C::GY * C::GX) + g.t2 * C::GX + g.t1;   // node 0, variable 0
             if (MODE == DG_MODE_RESIDUAL) {
 #pragma unroll
                 for (int s = 0; s < NV; ++s)
@@ -434,8 +448,8 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
                         const size_t go = g0 + (size_t)n * C::NODES + (size_t)i * (C::GY * C::GX);
                         const double Kn = fma(cR, V[s][i], K0[n * PLANE + i * S]);
                         const double Qn = fma(rkB, Kn, Q0w[n * PLANE + i * S]);
-                        a.K[go] = Kn;
-                        a.Q[go] = Qn;
+                        __stcs(a.K + go, Kn);   // streaming: written once, not read again in this stage
+                        __stcs(a.Q + go, Qn);
                         Q0w[n * PLANE + i * S] = Qn;
                         tp = fma(a.ops.lp[i], Qn, tp);
                         tm = fma(a.ops.lm[i], Qn, tm);
@@ -480,7 +494,7 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
         if (readK) stage_in<C>(Ks, a.K + qbase, tid);
         cp_async_commit();
         const int next = brick + a.grid;
-        if (next < nbricks) prefetch_brick<C>(a, next, tid, readK, MODE != DG_MODE_TRACES);
+        if (next < nbricks && (a.flags & 2)) prefetch_brick<C>(a, next, tid, readK, MODE != DG_MODE_TRACES);
 
         const int ext0 = min(C::BX, a.nx - bxi * C::BX);   // elements of this brick per axis (ragged last brick)
         const int ext1 = min(C::BY, a.ny - byi * C::BY);
@@ -503,6 +517,8 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
             axis_pass<C, 1, MODE>(a, gy, l, acty, ext1, halo_source<C, 1>(a, bxi, byi, bzi, 0),
                                   halo_source<C, 1>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, cR, qbase, Tbrick);
             __syncthreads();
+            // the brick that takes this block's place: ask L2 for its data now, about a third of a brick ahead
+            if (next < nbricks && !(a.flags & 3)) prefetch_brick<C>(a, next, tid, readK, true);
             axis_pass<C, 2, MODE>(a, gz, l, actz, ext2, halo_source<C, 2>(a, bxi, byi, bzi, 0),
                                   halo_source<C, 2>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, cR, qbase, Tbrick);
         } else {
@@ -641,43 +657,43 @@ constexpr DgKernelTable make_table() {
                          &prepare<C>, &launch_stage<C>, &launch_layout<C>, &launch_wavespeed<C>};
 }
 
-// Brick shapes per N (default first): Cfg<N, BX, BY, BZ, min blocks per SM>.
-// DESIGN.md "brick shapes" explains the choice.
+// Variants per N (default first): Cfg<N, BX, BY, BZ, min blocks per SM, RELOAD, P, PP, OX, OY, OZ>.
+// DESIGN.md "brick shapes" and "shared-memory layout" explain the choices.
 #if DG_N == 2
-using V0 = Cfg<2, 4, 4, 4, 2, 0>;
-using V1 = Cfg<2, 4, 4, 4, 3, 1>;
-using V2 = Cfg<2, 4, 4, 2, 4, 0>;
-using V3 = Cfg<2, 4, 4, 2, 6, 1>;
+using V0 = Cfg<2, 4, 4, 2, 6, 1, 9, 76, 1, 1, 2>;
+using V1 = Cfg<2, 4, 4, 2, 4, 0, 9, 76, 1, 1, 2>;
+using V2 = Cfg<2, 4, 4, 4, 3, 1, 8, 65, 1, 0, 0>;
+using V3 = Cfg<2, 4, 4, 4, 2, 0, 8, 65, 1, 0, 0>;
 #elif DG_N == 3
-using V0 = Cfg<3, 4, 4, 2, 2, 1>;
-using V1 = Cfg<3, 4, 4, 2, 1, 0>;
-using V2 = Cfg<3, 2, 2, 2, 5, 0>;
-using V3 = Cfg<3, 2, 2, 2, 7, 1>;
+using V0 = Cfg<3, 2, 2, 2, 7, 1, 6, 38, 2, 0, 0>;
+using V1 = Cfg<3, 2, 2, 2, 5, 0, 6, 38, 2, 0, 0>;
+using V2 = Cfg<3, 4, 4, 2, 2, 1, 12, 156, 3, 0, 0>;
+using V3 = Cfg<3, 4, 4, 2, 1, 0, 12, 156, 3, 0, 0>;
 #elif DG_N == 4
-using V0 = Cfg<4, 2, 2, 2, 3, 1>;
-using V1 = Cfg<4, 2, 2, 2, 2, 0>;
-using V2 = Cfg<4, 2, 2, 1, 4, 0>;
-using V3 = Cfg<4, 2, 2, 1, 6, 1>;
+using V0 = Cfg<4, 2, 2, 2, 3, 1, 9, 74, 1, 1, 2>;
+using V1 = Cfg<4, 2, 2, 2, 3, 0, 9, 74, 1, 1, 2>;
+using V2 = Cfg<4, 2, 2, 1, 6, 1, 8, 65, 3, 0, 0>;
+using V3 = Cfg<4, 2, 2, 1, 4, 0, 8, 65, 3, 0, 0>;
 #elif DG_N == 5
-using V0 = Cfg<5, 1, 2, 2, 4, 1>;
-using V1 = Cfg<5, 1, 2, 2, 3, 1>;
-using V2 = Cfg<5, 1, 2, 2, 2, 0>;
-using V3 = Cfg<5, 1, 2, 3, 3, 1>;
+using V0 = Cfg<5, 1, 2, 2, 4, 1, 0, 0, 0, 1, 0>;
+using V1 = Cfg<5, 1, 2, 2, 3, 0, 0, 0, 0, 1, 0>;
+using V2 = Cfg<5, 1, 2, 3, 3, 1, 0, 0, 0, 1, 0>;
+using V3 = Cfg<5, 1, 2, 3, 2, 0, 0, 0, 0, 1, 0>;
 #elif DG_N == 6
-using V0 = Cfg<6, 1, 1, 2, 4, 1>;
-using V1 = Cfg<6, 1, 1, 2, 3, 0>;
-using V2 = Cfg<6, 1, 2, 2, 2, 1>;
-using V3 = Cfg<6, 1, 1, 1, 8, 1>;
+using V0 = Cfg<6, 1, 1, 2, 4, 1, 6, 38, 1, 0, 0>;
+using V1 = Cfg<6, 1, 1, 2, 3, 0, 6, 38, 1, 0, 0>;
+using V2 = Cfg<6, 1, 2, 2, 2, 1, 6, 75, 0, 3, 0>;
+using V3 = Cfg<6, 1, 2, 2, 2, 0, 6, 75, 0, 3, 0>;
 #elif DG_N == 7
-using V0 = Cfg<7, 1, 1, 2, 3, 1>;
-using V1 = Cfg<7, 1, 1, 2, 2, 0>;
-using V2 = Cfg<7, 1, 2, 2, 1, 0>;
-using V3 = Cfg<7, 1, 1, 1, 6, 1>;
+using V0 = Cfg<7, 1, 1, 2, 3, 1, 7, 55, 1, 0, 0>;
+using V1 = Cfg<7, 1, 1, 2, 2, 0, 7, 55, 1, 0, 0>;
+using V2 = Cfg<7, 1, 1, 1, 6, 1, 7, 55, 1, 0, 0>;
+using V3 = Cfg<7, 1, 1, 1, 4, 0, 7, 55, 1, 0, 0>;
 #elif DG_N == 8
-using V0 = Cfg<8, 1, 1, 2, 2, 1>;
-using V1 = Cfg<8, 1, 1, 2, 2, 0>;
-using V2 = Cfg<8, 1, 1, 1, 4, 1>;
-using V3 = Cfg<8, 1, 1, 1, 4, 0>;
+using V0 = Cfg<8, 1, 1, 2, 2, 1, 8, 65, 1, 1, 0>;
+using V1 = Cfg<8, 1, 1, 2, 2, 0, 8, 65, 1, 1, 0>;
+using V2 = Cfg<8, 1, 1, 1, 4, 1, 8, 65, 1, 0, 0>;
+using V3 = Cfg<8, 1, 1, 1, 4, 0, 8, 65, 1, 0, 0>;
 #else
 #error "DG_N must be 2..8"
 #endif
