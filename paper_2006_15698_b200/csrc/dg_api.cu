@@ -93,11 +93,22 @@ void build_device_ops(int N, const double g[3], DgOps &d) {
         d.lm[i] = (double)o.lm[i];
         for (int a = 0; a < 3; ++a) {
             const long double ga = (long double)g[a];
-            d.lpg[a][i] = (double)(ga * o.lp[i] / o.w[i]);
-            d.lmg[a][i] = (double)(ga * o.lm[i] / o.w[i]);
+            d.lpg[a][i] = (double)(0.5L * ga * o.lp[i] / o.w[i]);   // 1/2: the kernel's interface flux is 2 F*
+            d.lmg[a][i] = (double)(0.5L * ga * o.lm[i] / o.w[i]);
             for (int q = 0; q < N; ++q) d.Dg[a][q][i] = (double)(ga * o.w[q] * o.D[q][i] / o.w[i]);
         }
     }
+}
+
+// The same tables with the time step folded in: the stage kernel then accumulates dt * L(Q) directly.
+void scale_ops(const DgOps &in, double dt, DgOps &out) {
+    out = in;
+    for (int a = 0; a < 3; ++a)
+        for (int i = 0; i < DG_NMAX; ++i) {
+            out.lpg[a][i] = dt * in.lpg[a][i];
+            out.lmg[a][i] = dt * in.lmg[a][i];
+            for (int q = 0; q < DG_NMAX; ++q) out.Dg[a][q][i] = dt * in.Dg[a][q][i];
+        }
 }
 
 // Carpenter-Kennedy (5,4) 2N-storage Runge-Kutta, "LSERK45" (reading R9).
@@ -397,9 +408,12 @@ int dg_rk_step(dg_ctx *c, double dt, int nsteps) {
     if (!c) return DG_EINVAL;
     if (nsteps < 0 || !std::isfinite(dt)) return fail(c, DG_EINVAL, "nsteps < 0 or dt not finite");
     if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_rk_step needs dg_bind and dg_set_state first");
+    DgOps scaled;
+    scale_ops(c->ops, dt, scaled);
     for (int step = 0; step < nsteps; ++step) {
         for (int s = 0; s < 5; ++s) {
             DgStageArgs a = stage_args(c, DG_MODE_STAGE);
+            a.ops = scaled;
             a.rkA = (double)kRkA[s];
             a.rkB = (double)kRkB[s];
             a.dt = dt;

@@ -10,12 +10,13 @@
 
 // 1-D operators of the collocated Gauss-Legendre Lagrange basis, built on the
 // host in long double (dg_api.cu) with the constant geometric factor 2/h_a of each axis
-// folded in, rounded to double once.  They travel inside the kernel
+// folded in, rounded to double once.  In the Runge-Kutta stage kernel Dg, lpg and lmg
+// are additionally multiplied by the time step (dg_rk_step), so the kernel accumulates dt * L(Q).  They travel inside the kernel
 // arguments (constant bank; per context, so contexts with different meshes can coexist).
 struct DgOps {
     double Dg[3][DG_NMAX][DG_NMAX];     // Dg[a][q][i] = (2/h_a) w_q l_i'(xi_q) / w_i   (eq (5) 2nd term / mass)
-    double lpg[3][DG_NMAX];             // (2/h_a) l_i(+1) / w_i                        (lift / mass)
-    double lmg[3][DG_NMAX];             // (2/h_a) l_i(-1) / w_i
+    double lpg[3][DG_NMAX];             // 1/2 (2/h_a) l_i(+1) / w_i     (lift / mass; the kernel forms 2 F*)
+    double lmg[3][DG_NMAX];             // 1/2 (2/h_a) l_i(-1) / w_i
     double lp[DG_NMAX], lm[DG_NMAX];    // l_i(+1), l_i(-1)                             (face traces)
 };
 

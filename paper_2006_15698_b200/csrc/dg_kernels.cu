@@ -118,28 +118,30 @@ __device__ __forceinline__ void euler_flux_normal(const double (&Q)[DG_NV], doub
                                                   double &vel, double &pres, double &oneOrho) {
     oneOrho = rcp_pos(Q[0]);
     vel = Q[1] * oneOrho;
-    const double ub = Q[2] * oneOrho, uc = Q[3] * oneOrho;
-    pres = gm1 * (Q[4] - 0.5 * Q[0] * (vel * vel + ub * ub + uc * uc));
-    F[0] = Q[0] * vel;
-    F[1] = Q[1] * vel + pres;
+    // 1/2 rho |u|^2 = 1/2 |rho u|^2 / rho
+    const double m2 = fma(Q[3], Q[3], fma(Q[2], Q[2], Q[1] * Q[1]));
+    pres = gm1 * fma(-0.5, m2 * oneOrho, Q[4]);
+    F[0] = Q[1];                                    // rho u_a
+    F[1] = fma(Q[1], vel, pres);
     F[2] = Q[2] * vel;
     F[3] = Q[3] * vel;
     F[4] = (Q[4] + pres) * vel;
 }
 
-// Local Lax-Friedrichs flux (reading R3), rotated slots as above:
-//   F* = 1/2 (F(QL) + F(QR)) - 1/2 lam (QR - QL),  lam = max(|u_a^L| + c_L, |u_a^R| + c_R)
+// Local Lax-Friedrichs flux (reading R3), rotated slots as above, returned DOUBLED
+// (the factor 1/2 is folded into the lift tables):
+//   2 F* = F(QL) + F(QR) - lam (QR - QL),  lam = max(|u_a^L| + c_L, |u_a^R| + c_R)
 // written for (own, other) with sgn = +1 when own is the left state, -1 when it is the right one.
-__device__ __forceinline__ void lax_friedrichs(const double (&Qown)[DG_NV], const double (&Qoth)[DG_NV], double sgn,
-                                               double gamma, double gm1, double (&Fs)[DG_NV]) {
+__device__ __forceinline__ void lax_friedrichs2(const double (&Qown)[DG_NV], const double (&Qoth)[DG_NV], double sgn,
+                                                double gamma, double gm1, double (&Fs)[DG_NV]) {
     double Fa[DG_NV], Fb[DG_NV], ua, ub, pa, pb, ra, rb;
     euler_flux_normal(Qown, gm1, Fa, ua, pa, ra);
     euler_flux_normal(Qoth, gm1, Fb, ub, pb, rb);
     const double lama = fabs(ua) + sqrt_pos(gamma * pa * ra);
     const double lamb = fabs(ub) + sqrt_pos(gamma * pb * rb);
-    const double hl = 0.5 * sgn * ((lama > lamb) ? lama : lamb);
+    const double sl = sgn * ((lama > lamb) ? lama : lamb);
 #pragma unroll
-    for (int n = 0; n < DG_NV; ++n) Fs[n] = 0.5 * (Fa[n] + Fb[n]) - hl * (Qoth[n] - Qown[n]);
+    for (int n = 0; n < DG_NV; ++n) Fs[n] = fma(-sl, Qoth[n] - Qown[n], Fa[n] + Fb[n]);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -323,7 +325,7 @@ __device__ __forceinline__ void load_halo(const Geo &g, bool act, int exta, cons
 template <class C, int AX, int MODE>
 __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, int l, bool act, int exta,
                                           const double *halo_lo, const double *halo_hi, double *Qs, double *Ks,
-                                          double *Tms, double *Fss, bool readK, double cR, size_t qbase,
+                                          double *Tms, double *Fss, bool readK, size_t qbase,
                                           double *Tbrick) {
     using A = Axis<C, AX>;
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE, L = C::L, S = A::S, Ca = A::Ca;
@@ -362,12 +364,12 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
 #pragma unroll
             for (int n = 0; n < NV; ++n) Hhi[n] = Tms[n * L + lb + Ca];   // T- of the next element of this brick
         }
-        lax_friedrichs(Tp, Hhi, 1.0, a.gamma, a.gm1, Fp);
+        lax_friedrichs2(Tp, Hhi, 1.0, a.gamma, a.gm1, Fp);
         if (A::MULTI) {
 #pragma unroll
             for (int n = 0; n < NV; ++n) Fss[n * L + lb] = Fp[n];
         }
-        if (first) lax_friedrichs(Tm, Hlo, -1.0, a.gamma, a.gm1, Fm);
+        if (first) lax_friedrichs2(Tm, Hlo, -1.0, a.gamma, a.gm1, Fm);
     }
     if (A::MULTI) __syncthreads();
 
@@ -407,13 +409,13 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
 #pragma unroll
                     for (int i = 0; i < N; ++i) {
                         double *p = K0 + var_of_slot<C, AX>(s) * PLANE + i * S;
-                        *p = fma(rkA, *p, cR * V[s][i]);
+                        *p = fma(rkA, *p, V[s][i]);
                     }
             } else {
 #pragma unroll
                 for (int s = 0; s < NV; ++s)
 #pragma unroll
-                    for (int i = 0; i < N; ++i) K0[var_of_slot<C, AX>(s) * PLANE + i * S] = cR * V[s][i];
+                    for (int i = 0; i < N; ++i) K0[var_of_slot<C, AX>(s) * PLANE + i * S] = V[s][i];
             }
         } else if (AX == 1) {
 #pragma unroll
@@ -421,7 +423,7 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
 #pragma unroll
                 for (int i = 0; i < N; ++i) {
                     double *p = K0 + var_of_slot<C, AX>(s) * PLANE + i * S;
-                    *p = fma(cR, V[s][i], *p);
+                    *p += V[s][i];
                 }
         } else {
             // z lines: consecutive threads hold consecutive (gx, gy), so HBM accesses coalesce
@@ -433,7 +435,7 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
                     for (int i = 0; i < N; ++i) {
                         const int n = var_of_slot<C, AX>(s);
                         a.Rout[g0 + (size_t)n * C::NODES + (size_t)i * (C::GY * C::GX)] =
-                            fma(cR, V[s][i], K0[n * PLANE + i * S]);
+                            K0[n * PLANE + i * S] + V[s][i];
                     }
             } else {
                 const double rkB = a.rkB;
@@ -442,20 +444,30 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
 #pragma unroll
                 for (int s = 0; s < NV; ++s) {
                     const int n = var_of_slot<C, AX>(s);
-                    double tp = 0.0, tm = 0.0;
+                    double Qn[N];
 #pragma unroll
                     for (int i = 0; i < N; ++i) {
                         const size_t go = g0 + (size_t)n * C::NODES + (size_t)i * (C::GY * C::GX);
-                        const double Kn = fma(cR, V[s][i], K0[n * PLANE + i * S]);
-                        const double Qn = fma(rkB, Kn, Q0w[n * PLANE + i * S]);
+                        const double Kn = K0[n * PLANE + i * S] + V[s][i];
+                        const double Qold = C::RELOAD ? Q0w[n * PLANE + i * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : i];
+                        Qn[i] = fma(rkB, Kn, Qold);
                         __stcs(a.K + go, Kn);   // streaming: written once, not read again in this stage
-                        __stcs(a.Q + go, Qn);
-                        Q0w[n * PLANE + i * S] = Qn;
-                        tp = fma(a.ops.lp[i], Qn, tp);
-                        tm = fma(a.ops.lm[i], Qn, tm);
+                        __stcs(a.Q + go, Qn[i]);
+                        Q0w[n * PLANE + i * S] = Qn[i];
                     }
-                    if (first) dst[n * Ca] = tm;
-                    if (last) dst[(NV + n) * Ca] = tp;
+                    // PE for the z faces: traces of the updated Q, only at the ends that lie on the brick boundary
+                    if (first) {
+                        double tm = 0.0;
+#pragma unroll
+                        for (int i = 0; i < N; ++i) tm = fma(a.ops.lm[i], Qn[i], tm);
+                        dst[n * Ca] = tm;
+                    }
+                    if (last) {
+                        double tp = 0.0;
+#pragma unroll
+                        for (int i = 0; i < N; ++i) tp = fma(a.ops.lp[i], Qn[i], tp);
+                        dst[(NV + n) * Ca] = tp;
+                    }
                 }
             }
         }
@@ -478,7 +490,6 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
     const int tid = threadIdx.x, l = tid;
     const int nbricks = a.nbx * a.nby * a.nbz;
     const bool readK = (MODE == DG_MODE_STAGE) && (a.rkA != 0.0);
-    const double cR = (MODE == DG_MODE_STAGE) ? a.dt : 1.0;
     const Geo gx = make_geo<C, 0>(l), gy = make_geo<C, 1>(l), gz = make_geo<C, 2>(l);
     const bool inL = l < L;
 
@@ -512,15 +523,15 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
             cp_async_wait<0>();
             __syncthreads();
             axis_pass<C, 0, MODE>(a, gx, l, actx, ext0, halo_source<C, 0>(a, bxi, byi, bzi, 0),
-                                  halo_source<C, 0>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, cR, qbase, Tbrick);
+                                  halo_source<C, 0>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, qbase, Tbrick);
             __syncthreads();
             axis_pass<C, 1, MODE>(a, gy, l, acty, ext1, halo_source<C, 1>(a, bxi, byi, bzi, 0),
-                                  halo_source<C, 1>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, cR, qbase, Tbrick);
+                                  halo_source<C, 1>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, qbase, Tbrick);
             __syncthreads();
             // the brick that takes this block's place: ask L2 for its data now, about a third of a brick ahead
             if (next < nbricks && !(a.flags & 3)) prefetch_brick<C>(a, next, tid, readK, true);
             axis_pass<C, 2, MODE>(a, gz, l, actz, ext2, halo_source<C, 2>(a, bxi, byi, bzi, 0),
-                                  halo_source<C, 2>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, cR, qbase, Tbrick);
+                                  halo_source<C, 2>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, qbase, Tbrick);
         } else {
             cp_async_wait<0>();
             __syncthreads();
