@@ -63,7 +63,7 @@ int dg_create(dg_ctx **out, int nx, int ny, int nz, int p, double gamma, const d
  * bx=by=bz=0 restores the default.  Changes layout sizes, so it is refused after dg_bind. */
 int dg_set_brick(dg_ctx *ctx, int bx, int by, int bz);
 
-/* Number of stage-kernel variants (brick shape x buffering depth x residency) compiled into the
+/* Number of stage-kernel variants (brick shape x shared-memory layout x residency) compiled into the
  * library for degree p; 0 when p is outside 1..7.  Variant 0 is the default. */
 int dg_variant_count(int p);
 
@@ -111,9 +111,15 @@ int dg_nodes(const dg_ctx *ctx, double *xi, double *w);
 unsigned long long dg_launch_count(const dg_ctx *ctx);
 
 /* Launch geometry of the fused stage kernel, for reports: out[0..7] = brick elements bx,by,bz,
- * threads per block, dynamic shared bytes per block, grid size (persistent blocks once bound, bricks before), internal (padded)
+ * threads per block, dynamic shared bytes per block, resident blocks of the whole GPU (once bound; bricks before), internal (padded)
  * state length in doubles / 2^20 rounded up, face-trace doubles per brick. */
 int dg_kernel_info(const dg_ctx *ctx, long long out[8]);
+
+/* Self-test of the two device arithmetic helpers the kernels use instead of IEEE division and square
+ * root (Newton-corrected hardware seeds, no slow-path branches): rcp_out[i] = 1/x[i] and
+ * sqrt_out[i] = sqrt(x[i]) for n positive normal doubles.  All three are DEVICE pointers; the call is
+ * enqueued on `cuda_stream` (cudaStream_t as void*).  Test entry, not part of the hot path. */
+int dg_selftest_fastmath(const double *x_dev, double *rcp_out_dev, double *sqrt_out_dev, size_t n, void *cuda_stream);
 
 /* Release the context (never the borrowed workspace).  NULL is accepted. */
 int dg_destroy(dg_ctx *ctx);

@@ -31,10 +31,25 @@ SYMBOLS = {
     "dg_nodes": (ctypes.c_int, [ctypes.c_void_p, _DP, _DP]),
     "dg_launch_count": (ctypes.c_ulonglong, [ctypes.c_void_p]),
     "dg_kernel_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_longlong)]),
+    "dg_selftest_fastmath": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t,
+                                            ctypes.c_void_p]),
     "dg_destroy": (ctypes.c_int, [ctypes.c_void_p]),
     "dg_last_error": (ctypes.c_char_p, [ctypes.c_void_p]),
 }
 ERRORS = {1: "DG_EINVAL", 2: "DG_EUNSUPPORTED", 3: "DG_ENOMEM", 4: "DG_ECUDA", 5: "DG_ESTATE"}
+
+
+def selftest_fastmath(x):
+    """(1/x, sqrt(x)) of a float64 CUDA tensor as the kernels compute them (dg_selftest_fastmath)."""
+    import torch
+    lib = load_library()
+    assert x.is_cuda and x.dtype == torch.float64 and x.is_contiguous()
+    r, q = torch.empty_like(x), torch.empty_like(x)
+    rc = lib.dg_selftest_fastmath(x.data_ptr(), r.data_ptr(), q.data_ptr(), x.numel(),
+                                  torch.cuda.current_stream(x.device).cuda_stream)
+    if rc != 0:
+        raise DGError(rc, "dg_selftest_fastmath")
+    return r, q
 
 
 class DGError(RuntimeError):

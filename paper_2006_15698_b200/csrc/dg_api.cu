@@ -136,6 +136,14 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 }  // namespace
 
+__global__ void dg_fastmath_kernel(const double *x, double *r, double *q, size_t n) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) {
+        r[i] = rcp_pos(x[i]);
+        q[i] = sqrt_pos(x[i]);
+    }
+}
+
 struct dg_ctx {
     int nx, ny, nz, p, N;
     double gamma;
@@ -454,6 +462,13 @@ int dg_kernel_info(const dg_ctx *c, long long out[8]) {
     out[6] = (long long)((c->int_len + (1u << 20) - 1) >> 20);
     out[7] = c->kt->tslot;
     return DG_OK;
+}
+
+int dg_selftest_fastmath(const double *x, double *r, double *q, size_t n, void *stream) {
+    if (!x || !r || !q) return DG_EINVAL;
+    if (n == 0) return DG_OK;
+    dg_fastmath_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(x, r, q, n);
+    return cudaGetLastError() == cudaSuccess ? DG_OK : DG_ECUDA;
 }
 
 int dg_destroy(dg_ctx *c) {

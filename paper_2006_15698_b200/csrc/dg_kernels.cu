@@ -90,26 +90,6 @@ __device__ __forceinline__ void l2_prefetch(const void *ptr, unsigned bytes) {
 // Compiler-level fence on memory operations: bounds how far loads are hoisted (register pressure).
 __device__ __forceinline__ void sched_fence() { asm volatile("" ::: "memory"); }
 
-// Branch-free reciprocal and square root for positive, normal arguments (densities, gamma p / rho):
-// hardware seed (MUFU.RCP64H / MUFU.RSQ64H), one cubic and one quadratic correction; the result is within
-// about one unit in the last place (tests/test_gpu_parity.py::test_fast_math measures it), with none of
-// the slow-path branches of the IEEE-rounded library routines.
-__device__ __forceinline__ double rcp_pos(double x) {
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-    const double e = fma(-x, r, 1.0);
-    r = fma(r, fma(e, e, e), r);                    // r (1 + e + e^2)
-    return fma(r, fma(-x, r, 1.0), r);
-}
-__device__ __forceinline__ double sqrt_pos(double x) {
-    double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    const double e = fma(-(x * y), y, 1.0);         // 1 - x y^2
-    y = fma(y, e * fma(0.375, e, 0.5), y);          // y (1 + e/2 + 3 e^2/8)
-    const double s = x * y;
-    return fma(fma(-s, s, x), 0.5 * y, s);          // s + (x - s^2) / (2 sqrt x)
-}
-
 // Euler flux along the face/line normal, eq (2)-(3) (listing lines 186-217), for a state
 // whose momentum components have been ROTATED so that slot 1 is the normal one:
 //   slots = (rho, rho u_a, rho u_b, rho u_c, rho E),  (a,b,c) = (x,y,z), (y,z,x) or (z,x,y).
@@ -522,6 +502,32 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
         if (MODE != DG_MODE_TRACES) {
             cp_async_wait<0>();
             __syncthreads();
+            if (a.flags & 8) {   // EXPERIMENT: memory traffic of a stage without its arithmetic
+                if (next < nbricks) prefetch_brick<C>(a, next, tid, readK, true);
+                if (actz) {
+                    double h = 0.0;
+                    const double *hl = halo_source<C, 2>(a, bxi, byi, bzi, 0), *hh = halo_source<C, 2>(a, bxi, byi, bzi, 1);
+                    const double *xl = halo_source<C, 0>(a, bxi, byi, bzi, 0), *xh = halo_source<C, 0>(a, bxi, byi, bzi, 1);
+                    const double *yl = halo_source<C, 1>(a, bxi, byi, bzi, 0), *yh = halo_source<C, 1>(a, bxi, byi, bzi, 1);
+                    for (int s = 0; s < NV; ++s) {
+                        if (gz.e == 0) h += hl[s * C::CZ + gz.c];
+                        if (gz.e == ext2 - 1) h += hh[s * C::CZ + gz.c];
+                        if (gx.e == 0) h += xl[s * C::CX + gx.c];
+                        if (gx.e == ext0 - 1) h += xh[s * C::CX + gx.c];
+                        if (gy.e == 0) h += yl[s * C::CY + gy.c];
+                        if (gy.e == ext1 - 1) h += yh[s * C::CY + gy.c];
+                    }
+                    const size_t g0 = qbase + (size_t)(gz.e * C::N) * (C::GY * C::GX) + gz.t2 * C::GX + gz.t1;
+                    for (int n = 0; n < NV; ++n)
+                        for (int i = 0; i < C::N; ++i) {
+                            const size_t go = g0 + (size_t)n * C::NODES + (size_t)i * (C::GY * C::GX);
+                            const double Kn = Ks[gz.base + n * PLANE + i * C::PP] * 0.5 + 1e-300 * h;
+                            __stcs(a.K + go, Kn);
+                            __stcs(a.Q + go, Qs[gz.base + n * PLANE + i * C::PP] + 1e-300 * Kn);
+                        }
+                    boundary_traces<C, 2>(gz, actz, ext2, Qs, Tbrick, a);
+                }
+            } else {
             axis_pass<C, 0, MODE>(a, gx, l, actx, ext0, halo_source<C, 0>(a, bxi, byi, bzi, 0),
                                   halo_source<C, 0>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, qbase, Tbrick);
             __syncthreads();
@@ -532,6 +538,7 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
             if (next < nbricks && !(a.flags & 3)) prefetch_brick<C>(a, next, tid, readK, true);
             axis_pass<C, 2, MODE>(a, gz, l, actz, ext2, halo_source<C, 2>(a, bxi, byi, bzi, 0),
                                   halo_source<C, 2>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, qbase, Tbrick);
+            }
         } else {
             cp_async_wait<0>();
             __syncthreads();
@@ -672,34 +679,34 @@ constexpr DgKernelTable make_table() {
 // DESIGN.md "brick shapes" and "shared-memory layout" explain the choices.
 #if DG_N == 2
 using V0 = Cfg<2, 4, 4, 2, 6, 1, 9, 76, 1, 1, 2>;
-using V1 = Cfg<2, 4, 4, 2, 4, 0, 9, 76, 1, 1, 2>;
+using V1 = Cfg<2, 4, 4, 2, 6, 0, 9, 76, 1, 1, 2>;
 using V2 = Cfg<2, 4, 4, 4, 3, 1, 8, 65, 1, 0, 0>;
-using V3 = Cfg<2, 4, 4, 4, 2, 0, 8, 65, 1, 0, 0>;
+using V3 = Cfg<2, 4, 4, 4, 3, 0, 8, 65, 1, 0, 0>;
 #elif DG_N == 3
-using V0 = Cfg<3, 2, 2, 2, 7, 1, 6, 38, 2, 0, 0>;
-using V1 = Cfg<3, 2, 2, 2, 5, 0, 6, 38, 2, 0, 0>;
-using V2 = Cfg<3, 4, 4, 2, 2, 1, 12, 156, 3, 0, 0>;
-using V3 = Cfg<3, 4, 4, 2, 1, 0, 12, 156, 3, 0, 0>;
+using V0 = Cfg<3, 4, 4, 2, 2, 1, 12, 156, 3, 0, 0>;
+using V1 = Cfg<3, 2, 2, 2, 7, 0, 6, 38, 2, 0, 0>;
+using V2 = Cfg<3, 2, 2, 2, 7, 1, 6, 38, 2, 0, 0>;
+using V3 = Cfg<3, 4, 4, 2, 2, 0, 12, 156, 3, 0, 0>;
 #elif DG_N == 4
 using V0 = Cfg<4, 2, 2, 2, 3, 1, 9, 74, 1, 1, 2>;
 using V1 = Cfg<4, 2, 2, 2, 3, 0, 9, 74, 1, 1, 2>;
 using V2 = Cfg<4, 2, 2, 1, 6, 1, 8, 65, 3, 0, 0>;
-using V3 = Cfg<4, 2, 2, 1, 4, 0, 8, 65, 3, 0, 0>;
+using V3 = Cfg<4, 2, 2, 1, 6, 0, 8, 65, 3, 0, 0>;
 #elif DG_N == 5
 using V0 = Cfg<5, 1, 2, 2, 4, 1, 0, 0, 0, 1, 0>;
-using V1 = Cfg<5, 1, 2, 2, 3, 0, 0, 0, 0, 1, 0>;
+using V1 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0>;
 using V2 = Cfg<5, 1, 2, 3, 3, 1, 0, 0, 0, 1, 0>;
-using V3 = Cfg<5, 1, 2, 3, 2, 0, 0, 0, 0, 1, 0>;
+using V3 = Cfg<5, 2, 2, 2, 2, 1, 10, 106, 2, 0, 0>;
 #elif DG_N == 6
 using V0 = Cfg<6, 1, 1, 2, 4, 1, 6, 38, 1, 0, 0>;
-using V1 = Cfg<6, 1, 1, 2, 3, 0, 6, 38, 1, 0, 0>;
+using V1 = Cfg<6, 1, 1, 2, 4, 0, 6, 38, 1, 0, 0>;
 using V2 = Cfg<6, 1, 2, 2, 2, 1, 6, 75, 0, 3, 0>;
 using V3 = Cfg<6, 1, 2, 2, 2, 0, 6, 75, 0, 3, 0>;
 #elif DG_N == 7
 using V0 = Cfg<7, 1, 1, 2, 3, 1, 7, 55, 1, 0, 0>;
-using V1 = Cfg<7, 1, 1, 2, 2, 0, 7, 55, 1, 0, 0>;
+using V1 = Cfg<7, 1, 1, 2, 3, 0, 7, 55, 1, 0, 0>;
 using V2 = Cfg<7, 1, 1, 1, 6, 1, 7, 55, 1, 0, 0>;
-using V3 = Cfg<7, 1, 1, 1, 4, 0, 7, 55, 1, 0, 0>;
+using V3 = Cfg<7, 1, 1, 1, 6, 0, 7, 55, 1, 0, 0>;
 #elif DG_N == 8
 using V0 = Cfg<8, 1, 1, 2, 2, 1, 8, 65, 1, 1, 0>;
 using V1 = Cfg<8, 1, 1, 2, 2, 0, 8, 65, 1, 1, 0>;
