@@ -159,14 +159,14 @@ def run_reference(args, rank):
 # ----------------------------------------------------------------------------------------------
 # the CUDA path
 # ----------------------------------------------------------------------------------------------
-def time_workload(workload, K, W, device, dist, sampler_index=None, want_e2e=False):
+def time_workload(workload, K, W, device, dist, sampler_index=None, want_e2e=False, variant=None):
     import torch
     from paper_2006_15698_b200 import DG
     from paper_2006_15698_b200 import inputs as I
     c = I.CONFIGS[workload]
     p, ext, n = c["p"], c["extent"], (c["nx"], c["ny"], c["nz"])
     q = I.make_field(workload, xp=torch, device=device)
-    dg = DG(*n, p, GAMMA, ext, device=device)
+    dg = DG(*n, p, GAMMA, ext, device=device, variant=variant)
     dg.set_state(q)
     dt = I.cfl_dt(dg.max_wavespeed(), p, ext, n, 0.1)
     dof = n[0] * n[1] * n[2] * (p + 1) ** 3
@@ -222,6 +222,22 @@ def time_workload(workload, K, W, device, dist, sampler_index=None, want_e2e=Fal
     del q
     torch.cuda.empty_cache()
     return out
+
+
+def run_variant_sweep(args):
+    """Tuning aid: one JSON line per compiled stage-kernel variant of the workload's degree (1 GPU)."""
+    import torch
+    from paper_2006_15698_b200 import inputs as I
+    from paper_2006_15698_b200.binding import load_library
+    device = torch.device("cuda:0")
+    torch.cuda.set_device(device)
+    peak, _ = measured_peaks()
+    p = I.CONFIGS[args.workload]["p"]
+    for v in range(load_library().dg_variant_count(p)):
+        r = time_workload(args.workload, args.steps, max(3, args.warmup), device, None, variant=v)
+        rate = r["dof"] * STAGES * args.steps / (r["ms"] * 1e-3)
+        print(json.dumps({"workload": args.workload, "variant": v, "kernel": r["kernel"], "value": rate, "unit": UNIT,
+                          "roofline_frac": rate * ALGO_BYTES_PER_DOF_STAGE / 1e9 / peak, "finite": r["finite"]}), flush=True)
 
 
 def run_ours(args, rank, world, local_rank):
@@ -309,11 +325,14 @@ def main():
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--sweep-variants", action="store_true", help="time every compiled variant of --workload")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.sweep_variants:
+        run_variant_sweep(args)
+    elif args.impl == "reference":
         run_reference(args, rank)
     else:
         run_ours(args, rank, world, local_rank)

@@ -344,14 +344,12 @@ int dg_bind(dg_ctx *c, void *ws, size_t bytes, void *stream) {
     if (e != cudaSuccess) return cuda_fail(c, e, "workspace memset");
     const double g[3] = {2.0 / (c->extent[0] / c->nx), 2.0 / (c->extent[1] / c->ny), 2.0 / (c->extent[2] / c->nz)};
     build_device_ops(c->N, g, c->ops);
-    int dev = 0, sms = 0, per_sm = 0;
-    e = cudaGetDevice(&dev);
-    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (e == cudaSuccess) e = c->kt->prepare(&per_sm);
+    int resident = 0;
+    e = c->kt->prepare(&resident);
     if (e != cudaSuccess) return cuda_fail(c, e, "stage kernel setup");
-    if (per_sm < 1 || sms < 1) return fail(c, DG_ECUDA, "stage kernel does not fit on an SM");
-    const size_t resident = (size_t)per_sm * (size_t)sms;
-    c->grid = (int)(c->nbricks < resident ? c->nbricks : resident);
+    if (resident < 1) return fail(c, DG_ECUDA, "stage kernel does not fit on the GPU");
+    if (c->nby > 65535 || c->nbz > 65535) return fail(c, DG_EUNSUPPORTED, "more than 65535 bricks along y or z");
+    c->grid = resident;   // how far ahead (in dispatch order) the L2 prefetch looks
     c->bound = true;
     c->err[0] = 0;
     return DG_OK;

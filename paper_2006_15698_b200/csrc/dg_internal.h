@@ -87,7 +87,7 @@ struct DgKernelTable {
     int smem_bytes;          // dynamic shared memory of the stage kernel
     long long slot;          // doubles per brick in Q/K/R (5 * nodes per brick)
     long long tslot;         // face-trace doubles per brick
-    cudaError_t (*prepare)(int *blocks_per_sm);   // opt in to the shared memory size; resident blocks per SM
+    cudaError_t (*prepare)(int *resident);        // opt in to the shared memory size; resident blocks of the GPU
     cudaError_t (*launch_stage)(const DgStageArgs &a, cudaStream_t s);
     cudaError_t (*launch_layout)(const DgLayoutArgs &a, cudaStream_t s);
     cudaError_t (*launch_wavespeed)(const DgWaveArgs &a, cudaStream_t s);

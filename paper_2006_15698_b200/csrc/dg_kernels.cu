@@ -44,9 +44,12 @@ namespace {
 // per brick shape so that the 16 lanes of a half-warp hit 16 different 8-byte bank pairs in all three
 // passes (0 = dense).  z lines keep t1 = gx fastest: their lanes also
 // address HBM.
+// CLX x CLY x CLZ > 1: the blocks of that many neighbouring bricks form a thread-block CLUSTER and hand the traces
+// of the faces they share to each other through distributed shared memory instead of the HBM trace buffer.
 template <int N_, int BX_, int BY_, int BZ_, int MINB_, int RELOAD_ = 0, int P_ = 0, int PP_ = 0, int OX_ = 0,
-          int OY_ = 0, int OZ_ = 0>
+          int OY_ = 0, int OZ_ = 0, int CLX_ = 1, int CLY_ = 1, int CLZ_ = 1>
 struct Cfg {
+    static constexpr int CLX = CLX_, CLY = CLY_, CLZ = CLZ_, CLUSTER = CLX_ * CLY_ * CLZ_;
     static constexpr int N = N_, BX = BX_, BY = BY_, BZ = BZ_, MINB = MINB_;
     // RELOAD = 1: the volume term reads the line's Q from shared memory a second time instead of keeping
     // it in 10 N registers across the interface fluxes (fewer registers, more blocks per SM, 15 more
@@ -65,7 +68,11 @@ struct Cfg {
     static constexpr int TSLOT = 2 * DG_NV * (CX + CY + CZ);       // trace doubles per brick
     static constexpr bool MULTI = (BX > 1) || (BY > 1) || (BZ > 1);
     static constexpr int LINEBUF = MULTI ? DG_NV * L : 0;          // T- / F* hand-over between elements of a brick
-    static constexpr int SMEM_DOUBLES = 2 * DG_NV * PLANE + 2 * LINEBUF;
+    static constexpr int EXFACE = (CLX > 1 ? CX : 0) > (CLY > 1 ? CY : 0)
+                                      ? ((CLX > 1 ? CX : 0) > (CLZ > 1 ? CZ : 0) ? (CLX > 1 ? CX : 0) : (CLZ > 1 ? CZ : 0))
+                                      : ((CLY > 1 ? CY : 0) > (CLZ > 1 ? CZ : 0) ? (CLY > 1 ? CY : 0) : (CLZ > 1 ? CZ : 0));
+    static constexpr int EXBUF = 2 * DG_NV * EXFACE;               // traces exported to the cluster neighbours
+    static constexpr int SMEM_DOUBLES = 2 * DG_NV * PLANE + 2 * LINEBUF + EXBUF;
     static constexpr int SMEM_BYTES = SMEM_DOUBLES * 8;
     static_assert(P >= GX && PP >= GY * P, "pitches too small");
     static_assert(OZ == 0 || OZ == 2, "z lines must keep gx fastest across lanes");
@@ -89,6 +96,21 @@ __device__ __forceinline__ void l2_prefetch(const void *ptr, unsigned bytes) {
 
 // Compiler-level fence on memory operations: bounds how far loads are hoisted (register pressure).
 __device__ __forceinline__ void sched_fence() { asm volatile("" ::: "memory"); }
+
+// Thread-block cluster primitives (split barrier; distributed shared memory loads).
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+__device__ __forceinline__ unsigned map_to_rank(const void *smem_ptr, unsigned rank) {
+    const unsigned a = (unsigned)__cvta_generic_to_shared(smem_ptr);
+    unsigned r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ double ld_cluster(unsigned addr) {
+    double v;
+    asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(addr) : "memory");
+    return v;
+}
 
 // Euler flux along the face/line normal, eq (2)-(3) (listing lines 186-217), for a state
 // whose momentum components have been ROTATED so that slot 1 is the normal one:
@@ -139,6 +161,7 @@ struct Axis {
     static constexpr int B = (AX == 0) ? C::BX : (AX == 1) ? C::BY : C::BZ;            // elements along the axis
     static constexpr int TBASE = (AX == 0) ? 0 : (AX == 1) ? 2 * DG_NV * C::CX : 2 * DG_NV * (C::CX + C::CY);
     static constexpr bool MULTI = B > 1;
+    static constexpr int CL = (AX == 0) ? C::CLX : (AX == 1) ? C::CLY : C::CLZ;     // cluster blocks along the axis
     // momentum slots rotated so that slot 1 is the component along this axis: slot s holds variable VAR[s]
     static constexpr int M1 = 1 + AX, M2 = (AX == 2) ? 1 : 2 + AX, M3 = (AX == 0) ? 3 : AX;
 };
@@ -239,10 +262,11 @@ __device__ __forceinline__ void prefetch_brick(const DgStageArgs &a, int brick, 
 // PE for one axis: traces of the (updated) Q in shared memory on the brick boundary -> Tnew.
 template <class C, int AX>
 __device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta, const double *Qs, double *Tbrick,
-                                                const DgStageArgs &a) {
+                                                const DgStageArgs &a, bool wlo = true, bool whi = true) {
     using A = Axis<C, AX>;
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE;
-    const bool first = g.e == 0, last = g.e == exta - 1;
+    // wlo / whi: does the low / high face of the brick go through HBM (false: a cluster neighbour takes it)
+    const bool first = g.e == 0 && wlo, last = g.e == exta - 1 && whi;
     if (!act || !(first || last)) return;
     double *dst = Tbrick + A::TBASE + g.c;
     const double *Q0 = Qs + g.base;
@@ -286,13 +310,14 @@ __device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta
 // PH: the neighbour bricks' traces this line touches, momentum slots rotated, HBM/L2 -> registers.
 template <class C, int AX>
 __device__ __forceinline__ void load_halo(const Geo &g, bool act, int exta, const double *halo_lo,
-                                          const double *halo_hi, double (&Hlo)[DG_NV], double (&Hhi)[DG_NV]) {
+                                          const double *halo_hi, bool ilo, bool ihi, double (&Hlo)[DG_NV],
+                                          double (&Hhi)[DG_NV]) {
     constexpr int Ca = Axis<C, AX>::Ca;
-    if (act && g.e == 0) {
+    if (act && g.e == 0 && !ilo) {
 #pragma unroll
         for (int s = 0; s < DG_NV; ++s) Hlo[s] = __ldg(halo_lo + var_of_slot<C, AX>(s) * Ca + g.c);
     }
-    if (act && g.e == exta - 1) {
+    if (act && g.e == exta - 1 && !ihi) {
 #pragma unroll
         for (int s = 0; s < DG_NV; ++s) Hhi[s] = __ldg(halo_hi + var_of_slot<C, AX>(s) * Ca + g.c);
     }
@@ -302,17 +327,22 @@ __device__ __forceinline__ void load_halo(const Geo &g, bool act, int exta, cons
 // face traces and the two interface fluxes come first (no accumulators alive yet); the accumulators then
 // START from the lift term and the volume term is added node by node.
 //   r_i = sum_q Dhat_iq F_q - (l_i(+1) F*_+ - l_i(-1) F*_-) (2/h_a)/w_i
-template <class C, int AX, int MODE>
+// Cluster variants (A::CL > 1): `ilo` / `ihi` say that the low / high face of the brick is shared with the
+// cluster block of rank `rlo` / `rhi`; the traces on those faces are exported to Ex in this block's shared
+// memory and the neighbour's are read from ITS Ex.  One cluster barrier between export and import; the
+// barrier that protects Ex against the next export is split (arrive after the import, wait before the next
+// export or the end of the kernel: PENDING says that such a wait is still owed on entry).
+template <class C, int AX, int MODE, bool PENDING>
 __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, int l, bool act, int exta,
                                           const double *halo_lo, const double *halo_hi, double *Qs, double *Ks,
-                                          double *Tms, double *Fss, bool readK, size_t qbase,
-                                          double *Tbrick) {
+                                          double *Tms, double *Fss, double *Ex, bool readK, size_t qbase,
+                                          double *Tbrick, bool ilo, bool ihi, unsigned rlo, unsigned rhi) {
     using A = Axis<C, AX>;
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE, L = C::L, S = A::S, Ca = A::Ca;
     const bool first = g.e == 0, last = g.e == exta - 1;
     const int lb = g.e * Ca + g.c;   // slot of this line in the hand-over buffers
     double Hlo[NV], Hhi[NV];
-    load_halo<C, AX>(g, act, exta, halo_lo, halo_hi, Hlo, Hhi);
+    load_halo<C, AX>(g, act, exta, halo_lo, halo_hi, ilo, ihi, Hlo, Hhi);
 
     double QL[C::RELOAD ? 1 : NV][C::RELOAD ? 1 : N], Tp[NV], Tm[NV];
     if (act) {
@@ -335,7 +365,21 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
             for (int n = 0; n < NV; ++n) Tms[n * L + lb] = Tm[n];
         }
     }
-    if (A::MULTI) __syncthreads();
+    if (A::CL > 1) {
+        if (PENDING) cluster_wait();   // the neighbours are done with the previous axis' exports
+        if (act && first && ilo) {
+#pragma unroll
+            for (int n = 0; n < NV; ++n) Ex[n * Ca + g.c] = Tm[n];
+        }
+        if (act && last && ihi) {
+#pragma unroll
+            for (int n = 0; n < NV; ++n) Ex[(NV + n) * Ca + g.c] = Tp[n];
+        }
+        cluster_arrive();              // (a cluster barrier is also a block barrier: covers Tms)
+        cluster_wait();
+    } else if (A::MULTI) {
+        __syncthreads();
+    }
 
     // ------------- PB: interface fluxes ----------------------------------------------------------------
     double Fp[NV], Fm[NV];
@@ -343,6 +387,13 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
         if (A::MULTI && !last) {
 #pragma unroll
             for (int n = 0; n < NV; ++n) Hhi[n] = Tms[n * L + lb + Ca];   // T- of the next element of this brick
+        } else if (A::CL > 1 && ihi) {
+#pragma unroll
+            for (int n = 0; n < NV; ++n) Hhi[n] = ld_cluster(map_to_rank(Ex + n * Ca + g.c, rhi));        // its T-
+        }
+        if (A::CL > 1 && first && ilo) {
+#pragma unroll
+            for (int n = 0; n < NV; ++n) Hlo[n] = ld_cluster(map_to_rank(Ex + (NV + n) * Ca + g.c, rlo));  // its T+
         }
         lax_friedrichs2(Tp, Hhi, 1.0, a.gamma, a.gm1, Fp);
         if (A::MULTI) {
@@ -351,6 +402,7 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
         }
         if (first) lax_friedrichs2(Tm, Hlo, -1.0, a.gamma, a.gm1, Fm);
     }
+    if (A::CL > 1) cluster_arrive();   // done reading the neighbours' exports (waited for before Ex is reused)
     if (A::MULTI) __syncthreads();
 
     if (act) {
@@ -436,13 +488,13 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
                         Q0w[n * PLANE + i * S] = Qn[i];
                     }
                     // PE for the z faces: traces of the updated Q, only at the ends that lie on the brick boundary
-                    if (first) {
+                    if (first && !ilo) {
                         double tm = 0.0;
 #pragma unroll
                         for (int i = 0; i < N; ++i) tm = fma(a.ops.lm[i], Qn[i], tm);
                         dst[n * Ca] = tm;
                     }
-                    if (last) {
+                    if (last && !ihi) {
                         double tp = 0.0;
 #pragma unroll
                         for (int i = 0; i < N; ++i) tp = fma(a.ops.lp[i], Qn[i], tp);
@@ -461,97 +513,96 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
 template <class C, int MODE>
 __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __grid_constant__ DgStageArgs a) {
     constexpr int NV = DG_NV, PLANE = C::PLANE, L = C::L;
+    constexpr bool EXCH = (C::CLUSTER > 1) && (MODE != DG_MODE_TRACES);   // do cluster neighbours trade traces?
     extern __shared__ __align__(16) double smem[];
     double *Qs = smem;                     // [5][PLANE] nodal values of the brick (old, then updated)
     double *Ks = Qs + NV * PLANE;          // [5][PLANE] Runge-Kutta register of the brick, accumulated in place
     double *Tms = Ks + NV * PLANE;         // [5][L]     T- of every line (right state of the line below)
     double *Fss = Tms + C::LINEBUF;        // [5][L]     F* at the + end of every line
+    double *Ex = Fss + C::LINEBUF;         // [2][5][EXFACE] traces exported to the cluster neighbours
 
+    // One brick per block, blockIdx = brick coordinates (no persistent loop: a loop over bricks makes the
+    // compiler hoist the operator tables out of it into registers).  The grid is rounded up to whole
+    // clusters; a block past the last brick only takes part in the cluster barriers.
     const int tid = threadIdx.x, l = tid;
-    const int nbricks = a.nbx * a.nby * a.nbz;
+    const int bxi = blockIdx.x, byi = blockIdx.y, bzi = blockIdx.z;
+    const bool real = bxi < a.nbx && byi < a.nby && bzi < a.nbz;
+    const int brick = bxi + a.nbx * (byi + a.nby * bzi);
     const bool readK = (MODE == DG_MODE_STAGE) && (a.rkA != 0.0);
     const Geo gx = make_geo<C, 0>(l), gy = make_geo<C, 1>(l), gz = make_geo<C, 2>(l);
-    const bool inL = l < L;
+    const bool inL = (l < L) && real;
+    const size_t qbase = (size_t)brick * C::SLOT;
 
-    // One brick per block (no persistent loop: a loop over bricks makes the compiler hoist the operator
-    // tables out of it into registers).  Blocks are dispatched in index order, so the brick that is
-    // `a.grid` (= resident blocks of the whole GPU) ahead is the one that starts when this one ends.
-    {
-        const int brick = blockIdx.x;
-        const int bxi = brick % a.nbx, byi = (brick / a.nbx) % a.nby, bzi = brick / (a.nbx * a.nby);
-        const size_t qbase = (size_t)brick * C::SLOT;
-        // ---------------- P0: this brick's Q and K come in; the next brick's data is asked into L2 ------
+    // ---------------- P0: this brick's Q and K come in ----------------------------------------------------
+    if (real) {
         stage_in<C>(Qs, a.Q + qbase, tid);
         if (readK) stage_in<C>(Ks, a.K + qbase, tid);
-        cp_async_commit();
-        const int next = brick + a.grid;
-        if (next < nbricks && (a.flags & 2)) prefetch_brick<C>(a, next, tid, readK, MODE != DG_MODE_TRACES);
-
-        const int ext0 = min(C::BX, a.nx - bxi * C::BX);   // elements of this brick per axis (ragged last brick)
-        const int ext1 = min(C::BY, a.ny - byi * C::BY);
-        const int ext2 = min(C::BZ, a.nz - bzi * C::BZ);
-        const bool full = (ext0 == C::BX) && (ext1 == C::BY) && (ext2 == C::BZ);
-        bool actx = inL, acty = inL, actz = inL;
-        if (!full) {
-            actx = inL && line_inside<C, 0>(gx, ext0, ext1, ext2);
-            acty = inL && line_inside<C, 1>(gy, ext0, ext1, ext2);
-            actz = inL && line_inside<C, 2>(gz, ext0, ext1, ext2);
-        }
-        double *Tbrick = a.Tnew + (size_t)brick * C::TSLOT;
-
-        if (MODE != DG_MODE_TRACES) {
-            cp_async_wait<0>();
-            __syncthreads();
-            if (a.flags & 8) {   // EXPERIMENT: memory traffic of a stage without its arithmetic
-                if (next < nbricks) prefetch_brick<C>(a, next, tid, readK, true);
-                if (actz) {
-                    double h = 0.0;
-                    const double *hl = halo_source<C, 2>(a, bxi, byi, bzi, 0), *hh = halo_source<C, 2>(a, bxi, byi, bzi, 1);
-                    const double *xl = halo_source<C, 0>(a, bxi, byi, bzi, 0), *xh = halo_source<C, 0>(a, bxi, byi, bzi, 1);
-                    const double *yl = halo_source<C, 1>(a, bxi, byi, bzi, 0), *yh = halo_source<C, 1>(a, bxi, byi, bzi, 1);
-                    for (int s = 0; s < NV; ++s) {
-                        if (gz.e == 0) h += hl[s * C::CZ + gz.c];
-                        if (gz.e == ext2 - 1) h += hh[s * C::CZ + gz.c];
-                        if (gx.e == 0) h += xl[s * C::CX + gx.c];
-                        if (gx.e == ext0 - 1) h += xh[s * C::CX + gx.c];
-                        if (gy.e == 0) h += yl[s * C::CY + gy.c];
-                        if (gy.e == ext1 - 1) h += yh[s * C::CY + gy.c];
-                    }
-                    const size_t g0 = qbase + (size_t)(gz.e * C::N) * (C::GY * C::GX) + gz.t2 * C::GX + gz.t1;
-                    for (int n = 0; n < NV; ++n)
-                        for (int i = 0; i < C::N; ++i) {
-                            const size_t go = g0 + (size_t)n * C::NODES + (size_t)i * (C::GY * C::GX);
-                            const double Kn = Ks[gz.base + n * PLANE + i * C::PP] * 0.5 + 1e-300 * h;
-                            __stcs(a.K + go, Kn);
-                            __stcs(a.Q + go, Qs[gz.base + n * PLANE + i * C::PP] + 1e-300 * Kn);
-                        }
-                    boundary_traces<C, 2>(gz, actz, ext2, Qs, Tbrick, a);
-                }
-            } else {
-            axis_pass<C, 0, MODE>(a, gx, l, actx, ext0, halo_source<C, 0>(a, bxi, byi, bzi, 0),
-                                  halo_source<C, 0>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, qbase, Tbrick);
-            __syncthreads();
-            axis_pass<C, 1, MODE>(a, gy, l, acty, ext1, halo_source<C, 1>(a, bxi, byi, bzi, 0),
-                                  halo_source<C, 1>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, qbase, Tbrick);
-            __syncthreads();
-            // the brick that takes this block's place: ask L2 for its data now, about a third of a brick ahead
-            if (next < nbricks && !(a.flags & 3)) prefetch_brick<C>(a, next, tid, readK, true);
-            axis_pass<C, 2, MODE>(a, gz, l, actz, ext2, halo_source<C, 2>(a, bxi, byi, bzi, 0),
-                                  halo_source<C, 2>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, readK, qbase, Tbrick);
-            }
-        } else {
-            cp_async_wait<0>();
-            __syncthreads();
-        }
-        // ---------------- PE: traces of the updated Q on the brick boundary (z came from registers) ----
-        if (MODE != DG_MODE_RESIDUAL) {
-            if (MODE == DG_MODE_STAGE) __syncthreads();
-            boundary_traces<C, 0>(gx, actx, ext0, Qs, Tbrick, a);
-            boundary_traces<C, 1>(gy, acty, ext1, Qs, Tbrick, a);
-            if (MODE == DG_MODE_TRACES) boundary_traces<C, 2>(gz, actz, ext2, Qs, Tbrick, a);
-        }
     }
+    cp_async_commit();
+
+    // The brick that takes this block's place when it ends: blocks are dispatched cluster by cluster in
+    // index order, so it is the one `a.grid` (= resident blocks of the whole GPU) further on in that order.
+    int next = -1;
+    {
+        const int ncx = gridDim.x / C::CLX, ncy = gridDim.y / C::CLY;
+        const int px = bxi % C::CLX, py = byi % C::CLY, pz = bzi % C::CLZ;
+        const long long cid = (bxi / C::CLX) + (long long)ncx * ((byi / C::CLY) + (long long)ncy * (bzi / C::CLZ));
+        const long long d = cid * C::CLUSTER + (px + C::CLX * (py + C::CLY * pz)) + a.grid;
+        const long long ncid = d / C::CLUSTER;
+        const int r = (int)(d - ncid * C::CLUSTER);
+        const int cx = (int)(ncid % ncx), cy = (int)((ncid / ncx) % ncy), cz = (int)(ncid / ((long long)ncx * ncy));
+        const int nx_ = cx * C::CLX + r % C::CLX, ny_ = cy * C::CLY + (r / C::CLX) % C::CLY, nz_ = cz * C::CLZ + r / (C::CLX * C::CLY);
+        if (nx_ < a.nbx && ny_ < a.nby && nz_ < a.nbz) next = nx_ + a.nbx * (ny_ + a.nby * nz_);
+    }
+
+    const int ext0 = min(C::BX, a.nx - bxi * C::BX);   // elements of this brick per axis (ragged last brick)
+    const int ext1 = min(C::BY, a.ny - byi * C::BY);
+    const int ext2 = min(C::BZ, a.nz - bzi * C::BZ);
+    const bool full = (ext0 == C::BX) && (ext1 == C::BY) && (ext2 == C::BZ);
+    bool actx = inL, acty = inL, actz = inL;
+    if (!full && real) {
+        actx = inL && line_inside<C, 0>(gx, ext0, ext1, ext2);
+        acty = inL && line_inside<C, 1>(gy, ext0, ext1, ext2);
+        actz = inL && line_inside<C, 2>(gz, ext0, ext1, ext2);
+    }
+    double *Tbrick = a.Tnew + (size_t)brick * C::TSLOT;
+
+    // faces shared with a block of the same cluster (never across the periodic wrap, never with a padding block)
+    const int px = bxi % C::CLX, py = byi % C::CLY, pz = bzi % C::CLZ;
+    const unsigned rank = px + C::CLX * (py + C::CLY * pz);
+    const bool ixl = EXCH && px > 0, ixh = EXCH && px < C::CLX - 1 && bxi + 1 < a.nbx;
+    const bool iyl = EXCH && py > 0, iyh = EXCH && py < C::CLY - 1 && byi + 1 < a.nby;
+    const bool izl = EXCH && pz > 0, izh = EXCH && pz < C::CLZ - 1 && bzi + 1 < a.nbz;
+
+    cp_async_wait<0>();
+    __syncthreads();
+    if (MODE != DG_MODE_TRACES) {
+        constexpr bool PY = C::CLX > 1, PZ = (C::CLX > 1) || (C::CLY > 1);
+        axis_pass<C, 0, MODE, false>(a, gx, l, actx, ext0, halo_source<C, 0>(a, bxi, byi, bzi, 0),
+                                     halo_source<C, 0>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, Ex, readK, qbase, Tbrick,
+                                     ixl, ixh, rank - 1, rank + 1);
+        __syncthreads();
+        axis_pass<C, 1, MODE, PY>(a, gy, l, acty, ext1, halo_source<C, 1>(a, bxi, byi, bzi, 0),
+                                  halo_source<C, 1>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, Ex, readK, qbase, Tbrick,
+                                  iyl, iyh, rank - C::CLX, rank + C::CLX);
+        __syncthreads();
+        // ask L2 for the follow-on brick's data now, about a third of a brick ahead of its use
+        if (next >= 0 && !(a.flags & 1)) prefetch_brick<C>(a, next, tid, readK, true);
+        axis_pass<C, 2, MODE, PZ>(a, gz, l, actz, ext2, halo_source<C, 2>(a, bxi, byi, bzi, 0),
+                                  halo_source<C, 2>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, Ex, readK, qbase, Tbrick,
+                                  izl, izh, rank - C::CLX * C::CLY, rank + C::CLX * C::CLY);
+    }
+    // ---------------- PE: traces of the updated Q on the brick boundary (z came from registers) --------
+    if (MODE != DG_MODE_RESIDUAL) {
+        if (MODE == DG_MODE_STAGE) __syncthreads();
+        boundary_traces<C, 0>(gx, actx, ext0, Qs, Tbrick, a, !ixl, !ixh);
+        boundary_traces<C, 1>(gy, acty, ext1, Qs, Tbrick, a, !iyl, !iyh);
+        if (MODE == DG_MODE_TRACES) boundary_traces<C, 2>(gz, actz, ext2, Qs, Tbrick, a);
+    }
+    // nobody may leave while a cluster neighbour can still read its exports
+    if (EXCH) cluster_wait();
 }
+
 // ------------------------------------------------------------------------------------------------
 // layout conversion canonical [e][k][j][i][n] <-> internal [brick][n][gz][gy][gx]
 // one thread per node; canonical side reads/writes 40 contiguous bytes per thread
@@ -621,7 +672,24 @@ __global__ void __launch_bounds__(256) dg_wavespeed_kernel(const DgWaveArgs a) {
 // host-side launchers, one table per variant
 // ------------------------------------------------------------------------------------------------
 template <class C>
-cudaError_t prepare(int *blocks_per_sm) {
+void stage_config(cudaLaunchConfig_t &cfg, cudaLaunchAttribute &attr, int nbx, int nby, int nbz, cudaStream_t s) {
+    // one block per brick, blockIdx = brick coordinates, rounded up to whole clusters
+    cfg.gridDim = dim3((unsigned)((nbx + C::CLX - 1) / C::CLX * C::CLX), (unsigned)((nby + C::CLY - 1) / C::CLY * C::CLY),
+                       (unsigned)((nbz + C::CLZ - 1) / C::CLZ * C::CLZ));
+    cfg.blockDim = dim3(C::THREADS, 1, 1);
+    cfg.dynamicSmemBytes = C::SMEM_BYTES;
+    cfg.stream = s;
+    attr.id = cudaLaunchAttributeClusterDimension;
+    attr.val.clusterDim.x = C::CLX;
+    attr.val.clusterDim.y = C::CLY;
+    attr.val.clusterDim.z = C::CLZ;
+    cfg.attrs = &attr;
+    cfg.numAttrs = 1;
+}
+
+// Opt in to the shared-memory size; *resident = blocks of the stage kernel the whole GPU holds at once.
+template <class C>
+cudaError_t prepare(int *resident) {
     cudaError_t err = cudaFuncSetAttribute(dg_stage_kernel<C, DG_MODE_STAGE>,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
     if (err == cudaSuccess)
@@ -631,21 +699,34 @@ cudaError_t prepare(int *blocks_per_sm) {
         err = cudaFuncSetAttribute(dg_stage_kernel<C, DG_MODE_TRACES>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    C::SMEM_BYTES);
     if (err != cudaSuccess) return err;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, dg_stage_kernel<C, DG_MODE_STAGE>,
-                                                         C::THREADS, C::SMEM_BYTES);
+    if (C::CLUSTER > 1) {
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute attr;
+        stage_config<C>(cfg, attr, C::CLX * 64, C::CLY * 64, C::CLZ * 64, 0);
+        int clusters = 0;
+        err = cudaOccupancyMaxActiveClusters(&clusters, dg_stage_kernel<C, DG_MODE_STAGE>, &cfg);
+        *resident = clusters * C::CLUSTER;
+        return err;
+    }
+    int dev = 0, sms = 0, per_sm = 0;
+    err = cudaGetDevice(&dev);
+    if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (err == cudaSuccess)
+        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, dg_stage_kernel<C, DG_MODE_STAGE>, C::THREADS,
+                                                            C::SMEM_BYTES);
+    *resident = per_sm * sms;
+    return err;
 }
 
 template <class C>
 cudaError_t launch_stage(const DgStageArgs &a, cudaStream_t s) {
     if (a.grid <= 0) return cudaErrorInvalidConfiguration;
-    const unsigned blocks = (unsigned)(a.nbx * a.nby * a.nbz);   // one block per brick
-    if (a.mode == DG_MODE_STAGE)
-        dg_stage_kernel<C, DG_MODE_STAGE><<<blocks, C::THREADS, C::SMEM_BYTES, s>>>(a);
-    else if (a.mode == DG_MODE_RESIDUAL)
-        dg_stage_kernel<C, DG_MODE_RESIDUAL><<<blocks, C::THREADS, C::SMEM_BYTES, s>>>(a);
-    else
-        dg_stage_kernel<C, DG_MODE_TRACES><<<blocks, C::THREADS, C::SMEM_BYTES, s>>>(a);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr;
+    stage_config<C>(cfg, attr, a.nbx, a.nby, a.nbz, s);
+    if (a.mode == DG_MODE_STAGE) return cudaLaunchKernelEx(&cfg, dg_stage_kernel<C, DG_MODE_STAGE>, a);
+    if (a.mode == DG_MODE_RESIDUAL) return cudaLaunchKernelEx(&cfg, dg_stage_kernel<C, DG_MODE_RESIDUAL>, a);
+    return cudaLaunchKernelEx(&cfg, dg_stage_kernel<C, DG_MODE_TRACES>, a);
 }
 
 inline unsigned flat_grid(size_t total) {
@@ -695,8 +776,8 @@ using V3 = Cfg<4, 2, 2, 1, 6, 0, 8, 65, 3, 0, 0>;
 #elif DG_N == 5
 using V0 = Cfg<5, 1, 2, 2, 4, 1, 0, 0, 0, 1, 0>;
 using V1 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0>;
-using V2 = Cfg<5, 1, 2, 3, 3, 1, 0, 0, 0, 1, 0>;
-using V3 = Cfg<5, 2, 2, 2, 2, 1, 10, 106, 2, 0, 0>;
+using V2 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0, 2, 2, 2>;
+using V3 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0, 2, 1, 1>;
 #elif DG_N == 6
 using V0 = Cfg<6, 1, 1, 2, 4, 1, 6, 38, 1, 0, 0>;
 using V1 = Cfg<6, 1, 1, 2, 4, 0, 6, 38, 1, 0, 0>;
