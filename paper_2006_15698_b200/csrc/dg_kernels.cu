@@ -1,23 +1,23 @@
 // dg_kernels.cu -- CUDA kernels of the DG Euler time step for one N = p+1 (compile with -DDG_N=<N>,
 // -gencode arch=compute_100a,code=sm_100a).  Hand-written for B200; fp64 throughout.
 //
-// The fused stage kernel (v4) is PERSISTENT: a thread block strides over "bricks" of BX x BY x BZ elements.
-// The geometry of a thread's three node lines (one per axis) does not depend on the brick, so it is computed
-// once per kernel; every shared-memory stride below is a compile-time constant.  Per brick, in ONE sweep
-// over HBM:
-//   P0  cp.async (no registers) of the brick's Q and K (5 x nodes each) into shared memory; one L2 prefetch
-//       instruction each for the NEXT brick's Q, K and 6 neighbour trace blocks
-//   then, one thread per node LINE, for the axes x, y, z in turn (three instances of one template):
+// The fused stage kernel (v4): ONE thread block per "brick" of BX x BY x BZ elements, one thread per node
+// LINE, every shared-memory stride a compile-time constant.  Per brick, in ONE sweep over HBM:
+//   P0  cp.async (no registers) of the brick's Q and K (5 x nodes each, separate groups) into shared memory
+//   then, for the axes x, y, z in turn (three instances of one template):
 //   PH  the neighbour bricks' face traces this line touches go straight from HBM/L2 into registers
-//   PA  pointwise Euler flux (eq (2)-(3)) at the line's N nodes,
-//       V_i = sum_q Dhat_iq F_q in registers (eq (5) 2nd term, the contraction of
-//       listing lines 220-237), and the two face traces T+- = sum_q l_q(+-1) Q_q
-//   PB  local Lax-Friedrichs interface flux at the + end of the line, and at the - end of
-//       the lines that start on the brick boundary
-//   PC  lift with 2/h folded in: r_i = V_i - (l_i(+1) F*_+ - l_i(-1) F*_-) (2/h_a)/w_i  (eq (5) 3rd term)
-//   PD  LSERK45 accumulated in place on the staged K:  x: K = A K + dt r_x,
-//       y: K += dt r_y,  z: K += dt r_z, Q += B K, both written straight to HBM from the z lines
-//       (coalesced); or R itself in residual mode
+//   PT  the line's N nodal values into registers (RELOAD variants: read again later instead) and the two
+//       face traces T+- = sum_q l_q(+-1) Q_q
+//   PB  local Lax-Friedrichs interface flux, doubled, at the + end of the line, and at the
+//       - end of the lines that start on the brick boundary (faces inside a brick: once, handed over
+//       through shared memory; cluster variants: also across the blocks of a cluster)
+//   PC  lift with 2/h, 1/2 and dt folded into the tables starts the accumulators:
+//       r_i = sum_q Dhat_iq F_q - (l_i(+1) F*_+ - l_i(-1) F*_-) (2/h_a)/w_i       (eq (5) 3rd and 2nd term)
+//   PA  pointwise Euler flux (eq (2)-(3)) at the line's N nodes and the sum-factorised
+//       derivative (the contraction of listing lines 220-237), all in registers
+//   PD  LSERK45 accumulated in place on the staged K:  x: K = A K + r_x,  y: K += r_y,
+//       z: K += r_z, Q += B K, both written straight to HBM from the z lines (coalesced, streaming);
+//       or R itself in residual mode.  Before the z pass: L2 prefetch of the follow-on brick's data.
 //   PE  face traces of the UPDATED Q on the brick boundary, written to the other trace buffer
 // so that Q and K are read once and written once per stage and no element ever needs another
 // element's nodal values: neighbours meet only through the double-buffered brick-boundary traces.
@@ -405,13 +405,13 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
     if (A::CL > 1) cluster_arrive();   // done reading the neighbours' exports (waited for before Ex is reused)
     if (A::MULTI) __syncthreads();
 
+    double V[NV][N];
     if (act) {
         if (A::MULTI && !first) {
 #pragma unroll
             for (int n = 0; n < NV; ++n) Fm[n] = Fss[n * L + lb - Ca];
         }
         // ------------- PC: lift (2/h and 1/w folded into the tables) starts the accumulators -----------
-        double V[NV][N];
 #pragma unroll
         for (int i = 0; i < N; ++i) {
             const double cp = a.ops.lpg[AX][i], cm = a.ops.lmg[AX][i];
@@ -431,6 +431,12 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
 #pragma unroll
                 for (int i = 0; i < N; ++i) V[n][i] = fma(a.ops.Dg[AX][q][i], F[n], V[n][i]);
         }
+    }
+    if (AX == 0) {
+        cp_async_wait<0>();            // the staged K (its own cp.async group) has landed
+        if (readK) __syncthreads();
+    }
+    if (act) {
         // ------------- PD: Runge-Kutta accumulation on the staged K ------------------------------------
         double *K0 = Ks + g.base;
         if (AX == 0) {
@@ -534,11 +540,10 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
     const size_t qbase = (size_t)brick * C::SLOT;
 
     // ---------------- P0: this brick's Q and K come in ----------------------------------------------------
-    if (real) {
-        stage_in<C>(Qs, a.Q + qbase, tid);
-        if (readK) stage_in<C>(Ks, a.K + qbase, tid);
-    }
+    if (real) stage_in<C>(Qs, a.Q + qbase, tid);
     cp_async_commit();
+    if (real && readK) stage_in<C>(Ks, a.K + qbase, tid);
+    cp_async_commit();   // K is not needed before the end of the x pass: its own group
 
     // The brick that takes this block's place when it ends: blocks are dispatched cluster by cluster in
     // index order, so it is the one `a.grid` (= resident blocks of the whole GPU) further on in that order.
@@ -574,7 +579,7 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
     const bool iyl = EXCH && py > 0, iyh = EXCH && py < C::CLY - 1 && byi + 1 < a.nby;
     const bool izl = EXCH && pz > 0, izh = EXCH && pz < C::CLZ - 1 && bzi + 1 < a.nbz;
 
-    cp_async_wait<0>();
+    cp_async_wait<1>();   // Q has landed
     __syncthreads();
     if (MODE != DG_MODE_TRACES) {
         constexpr bool PY = C::CLX > 1, PZ = (C::CLX > 1) || (C::CLY > 1);
@@ -774,8 +779,8 @@ using V1 = Cfg<4, 2, 2, 2, 3, 0, 9, 74, 1, 1, 2>;
 using V2 = Cfg<4, 2, 2, 1, 6, 1, 8, 65, 3, 0, 0>;
 using V3 = Cfg<4, 2, 2, 1, 6, 0, 8, 65, 3, 0, 0>;
 #elif DG_N == 5
-using V0 = Cfg<5, 1, 2, 2, 4, 1, 0, 0, 0, 1, 0>;
-using V1 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0>;
+using V0 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0>;
+using V1 = Cfg<5, 1, 2, 2, 4, 1, 0, 0, 0, 1, 0>;
 using V2 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0, 2, 2, 2>;
 using V3 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0, 2, 1, 1>;
 #elif DG_N == 6
