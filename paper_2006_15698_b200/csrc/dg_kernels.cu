@@ -40,6 +40,7 @@ namespace {
 // plane, and, per axis, the order in which a warp's lanes walk the node lines (ORD):
 //   0: t1 fastest, then t2, then the element e along the axis      1: t2, t1, e
 //   2: t1, e, t2                                                   3: t2, e, t1
+//   4: e, t1, t2                                                   5: e, t2, t1
 // (t1,t2) = (gy,gz) for x lines, (gx,gz) for y lines, (gx,gy) for z lines.  P, PP and the orders are picked
 // per brick shape so that the 16 lanes of a half-warp hit 16 different 8-byte bank pairs in all three
 // passes (0 = dense).  z lines keep t1 = gx fastest: their lanes also
@@ -197,10 +198,20 @@ __device__ __forceinline__ Geo make_geo(int l) {
         g.e = (l / T1) % B;
         g.t2 = l / (T1 * B);
         g.c = g.t2 * T1 + g.t1;
-    } else {
+    } else if (A::ORD == 3) {
         g.t2 = l % T2;
         g.e = (l / T2) % B;
         g.t1 = l / (T2 * B);
+        g.c = g.t1 * T2 + g.t2;
+    } else if (A::ORD == 4) {
+        g.e = l % B;
+        g.t1 = (l / B) % T1;
+        g.t2 = l / (B * T1);
+        g.c = g.t2 * T1 + g.t1;
+    } else {
+        g.e = l % B;
+        g.t2 = (l / B) % T2;
+        g.t1 = l / (B * T2);
         g.c = g.t1 * T2 + g.t2;
     }
     if (AX == 0) g.base = g.t2 * C::PP + g.t1 * C::P + g.e * N;
@@ -783,6 +794,9 @@ using V0 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0>;
 using V1 = Cfg<5, 1, 2, 2, 4, 1, 0, 0, 0, 1, 0>;
 using V2 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0, 2, 2, 2>;
 using V3 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0, 2, 1, 1>;
+using V4 = Cfg<5, 5, 1, 1, 3, 0, 0, 0, 4, 1, 0>;   // 125 lines on 128 threads
+using V5 = Cfg<5, 1, 2, 3, 3, 1, 0, 0, 0, 1, 0>;
+#define DG_MORE_VARIANTS make_table<V4>(), make_table<V5>(),
 #elif DG_N == 6
 using V0 = Cfg<6, 1, 1, 2, 4, 1, 6, 38, 1, 0, 0>;
 using V1 = Cfg<6, 1, 1, 2, 4, 0, 6, 38, 1, 0, 0>;
@@ -804,8 +818,11 @@ using V3 = Cfg<8, 1, 1, 1, 4, 0, 8, 65, 1, 0, 0>;
 
 using VE = Cfg<DG_N, 1, 1, 1, 4, 1>;   // one element per block: always there (tiny and ragged meshes, tests)
 
+#ifndef DG_MORE_VARIANTS
+#define DG_MORE_VARIANTS
+#endif
 const DgKernelTable k_tables[] = {make_table<V0>(), make_table<V1>(), make_table<V2>(), make_table<V3>(),
-                                  make_table<VE>()};
+                                  DG_MORE_VARIANTS make_table<VE>()};
 
 }  // namespace
 
