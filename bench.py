@@ -45,7 +45,9 @@ def ncu_traffic(workload):
     path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
     if os.path.exists(path):
         with open(path) as f:
-            return json.load(f).get(workload)
+            entry = json.load(f).get(workload)
+        if entry:
+            return entry.get("dram_bytes_per_launch")
     return None
 
 
@@ -300,7 +302,7 @@ def run_ours(args, rank, world, local_rank):
                      "frac": achieved / peak, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": ALGO_BYTES_PER_DOF_STAGE * dof,
                      "avg_launch_ms": launch_s * 1e3, "frac_of_8TBs_nominal": achieved / 8000.0,
-                     "traffic": ncu_traffic(args.workload)},
+                     "traffic": ncu_traffic(args.workload), "traffic_unit": "DRAM bytes per launch (ncu, profiles/)"},
         "e2e": {"value": world * dof * STAGES * e2e["steps"] / e2e_s, "unit": UNIT,
                 "h2d_bytes_per_step": e2e["bytes_each_way"], "d2h_bytes_per_step": e2e["bytes_each_way"],
                 "steps": e2e["steps"], "api": "DG.set_state(pinned host) -> DG.rk_step(dt,1) -> DG.get_state(pinned host)"},
