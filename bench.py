@@ -226,6 +226,21 @@ def time_workload(workload, K, W, device, dist, sampler_index=None, want_e2e=Fal
     return out
 
 
+def reduce_max(x, dist, device):
+    """Max over ranks of a per-rank time (replicas: the slowest replica sets the whole-job rate)."""
+    if dist is None:
+        return x
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(dof_per_rank, steps, ms, world):
+    """DOF-updates/s per RK stage of the whole job: every rank advances its own replica (weak scaling)."""
+    return world * dof_per_rank * STAGES * steps / (ms * 1e-3)
+
+
 def run_variant_sweep(args):
     """Tuning aid: one JSON line per compiled stage-kernel variant of the workload's degree (1 GPU)."""
     import torch
@@ -256,15 +271,8 @@ def run_ours(args, rank, world, local_rank):
     K, W = args.steps, max(3, args.warmup)
     main = time_workload(args.workload, K, W, device, dist, physical_gpu_index(local_rank), want_e2e=True)
 
-    def reduce_max(x):
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
-    ms = reduce_max(main["ms"])
-    e2e_s = reduce_max(main["e2e"]["seconds"])
+    ms = reduce_max(main["ms"], dist, device)
+    e2e_s = reduce_max(main["e2e"]["seconds"], dist, device)
     sweep = []
     if not args.no_sweep and world == 1:
         for p in range(1, 8):
@@ -279,7 +287,7 @@ def run_ours(args, rank, world, local_rank):
         return
     peak, peak_src = measured_peaks()
     dof = main["dof"]
-    value = world * dof * STAGES * K / (ms * 1e-3)
+    value = whole_job_rate(dof, K, ms, world)
     launch_s = ms * 1e-3 / main["launches"]                       # the step IS 5 stage-kernel launches
     achieved = ALGO_BYTES_PER_DOF_STAGE * dof / launch_s / 1e9
     for s in sweep:
@@ -303,7 +311,7 @@ def run_ours(args, rank, world, local_rank):
                      "algorithmic_bytes_per_launch": ALGO_BYTES_PER_DOF_STAGE * dof,
                      "avg_launch_ms": launch_s * 1e3, "frac_of_8TBs_nominal": achieved / 8000.0,
                      "traffic": ncu_traffic(args.workload), "traffic_unit": "DRAM bytes per launch (ncu, profiles/)"},
-        "e2e": {"value": world * dof * STAGES * e2e["steps"] / e2e_s, "unit": UNIT,
+        "e2e": {"value": whole_job_rate(dof, e2e["steps"], e2e_s * 1e3, world), "unit": UNIT,
                 "h2d_bytes_per_step": e2e["bytes_each_way"], "d2h_bytes_per_step": e2e["bytes_each_way"],
                 "steps": e2e["steps"], "api": "DG.set_state(pinned host) -> DG.rk_step(dt,1) -> DG.get_state(pinned host)"},
         "p_sweep": sweep,
