@@ -55,7 +55,7 @@ class ClockSampler:
     """Samples SM clock and throttle reasons with NVML while the timed region runs."""
 
     def __init__(self, index):
-        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.samples, self.power, self.reasons, self.max_mhz, self.power_limit = [], [], set(), None, None
         self._stop = threading.Event()
         self._thread = None
         try:
@@ -64,6 +64,7 @@ class ClockSampler:
             self.nv = pynvml
             self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
             self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.power_limit = pynvml.nvmlDeviceGetEnforcedPowerLimit(self.h) / 1000.0
         except Exception:
             self.nv = None
 
@@ -76,6 +77,7 @@ class ClockSampler:
         while not self._stop.is_set():
             try:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
                 bits = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
                 for k, v in names.items():
                     if bits & v:
@@ -99,8 +101,9 @@ class ClockSampler:
         if not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
         s = sorted(self.samples)
+        pw = sorted(self.power)
         return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
-                "samples": len(s)}
+                "samples": len(s), "power_w": pw[len(pw) // 2] if pw else None, "power_limit_w": self.power_limit}
 
 
 def physical_gpu_index(local_rank):
@@ -200,6 +203,14 @@ def time_workload(workload, K, W, device, dist, sampler_index=None, want_e2e=Fal
            "clocks": sampler.summary() if sampler else None}
 
     if want_e2e:
+        # second device-timed number: the max-wavespeed reduction (CFL time step) executed before every step
+        steps_a = min(K, 10)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(steps_a):
+            dg.rk_step(I.cfl_dt(dg.max_wavespeed(), p, ext, n, 0.1), 1)      # max_wavespeed synchronises
+        torch.cuda.synchronize(device)
+        out["adaptive_dt"] = {"seconds": time.perf_counter() - t0, "steps": steps_a}
         # end to end through the public API with HOST buffers: every step copies the state in from
         # pinned host memory, advances one LSERK45 step and copies the result back.
         steps = min(K, 10)
@@ -314,6 +325,9 @@ def run_ours(args, rank, world, local_rank):
         "e2e": {"value": whole_job_rate(dof, e2e["steps"], e2e_s * 1e3, world), "unit": UNIT,
                 "h2d_bytes_per_step": e2e["bytes_each_way"], "d2h_bytes_per_step": e2e["bytes_each_way"],
                 "steps": e2e["steps"], "api": "DG.set_state(pinned host) -> DG.rk_step(dt,1) -> DG.get_state(pinned host)"},
+        "adaptive_dt": {"value": whole_job_rate(dof, main["adaptive_dt"]["steps"], main["adaptive_dt"]["seconds"] * 1e3, world),
+                        "unit": UNIT, "steps": main["adaptive_dt"]["steps"],
+                        "what": "dg_max_wavespeed (device reduction + 8-byte read-back) before every step, dt = CFL rule"},
         "p_sweep": sweep,
         "context": "paper: 1.13e9 DOF-updates/s per V100 (kernels only, derived from Table II, PAPER.md:264-269); "
                    "another machine, not a target",

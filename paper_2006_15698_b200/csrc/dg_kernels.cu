@@ -785,8 +785,8 @@ using V1 = Cfg<3, 2, 2, 2, 7, 0, 6, 38, 2, 0, 0>;
 using V2 = Cfg<3, 2, 2, 2, 7, 1, 6, 38, 2, 0, 0>;
 using V3 = Cfg<3, 4, 4, 2, 2, 0, 12, 156, 3, 0, 0>;
 #elif DG_N == 4
-using V0 = Cfg<4, 2, 2, 2, 3, 1, 9, 74, 1, 1, 2>;
-using V1 = Cfg<4, 2, 2, 2, 3, 0, 9, 74, 1, 1, 2>;
+using V0 = Cfg<4, 2, 2, 2, 3, 0, 9, 74, 1, 1, 2>;
+using V1 = Cfg<4, 2, 2, 2, 3, 1, 9, 74, 1, 1, 2>;
 using V2 = Cfg<4, 2, 2, 1, 6, 1, 8, 65, 3, 0, 0>;
 using V3 = Cfg<4, 2, 2, 1, 6, 0, 8, 65, 3, 0, 0>;
 #elif DG_N == 5
@@ -808,8 +808,8 @@ using V1 = Cfg<7, 1, 1, 2, 3, 0, 7, 55, 1, 0, 0>;
 using V2 = Cfg<7, 1, 1, 1, 6, 1, 7, 55, 1, 0, 0>;
 using V3 = Cfg<7, 1, 1, 1, 6, 0, 7, 55, 1, 0, 0>;
 #elif DG_N == 8
-using V0 = Cfg<8, 1, 1, 2, 2, 1, 8, 65, 1, 1, 0>;
-using V1 = Cfg<8, 1, 1, 2, 2, 0, 8, 65, 1, 1, 0>;
+using V0 = Cfg<8, 1, 1, 2, 2, 0, 8, 65, 1, 1, 0>;
+using V1 = Cfg<8, 1, 1, 2, 2, 1, 8, 65, 1, 1, 0>;
 using V2 = Cfg<8, 1, 1, 1, 4, 1, 8, 65, 1, 0, 0>;
 using V3 = Cfg<8, 1, 1, 1, 4, 0, 8, 65, 1, 0, 0>;
 #else
