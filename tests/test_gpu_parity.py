@@ -194,3 +194,20 @@ def test_fast_math():
     ulp_q = np.abs(q - np.sqrt(x)) / np.spacing(np.sqrt(x))
     assert ulp_r.max() <= 2.0, ulp_r.max()
     assert ulp_q.max() <= 2.0, ulp_q.max()
+
+
+@pytest.mark.parametrize("gamma", [5.0 / 3.0, 1.1])
+def test_other_gas_constants_and_high_orders_on_odd_meshes(gamma):
+    """gamma other than 1.4 (it enters the pressure, the wavespeed and the interface flux), p = 5..7 on meshes
+    that are ragged against the default bricks, residual and two LSERK45 steps."""
+    for p, shape in ((5, (3, 2, 3)), (6, (2, 3, 3)), (7, (3, 3, 1))):
+        nx, ny, nz = shape
+        ext = (0.9, 1.0, 1.7)
+        q = rough_field(nx, ny, nz, p, ext, seed=11)
+        dg = DG(nx, ny, nz, p, gamma, ext)
+        e = relerr(dg.set_state(q).residual(), ORC.residual(q, p, gamma, ext))
+        assert e < TOL_RES, (gamma, p, e)
+        dt = I.cfl_dt(ORC.max_wavespeed(q, p, gamma), p, ext, shape, 0.1)
+        e = relerr(dg.rk_step(dt, 2).get_state(), ORC.rk_step(q, p, gamma, ext, dt, 2))
+        assert e < 1e-12, (gamma, p, e)
+        dg.close()
