@@ -290,7 +290,7 @@ def run_ours(args, rank, world, local_rank):
             s = time_workload(f"cfg4_p{p}", 20, 3, device, None)
             rate = s["dof"] * STAGES * 20 / (s["ms"] * 1e-3)
             sweep.append({"p": p, "elements_per_side": s["elements"][0], "dof": s["dof"], "value": rate,
-                          "ms_per_step": s["ms"] / 20, "brick": [s["kernel"][k] for k in ("bx", "by", "bz")],
+                          "ms_per_step": s["ms"] / 20, "brick": [s["kernel"][k] for k in ("bx", "by", "lz")],
                           "finite": s["finite"]})
     if rank != 0:
         if dist is not None:

@@ -11,16 +11,22 @@
  *
  * Memory ownership: the CALLER allocates all device memory (one workspace of
  * dg_workspace_bytes(), e.g. a torch uint8 tensor) and owns the CUDA stream; the library borrows
- * both from dg_bind() until dg_destroy().  The context itself (host struct + small operator
- * tables in __constant__ memory) is owned by the library.
+ * both from dg_bind() until dg_destroy().  The context itself (a host struct holding the small
+ * operator tables, which travel to the GPU inside the kernel arguments) is owned by the library.
+ *
+ * Stream and device contract: every call after dg_bind() enqueues its work on the stream given to
+ * dg_bind() and assumes that the workspace's device is the calling thread's CURRENT device (the
+ * library never calls cudaSetDevice).  Device pointers passed to dg_set_state / dg_get_state /
+ * dg_residual are read or written in that stream's order: data produced or consumed on another
+ * stream must be ordered against it by the caller (event or synchronise).
  *
  * Canonical array layout of every state-sized argument (`q`, `r`), N = p+1:
  *     a[ ((((e*N + k)*N + j)*N + i)*5 + n ],   n = rho, rho u, rho v, rho w, rho E   (eq (2))
  *     e = ex + nx*(ey + ny*ez)                 (element order: DESIGN.md reading R13)
  * Node (i,j,k) of element (ex,ey,ez) is at x = (ex + (xi_i+1)/2) Lx/nx, ... with xi the
  * N Gauss-Legendre points on [-1,1], ascending.  The library keeps the state in its
- * own brick-major, variable-planar layout; dg_set_state/dg_get_state
- * convert on the device.
+ * own column-layer-major, variable-planar layout; dg_set_state /
+ * dg_get_state convert on the device.
  *
  * Pointers flagged `on_device` are device pointers (same device as the workspace) when
  * on_device != 0, host pointers otherwise (pinned memory makes the copies asynchronous).
@@ -58,29 +64,32 @@ enum {
  * gamma > 1; extents > 0.  Touches no GPU.  *out is set only on DG_OK. */
 int dg_create(dg_ctx **out, int nx, int ny, int nz, int p, double gamma, const double extent[3]);
 
-/* Optional tuning knob, before dg_bind: elements per thread-block "brick" along each axis.  Only
- * the shapes compiled into the library for this p are accepted (DG_EUNSUPPORTED otherwise);
- * bx=by=bz=0 restores the default.  Changes layout sizes, so it is refused after dg_bind. */
-int dg_set_brick(dg_ctx *ctx, int bx, int by, int bz);
+/* Optional tuning knob, before dg_bind: the stage kernel cuts the mesh into COLUMNS of bx x by elements
+ * and a thread block marches through lz consecutive z layers of one column.  Only the
+ * column shapes compiled into the library for this p are accepted (DG_EUNSUPPORTED otherwise);
+ * bx = by = 0 keeps the current shape; lz = 0 lets the library choose the chunk length.  Changes layout
+ * sizes, so it is refused after dg_bind (DG_ESTATE). */
+int dg_set_brick(dg_ctx *ctx, int bx, int by, int lz);
 
-/* Number of stage-kernel variants (brick shape x shared-memory layout x residency) compiled into the
- * library for degree p; 0 when p is outside 1..7.  Variant 0 is the default. */
+/* Number of stage-kernel variants (column shape x shared-memory layout x residency) compiled into the
+ * library for degree p; 0 when p is outside 1..7.  dg_create picks the first variant whose columns
+ * pad the mesh by less than 4 % (variants are listed fastest first). */
 int dg_variant_count(int p);
 
-/* Tuning knob, before dg_bind: select variant 0 <= index < dg_variant_count(p) (DG_EINVAL otherwise).
- * The environment variable DG_VARIANT=<index> sets the default picked by dg_create. */
+/* Tuning knob, before dg_bind: select variant 0 <= index < dg_variant_count(p) (DG_EINVAL otherwise). */
 int dg_set_variant(dg_ctx *ctx, int index);
 
 /* 5*(p+1)^3*nx*ny*nz: number of doubles in a canonical state vector (size_t: config 5 > 2^31). */
 size_t dg_state_len(const dg_ctx *ctx);
 
 /* Device bytes the caller must provide to dg_bind: state Q, Runge-Kutta register K, one
- * canonical staging vector, two face-trace buffers, scalars. */
+ * canonical staging vector, two pairs of face-trace buffers (column boundaries, chunk ends), scalars. */
 size_t dg_workspace_bytes(const dg_ctx *ctx);
 
 /* Borrow `bytes` (>= dg_workspace_bytes) of device memory, 256-byte aligned, and a CUDA stream
  * (cudaStream_t passed as void*; NULL = legacy default stream).  All later work of this context
- * is enqueued on that stream.  Uploads the operator tables (first CUDA call). */
+ * is enqueued on that stream.  First CUDA call of the context: queries the device, opts the kernels in
+ * to their shared-memory size, and zero-fills Q and K when the layout has padding nodes. */
 int dg_bind(dg_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream);
 
 /* Copy a canonical state vector in (host or device), convert it to the internal layout and
@@ -93,13 +102,24 @@ int dg_set_state(dg_ctx *ctx, const double *q, int on_device);
 int dg_residual(dg_ctx *ctx, double *r_out, int on_device);
 
 /* *lam_host = max over nodes of sqrt(u^2+v^2+w^2) + sqrt(gamma p/rho) of the current state
- * (for the caller's CFL time step, reading R10).  Synchronises the stream. */
+ * (for the caller's CFL time step; not in the paper: DESIGN.md reading R10).  After dg_set_state or
+ * dg_rk_step this runs a reduction kernel over the state; after dg_rk_step_cfl the last stage has
+ * already reduced it and the call is an 8-byte read-back.  NaN if any node is non-finite or has
+ * negative pressure or density.  Synchronises the stream. */
 int dg_max_wavespeed(dg_ctx *ctx, double *lam_host);
 
 /* Advance nsteps >= 0 LSERK45 steps of fixed dt:
  * K = 0; for s = 1..5: K = A_s K + dt L(Q); Q = Q + B_s K.  One fused kernel per stage,
  * enqueued on the stream, no host synchronisation. */
 int dg_rk_step(dg_ctx *ctx, double dt, int nsteps);
+
+/* nsteps >= 0 LSERK45 steps, each with its own time step from the CFL rule of reading R10,
+ *     dt = cfl * min(hx,hy,hz) / ((2p+1) * lam_max(Q at the start of the step)),
+ * lam_max reduced on the device by the last stage of the previous step (no extra sweep over the
+ * state; one 8-byte read-back and stream synchronisation per step).  cfl > 0.  On return
+ * *t_advanced = sum of the time steps taken and *dt_last = the last one (host pointers, either may be
+ * NULL).  DG_ESTATE if the wavespeed is not positive and finite. */
+int dg_rk_step_cfl(dg_ctx *ctx, double cfl, int nsteps, double *t_advanced, double *dt_last);
 
 /* Copy the current state out in canonical layout.  Synchronises when q_out is a host pointer. */
 int dg_get_state(dg_ctx *ctx, double *q_out, int on_device);
@@ -110,16 +130,11 @@ int dg_nodes(const dg_ctx *ctx, double *xi, double *w);
 /* Number of CUDA kernels this context has launched so far (bench.py's `gpu_launches`). */
 unsigned long long dg_launch_count(const dg_ctx *ctx);
 
-/* Launch geometry of the fused stage kernel, for reports: out[0..7] = brick elements bx,by,bz,
- * threads per block, dynamic shared bytes per block, resident blocks of the whole GPU (once bound; bricks before), internal (padded)
- * state length in doubles / 2^20 rounded up, face-trace doubles per brick. */
+/* Launch geometry of the fused stage kernel, for reports: out[0..7] = column elements bx, by, layers per
+ * chunk lz, threads per block, dynamic shared bytes per block, resident blocks of the whole GPU (once
+ * bound; thread blocks per launch before), internal (padded) state length in doubles / 2^20 rounded
+ * up, index of the variant in use. */
 int dg_kernel_info(const dg_ctx *ctx, long long out[8]);
-
-/* Self-test of the two device arithmetic helpers the kernels use instead of IEEE division and square
- * root (Newton-corrected hardware seeds, no slow-path branches): rcp_out[i] = 1/x[i] and
- * sqrt_out[i] = sqrt(x[i]) for n positive normal doubles.  All three are DEVICE pointers; the call is
- * enqueued on `cuda_stream` (cudaStream_t as void*).  Test entry, not part of the hot path. */
-int dg_selftest_fastmath(const double *x_dev, double *rcp_out_dev, double *sqrt_out_dev, size_t n, void *cuda_stream);
 
 /* Release the context (never the borrowed workspace).  NULL is accepted. */
 int dg_destroy(dg_ctx *ctx);

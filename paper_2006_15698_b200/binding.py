@@ -27,6 +27,7 @@ SYMBOLS = {
     "dg_residual": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
     "dg_max_wavespeed": (ctypes.c_int, [ctypes.c_void_p, _DP]),
     "dg_rk_step": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int]),
+    "dg_rk_step_cfl": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int, _DP, _DP]),
     "dg_get_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
     "dg_nodes": (ctypes.c_int, [ctypes.c_void_p, _DP, _DP]),
     "dg_launch_count": (ctypes.c_ulonglong, [ctypes.c_void_p]),
@@ -142,7 +143,7 @@ class DG:
     def kernel_info(self):
         out = (ctypes.c_longlong * 8)()
         self._check(self.lib.dg_kernel_info(self._h, out))
-        keys = ("bx", "by", "bz", "threads", "smem_bytes", "grid", "internal_mdoubles", "trace_doubles_per_brick")
+        keys = ("bx", "by", "lz", "threads", "smem_bytes", "grid", "internal_mdoubles", "variant")
         return dict(zip(keys, [int(v) for v in out]))
 
     def nodes(self):
@@ -189,6 +190,14 @@ class DG:
         with self._torch.cuda.device(self.device):
             self._check(self.lib.dg_rk_step(self._h, float(dt), int(nsteps)))
         return self
+
+    def rk_step_cfl(self, cfl, nsteps=1):
+        """nsteps LSERK45 steps, each with dt = cfl * min(h) / ((2p+1) * max wavespeed) of its own initial state.
+        Returns (time advanced, last dt)."""
+        t, dt = ctypes.c_double(0.0), ctypes.c_double(0.0)
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.dg_rk_step_cfl(self._h, float(cfl), int(nsteps), ctypes.byref(t), ctypes.byref(dt)))
+        return t.value, dt.value
 
     def get_state(self, out=None):
         if out is None:

@@ -25,7 +25,8 @@ NVCC_FLAGS = [
 
 def _sources():
     return [os.path.join(CSRC, f) for f in ("dg_kernels.cu", "dg_api.cu", "dg_internal.h")] + [
-        os.path.join(os.path.dirname(HERE), "include", "dg_b200.h")]
+        os.path.join(os.path.dirname(HERE), "include", "dg_b200.h"),
+        os.path.join(os.path.dirname(HERE), "include", "dg_b200_test.h")]
 
 
 def _stale(target, deps):

@@ -2,6 +2,7 @@
 // tables and kernel launches.  No arithmetic of the method runs here; it all runs in dg_kernels.cu.
 // Shares nothing with oracle/ (the operator construction below is written independently).
 #include "../../include/dg_b200.h"
+#include "../../include/dg_b200_test.h"
 #include "dg_internal.h"
 
 #include <cmath>
@@ -149,17 +150,21 @@ struct dg_ctx {
     double gamma;
     double extent[3];
     const DgKernelTable *kt;
-    int nbx, nby, nbz;
-    size_t nbricks;
+    int variant;
+    int nbx, nby;       // columns of bx x by elements
+    int lz, nchunks;    // layers per chunk (one thread block marches through one chunk of one column)
+    int lz_user;        // 0 = heuristic
+    size_t nslots;      // layer slots = nbx * nby * nz
     size_t state_len;   // canonical doubles
-    size_t int_len;     // internal (brick-padded) doubles
-    size_t trace_len;   // doubles per trace buffer
+    size_t int_len;     // internal (column-padded) doubles
+    size_t txy_len;     // doubles per x/y trace buffer
+    size_t tz_len;      // doubles per z trace buffer
     // borrowed workspace
-    double *Q, *K, *S, *T[2];
+    double *Q, *K, *S, *Txy[2], *Tz[2];
     unsigned long long *scal;
-    int tcur;           // T[tcur] holds the traces of the current Q
-    int grid;           // resident blocks per SM x SMs, capped by the brick count (L2 prefetch distance)
-    int flags;          // DG_FLAGS tuning knobs, see DgStageArgs
+    int tcur;           // Txy[tcur], Tz[tcur] hold the traces of the current Q
+    bool lam_valid;     // scal[0] holds the max wavespeed of the current Q (reduced by the last stage)
+    int sms, blocks_per_sm;
     DgOps ops;          // device operator tables of this mesh (travel in the kernel arguments)
     bool bound, has_state;
     cudaStream_t stream;
@@ -183,18 +188,42 @@ int cuda_fail(dg_ctx *c, cudaError_t e, const char *what) {
     return fail(c, DG_ECUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 
-void set_layout(dg_ctx *c, const DgKernelTable *kt) {
+// Layers per chunk: enough blocks to fill the GPU several times over with a small tail, chunks long enough
+// that the extra work at their two ends (pipeline fill, one more interface flux, z traces through HBM)
+// stays small.  `resident` = thread blocks the whole GPU holds at once.
+int pick_lz(int columns, int nz, long long resident) {
+    int best = 1;
+    double best_score = -1.0;
+    for (int lz = 1; lz <= nz && lz <= 64; ++lz) {
+        const long long blocks = (long long)columns * ((nz + lz - 1) / lz);
+        const double waves = (double)blocks / (double)resident;
+        const double fill = waves / std::ceil(waves);
+        const double score = fill * (double)lz / ((double)lz + 0.6);
+        if (score > best_score + 1e-12) {
+            best_score = score;
+            best = lz;
+        }
+    }
+    return best;
+}
+
+void set_layout(dg_ctx *c, int variant, const DgKernelTable *kt) {
     c->kt = kt;
+    c->variant = variant;
     c->nbx = (c->nx + kt->bx - 1) / kt->bx;
     c->nby = (c->ny + kt->by - 1) / kt->by;
-    c->nbz = (c->nz + kt->bz - 1) / kt->bz;
-    c->nbricks = (size_t)c->nbx * c->nby * c->nbz;
-    c->int_len = c->nbricks * (size_t)kt->slot;
-    c->trace_len = c->nbricks * (size_t)kt->tslot;
+    const int sms = c->sms > 0 ? c->sms : 148;
+    c->lz = c->lz_user > 0 ? (c->lz_user < c->nz ? c->lz_user : c->nz)
+                           : pick_lz(c->nbx * c->nby, c->nz, (long long)sms * (kt->minb > 0 ? kt->minb : 1));
+    c->nchunks = (c->nz + c->lz - 1) / c->lz;
+    c->nslots = (size_t)c->nbx * c->nby * c->nz;
+    c->int_len = c->nslots * (size_t)kt->slot;
+    c->txy_len = c->nslots * (size_t)kt->txy;
+    c->tz_len = (size_t)c->nbx * c->nby * c->nchunks * (size_t)kt->tz;
 }
 
 struct Carve {
-    size_t q, k, s, t0, t1, scal, total;
+    size_t q, k, s, txy0, txy1, tz0, tz1, scal, total;
 };
 Carve carve(const dg_ctx *c) {
     Carve v;
@@ -202,8 +231,10 @@ Carve carve(const dg_ctx *c) {
     v.q = off;    off += align_up(c->int_len * 8 + 16, 256);   // +16: the L2 prefetch rounds out to 16-byte granules
     v.k = off;    off += align_up(c->int_len * 8 + 16, 256);
     v.s = off;    off += align_up(c->state_len * 8, 256);
-    v.t0 = off;   off += align_up(c->trace_len * 8, 256);
-    v.t1 = off;   off += align_up(c->trace_len * 8, 256);
+    v.txy0 = off; off += align_up(c->txy_len * 8 + 16, 256);
+    v.txy1 = off; off += align_up(c->txy_len * 8 + 16, 256);
+    v.tz0 = off;  off += align_up(c->tz_len * 8, 256);
+    v.tz1 = off;  off += align_up(c->tz_len * 8, 256);
     v.scal = off; off += 256;
     v.total = off;
     return v;
@@ -213,17 +244,18 @@ DgStageArgs stage_args(const dg_ctx *c, int mode) {
     DgStageArgs a;
     std::memset(&a, 0, sizeof(a));
     a.Q = c->Q;
-    a.K = c->K;
-    a.Rout = c->K;   // the Runge-Kutta register is dead between steps: residual output lands there
-    a.Told = c->T[c->tcur];
-    a.Tnew = c->T[1 - c->tcur];
+    a.K = c->K;   // residual mode: the Runge-Kutta register is dead between steps, the residual lands there
+    a.Txy_old = c->Txy[c->tcur];
+    a.Txy_new = c->Txy[1 - c->tcur];
+    a.Tz_old = c->Tz[c->tcur];
+    a.Tz_new = c->Tz[1 - c->tcur];
+    a.lam_bits = c->scal;
     a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
-    a.nbx = c->nbx; a.nby = c->nby; a.nbz = c->nbz;
+    a.nbx = c->nbx; a.nby = c->nby;
+    a.lz = c->lz; a.nchunks = c->nchunks;
     a.gamma = c->gamma;
     a.gm1 = c->gamma - 1.0;
     a.mode = mode;
-    a.grid = c->grid;
-    a.flags = c->flags;
     a.ops = c->ops;
     return a;
 }
@@ -233,9 +265,9 @@ int launch_layout(dg_ctx *c, double *internal, double *canonical, int to_interna
     a.internal = internal;
     a.canonical = canonical;
     a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
-    a.nbx = c->nbx; a.nby = c->nby; a.nbz = c->nbz;
+    a.nbx = c->nbx; a.nby = c->nby;
     a.to_internal = to_internal;
-    cudaError_t e = c->kt->launch_layout(a, c->stream);
+    cudaError_t e = c->kt->launch_layout(a, c->sms, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "layout kernel");
     c->launches++;
     return DG_OK;
@@ -250,6 +282,51 @@ int export_vector(dg_ctx *c, double *internal, double *out, int on_device, const
     if (e != cudaSuccess) return cuda_fail(c, e, what);
     e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, what);
+    return DG_OK;
+}
+
+// One LSERK45 step = 5 launches of the fused stage kernel; the last stage can reduce the max wavespeed
+// of the state it produces on the way (a9 fused: no extra sweep over the state).
+int enqueue_step(dg_ctx *c, const DgOps &scaled, bool want_lam) {
+    for (int s = 0; s < 5; ++s) {
+        DgStageArgs a = stage_args(c, DG_MODE_STAGE);
+        a.ops = scaled;
+        a.rkA = (double)kRkA[s];
+        a.rkB = (double)kRkB[s];
+        a.want_lam = (want_lam && s == 4) ? 1 : 0;
+        if (a.want_lam) {
+            cudaError_t e = cudaMemsetAsync(c->scal, 0, 8, c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e, "memset");
+        }
+        cudaError_t e = c->kt->launch_stage(a, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "stage kernel");
+        c->launches++;
+        c->tcur = 1 - c->tcur;
+    }
+    c->lam_valid = want_lam;
+    return DG_OK;
+}
+
+int read_lam(dg_ctx *c, double *lam_host) {
+    if (!c->lam_valid) {
+        cudaError_t e = cudaMemsetAsync(c->scal, 0, 8, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "memset");
+        DgWaveArgs a;
+        a.Q = c->Q;
+        a.lam_bits = c->scal;
+        a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
+        a.nbx = c->nbx; a.nby = c->nby;
+        a.gamma = c->gamma;
+        a.gm1 = c->gamma - 1.0;
+        e = c->kt->launch_wavespeed(a, c->sms, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "wavespeed kernel");
+        c->launches++;
+        c->lam_valid = true;
+    }
+    cudaError_t e = cudaMemcpyAsync(lam_host, c->scal, 8, cudaMemcpyDeviceToHost, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "device->host copy");
+    e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "synchronise");
     return DG_OK;
 }
 
@@ -274,32 +351,45 @@ int dg_create(dg_ctx **out, int nx, int ny, int nz, int p, double gamma, const d
     c->gamma = gamma;
     for (int a = 0; a < 3; ++a) c->extent[a] = extent[a];
     c->state_len = (size_t)nx * ny * nz * (size_t)(c->N * c->N * c->N) * DG_NV;
+    // default variant: the first compiled column shape that wastes < 4 % of its nodes on padding of ragged
+    // columns (they are listed fastest first), else the one that wastes least
     int pick = 0;
-    if (const char *ev = std::getenv("DG_VARIANT")) {   // tuning knob: index into this p's compiled variants
-        const int v = std::atoi(ev);
-        if (v >= 0 && v < count) pick = v;
+    double best_waste = 1e30;
+    for (int v = 0; v < count; ++v) {
+        const double padded = (double)((nx + kt[v].bx - 1) / kt[v].bx * kt[v].bx) * ((ny + kt[v].by - 1) / kt[v].by * kt[v].by);
+        const double waste = padded / ((double)nx * ny) - 1.0;
+        if (waste < 0.04) {
+            pick = v;
+            break;
+        }
+        if (waste < best_waste) {
+            best_waste = waste;
+            pick = v;
+        }
     }
-    if (const char *ev = std::getenv("DG_FLAGS")) c->flags = std::atoi(ev);
-    set_layout(c, &kt[pick]);
+    set_layout(c, pick, &kt[pick]);
     *out = c;
     return DG_OK;
 }
 
-int dg_set_brick(dg_ctx *c, int bx, int by, int bz) {
+int dg_set_brick(dg_ctx *c, int bx, int by, int lz) {
     if (!c) return DG_EINVAL;
     if (c->bound) return fail(c, DG_ESTATE, "dg_set_brick after dg_bind");
+    if (bx < 0 || by < 0 || lz < 0) return fail(c, DG_EINVAL, "negative brick size");
     int count = 0;
     const DgKernelTable *kt = variants_for(c->N, &count);
-    if (bx == 0 && by == 0 && bz == 0) {
-        set_layout(c, &kt[0]);
+    if (bx == 0 && by == 0) {
+        c->lz_user = lz;
+        set_layout(c, c->variant, c->kt);
         return DG_OK;
     }
     for (int v = 0; v < count; ++v)
-        if (kt[v].bx == bx && kt[v].by == by && kt[v].bz == bz) {
-            set_layout(c, &kt[v]);
+        if (kt[v].bx == bx && kt[v].by == by) {
+            c->lz_user = lz;
+            set_layout(c, v, &kt[v]);
             return DG_OK;
         }
-    return fail(c, DG_EUNSUPPORTED, "brick %dx%dx%d is not compiled for p=%d", bx, by, bz, c->p);
+    return fail(c, DG_EUNSUPPORTED, "column %dx%d is not compiled for p=%d", bx, by, c->p);
 }
 
 int dg_variant_count(int p) {
@@ -315,7 +405,7 @@ int dg_set_variant(dg_ctx *c, int index) {
     int count = 0;
     const DgKernelTable *kt = variants_for(c->N, &count);
     if (index < 0 || index >= count) return fail(c, DG_EINVAL, "variant %d outside 0..%d", index, count - 1);
-    set_layout(c, &kt[index]);
+    set_layout(c, index, &kt[index]);
     return DG_OK;
 }
 
@@ -328,28 +418,41 @@ int dg_bind(dg_ctx *c, void *ws, size_t bytes, void *stream) {
     if (!ws || ((size_t)ws & 255u)) return fail(c, DG_EINVAL, "workspace must be a 256-byte aligned device pointer");
     const Carve v = carve(c);
     if (bytes < v.total) return fail(c, DG_ENOMEM, "workspace %zu bytes < required %zu", bytes, v.total);
-    if (c->nbricks > 2147483647ull) return fail(c, DG_EUNSUPPORTED, "more than 2^31-1 bricks");
+    if (c->nby > 65535 || c->nchunks > 65535) return fail(c, DG_EUNSUPPORTED, "more than 65535 columns along y or chunks");
     char *base = (char *)ws;
     c->Q = (double *)(base + v.q);
     c->K = (double *)(base + v.k);
     c->S = (double *)(base + v.s);
-    c->T[0] = (double *)(base + v.t0);
-    c->T[1] = (double *)(base + v.t1);
+    c->Txy[0] = (double *)(base + v.txy0);
+    c->Txy[1] = (double *)(base + v.txy1);
+    c->Tz[0] = (double *)(base + v.tz0);
+    c->Tz[1] = (double *)(base + v.tz1);
     c->scal = (unsigned long long *)(base + v.scal);
     c->stream = (cudaStream_t)stream;
     c->tcur = 0;
     c->has_state = false;
-    // bricks of a ragged mesh carry padding nodes that are staged but never used: give them a defined value
-    cudaError_t e = cudaMemsetAsync(base, 0, v.total, c->stream);
+    c->lam_valid = false;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return cuda_fail(c, e, "device query");
+    // The nodes that pad ragged columns (and the even-pitch pad of every plane) travel with the bulk copies but are
+    // never used: give them a defined value.  Only Q and K have such nodes; a mesh the columns tile exactly
+    // with even planes has none.
+    const bool padded = (c->nx % c->kt->bx) || (c->ny % c->kt->by) ||
+                        ((size_t)c->kt->slot != (size_t)DG_NV * c->N * c->N * c->N * c->kt->bx * c->kt->by);
+    if (padded) {
+        e = cudaMemsetAsync(c->Q, 0, c->int_len * 8, c->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->K, 0, c->int_len * 8, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "workspace memset");
+    }
+    e = cudaMemsetAsync(c->scal, 0, 256, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "workspace memset");
     const double g[3] = {2.0 / (c->extent[0] / c->nx), 2.0 / (c->extent[1] / c->ny), 2.0 / (c->extent[2] / c->nz)};
     build_device_ops(c->N, g, c->ops);
-    int resident = 0;
-    e = c->kt->prepare(&resident);
+    e = c->kt->prepare(&c->blocks_per_sm);
     if (e != cudaSuccess) return cuda_fail(c, e, "stage kernel setup");
-    if (resident < 1) return fail(c, DG_ECUDA, "stage kernel does not fit on the GPU");
-    if (c->nby > 65535 || c->nbz > 65535) return fail(c, DG_EUNSUPPORTED, "more than 65535 bricks along y or z");
-    c->grid = resident;   // how far ahead (in dispatch order) the L2 prefetch looks
+    if (c->blocks_per_sm < 1) return fail(c, DG_ECUDA, "stage kernel does not fit on the GPU");
     c->bound = true;
     c->err[0] = 0;
     return DG_OK;
@@ -366,15 +469,25 @@ int dg_set_state(dg_ctx *c, const double *q, int on_device) {
     }
     int rc = launch_layout(c, c->Q, const_cast<double *>(src), 1);
     if (rc != DG_OK) return rc;
-    // traces of the new state into T[tcur]
+    // traces of the new state into buffer 0
     c->tcur = 0;
-    DgStageArgs a = stage_args(c, DG_MODE_TRACES);
-    a.Tnew = c->T[0];
-    a.Told = c->T[1];
-    cudaError_t e = c->kt->launch_stage(a, c->stream);
+    DgTraceArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.Q = c->Q;
+    a.Txy = c->Txy[0];
+    a.Tz = c->Tz[0];
+    a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
+    a.nbx = c->nbx; a.nby = c->nby;
+    a.lz = c->lz; a.nchunks = c->nchunks;
+    for (int i = 0; i < DG_NMAX; ++i) {
+        a.lp[i] = c->ops.lp[i];
+        a.lm[i] = c->ops.lm[i];
+    }
+    cudaError_t e = c->kt->launch_traces(a, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "trace kernel");
     c->launches++;
     c->has_state = true;
+    c->lam_valid = false;
     return DG_OK;
 }
 
@@ -391,23 +504,7 @@ int dg_residual(dg_ctx *c, double *r_out, int on_device) {
 int dg_max_wavespeed(dg_ctx *c, double *lam_host) {
     if (!c || !lam_host) return c ? fail(c, DG_EINVAL, "null pointer") : DG_EINVAL;
     if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_max_wavespeed needs dg_bind and dg_set_state first");
-    cudaError_t e = cudaMemsetAsync(c->scal, 0, 8, c->stream);
-    if (e != cudaSuccess) return cuda_fail(c, e, "memset");
-    DgWaveArgs a;
-    a.Q = c->Q;
-    a.lam_bits = c->scal;
-    a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
-    a.nbx = c->nbx; a.nby = c->nby; a.nbz = c->nbz;
-    a.gamma = c->gamma;
-    a.gm1 = c->gamma - 1.0;
-    e = c->kt->launch_wavespeed(a, c->stream);
-    if (e != cudaSuccess) return cuda_fail(c, e, "wavespeed kernel");
-    c->launches++;
-    e = cudaMemcpyAsync(lam_host, c->scal, 8, cudaMemcpyDeviceToHost, c->stream);
-    if (e != cudaSuccess) return cuda_fail(c, e, "device->host copy");
-    e = cudaStreamSynchronize(c->stream);
-    if (e != cudaSuccess) return cuda_fail(c, e, "synchronise");
-    return DG_OK;
+    return read_lam(c, lam_host);
 }
 
 int dg_rk_step(dg_ctx *c, double dt, int nsteps) {
@@ -417,18 +514,34 @@ int dg_rk_step(dg_ctx *c, double dt, int nsteps) {
     DgOps scaled;
     scale_ops(c->ops, dt, scaled);
     for (int step = 0; step < nsteps; ++step) {
-        for (int s = 0; s < 5; ++s) {
-            DgStageArgs a = stage_args(c, DG_MODE_STAGE);
-            a.ops = scaled;
-            a.rkA = (double)kRkA[s];
-            a.rkB = (double)kRkB[s];
-            a.dt = dt;
-            cudaError_t e = c->kt->launch_stage(a, c->stream);
-            if (e != cudaSuccess) return cuda_fail(c, e, "stage kernel");
-            c->launches++;
-            c->tcur = 1 - c->tcur;
-        }
+        const int rc = enqueue_step(c, scaled, false);
+        if (rc != DG_OK) return rc;
     }
+    return DG_OK;
+}
+
+int dg_rk_step_cfl(dg_ctx *c, double cfl, int nsteps, double *t_advanced, double *dt_last) {
+    if (!c) return DG_EINVAL;
+    if (nsteps < 0 || !(cfl > 0.0) || !std::isfinite(cfl)) return fail(c, DG_EINVAL, "nsteps < 0 or cfl not positive");
+    if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_rk_step_cfl needs dg_bind and dg_set_state first");
+    double hmin = c->extent[0] / c->nx;
+    if (c->extent[1] / c->ny < hmin) hmin = c->extent[1] / c->ny;
+    if (c->extent[2] / c->nz < hmin) hmin = c->extent[2] / c->nz;
+    double t = 0.0, dt = 0.0;
+    for (int step = 0; step < nsteps; ++step) {
+        double lam = 0.0;
+        int rc = read_lam(c, &lam);   // 8-byte read-back; reduced by the previous step's last stage
+        if (rc != DG_OK) return rc;
+        if (!(lam > 0.0) || !std::isfinite(lam)) return fail(c, DG_ESTATE, "max wavespeed %g is not positive and finite", lam);
+        dt = cfl * hmin / ((2.0 * c->p + 1.0) * lam);
+        DgOps scaled;
+        scale_ops(c->ops, dt, scaled);
+        rc = enqueue_step(c, scaled, true);
+        if (rc != DG_OK) return rc;
+        t += dt;
+    }
+    if (t_advanced) *t_advanced = t;
+    if (dt_last) *dt_last = dt;
     return DG_OK;
 }
 
@@ -453,12 +566,12 @@ unsigned long long dg_launch_count(const dg_ctx *c) { return c ? c->launches : 0
 
 int dg_kernel_info(const dg_ctx *c, long long out[8]) {
     if (!c || !out) return DG_EINVAL;
-    out[0] = c->kt->bx; out[1] = c->kt->by; out[2] = c->kt->bz;
+    out[0] = c->kt->bx; out[1] = c->kt->by; out[2] = c->lz;
     out[3] = c->kt->threads;
     out[4] = c->kt->smem_bytes;
-    out[5] = c->bound ? (long long)c->grid : (long long)c->nbricks;
+    out[5] = c->bound ? (long long)c->blocks_per_sm * c->sms : (long long)c->nbx * c->nby * c->nchunks;
     out[6] = (long long)((c->int_len + (1u << 20) - 1) >> 20);
-    out[7] = c->kt->tslot;
+    out[7] = c->variant;
     return DG_OK;
 }
 

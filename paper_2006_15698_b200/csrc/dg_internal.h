@@ -11,8 +11,8 @@
 // 1-D operators of the collocated Gauss-Legendre Lagrange basis, built on the
 // host in long double (dg_api.cu) with the constant geometric factor 2/h_a of each axis
 // folded in, rounded to double once.  In the Runge-Kutta stage kernel Dg, lpg and lmg
-// are additionally multiplied by the time step (dg_rk_step), so the kernel accumulates dt * L(Q).  They travel inside the kernel
-// arguments (constant bank; per context, so contexts with different meshes can coexist).
+// are additionally multiplied by the time step (dg_rk_step), so the kernel accumulates dt * L(Q).  They
+// travel inside the kernel arguments (constant bank; per context, so contexts with different meshes coexist).
 struct DgOps {
     double Dg[3][DG_NMAX][DG_NMAX];     // Dg[a][q][i] = (2/h_a) w_q l_i'(xi_q) / w_i   (eq (5) 2nd term / mass)
     double lpg[3][DG_NMAX];             // 1/2 (2/h_a) l_i(+1) / w_i     (lift / mass; the kernel forms 2 F*)
@@ -23,9 +23,9 @@ struct DgOps {
 #ifdef __CUDACC__
 // Branch-free reciprocal and square root for positive, normal arguments (densities, gamma p / rho):
 // hardware seed (MUFU.RCP64H / MUFU.RSQ64H, good to about 2^-20) and ONE cubic correction; measured error
-// <= 1 ulp (reciprocal) and <= 2 ulp (square root) over 14 decades (dg_selftest_fastmath exposes them;
-// tests/test_gpu_parity.py::test_fast_math), with none of the slow-path branches of the IEEE-rounded
-// library routines and about half their operations.
+// <= 1 ulp (reciprocal) and <= 2 ulp (square root) over 14 decades (dg_selftest_fastmath in dg_b200_test.h
+// exposes them; tests/test_gpu_parity.py::test_fast_math), with none of the slow-path branches of the
+// IEEE-rounded library routines and about half their operations.
 __device__ __forceinline__ double rcp_pos(double x) {
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
@@ -39,57 +39,72 @@ __device__ __forceinline__ double sqrt_pos(double x) {
     y = fma(y, e * fma(0.375, e, 0.5), y);          // y (1 + e/2 + 3 e^2/8)
     return x * y;
 }
-
 #endif
 
 enum DgMode {
     DG_MODE_STAGE = 0,     // full Runge-Kutta stage: residual + K,Q update + new traces
-    DG_MODE_RESIDUAL = 1,  // residual only, written to Rout (internal layout)
-    DG_MODE_TRACES = 2     // face traces of Q only (after dg_set_state)
+    DG_MODE_RESIDUAL = 1   // residual only, written to the K array (internal layout)
 };
 
 // Arguments of the fused stage kernel (passed by value, lives in the constant bank).
+//
+// Internal layout: the mesh is cut into COLUMNS of BX x BY elements; one "layer" of a column
+// (BX x BY x 1 elements) is one contiguous slot [n][k][HP] of Q and K, HP = the (gy,gx) node plane padded to
+// an even number of doubles; slot index = (ez * nby + by) * nbx + bx.
 struct DgStageArgs {
-    double *Q;            // state, internal layout [brick][n][gz][gy][gx]
-    double *K;            // Runge-Kutta register, same layout
-    double *Rout;         // residual output (mode RESIDUAL)
-    const double *Told;   // brick-boundary face traces of the current Q
-    double *Tnew;         // ... of the updated Q (mode STAGE / TRACES)
+    double *Q;            // state
+    double *K;            // Runge-Kutta register (RESIDUAL mode: the residual lands here)
+    const double *Txy_old;  // x and y face traces of the current Q on the column boundaries, per layer slot
+    double *Txy_new;        // ... of the updated Q
+    const double *Tz_old;   // z face traces of the current Q at the ends of every chunk of lz layers, per chunk slot
+    double *Tz_new;
+    unsigned long long *lam_bits;   // LAM kernels: max wavespeed of the updated state (bit pattern, atomicMax)
     int nx, ny, nz;       // elements per axis
-    int nbx, nby, nbz;    // bricks per axis
+    int nbx, nby;         // columns per axis
+    int lz, nchunks;      // layers per chunk (the unit of work of one thread block), chunks per column
     double gamma, gm1;
-    double rkA, rkB, dt;  // stage coefficients; rkA == 0 means "do not read K" (stage 1)
+    double rkA, rkB;      // stage coefficients; rkA == 0 means "do not read K" (stage 1)
     int mode;
-    int grid;             // resident blocks of the whole GPU = how far ahead (in bricks) the L2 prefetch looks
-    int flags;            // tuning knobs (DG_FLAGS): 1 = no L2 prefetch, 2 = prefetch at block start
+    int want_lam;
     DgOps ops;
 };
 
+struct DgTraceArgs {
+    const double *Q;
+    double *Txy, *Tz;
+    int nx, ny, nz, nbx, nby, lz, nchunks;
+    double lp[DG_NMAX], lm[DG_NMAX];
+};
+
 struct DgLayoutArgs {
-    double *internal;       // [brick][n][gz][gy][gx]
+    double *internal;
     double *canonical;      // [e][k][j][i][n]
-    int nx, ny, nz, nbx, nby, nbz;
+    int nx, ny, nz, nbx, nby;
     int to_internal;        // 1: canonical -> internal, 0: internal -> canonical
 };
 
 struct DgWaveArgs {
     const double *Q;
     unsigned long long *lam_bits;  // max reduced on the bit pattern (non-negative doubles order as integers)
-    int nx, ny, nz, nbx, nby, nbz;
+    int nx, ny, nz, nbx, nby;
     double gamma, gm1;
 };
 
-// One compiled (N, brick shape) variant.
+// One compiled (N, column shape) variant.
 struct DgKernelTable {
-    int N, bx, by, bz;
-    int threads;             // threads per block of the stage kernel
+    int N, bx, by;
+    int threads;             // threads per block of the stage kernel (compute warps + 1 copy warp)
     int smem_bytes;          // dynamic shared memory of the stage kernel
-    long long slot;          // doubles per brick in Q/K/R (5 * nodes per brick)
-    long long tslot;         // face-trace doubles per brick
-    cudaError_t (*prepare)(int *resident);        // opt in to the shared memory size; resident blocks of the GPU
+    long long slot;          // doubles per layer slot in Q/K
+    long long txy;           // x/y face-trace doubles per layer slot
+    long long tz;            // z face-trace doubles per chunk slot
+    int reload;
+    int minb;                // blocks per SM the kernel is compiled for (__launch_bounds__)
+    cudaError_t (*prepare)(int *blocks_per_sm);   // opt in to the shared memory size; resident blocks per SM
     cudaError_t (*launch_stage)(const DgStageArgs &a, cudaStream_t s);
-    cudaError_t (*launch_layout)(const DgLayoutArgs &a, cudaStream_t s);
-    cudaError_t (*launch_wavespeed)(const DgWaveArgs &a, cudaStream_t s);
+    cudaError_t (*launch_traces)(const DgTraceArgs &a, cudaStream_t s);
+    cudaError_t (*launch_layout)(const DgLayoutArgs &a, int sms, cudaStream_t s);
+    cudaError_t (*launch_wavespeed)(const DgWaveArgs &a, int sms, cudaStream_t s);
 };
 
 // Each kernel TU exports its variants: dg_variants_N<N>(&count) -> array of tables, default first.

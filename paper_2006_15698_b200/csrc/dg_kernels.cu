@@ -1,26 +1,29 @@
 // dg_kernels.cu -- CUDA kernels of the DG Euler time step for one N = p+1 (compile with -DDG_N=<N>,
 // -gencode arch=compute_100a,code=sm_100a).  Hand-written for B200; fp64 throughout.
 //
-// The fused stage kernel (v4): ONE thread block per "brick" of BX x BY x BZ elements, one thread per node
-// LINE, every shared-memory stride a compile-time constant.  Per brick, in ONE sweep over HBM:
-//   P0  cp.async (no registers) of the brick's Q and K (5 x nodes each, separate groups) into shared memory
-//   then, for the axes x, y, z in turn (three instances of one template):
-//   PH  the neighbour bricks' face traces this line touches go straight from HBM/L2 into registers
-//   PT  the line's N nodal values into registers (RELOAD variants: read again later instead) and the two
-//       face traces T+- = sum_q l_q(+-1) Q_q
-//   PB  local Lax-Friedrichs interface flux, doubled, at the + end of the line, and at the
-//       - end of the lines that start on the brick boundary (faces inside a brick: once, handed over
-//       through shared memory; cluster variants: also across the blocks of a cluster)
+// The fused stage kernel (v5, "column sweep"): the mesh is cut into columns of BX x BY elements; ONE thread
+// block marches through `lz` consecutive z layers (BX x BY x 1 elements each) of one column.  Per layer, in
+// ONE sweep over HBM:
+//   copy warp   cp.async.bulk (TMA engine, mbarrier completion) brings the layer's Q and K slots into a ring
+//               of shared-memory buffers one to two layers ahead of their use and writes the updated Q and K
+//               back with cp.async.bulk stores: no thread ever touches Q or K in global memory
+//   compute warps, one thread per node LINE, for the axes x, y, z in turn (instances of one template):
+//   PH  the neighbour columns' face traces this line touches go straight from HBM/L2 into registers (x, y);
+//       along z the upper neighbour is the NEXT layer of the ring (its trace is taken from shared memory) and
+//       the lower face's flux is the one this thread computed for the previous layer (kept in registers):
+//       z traces go through HBM only at the two ends of a chunk
+//   PT  the line's N nodal values into registers and the two face traces T+- = sum_q l_q(+-1) Q_q
+//   PB  local Lax-Friedrichs interface flux, doubled: faces inside a column once (x, y: handed
+//       over through shared memory; z: carried in registers), faces on the column boundary by both sides
 //   PC  lift with 2/h, 1/2 and dt folded into the tables starts the accumulators:
 //       r_i = sum_q Dhat_iq F_q - (l_i(+1) F*_+ - l_i(-1) F*_-) (2/h_a)/w_i       (eq (5) 3rd and 2nd term)
 //   PA  pointwise Euler flux (eq (2)-(3)) at the line's N nodes and the sum-factorised
 //       derivative (the contraction of listing lines 220-237), all in registers
 //   PD  LSERK45 accumulated in place on the staged K:  x: K = A K + r_x,  y: K += r_y,
-//       z: K += r_z, Q += B K, both written straight to HBM from the z lines (coalesced, streaming);
-//       or R itself in residual mode.  Before the z pass: L2 prefetch of the follow-on brick's data.
-//   PE  face traces of the UPDATED Q on the brick boundary, written to the other trace buffer
-// so that Q and K are read once and written once per stage and no element ever needs another
-// element's nodal values: neighbours meet only through the double-buffered brick-boundary traces.
+//       z: K += r_z, Q += B K, both left in shared memory for the copy warp; or R itself in residual mode
+//   PE  x / y face traces of the UPDATED Q on the column boundary, written to the other trace buffer
+// so that Q and K are read once and written once per stage and no block ever needs another block's nodal
+// values: neighbours meet only through the double-buffered column-boundary traces.
 //
 // Nothing here is shared with oracle/ (separate source, separate operator construction).
 #include "dg_internal.h"
@@ -36,81 +39,100 @@ namespace {
 // ------------------------------------------------------------------------------------------------
 // compile-time geometry of one variant
 // ------------------------------------------------------------------------------------------------
-// Shared-memory layout of a brick: [5][GZ] planes of pitch PP doubles, rows of pitch P doubles inside a
-// plane, and, per axis, the order in which a warp's lanes walk the node lines (ORD):
+// Shared-memory layout of a layer: [5][N] planes (variable, z node k) of pitch PP doubles, dense rows of GX
+// doubles inside a plane, and, per axis, the order in which a warp's lanes walk the node lines (ORD):
 //   0: t1 fastest, then t2, then the element e along the axis      1: t2, t1, e
 //   2: t1, e, t2                                                   3: t2, e, t1
 //   4: e, t1, t2                                                   5: e, t2, t1
-// (t1,t2) = (gy,gz) for x lines, (gx,gz) for y lines, (gx,gy) for z lines.  P, PP and the orders are picked
-// per brick shape so that the 16 lanes of a half-warp hit 16 different 8-byte bank pairs in all three
-// passes (0 = dense).  z lines keep t1 = gx fastest: their lanes also
-// address HBM.
-// CLX x CLY x CLZ > 1: the blocks of that many neighbouring bricks form a thread-block CLUSTER and hand the traces
-// of the faces they share to each other through distributed shared memory instead of the HBM trace buffer.
-template <int N_, int BX_, int BY_, int BZ_, int MINB_, int RELOAD_ = 0, int P_ = 0, int PP_ = 0, int OX_ = 0,
-          int OY_ = 0, int OZ_ = 0, int CLX_ = 1, int CLY_ = 1, int CLZ_ = 1>
+// (t1,t2) = (gy,k) for x lines, (gx,k) for y lines, (gx,gy) for z lines.  PP (even: planes stay 16-byte
+// aligned for the bulk copies) and the orders are picked per column shape so that the 16 lanes of a
+// half-warp hit different 8-byte bank pairs where such a choice exists.
+template <int N_, int BX_, int BY_, int MINB_, int RELOAD_ = 0, int PP_ = 0, int OX_ = 0, int OY_ = 0>
 struct Cfg {
-    static constexpr int CLX = CLX_, CLY = CLY_, CLZ = CLZ_, CLUSTER = CLX_ * CLY_ * CLZ_;
-    static constexpr int N = N_, BX = BX_, BY = BY_, BZ = BZ_, MINB = MINB_;
+    static constexpr int N = N_, BX = BX_, BY = BY_, MINB = MINB_;
     // RELOAD = 1: the volume term reads the line's Q from shared memory a second time instead of keeping
-    // it in 10 N registers across the interface fluxes (fewer registers, more blocks per SM, 15 more
-    // shared loads per node)
+    // it in 10 N registers across the interface fluxes
     static constexpr bool RELOAD = RELOAD_ != 0;
-    static constexpr int GX = BX * N, GY = BY * N, GZ = BZ * N;   // nodes of the brick per axis
-    static constexpr int NODES = GX * GY * GZ;
-    static constexpr int SLOT = DG_NV * NODES;                     // doubles per brick in Q, K, R (HBM, dense)
-    static constexpr int P = P_ ? P_ : GX;                         // shared-memory row pitch
-    static constexpr int PP = PP_ ? PP_ : GY * P;                  // shared-memory plane pitch
-    static constexpr int PLANE = GZ * PP;                          // shared doubles per variable
-    static constexpr int OX = OX_, OY = OY_, OZ = OZ_;
-    static constexpr int L = NODES / N;                            // node lines per axis = threads that work
-    static constexpr int THREADS = (L + 31) / 32 * 32;
-    static constexpr int CX = GY * GZ, CY = GX * GZ, CZ = GX * GY; // face nodes of a brick side per axis
-    static constexpr int TSLOT = 2 * DG_NV * (CX + CY + CZ);       // trace doubles per brick
-    static constexpr bool MULTI = (BX > 1) || (BY > 1) || (BZ > 1);
-    static constexpr int LINEBUF = MULTI ? DG_NV * L : 0;          // T- / F* hand-over between elements of a brick
-    static constexpr int EXFACE = (CLX > 1 ? CX : 0) > (CLY > 1 ? CY : 0)
-                                      ? ((CLX > 1 ? CX : 0) > (CLZ > 1 ? CZ : 0) ? (CLX > 1 ? CX : 0) : (CLZ > 1 ? CZ : 0))
-                                      : ((CLY > 1 ? CY : 0) > (CLZ > 1 ? CZ : 0) ? (CLY > 1 ? CY : 0) : (CLZ > 1 ? CZ : 0));
-    static constexpr int EXBUF = 2 * DG_NV * EXFACE;               // traces exported to the cluster neighbours
-    static constexpr int SMEM_DOUBLES = 2 * DG_NV * PLANE + 2 * LINEBUF + EXBUF;
-    static constexpr int SMEM_BYTES = SMEM_DOUBLES * 8;
-    static_assert(P >= GX && PP >= GY * P, "pitches too small");
-    static_assert(OZ == 0 || OZ == 2, "z lines must keep gx fastest across lanes");
+    static constexpr int GX = BX * N, GY = BY * N;                 // nodes of a layer per axis (z: N)
+    static constexpr int NODES = GX * GY * N;
+    static constexpr int HP = (GX * GY + 1) & ~1;                  // HBM pitch of one (gy,gx) plane, doubles (even)
+    static constexpr int NPL = DG_NV * N;                          // planes per slot
+    static constexpr int SLOT = (NPL * HP + 15) & ~15;             // doubles per layer slot in Q, K (128-byte multiple)
+    static constexpr int P = GX;                                   // shared-memory row pitch (dense)
+    static constexpr int PP = PP_ ? PP_ : HP;                      // shared-memory plane pitch
+    static constexpr int PLANE = N * PP;                           // shared doubles per variable
+    static constexpr int BUF = DG_NV * PLANE;                      // shared doubles per layer buffer
+    static constexpr int OX = OX_, OY = OY_;
+    static constexpr int L = GX * GY;                              // node lines per axis = threads that work
+    static constexpr int NCOMP = (L + 31) / 32 * 32;               // compute threads
+    static constexpr int THREADS = NCOMP + 32;                     // + the copy warp
+    static constexpr int CX = GY * N, CY = GX * N, CZ = GX * GY;   // face nodes of a layer side per axis
+    static constexpr int TXY = 2 * DG_NV * (CX + CY);              // x/y trace doubles per layer slot
+    static constexpr int TZ = 2 * DG_NV * CZ;                      // z trace doubles per chunk slot
+    static constexpr bool MULTI = (BX > 1) || (BY > 1);
+    static constexpr int LINEBUF = MULTI ? DG_NV * L : 0;          // T- / F* hand-over between elements of a layer
+    static constexpr int SMEM_DOUBLES = 3 * BUF + 2 * LINEBUF;
+    static constexpr int SMEM_BYTES = SMEM_DOUBLES * 8 + 64;       // + mbarriers
+    static_assert(PP >= HP && (PP % 2) == 0, "plane pitch must be even and hold a plane");
+    static_assert((BUF % 2) == 0 && (LINEBUF % 2) == 0, "buffers must stay 16-byte aligned");
 };
 
-__device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) {
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gsrc) : "memory");
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+// ---- mbarrier + bulk-copy (TMA engine) primitives ---------------------------------------------------------
+__device__ __forceinline__ void mbar_init(uint64_t *b, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int PENDING>
-__device__ __forceinline__ void cp_async_wait() {
-    asm volatile("cp.async.wait_group %0;" ::"n"(PENDING) : "memory");
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *b, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint64_t *b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *b, unsigned parity) {
+    const unsigned addr = smem_u32(b);
+    unsigned done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(addr), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+// global -> shared, completion counted in bytes on an mbarrier
+__device__ __forceinline__ void bulk_load(double *sdst, const double *gsrc, unsigned bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(sdst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+// shared -> global, completion tracked by the issuing thread's bulk groups
+__device__ __forceinline__ void bulk_store(double *gdst, const double *ssrc, unsigned bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(ssrc)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+// generic-proxy writes to shared memory become visible to the async proxy (the bulk stores)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // Ask L2 to fetch [ptr, ptr + bytes) (rounded out to 16-byte granules): one instruction per block of data.
 __device__ __forceinline__ void l2_prefetch(const void *ptr, unsigned bytes) {
     const uintptr_t lo = (uintptr_t)ptr & ~(uintptr_t)15;
     const uintptr_t hi = ((uintptr_t)ptr + bytes + 15) & ~(uintptr_t)15;
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(lo), "r"((unsigned)(hi - lo)) : "memory");
 }
-
-// Compiler-level fence on memory operations: bounds how far loads are hoisted (register pressure).
-__device__ __forceinline__ void sched_fence() { asm volatile("" ::: "memory"); }
-
-// Thread-block cluster primitives (split barrier; distributed shared memory loads).
-__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
-__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
-__device__ __forceinline__ unsigned map_to_rank(const void *smem_ptr, unsigned rank) {
-    const unsigned a = (unsigned)__cvta_generic_to_shared(smem_ptr);
-    unsigned r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
-    return r;
+// named barriers: 1 = the compute warps among themselves, 2 = compute warps -> copy warp ("layer finished")
+template <int NTHREADS>
+__device__ __forceinline__ void bar_sync(int id) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(NTHREADS) : "memory");
 }
-__device__ __forceinline__ double ld_cluster(unsigned addr) {
-    double v;
-    asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(addr) : "memory");
-    return v;
+template <int NTHREADS>
+__device__ __forceinline__ void bar_arrive(int id) {
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "n"(NTHREADS) : "memory");
 }
 
 // Euler flux along the face/line normal, eq (2)-(3) (listing lines 186-217), for a state
@@ -134,7 +156,8 @@ __device__ __forceinline__ void euler_flux_normal(const double (&Q)[DG_NV], doub
 // Local Lax-Friedrichs flux (reading R3), rotated slots as above, returned DOUBLED
 // (the factor 1/2 is folded into the lift tables):
 //   2 F* = F(QL) + F(QR) - lam (QR - QL),  lam = max(|u_a^L| + c_L, |u_a^R| + c_R)
-// written for (own, other) with sgn = +1 when own is the left state, -1 when it is the right one.
+// written for (own, other) with sgn = +1 when own is the left state, -1 when it is the right one; the two
+// evaluations of one face (by the blocks on either side) are bit-identical.
 __device__ __forceinline__ void lax_friedrichs2(const double (&Qown)[DG_NV], const double (&Qoth)[DG_NV], double sgn,
                                                 double gamma, double gm1, double (&Fs)[DG_NV]) {
     double Fa[DG_NV], Fb[DG_NV], ua, ub, pa, pb, ra, rb;
@@ -148,21 +171,20 @@ __device__ __forceinline__ void lax_friedrichs2(const double (&Qown)[DG_NV], con
 }
 
 // ------------------------------------------------------------------------------------------------
-// per-axis compile-time traits and the (brick-independent) geometry of a thread's node line
-//   line l = e * Ca + c,  e = element along the axis, c = face node = t2 * T1 + t1
-//   axis x: (t1,t2) = (gy,gz);  y: (gx,gz);  z: (gx,gy)
+// per-axis compile-time traits and the (layer-independent) geometry of a thread's node line
+//   line l = e * Ca + c,  e = element along the axis, c = face node = position in the lane order
+//   axis x: (t1,t2) = (gy,k);  y: (gx,k);  z: (gx,gy)
 // ------------------------------------------------------------------------------------------------
 template <class C, int AX>
 struct Axis {
     static constexpr int S = (AX == 0) ? 1 : (AX == 1) ? C::P : C::PP;                 // shared stride along the line
-    static constexpr int Ca = (AX == 0) ? C::CX : (AX == 1) ? C::CY : C::CZ;           // face nodes of a brick side
+    static constexpr int Ca = (AX == 0) ? C::CX : (AX == 1) ? C::CY : C::CZ;           // face nodes of a layer side
     static constexpr int T1 = (AX == 0) ? C::GY : C::GX;
-    static constexpr int T2 = (AX == 2) ? C::GY : C::GZ;
-    static constexpr int ORD = (AX == 0) ? C::OX : (AX == 1) ? C::OY : C::OZ;
-    static constexpr int B = (AX == 0) ? C::BX : (AX == 1) ? C::BY : C::BZ;            // elements along the axis
-    static constexpr int TBASE = (AX == 0) ? 0 : (AX == 1) ? 2 * DG_NV * C::CX : 2 * DG_NV * (C::CX + C::CY);
+    static constexpr int T2 = (AX == 2) ? C::GY : C::N;
+    static constexpr int ORD = (AX == 0) ? C::OX : (AX == 1) ? C::OY : 0;
+    static constexpr int B = (AX == 0) ? C::BX : (AX == 1) ? C::BY : 1;                // elements along the axis
+    static constexpr int TBASE = (AX == 0) ? 0 : 2 * DG_NV * C::CX;                    // inside a Txy slot
     static constexpr bool MULTI = B > 1;
-    static constexpr int CL = (AX == 0) ? C::CLX : (AX == 1) ? C::CLY : C::CLZ;     // cluster blocks along the axis
     // momentum slots rotated so that slot 1 is the component along this axis: slot s holds variable VAR[s]
     static constexpr int M1 = 1 + AX, M2 = (AX == 2) ? 1 : 2 + AX, M3 = (AX == 0) ? 3 : AX;
 };
@@ -172,8 +194,8 @@ __device__ __forceinline__ constexpr int var_of_slot(int s) {
 }
 
 struct Geo {
-    int base;   // shared-memory offset (doubles, inside one variable plane) of node 0 of the line
-    int c;      // face-node index of the line on the brick side (lane order: this is how the traces are stored)
+    int base;   // shared-memory offset (doubles, inside one variable's planes) of node 0 of the line
+    int c;      // face-node index of the line on the layer side (lane order: this is how the traces are stored)
     int e;      // element along the axis
     int t1, t2; // transverse node indices
 };
@@ -216,70 +238,27 @@ __device__ __forceinline__ Geo make_geo(int l) {
     }
     if (AX == 0) g.base = g.t2 * C::PP + g.t1 * C::P + g.e * N;
     else if (AX == 1) g.base = g.t2 * C::PP + g.e * N * C::P + g.t1;
-    else g.base = g.e * N * C::PP + g.t2 * C::P + g.t1;
+    else g.base = g.t2 * C::P + g.t1;
     return g;
 }
 
-// Is the line inside a ragged (last) brick of ext0 x ext1 x ext2 elements?
+// Is the line inside a ragged (last) column of ext0 x ext1 elements?
 template <class C, int AX>
-__device__ __forceinline__ bool line_inside(const Geo &g, int ext0, int ext1, int ext2) {
-    const int lim1 = ((AX == 0) ? ext1 : ext0) * C::N, lim2 = ((AX == 2) ? ext1 : ext2) * C::N;
-    const int exta = (AX == 0) ? ext0 : (AX == 1) ? ext1 : ext2;
-    return g.t1 < lim1 && g.t2 < lim2 && g.e < exta;
+__device__ __forceinline__ bool line_inside(const Geo &g, int ext0, int ext1) {
+    if (AX == 0) return g.t1 < ext1 * C::N && g.e < ext0;
+    if (AX == 1) return g.t1 < ext0 * C::N && g.e < ext1;
+    return g.t1 < ext0 * C::N && g.t2 < ext1 * C::N;
 }
 
-// P0: enqueue the asynchronous copy of one dense HBM slot [5][GZ][GY][GX] into the pitched shared planes.
-// Thread tid < L = BZ * GX * GY owns one node of a group of BZ consecutive z planes; the 5 N groups of the
-// slot are then a fixed stride apart on both sides, so the whole copy is 5 N instructions per thread with
-// immediate offsets (consecutive lanes read consecutive doubles of HBM).
-template <class C>
-__device__ __forceinline__ void stage_in(double *dst, const double *src, int tid) {
-    if (tid < C::L) {
-        const int pz = tid / (C::GX * C::GY), k = tid - pz * (C::GX * C::GY);
-        const int gy = k / C::GX, gx = k - gy * C::GX;
-        double *d = dst + pz * C::PP + gy * C::P + gx;
-        const double *g = src + tid;
-#pragma unroll
-        for (int j = 0; j < DG_NV * C::N; ++j) cp_async8(d + j * (C::BZ * C::PP), g + j * C::L);
-    }
-}
-
-// Trace block [5][Ca] a brick needs for (axis, side): side 0 = T+ of the brick below (stored as that brick's
-// side 1), side 1 = T- of the brick above (its side 0).  Periodic in every direction.
+// PE for one of the axes x, y: traces of the Q in shared memory on the column boundary -> Tslot.
 template <class C, int AX>
-__device__ __forceinline__ const double *halo_source(const DgStageArgs &a, int bx, int by, int bz, int side) {
-    using A = Axis<C, AX>;
-    if (AX == 0) bx = (side == 0) ? ((bx == 0) ? a.nbx - 1 : bx - 1) : ((bx + 1 == a.nbx) ? 0 : bx + 1);
-    else if (AX == 1) by = (side == 0) ? ((by == 0) ? a.nby - 1 : by - 1) : ((by + 1 == a.nby) ? 0 : by + 1);
-    else bz = (side == 0) ? ((bz == 0) ? a.nbz - 1 : bz - 1) : ((bz + 1 == a.nbz) ? 0 : bz + 1);
-    const size_t nbr = (size_t)bx + (size_t)a.nbx * ((size_t)by + (size_t)a.nby * bz);
-    return a.Told + nbr * C::TSLOT + A::TBASE + (side == 0 ? DG_NV * A::Ca : 0);
-}
-
-// L2 prefetch of everything the block's NEXT brick will read: 8 threads, one instruction each.
-template <class C>
-__device__ __forceinline__ void prefetch_brick(const DgStageArgs &a, int brick, int tid, bool want_k, bool want_halo) {
-    if (tid == 0) l2_prefetch(a.Q + (size_t)brick * C::SLOT, C::SLOT * 8);
-    if (tid == 1 && want_k) l2_prefetch(a.K + (size_t)brick * C::SLOT, C::SLOT * 8);
-    if (tid >= 2 && tid < 8 && want_halo) {
-        const int bx = brick % a.nbx, by = (brick / a.nbx) % a.nby, bz = brick / (a.nbx * a.nby);
-        const int side = tid & 1;
-        if (tid < 4) l2_prefetch(halo_source<C, 0>(a, bx, by, bz, side), DG_NV * C::CX * 8);
-        else if (tid < 6) l2_prefetch(halo_source<C, 1>(a, bx, by, bz, side), DG_NV * C::CY * 8);
-        else l2_prefetch(halo_source<C, 2>(a, bx, by, bz, side), DG_NV * C::CZ * 8);
-    }
-}
-
-// PE for one axis: traces of the (updated) Q in shared memory on the brick boundary -> Tnew.
-template <class C, int AX>
-__device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta, const double *Qs, double *Tbrick,
-                                                const DgStageArgs &a, bool wlo = true, bool whi = true) {
+__device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta, const double *Qs, double *Tslot,
+                                                const double (&lp)[DG_NMAX], const double (&lm)[DG_NMAX]) {
     using A = Axis<C, AX>;
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE;
-    // wlo / whi: does the low / high face of the brick go through HBM (false: a cluster neighbour takes it)
-    const bool first = g.e == 0 && wlo, last = g.e == exta - 1 && whi;
+    const bool first = g.e == 0, last = g.e == exta - 1;
     if (!act || !(first || last)) return;
-    double *dst = Tbrick + A::TBASE + g.c;
+    double *dst = Tslot + A::TBASE + g.c;
     const double *Q0 = Qs + g.base;
     if (first && last) {
         double Tp[NV], Tm[NV];
@@ -290,8 +269,8 @@ __device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta
 #pragma unroll
             for (int n = 0; n < NV; ++n) {
                 const double Qv = Q0[n * PLANE + q * A::S];
-                Tp[n] = fma(a.ops.lp[q], Qv, Tp[n]);
-                Tm[n] = fma(a.ops.lm[q], Qv, Tm[n]);
+                Tp[n] = fma(lp[q], Qv, Tp[n]);
+                Tm[n] = fma(lm[q], Qv, Tm[n]);
             }
 #pragma unroll
         for (int n = 0; n < NV; ++n) {
@@ -305,7 +284,7 @@ __device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta
         for (int n = 0; n < NV; ++n) T[n] = 0.0;
 #pragma unroll
         for (int q = 0; q < N; ++q) {
-            const double w = first ? a.ops.lm[q] : a.ops.lp[q];
+            const double w = first ? lm[q] : lp[q];
 #pragma unroll
             for (int n = 0; n < NV; ++n) T[n] = fma(w, Q0[n * PLANE + q * A::S], T[n]);
         }
@@ -315,141 +294,126 @@ __device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta
     }
 }
 
-// ------------------------------------------------------------------------------------------------
-// one axis of the residual for one brick
-// ------------------------------------------------------------------------------------------------
-// PH: the neighbour bricks' traces this line touches, momentum slots rotated, HBM/L2 -> registers.
+// Trace block [5][Ca] a column needs for (axis x or y, side) in layer ez: side 0 = T+ of the column below
+// (stored as that column's side 1), side 1 = T- of the column above (its side 0).  Periodic.
 template <class C, int AX>
-__device__ __forceinline__ void load_halo(const Geo &g, bool act, int exta, const double *halo_lo,
-                                          const double *halo_hi, bool ilo, bool ihi, double (&Hlo)[DG_NV],
-                                          double (&Hhi)[DG_NV]) {
-    constexpr int Ca = Axis<C, AX>::Ca;
-    if (act && g.e == 0 && !ilo) {
-#pragma unroll
-        for (int s = 0; s < DG_NV; ++s) Hlo[s] = __ldg(halo_lo + var_of_slot<C, AX>(s) * Ca + g.c);
-    }
-    if (act && g.e == exta - 1 && !ihi) {
-#pragma unroll
-        for (int s = 0; s < DG_NV; ++s) Hhi[s] = __ldg(halo_hi + var_of_slot<C, AX>(s) * Ca + g.c);
-    }
+__device__ __forceinline__ const double *halo_source(const double *T, int nbx, int nby, int bx, int by, int ez, int side) {
+    using A = Axis<C, AX>;
+    if (AX == 0) bx = (side == 0) ? ((bx == 0) ? nbx - 1 : bx - 1) : ((bx + 1 == nbx) ? 0 : bx + 1);
+    else by = (side == 0) ? ((by == 0) ? nby - 1 : by - 1) : ((by + 1 == nby) ? 0 : by + 1);
+    const size_t nbr = (size_t)bx + (size_t)nbx * ((size_t)by + (size_t)nby * ez);
+    return T + nbr * C::TXY + A::TBASE + (side == 0 ? DG_NV * A::Ca : 0);
 }
 
-// PA..PD for one axis.  Order chosen for register pressure: the line's Q goes into registers once; the
-// face traces and the two interface fluxes come first (no accumulators alive yet); the accumulators then
-// START from the lift term and the volume term is added node by node.
+// ------------------------------------------------------------------------------------------------
+// the x and y passes of one layer
+// ------------------------------------------------------------------------------------------------
+// Order chosen for register pressure: the line's Q goes into registers once; the face traces and the two
+// interface fluxes come first (no accumulators alive yet); the accumulators then START from the lift term
+// and the volume term is added node by node.
 //   r_i = sum_q Dhat_iq F_q - (l_i(+1) F*_+ - l_i(-1) F*_-) (2/h_a)/w_i
-// Cluster variants (A::CL > 1): `ilo` / `ihi` say that the low / high face of the brick is shared with the
-// cluster block of rank `rlo` / `rhi`; the traces on those faces are exported to Ex in this block's shared
-// memory and the neighbour's are read from ITS Ex.  One cluster barrier between export and import; the
-// barrier that protects Ex against the next export is split (arrive after the import, wait before the next
-// export or the end of the kernel: PENDING says that such a wait is still owed on entry).
-template <class C, int AX, int MODE, bool PENDING>
-__device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, int l, bool act, int exta,
-                                          const double *halo_lo, const double *halo_hi, double *Qs, double *Ks,
-                                          double *Tms, double *Fss, double *Ex, bool readK, size_t qbase,
-                                          double *Tbrick, bool ilo, bool ihi, unsigned rlo, unsigned rhi) {
+// Threads without a line of their own (`act` false: the tail of the last warp, lines in the padding of a ragged
+// column) run the arithmetic on a valid line all the same and only their stores are switched off: every
+// register is then defined on every path through the layer loop, which is what keeps the line's 10 N + 30
+// values from staying alive (and spilling) across the other two passes.
+template <class C, int AX, int MODE>
+__device__ __forceinline__ void xy_pass(const DgStageArgs &a, const Geo &g, bool act, int exta, const double *halo_lo,
+                                        const double *halo_hi, const double *Qs, double *KR, double *Tms, double *Fss,
+                                        bool readK, uint64_t *fullk, unsigned kparity) {
     using A = Axis<C, AX>;
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE, L = C::L, S = A::S, Ca = A::Ca;
     const bool first = g.e == 0, last = g.e == exta - 1;
     const int lb = g.e * Ca + g.c;   // slot of this line in the hand-over buffers
+    // PH: the neighbour columns' traces this line touches, momentum slots rotated, HBM/L2 -> registers
     double Hlo[NV], Hhi[NV];
-    load_halo<C, AX>(g, act, exta, halo_lo, halo_hi, ilo, ihi, Hlo, Hhi);
+#pragma unroll
+    for (int s = 0; s < NV; ++s) {
+        Hlo[s] = 1.0;
+        Hhi[s] = 1.0;
+    }
+    if (act && first) {
+#pragma unroll
+        for (int s = 0; s < NV; ++s) Hlo[s] = __ldg(halo_lo + var_of_slot<C, AX>(s) * Ca + g.c);
+    }
+    if (act && last) {
+#pragma unroll
+        for (int s = 0; s < NV; ++s) Hhi[s] = __ldg(halo_hi + var_of_slot<C, AX>(s) * Ca + g.c);
+    }
 
+    // ------------- PT: the line's nodal values (slot s holds variable var_of_slot(s)) and its traces ----
     double QL[C::RELOAD ? 1 : NV][C::RELOAD ? 1 : N], Tp[NV], Tm[NV];
-    if (act) {
-        // ------------- the line's nodal values (slot s holds variable var_of_slot(s)) and its traces ----
-        const double *Q0 = Qs + g.base;
+    const double *Q0 = Qs + g.base;
 #pragma unroll
-        for (int s = 0; s < NV; ++s) {
-            Tp[s] = 0.0;
-            Tm[s] = 0.0;
+    for (int s = 0; s < NV; ++s) {
+        Tp[s] = 0.0;
+        Tm[s] = 0.0;
 #pragma unroll
-            for (int q = 0; q < N; ++q) {
-                const double Qv = Q0[var_of_slot<C, AX>(s) * PLANE + q * S];
-                if (!C::RELOAD) QL[s][q] = Qv;
-                Tp[s] = fma(a.ops.lp[q], Qv, Tp[s]);
-                Tm[s] = fma(a.ops.lm[q], Qv, Tm[s]);
-            }
+        for (int q = 0; q < N; ++q) {
+            const double Qv = Q0[var_of_slot<C, AX>(s) * PLANE + q * S];
+            if (!C::RELOAD) QL[s][q] = Qv;
+            Tp[s] = fma(a.ops.lp[q], Qv, Tp[s]);
+            Tm[s] = fma(a.ops.lm[q], Qv, Tm[s]);
         }
-        if (A::MULTI) {
+    }
+    if (A::MULTI) {
+        if (act) {
 #pragma unroll
             for (int n = 0; n < NV; ++n) Tms[n * L + lb] = Tm[n];
         }
-    }
-    if (A::CL > 1) {
-        if (PENDING) cluster_wait();   // the neighbours are done with the previous axis' exports
-        if (act && first && ilo) {
-#pragma unroll
-            for (int n = 0; n < NV; ++n) Ex[n * Ca + g.c] = Tm[n];
-        }
-        if (act && last && ihi) {
-#pragma unroll
-            for (int n = 0; n < NV; ++n) Ex[(NV + n) * Ca + g.c] = Tp[n];
-        }
-        cluster_arrive();              // (a cluster barrier is also a block barrier: covers Tms)
-        cluster_wait();
-    } else if (A::MULTI) {
-        __syncthreads();
+        bar_sync<C::NCOMP>(1);
     }
 
     // ------------- PB: interface fluxes ----------------------------------------------------------------
     double Fp[NV], Fm[NV];
-    if (act) {
-        if (A::MULTI && !last) {
+    if (A::MULTI && act && !last) {
 #pragma unroll
-            for (int n = 0; n < NV; ++n) Hhi[n] = Tms[n * L + lb + Ca];   // T- of the next element of this brick
-        } else if (A::CL > 1 && ihi) {
-#pragma unroll
-            for (int n = 0; n < NV; ++n) Hhi[n] = ld_cluster(map_to_rank(Ex + n * Ca + g.c, rhi));        // its T-
-        }
-        if (A::CL > 1 && first && ilo) {
-#pragma unroll
-            for (int n = 0; n < NV; ++n) Hlo[n] = ld_cluster(map_to_rank(Ex + (NV + n) * Ca + g.c, rlo));  // its T+
-        }
-        lax_friedrichs2(Tp, Hhi, 1.0, a.gamma, a.gm1, Fp);
-        if (A::MULTI) {
+        for (int n = 0; n < NV; ++n) Hhi[n] = Tms[n * L + lb + Ca];   // T- of the next element of this layer
+    }
+    lax_friedrichs2(Tp, Hhi, 1.0, a.gamma, a.gm1, Fp);
+    if (A::MULTI) {
+        if (act) {
 #pragma unroll
             for (int n = 0; n < NV; ++n) Fss[n * L + lb] = Fp[n];
         }
         if (first) lax_friedrichs2(Tm, Hlo, -1.0, a.gamma, a.gm1, Fm);
-    }
-    if (A::CL > 1) cluster_arrive();   // done reading the neighbours' exports (waited for before Ex is reused)
-    if (A::MULTI) __syncthreads();
-
-    double V[NV][N];
-    if (act) {
-        if (A::MULTI && !first) {
+        bar_sync<C::NCOMP>(1);
+        if (!first) {
 #pragma unroll
             for (int n = 0; n < NV; ++n) Fm[n] = Fss[n * L + lb - Ca];
         }
-        // ------------- PC: lift (2/h and 1/w folded into the tables) starts the accumulators -----------
-#pragma unroll
-        for (int i = 0; i < N; ++i) {
-            const double cp = a.ops.lpg[AX][i], cm = a.ops.lmg[AX][i];
-#pragma unroll
-            for (int n = 0; n < NV; ++n) V[n][i] = fma(cm, Fm[n], -cp * Fp[n]);
-        }
-        // ------------- PA: pointwise flux and sum-factorised derivative --------------------------------
-#pragma unroll
-        for (int q = 0; q < N; ++q) {
-            double Qn[NV], F[NV], vel, pres, rinv;
-#pragma unroll
-            for (int s = 0; s < NV; ++s)
-                Qn[s] = C::RELOAD ? Qs[g.base + var_of_slot<C, AX>(s) * PLANE + q * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : q];
-            euler_flux_normal(Qn, a.gm1, F, vel, pres, rinv);
-#pragma unroll
-            for (int n = 0; n < NV; ++n)
-#pragma unroll
-                for (int i = 0; i < N; ++i) V[n][i] = fma(a.ops.Dg[AX][q][i], F[n], V[n][i]);
-        }
+    } else {
+        lax_friedrichs2(Tm, Hlo, -1.0, a.gamma, a.gm1, Fm);
     }
+
+    // ------------- PC: lift (2/h and 1/w folded into the tables) starts the accumulators -----------
+    double V[NV][N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        const double cp = a.ops.lpg[AX][i], cm = a.ops.lmg[AX][i];
+#pragma unroll
+        for (int n = 0; n < NV; ++n) V[n][i] = fma(cm, Fm[n], -cp * Fp[n]);
+    }
+    // ------------- PA: pointwise flux and sum-factorised derivative --------------------------------
+#pragma unroll
+    for (int q = 0; q < N; ++q) {
+        double Qn[NV], F[NV], vel, pres, rinv;
+#pragma unroll
+        for (int s = 0; s < NV; ++s)
+            Qn[s] = C::RELOAD ? Q0[var_of_slot<C, AX>(s) * PLANE + q * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : q];
+        euler_flux_normal(Qn, a.gm1, F, vel, pres, rinv);
+#pragma unroll
+        for (int n = 0; n < NV; ++n)
+#pragma unroll
+            for (int i = 0; i < N; ++i) V[n][i] = fma(a.ops.Dg[AX][q][i], F[n], V[n][i]);
+    }
+    // ------------- PD: Runge-Kutta accumulation on the staged K -----------------------------------------
     if (AX == 0) {
-        cp_async_wait<0>();            // the staged K (its own cp.async group) has landed
-        if (readK) __syncthreads();
+        mbar_wait(fullk, kparity);     // the copy warp has read the previous K out and this layer's K has landed
+    } else if (!A::MULTI) {
+        bar_sync<C::NCOMP>(1);         // the x pass of every line is done (with MULTI the two barriers above said so)
     }
     if (act) {
-        // ------------- PD: Runge-Kutta accumulation on the staged K ------------------------------------
-        double *K0 = Ks + g.base;
+        double *K0 = KR + g.base;
         if (AX == 0) {
             if (readK) {
                 const double rkA = a.rkA;
@@ -466,7 +430,99 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
 #pragma unroll
                     for (int i = 0; i < N; ++i) K0[var_of_slot<C, AX>(s) * PLANE + i * S] = V[s][i];
             }
-        } else if (AX == 1) {
+        } else {
+#pragma unroll
+            for (int s = 0; s < NV; ++s)
+#pragma unroll
+                for (int i = 0; i < N; ++i) {
+                    double *p = K0 + var_of_slot<C, AX>(s) * PLANE + i * S;
+                    *p += V[s][i];
+                }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// the z pass of one layer: thread (gx, gy) owns the z line; the flux on the lower face is carried in Fm
+// ------------------------------------------------------------------------------------------------
+template <class C, int MODE, bool LAM>
+__device__ __forceinline__ void z_pass(const DgStageArgs &a, const Geo &g, bool act, double *Qs, const double *Qnext,
+                                       const double *tz_lo, const double *tz_hi, double *tz_out, double *KR,
+                                       double (&Fm)[DG_NV], bool first_layer, bool last_layer, double &lam_best) {
+    constexpr int AX = 2;
+    using A = Axis<C, AX>;
+    constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE, S = A::S, Ca = A::Ca;
+    double QL[C::RELOAD ? 1 : NV][C::RELOAD ? 1 : N], V[NV][N], Fp[NV];
+    // PH: T- of the line above: from the next layer of the ring, or (top of the chunk) from HBM
+    double Hhi[NV];
+    if (!last_layer) {
+        const double *Q1 = Qnext + g.base;
+#pragma unroll
+        for (int s = 0; s < NV; ++s) {
+            double t = 0.0;
+#pragma unroll
+            for (int q = 0; q < N; ++q) t = fma(a.ops.lm[q], Q1[var_of_slot<C, AX>(s) * PLANE + q * S], t);
+            Hhi[s] = t;
+        }
+    } else {
+#pragma unroll
+        for (int s = 0; s < NV; ++s) Hhi[s] = __ldg(tz_hi + var_of_slot<C, AX>(s) * Ca + g.c);
+    }
+    // PT
+    double Tp[NV];
+    const double *Q0 = Qs + g.base;
+#pragma unroll
+    for (int s = 0; s < NV; ++s) {
+        Tp[s] = 0.0;
+#pragma unroll
+        for (int q = 0; q < N; ++q) {
+            const double Qv = Q0[var_of_slot<C, AX>(s) * PLANE + q * S];
+            if (!C::RELOAD) QL[s][q] = Qv;
+            Tp[s] = fma(a.ops.lp[q], Qv, Tp[s]);
+        }
+    }
+    // PB
+    if (first_layer) {   // bottom of the chunk: own T- against T+ of the layer below (from HBM)
+        double Tm[NV], Hlo[NV];
+#pragma unroll
+        for (int s = 0; s < NV; ++s) {
+            double t = 0.0;
+#pragma unroll
+            for (int q = 0; q < N; ++q) t = fma(a.ops.lm[q], Q0[var_of_slot<C, AX>(s) * PLANE + q * S], t);
+            Tm[s] = t;
+            Hlo[s] = __ldg(tz_lo + var_of_slot<C, AX>(s) * Ca + g.c);
+        }
+        lax_friedrichs2(Tm, Hlo, -1.0, a.gamma, a.gm1, Fm);
+    }
+    lax_friedrichs2(Tp, Hhi, 1.0, a.gamma, a.gm1, Fp);
+    // PC
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        const double cp = a.ops.lpg[AX][i], cm = a.ops.lmg[AX][i];
+#pragma unroll
+        for (int n = 0; n < NV; ++n) V[n][i] = fma(cm, Fm[n], -cp * Fp[n]);
+    }
+    // PA
+#pragma unroll
+    for (int q = 0; q < N; ++q) {
+        double Qn[NV], F[NV], vel, pres, rinv;
+#pragma unroll
+        for (int s = 0; s < NV; ++s)
+            Qn[s] = C::RELOAD ? Q0[var_of_slot<C, AX>(s) * PLANE + q * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : q];
+        euler_flux_normal(Qn, a.gm1, F, vel, pres, rinv);
+#pragma unroll
+        for (int n = 0; n < NV; ++n)
+#pragma unroll
+            for (int i = 0; i < N; ++i) V[n][i] = fma(a.ops.Dg[AX][q][i], F[n], V[n][i]);
+    }
+#pragma unroll
+    for (int n = 0; n < NV; ++n) Fm[n] = Fp[n];   // the next layer's lower face
+    bar_sync<C::NCOMP>(1);   // the y pass of every line is done with K (and, RELOAD, with Q)
+    if (act) {
+        // PD
+        double *K0 = KR + g.base;
+        double *Q0w = Qs + g.base;
+        if (MODE == DG_MODE_RESIDUAL) {
 #pragma unroll
             for (int s = 0; s < NV; ++s)
 #pragma unroll
@@ -475,48 +531,44 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
                     *p += V[s][i];
                 }
         } else {
-            // z lines: consecutive threads hold consecutive (gx, gy), so HBM accesses coalesce
-            const size_t g0 = qbase + (size_t)(g.e * N) * (C::GY * C::GX) + g.t2 * C::GX + g.t1;   // node 0, variable 0
-            if (MODE == DG_MODE_RESIDUAL) {
+            const double rkB = a.rkB;
+            double Qn[LAM ? NV : 1][N];
 #pragma unroll
-                for (int s = 0; s < NV; ++s)
+            for (int s = 0; s < NV; ++s) {
+                const int n = var_of_slot<C, AX>(s);
+                const int sq = LAM ? s : 0;
 #pragma unroll
-                    for (int i = 0; i < N; ++i) {
-                        const int n = var_of_slot<C, AX>(s);
-                        a.Rout[g0 + (size_t)n * C::NODES + (size_t)i * (C::GY * C::GX)] =
-                            K0[n * PLANE + i * S] + V[s][i];
-                    }
-            } else {
-                const double rkB = a.rkB;
-                double *Q0w = Qs + g.base;
-                double *dst = Tbrick + A::TBASE + g.c;
+                for (int i = 0; i < N; ++i) {
+                    const double Kn = K0[n * PLANE + i * S] + V[s][i];
+                    const double Qold = C::RELOAD ? Q0w[n * PLANE + i * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : i];
+                    Qn[sq][i] = fma(rkB, Kn, Qold);
+                    K0[n * PLANE + i * S] = Kn;
+                    Q0w[n * PLANE + i * S] = Qn[sq][i];
+                }
+                // PE for the z faces: traces of the updated Q, only at the two ends of the chunk
+                if (first_layer) {
+                    double tm = 0.0;
 #pragma unroll
-                for (int s = 0; s < NV; ++s) {
-                    const int n = var_of_slot<C, AX>(s);
-                    double Qn[N];
+                    for (int i = 0; i < N; ++i) tm = fma(a.ops.lm[i], Qn[sq][i], tm);
+                    tz_out[n * Ca + g.c] = tm;
+                }
+                if (last_layer) {
+                    double tp = 0.0;
 #pragma unroll
-                    for (int i = 0; i < N; ++i) {
-                        const size_t go = g0 + (size_t)n * C::NODES + (size_t)i * (C::GY * C::GX);
-                        const double Kn = K0[n * PLANE + i * S] + V[s][i];
-                        const double Qold = C::RELOAD ? Q0w[n * PLANE + i * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : i];
-                        Qn[i] = fma(rkB, Kn, Qold);
-                        __stcs(a.K + go, Kn);   // streaming: written once, not read again in this stage
-                        __stcs(a.Q + go, Qn[i]);
-                        Q0w[n * PLANE + i * S] = Qn[i];
-                    }
-                    // PE for the z faces: traces of the updated Q, only at the ends that lie on the brick boundary
-                    if (first && !ilo) {
-                        double tm = 0.0;
+                    for (int i = 0; i < N; ++i) tp = fma(a.ops.lp[i], Qn[sq][i], tp);
+                    tz_out[(NV + n) * Ca + g.c] = tp;
+                }
+            }
+            if (LAM) {
+                // max wavespeed of the updated state (reading R10), IEEE division and square root;
+                // slots are (rho, rho w, rho u, rho v, rho E): the speed does not care about the rotation
 #pragma unroll
-                        for (int i = 0; i < N; ++i) tm = fma(a.ops.lm[i], Qn[i], tm);
-                        dst[n * Ca] = tm;
-                    }
-                    if (last && !ihi) {
-                        double tp = 0.0;
-#pragma unroll
-                        for (int i = 0; i < N; ++i) tp = fma(a.ops.lp[i], Qn[i], tp);
-                        dst[(NV + n) * Ca] = tp;
-                    }
+                for (int i = 0; i < N; ++i) {
+                    const double rinv = 1.0 / Qn[0][i];
+                    const double u = Qn[LAM ? 2 : 0][i] * rinv, v = Qn[LAM ? 3 : 0][i] * rinv, w = Qn[LAM ? 1 : 0][i] * rinv;
+                    const double pres = a.gm1 * (Qn[LAM ? 4 : 0][i] - 0.5 * Qn[0][i] * (u * u + v * v + w * w));
+                    const double sp = sqrt(u * u + v * v + w * w) + sqrt(a.gamma * pres * rinv);
+                    if (!(sp <= lam_best)) lam_best = sp;   // NaN sticks
                 }
             }
         }
@@ -524,103 +576,209 @@ __device__ __forceinline__ void axis_pass(const DgStageArgs &a, const Geo &g, in
 }
 
 // ------------------------------------------------------------------------------------------------
+// the copy warp: every byte of Q and K between HBM and shared memory moves here, by the TMA engine
 // ------------------------------------------------------------------------------------------------
-// the fused, persistent stage kernel
-// ------------------------------------------------------------------------------------------------
+template <class C>
+__device__ __forceinline__ void copy_in(double *sdst, const double *gsrc, uint64_t *bar, int lane) {
+    constexpr unsigned BYTES = C::NPL * C::HP * 8;
+    if (C::PP == C::HP) {
+        if (lane == 0) {
+            mbar_expect_tx(bar, BYTES);
+            bulk_load(sdst, gsrc, BYTES, bar);
+        }
+    } else {
+        if (lane == 0) mbar_expect_tx(bar, BYTES);
+        __syncwarp();
+        for (int pl = lane; pl < C::NPL; pl += 32) bulk_load(sdst + pl * C::PP, gsrc + pl * C::HP, C::HP * 8, bar);
+    }
+}
+template <class C>
+__device__ __forceinline__ void copy_out(double *gdst, const double *ssrc, int lane) {
+    if (C::PP == C::HP) {
+        if (lane == 0) bulk_store(gdst, ssrc, C::NPL * C::HP * 8);
+    } else {
+        for (int pl = lane; pl < C::NPL; pl += 32) bulk_store(gdst + pl * C::HP, ssrc + pl * C::PP, C::HP * 8);
+    }
+}
+
 template <class C, int MODE>
-__global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __grid_constant__ DgStageArgs a) {
-    constexpr int NV = DG_NV, PLANE = C::PLANE, L = C::L;
-    constexpr bool EXCH = (C::CLUSTER > 1) && (MODE != DG_MODE_TRACES);   // do cluster neighbours trade traces?
-    extern __shared__ __align__(16) double smem[];
-    double *Qs = smem;                     // [5][PLANE] nodal values of the brick (old, then updated)
-    double *Ks = Qs + NV * PLANE;          // [5][PLANE] Runge-Kutta register of the brick, accumulated in place
-    double *Tms = Ks + NV * PLANE;         // [5][L]     T- of every line (right state of the line below)
-    double *Fss = Tms + C::LINEBUF;        // [5][L]     F* at the + end of every line
-    double *Ex = Fss + C::LINEBUF;         // [2][5][EXFACE] traces exported to the cluster neighbours
-
-    // One brick per block, blockIdx = brick coordinates (no persistent loop: a loop over bricks makes the
-    // compiler hoist the operator tables out of it into registers).  The grid is rounded up to whole
-    // clusters; a block past the last brick only takes part in the cluster barriers.
-    const int tid = threadIdx.x, l = tid;
-    const int bxi = blockIdx.x, byi = blockIdx.y, bzi = blockIdx.z;
-    const bool real = bxi < a.nbx && byi < a.nby && bzi < a.nbz;
-    const int brick = bxi + a.nbx * (byi + a.nby * bzi);
-    const bool readK = (MODE == DG_MODE_STAGE) && (a.rkA != 0.0);
-    const Geo gx = make_geo<C, 0>(l), gy = make_geo<C, 1>(l), gz = make_geo<C, 2>(l);
-    const bool inL = (l < L) && real;
-    const size_t qbase = (size_t)brick * C::SLOT;
-
-    // ---------------- P0: this brick's Q and K come in ----------------------------------------------------
-    if (real) stage_in<C>(Qs, a.Q + qbase, tid);
-    cp_async_commit();
-    if (real && readK) stage_in<C>(Ks, a.K + qbase, tid);
-    cp_async_commit();   // K is not needed before the end of the x pass: its own group
-
-    // The brick that takes this block's place when it ends: blocks are dispatched cluster by cluster in
-    // index order, so it is the one `a.grid` (= resident blocks of the whole GPU) further on in that order.
-    int next = -1;
-    {
-        const int ncx = gridDim.x / C::CLX, ncy = gridDim.y / C::CLY;
-        const int px = bxi % C::CLX, py = byi % C::CLY, pz = bzi % C::CLZ;
-        const long long cid = (bxi / C::CLX) + (long long)ncx * ((byi / C::CLY) + (long long)ncy * (bzi / C::CLZ));
-        const long long d = cid * C::CLUSTER + (px + C::CLX * (py + C::CLY * pz)) + a.grid;
-        const long long ncid = d / C::CLUSTER;
-        const int r = (int)(d - ncid * C::CLUSTER);
-        const int cx = (int)(ncid % ncx), cy = (int)((ncid / ncx) % ncy), cz = (int)(ncid / ((long long)ncx * ncy));
-        const int nx_ = cx * C::CLX + r % C::CLX, ny_ = cy * C::CLY + (r / C::CLX) % C::CLY, nz_ = cz * C::CLZ + r / (C::CLX * C::CLY);
-        if (nx_ < a.nbx && ny_ < a.nby && nz_ < a.nbz) next = nx_ + a.nbx * (ny_ + a.nby * nz_);
+__device__ __forceinline__ void copy_warp(const DgStageArgs &a, int lane, int bxi, int byi, int z0, int nl, bool readK,
+                                          double *Qb0, double *Qb1, double *KR, uint64_t *fullq, uint64_t *fullk) {
+    const size_t lstride = (size_t)a.nbx * a.nby;                    // slots per layer
+    const size_t slot0 = (size_t)z0 * lstride + (size_t)byi * a.nbx + bxi;
+    // L2 prefetch of the neighbour columns' traces of a layer (4 blocks of 5 Ca doubles)
+    auto prefetch_halo = [&](int ez) {
+        if (lane < 2) l2_prefetch(halo_source<C, 0>(a.Txy_old, a.nbx, a.nby, bxi, byi, ez, lane), DG_NV * C::CX * 8);
+        else if (lane < 4) l2_prefetch(halo_source<C, 1>(a.Txy_old, a.nbx, a.nby, bxi, byi, ez, lane - 2), DG_NV * C::CY * 8);
+    };
+    copy_in<C>(Qb0, a.Q + slot0 * C::SLOT, &fullq[0], lane);
+    if (readK) copy_in<C>(KR, a.K + slot0 * C::SLOT, fullk, lane);
+    else if (lane == 0) mbar_arrive(fullk);
+    if (nl > 1) copy_in<C>(Qb1, a.Q + (slot0 + lstride) * C::SLOT, &fullq[1], lane);
+    prefetch_halo(z0);
+    if (nl > 1) prefetch_halo(z0 + 1);
+    for (int it = 0; it < nl; ++it) {
+        double *Qcur = (it & 1) ? Qb1 : Qb0;
+        const size_t slot = slot0 + (size_t)it * lstride;
+        if (lane == 4 && readK && it + 2 < nl) l2_prefetch(a.K + (slot + 2 * lstride) * C::SLOT, C::NPL * C::HP * 8);
+        if (it + 2 < nl) prefetch_halo(z0 + it + 2);
+        bar_sync<C::THREADS>(2);                                     // the compute warps are done with layer `it`
+        copy_out<C>(a.K + slot * C::SLOT, KR, lane);
+        if (MODE == DG_MODE_STAGE) copy_out<C>(a.Q + slot * C::SLOT, Qcur, lane);
+        bulk_commit();
+        bulk_wait_read();                                            // shared memory has been read out
+        __syncwarp();
+        if (it + 1 < nl) {
+            if (readK) copy_in<C>(KR, a.K + (slot + lstride) * C::SLOT, fullk, lane);
+            else if (lane == 0) mbar_arrive(fullk);
+        }
+        if (it + 2 < nl) copy_in<C>(Qcur, a.Q + (slot + 2 * lstride) * C::SLOT, &fullq[it & 1], lane);
     }
-
-    const int ext0 = min(C::BX, a.nx - bxi * C::BX);   // elements of this brick per axis (ragged last brick)
-    const int ext1 = min(C::BY, a.ny - byi * C::BY);
-    const int ext2 = min(C::BZ, a.nz - bzi * C::BZ);
-    const bool full = (ext0 == C::BX) && (ext1 == C::BY) && (ext2 == C::BZ);
-    bool actx = inL, acty = inL, actz = inL;
-    if (!full && real) {
-        actx = inL && line_inside<C, 0>(gx, ext0, ext1, ext2);
-        acty = inL && line_inside<C, 1>(gy, ext0, ext1, ext2);
-        actz = inL && line_inside<C, 2>(gz, ext0, ext1, ext2);
-    }
-    double *Tbrick = a.Tnew + (size_t)brick * C::TSLOT;
-
-    // faces shared with a block of the same cluster (never across the periodic wrap, never with a padding block)
-    const int px = bxi % C::CLX, py = byi % C::CLY, pz = bzi % C::CLZ;
-    const unsigned rank = px + C::CLX * (py + C::CLY * pz);
-    const bool ixl = EXCH && px > 0, ixh = EXCH && px < C::CLX - 1 && bxi + 1 < a.nbx;
-    const bool iyl = EXCH && py > 0, iyh = EXCH && py < C::CLY - 1 && byi + 1 < a.nby;
-    const bool izl = EXCH && pz > 0, izh = EXCH && pz < C::CLZ - 1 && bzi + 1 < a.nbz;
-
-    cp_async_wait<1>();   // Q has landed
-    __syncthreads();
-    if (MODE != DG_MODE_TRACES) {
-        constexpr bool PY = C::CLX > 1, PZ = (C::CLX > 1) || (C::CLY > 1);
-        axis_pass<C, 0, MODE, false>(a, gx, l, actx, ext0, halo_source<C, 0>(a, bxi, byi, bzi, 0),
-                                     halo_source<C, 0>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, Ex, readK, qbase, Tbrick,
-                                     ixl, ixh, rank - 1, rank + 1);
-        __syncthreads();
-        axis_pass<C, 1, MODE, PY>(a, gy, l, acty, ext1, halo_source<C, 1>(a, bxi, byi, bzi, 0),
-                                  halo_source<C, 1>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, Ex, readK, qbase, Tbrick,
-                                  iyl, iyh, rank - C::CLX, rank + C::CLX);
-        __syncthreads();
-        // ask L2 for the follow-on brick's data now, about a third of a brick ahead of its use
-        if (next >= 0 && !(a.flags & 1)) prefetch_brick<C>(a, next, tid, readK, true);
-        axis_pass<C, 2, MODE, PZ>(a, gz, l, actz, ext2, halo_source<C, 2>(a, bxi, byi, bzi, 0),
-                                  halo_source<C, 2>(a, bxi, byi, bzi, 1), Qs, Ks, Tms, Fss, Ex, readK, qbase, Tbrick,
-                                  izl, izh, rank - C::CLX * C::CLY, rank + C::CLX * C::CLY);
-    }
-    // ---------------- PE: traces of the updated Q on the brick boundary (z came from registers) --------
-    if (MODE != DG_MODE_RESIDUAL) {
-        if (MODE == DG_MODE_STAGE) __syncthreads();
-        boundary_traces<C, 0>(gx, actx, ext0, Qs, Tbrick, a, !ixl, !ixh);
-        boundary_traces<C, 1>(gy, acty, ext1, Qs, Tbrick, a, !iyl, !iyh);
-        if (MODE == DG_MODE_TRACES) boundary_traces<C, 2>(gz, actz, ext2, Qs, Tbrick, a);
-    }
-    // nobody may leave while a cluster neighbour can still read its exports
-    if (EXCH) cluster_wait();
 }
 
 // ------------------------------------------------------------------------------------------------
-// layout conversion canonical [e][k][j][i][n] <-> internal [brick][n][gz][gy][gx]
+// the fused stage kernel: block (bx, by, chunk) marches through layers z0 .. z0 + nl - 1 of column (bx, by)
+// ------------------------------------------------------------------------------------------------
+template <class C, int MODE, bool LAM>
+__global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __grid_constant__ DgStageArgs a) {
+    constexpr int L = C::L;
+    extern __shared__ __align__(128) double smem[];
+    double *Qb0 = smem;                    // ring of two layers of Q (old, then updated in place)
+    double *Qb1 = Qb0 + C::BUF;
+    double *KR = Qb1 + C::BUF;             // Runge-Kutta register of the layer, accumulated in place
+    double *Tms = KR + C::BUF;             // [5][L] T- of every line (right state of the line below)
+    double *Fss = Tms + C::LINEBUF;        // [5][L] F* at the + end of every line
+    uint64_t *bars = reinterpret_cast<uint64_t *>(Fss + C::LINEBUF);
+    uint64_t *fullq = bars, *fullk = bars + 2;
+
+    const int tid = threadIdx.x;
+    const int bxi = blockIdx.x, byi = blockIdx.y, chunk = blockIdx.z;
+    const int z0 = chunk * a.lz;
+    const int nl = min(a.lz, a.nz - z0);
+    const bool readK = (MODE == DG_MODE_STAGE) && (a.rkA != 0.0);
+    if (tid == 0) {
+        mbar_init(&fullq[0], 1);
+        mbar_init(&fullq[1], 1);
+        mbar_init(fullk, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid >= C::NCOMP) {
+        copy_warp<C, MODE>(a, tid - C::NCOMP, bxi, byi, z0, nl, readK, Qb0, Qb1, KR, fullq, fullk);
+        return;
+    }
+
+    const int l = tid;
+    const int ext0 = min(C::BX, a.nx - bxi * C::BX);   // elements of this column per axis (ragged last column)
+    const int ext1 = min(C::BY, a.ny - byi * C::BY);
+    const bool inL = l < L;
+    const size_t cstride = (size_t)a.nbx * a.nby;
+    const size_t col = (size_t)byi * a.nbx + bxi;
+
+    double Fm[DG_NV] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    double lam_best = 0.0;
+#pragma unroll 1
+    for (int it = 0; it < nl; ++it) {
+        const int ez = z0 + it;
+        double *Qs = (it & 1) ? Qb1 : Qb0;
+        const double *Qnext = (it & 1) ? Qb0 : Qb1;
+        // The geometry of a thread's three lines is recomputed per layer from an opaque copy of the line index:
+        // kept across the loop it would cost ~20 registers in the sections that need every one of them.
+        int lx = min(l, L - 1);
+        asm volatile("" : "+r"(lx));
+        mbar_wait(&fullq[it & 1], (it >> 1) & 1);
+        {
+            const Geo gx = make_geo<C, 0>(lx);
+            const bool actx = inL && line_inside<C, 0>(gx, ext0, ext1);
+            xy_pass<C, 0, MODE>(a, gx, actx, ext0, halo_source<C, 0>(a.Txy_old, a.nbx, a.nby, bxi, byi, ez, 0),
+                                halo_source<C, 0>(a.Txy_old, a.nbx, a.nby, bxi, byi, ez, 1), Qs, KR, Tms, Fss, readK,
+                                fullk, it & 1);
+        }
+        asm volatile("" : "+r"(lx));
+        {
+            const Geo gy = make_geo<C, 1>(lx);
+            const bool acty = inL && line_inside<C, 1>(gy, ext0, ext1);
+            xy_pass<C, 1, MODE>(a, gy, acty, ext1, halo_source<C, 1>(a.Txy_old, a.nbx, a.nby, bxi, byi, ez, 0),
+                                halo_source<C, 1>(a.Txy_old, a.nbx, a.nby, bxi, byi, ez, 1), Qs, KR, Tms, Fss, readK,
+                                fullk, it & 1);
+        }
+        asm volatile("" : "+r"(lx));
+        const bool last_layer = it + 1 == nl;
+        if (!last_layer) mbar_wait(&fullq[(it + 1) & 1], ((it + 1) >> 1) & 1);
+        {
+            // z traces at the ends of the chunk: T+ of the chunk below (its side 1), T- of the chunk above (its side 0)
+            const int clo = (chunk == 0) ? a.nchunks - 1 : chunk - 1, chi = (chunk + 1 == a.nchunks) ? 0 : chunk + 1;
+            const double *tz_lo = a.Tz_old + ((size_t)clo * cstride + col) * C::TZ + DG_NV * C::CZ;
+            const double *tz_hi = a.Tz_old + ((size_t)chi * cstride + col) * C::TZ;
+            double *tz_out = a.Tz_new + ((size_t)chunk * cstride + col) * C::TZ;
+            const Geo gz = make_geo<C, 2>(lx);
+            const bool actz = inL && line_inside<C, 2>(gz, ext0, ext1);
+            z_pass<C, MODE, LAM>(a, gz, actz, Qs, Qnext, tz_lo, tz_hi, tz_out, KR, Fm, it == 0, last_layer, lam_best);
+        }
+        if (MODE == DG_MODE_STAGE) {
+            bar_sync<C::NCOMP>(1);   // the updated Q of the whole layer is in shared memory
+            asm volatile("" : "+r"(lx));
+            double *Tslot = a.Txy_new + ((size_t)ez * cstride + col) * C::TXY;
+            const Geo gx = make_geo<C, 0>(lx), gy = make_geo<C, 1>(lx);
+            boundary_traces<C, 0>(gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, Qs, Tslot, a.ops.lp, a.ops.lm);
+            boundary_traces<C, 1>(gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, Qs, Tslot, a.ops.lp, a.ops.lm);
+        }
+        fence_proxy_async();
+        bar_arrive<C::THREADS>(2);   // hand the layer to the copy warp
+    }
+    if (LAM) {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            const double o = __shfl_xor_sync(0xffffffffu, lam_best, off);
+            if (!(o <= lam_best)) lam_best = o;
+        }
+        if ((tid & 31) == 0) atomicMax(a.lam_bits, (unsigned long long)__double_as_longlong(lam_best));
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// face traces of a freshly set state (after dg_set_state): one block per layer slot
+// ------------------------------------------------------------------------------------------------
+template <class C>
+__global__ void __launch_bounds__(C::NCOMP) dg_traces_kernel(const __grid_constant__ DgTraceArgs a) {
+    constexpr int NV = DG_NV, N = C::N;
+    extern __shared__ __align__(128) double smem[];
+    const int tid = threadIdx.x, bxi = blockIdx.x, byi = blockIdx.y, ez = blockIdx.z;
+    const size_t cstride = (size_t)a.nbx * a.nby, col = (size_t)byi * a.nbx + bxi;
+    const size_t slot = (size_t)ez * cstride + col;
+    const double *src = a.Q + slot * C::SLOT;
+    for (int idx = tid; idx < C::NPL * C::HP; idx += C::NCOMP) {
+        const int pl = idx / C::HP;
+        smem[pl * C::PP + (idx - pl * C::HP)] = src[idx];
+    }
+    __syncthreads();
+    const Geo gx = make_geo<C, 0>(tid), gy = make_geo<C, 1>(tid), gz = make_geo<C, 2>(tid);
+    const int ext0 = min(C::BX, a.nx - bxi * C::BX), ext1 = min(C::BY, a.ny - byi * C::BY);
+    const bool inL = tid < C::L;
+    double *Tslot = a.Txy + slot * C::TXY;
+    boundary_traces<C, 0>(gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, smem, Tslot, a.lp, a.lm);
+    boundary_traces<C, 1>(gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, smem, Tslot, a.lp, a.lm);
+    const int chunk = ez / a.lz;
+    const bool zfirst = ez == chunk * a.lz, zlast = (ez + 1 == a.nz) || (ez + 1 == (chunk + 1) * a.lz);
+    if ((zfirst || zlast) && inL && line_inside<C, 2>(gz, ext0, ext1)) {
+        double *dst = a.Tz + ((size_t)chunk * cstride + col) * C::TZ + gz.c;
+#pragma unroll
+        for (int n = 0; n < NV; ++n) {
+            double tp = 0.0, tm = 0.0;
+#pragma unroll
+            for (int q = 0; q < N; ++q) {
+                const double Qv = smem[n * C::PLANE + gz.base + q * C::PP];
+                tp = fma(a.lp[q], Qv, tp);
+                tm = fma(a.lm[q], Qv, tm);
+            }
+            if (zfirst) dst[n * C::CZ] = tm;
+            if (zlast) dst[(NV + n) * C::CZ] = tp;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// layout conversion canonical [e][k][j][i][n] <-> internal [slot][n][k][HP: gy, gx]
 // one thread per node; canonical side reads/writes 40 contiguous bytes per thread
 // ------------------------------------------------------------------------------------------------
 template <class C>
@@ -636,50 +794,52 @@ __device__ __forceinline__ size_t internal_offset(size_t node, int nx, int ny, i
     r /= nx;
     const int ey = (int)(r % ny);
     const int ez = (int)(r / ny);
-    const int bxi = ex / C::BX, byi = ey / C::BY, bzi = ez / C::BZ;
-    const int gx = (ex - bxi * C::BX) * N + i, gy = (ey - byi * C::BY) * N + j, gz = (ez - bzi * C::BZ) * N + k;
-    const size_t brick = (size_t)bxi + (size_t)nbx * ((size_t)byi + (size_t)nby * bzi);
-    return brick * C::SLOT + (size_t)(gz * C::GY + gy) * C::GX + gx;
+    const int bxi = ex / C::BX, byi = ey / C::BY;
+    const int gx = (ex - bxi * C::BX) * N + i, gy = (ey - byi * C::BY) * N + j;
+    const size_t slot = (size_t)bxi + (size_t)nbx * ((size_t)byi + (size_t)nby * ez);
+    return slot * C::SLOT + (size_t)k * C::HP + (size_t)(gy * C::GX + gx);
 }
 
 template <class C>
 __global__ void __launch_bounds__(256) dg_layout_kernel(const DgLayoutArgs a) {
+    constexpr size_t VS = (size_t)C::N * C::HP;   // doubles per variable inside a slot
     const size_t total = (size_t)a.nx * a.ny * a.nz * (C::N * C::N * C::N);
     for (size_t node = (size_t)blockIdx.x * blockDim.x + threadIdx.x; node < total;
          node += (size_t)gridDim.x * blockDim.x) {
         const size_t io = internal_offset<C>(node, a.nx, a.ny, a.nbx, a.nby);
         if (a.to_internal) {
 #pragma unroll
-            for (int n = 0; n < DG_NV; ++n) a.internal[io + (size_t)n * C::NODES] = a.canonical[node * DG_NV + n];
+            for (int n = 0; n < DG_NV; ++n) a.internal[io + n * VS] = a.canonical[node * DG_NV + n];
         } else {
 #pragma unroll
-            for (int n = 0; n < DG_NV; ++n) a.canonical[node * DG_NV + n] = a.internal[io + (size_t)n * C::NODES];
+            for (int n = 0; n < DG_NV; ++n) a.canonical[node * DG_NV + n] = a.internal[io + n * VS];
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
 // max wavespeed  lam = max_nodes sqrt(u^2+v^2+w^2) + sqrt(gamma p / rho)   (reading R10)
+// of a freshly set state (after a Runge-Kutta step the last stage has already reduced it)
 // ------------------------------------------------------------------------------------------------
 template <class C>
 __global__ void __launch_bounds__(256) dg_wavespeed_kernel(const DgWaveArgs a) {
+    constexpr size_t VS = (size_t)C::N * C::HP;
     const size_t total = (size_t)a.nx * a.ny * a.nz * (C::N * C::N * C::N);
     double best = 0.0;
     for (size_t node = (size_t)blockIdx.x * blockDim.x + threadIdx.x; node < total;
          node += (size_t)gridDim.x * blockDim.x) {
         const size_t io = internal_offset<C>(node, a.nx, a.ny, a.nbx, a.nby);
-        const double Q0 = a.Q[io], Q1 = a.Q[io + (size_t)C::NODES], Q2 = a.Q[io + 2 * (size_t)C::NODES],
-                     Q3 = a.Q[io + 3 * (size_t)C::NODES], Q4 = a.Q[io + 4 * (size_t)C::NODES];
+        const double Q0 = a.Q[io], Q1 = a.Q[io + VS], Q2 = a.Q[io + 2 * VS], Q3 = a.Q[io + 3 * VS], Q4 = a.Q[io + 4 * VS];
         const double rinv = 1.0 / Q0;
         const double u = Q1 * rinv, v = Q2 * rinv, w = Q3 * rinv;
         const double pres = a.gm1 * (Q4 - 0.5 * Q0 * (u * u + v * v + w * w));
         const double s = sqrt(u * u + v * v + w * w) + sqrt(a.gamma * pres * rinv);
-        best = (s > best) ? s : best;
+        if (!(s <= best)) best = s;   // NaN sticks
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
         const double o = __shfl_xor_sync(0xffffffffu, best, off);
-        best = (o > best) ? o : best;
+        if (!(o <= best)) best = o;
     }
     if ((threadIdx.x & 31) == 0) atomicMax(a.lam_bits, (unsigned long long)__double_as_longlong(best));
 }
@@ -688,141 +848,94 @@ __global__ void __launch_bounds__(256) dg_wavespeed_kernel(const DgWaveArgs a) {
 // host-side launchers, one table per variant
 // ------------------------------------------------------------------------------------------------
 template <class C>
-void stage_config(cudaLaunchConfig_t &cfg, cudaLaunchAttribute &attr, int nbx, int nby, int nbz, cudaStream_t s) {
-    // one block per brick, blockIdx = brick coordinates, rounded up to whole clusters
-    cfg.gridDim = dim3((unsigned)((nbx + C::CLX - 1) / C::CLX * C::CLX), (unsigned)((nby + C::CLY - 1) / C::CLY * C::CLY),
-                       (unsigned)((nbz + C::CLZ - 1) / C::CLZ * C::CLZ));
-    cfg.blockDim = dim3(C::THREADS, 1, 1);
-    cfg.dynamicSmemBytes = C::SMEM_BYTES;
-    cfg.stream = s;
-    attr.id = cudaLaunchAttributeClusterDimension;
-    attr.val.clusterDim.x = C::CLX;
-    attr.val.clusterDim.y = C::CLY;
-    attr.val.clusterDim.z = C::CLZ;
-    cfg.attrs = &attr;
-    cfg.numAttrs = 1;
-}
-
-// Opt in to the shared-memory size; *resident = blocks of the stage kernel the whole GPU holds at once.
-template <class C>
-cudaError_t prepare(int *resident) {
-    cudaError_t err = cudaFuncSetAttribute(dg_stage_kernel<C, DG_MODE_STAGE>,
-                                           cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+cudaError_t prepare(int *blocks_per_sm) {
+    cudaError_t err = cudaSuccess;
+    auto opt_in = [&](auto kernel) {
+        if (err == cudaSuccess) err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    };
+    opt_in(dg_stage_kernel<C, DG_MODE_STAGE, false>);
+    opt_in(dg_stage_kernel<C, DG_MODE_STAGE, true>);
+    opt_in(dg_stage_kernel<C, DG_MODE_RESIDUAL, false>);
     if (err == cudaSuccess)
-        err = cudaFuncSetAttribute(dg_stage_kernel<C, DG_MODE_RESIDUAL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   C::SMEM_BYTES);
-    if (err == cudaSuccess)
-        err = cudaFuncSetAttribute(dg_stage_kernel<C, DG_MODE_TRACES>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   C::SMEM_BYTES);
+        err = cudaFuncSetAttribute(dg_traces_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::BUF * 8);
     if (err != cudaSuccess) return err;
-    if (C::CLUSTER > 1) {
-        cudaLaunchConfig_t cfg = {};
-        cudaLaunchAttribute attr;
-        stage_config<C>(cfg, attr, C::CLX * 64, C::CLY * 64, C::CLZ * 64, 0);
-        int clusters = 0;
-        err = cudaOccupancyMaxActiveClusters(&clusters, dg_stage_kernel<C, DG_MODE_STAGE>, &cfg);
-        *resident = clusters * C::CLUSTER;
-        return err;
-    }
-    int dev = 0, sms = 0, per_sm = 0;
-    err = cudaGetDevice(&dev);
-    if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (err == cudaSuccess)
-        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, dg_stage_kernel<C, DG_MODE_STAGE>, C::THREADS,
-                                                            C::SMEM_BYTES);
-    *resident = per_sm * sms;
-    return err;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, dg_stage_kernel<C, DG_MODE_STAGE, false>,
+                                                         C::THREADS, C::SMEM_BYTES);
 }
 
 template <class C>
 cudaError_t launch_stage(const DgStageArgs &a, cudaStream_t s) {
-    if (a.grid <= 0) return cudaErrorInvalidConfiguration;
-    cudaLaunchConfig_t cfg = {};
-    cudaLaunchAttribute attr;
-    stage_config<C>(cfg, attr, a.nbx, a.nby, a.nbz, s);
-    if (a.mode == DG_MODE_STAGE) return cudaLaunchKernelEx(&cfg, dg_stage_kernel<C, DG_MODE_STAGE>, a);
-    if (a.mode == DG_MODE_RESIDUAL) return cudaLaunchKernelEx(&cfg, dg_stage_kernel<C, DG_MODE_RESIDUAL>, a);
-    return cudaLaunchKernelEx(&cfg, dg_stage_kernel<C, DG_MODE_TRACES>, a);
-}
-
-inline unsigned flat_grid(size_t total) {
-    const size_t want = (total + 255) / 256;
-    const size_t cap = 148u * 16u;   // grid-stride: a few blocks per SM
-    return (unsigned)(want < cap ? (want ? want : 1) : cap);
-}
-
-template <class C>
-cudaError_t launch_layout(const DgLayoutArgs &a, cudaStream_t s) {
-    const size_t total = (size_t)a.nx * a.ny * a.nz * (C::N * C::N * C::N);
-    dg_layout_kernel<C><<<flat_grid(total), 256, 0, s>>>(a);
+    const dim3 grid((unsigned)a.nbx, (unsigned)a.nby, (unsigned)a.nchunks);
+    if (a.mode == DG_MODE_RESIDUAL) dg_stage_kernel<C, DG_MODE_RESIDUAL, false><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(a);
+    else if (a.want_lam) dg_stage_kernel<C, DG_MODE_STAGE, true><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(a);
+    else dg_stage_kernel<C, DG_MODE_STAGE, false><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(a);
     return cudaGetLastError();
 }
 
 template <class C>
-cudaError_t launch_wavespeed(const DgWaveArgs &a, cudaStream_t s) {
+cudaError_t launch_traces(const DgTraceArgs &a, cudaStream_t s) {
+    const dim3 grid((unsigned)a.nbx, (unsigned)a.nby, (unsigned)a.nz);
+    dg_traces_kernel<C><<<grid, C::NCOMP, C::BUF * 8, s>>>(a);
+    return cudaGetLastError();
+}
+
+inline unsigned flat_grid(size_t total, int sms) {
+    const size_t want = (total + 255) / 256;
+    const size_t cap = (size_t)(sms > 0 ? sms : 1) * 16u;   // grid-stride: a few blocks per SM
+    return (unsigned)(want < cap ? (want ? want : 1) : cap);
+}
+
+template <class C>
+cudaError_t launch_layout(const DgLayoutArgs &a, int sms, cudaStream_t s) {
     const size_t total = (size_t)a.nx * a.ny * a.nz * (C::N * C::N * C::N);
-    dg_wavespeed_kernel<C><<<flat_grid(total), 256, 0, s>>>(a);
+    dg_layout_kernel<C><<<flat_grid(total, sms), 256, 0, s>>>(a);
+    return cudaGetLastError();
+}
+
+template <class C>
+cudaError_t launch_wavespeed(const DgWaveArgs &a, int sms, cudaStream_t s) {
+    const size_t total = (size_t)a.nx * a.ny * a.nz * (C::N * C::N * C::N);
+    dg_wavespeed_kernel<C><<<flat_grid(total, sms), 256, 0, s>>>(a);
     return cudaGetLastError();
 }
 
 template <class C>
 constexpr DgKernelTable make_table() {
-    return DgKernelTable{C::N,       C::BX,          C::BY,           C::BZ,
-                         C::THREADS, C::SMEM_BYTES,  C::SLOT,         C::TSLOT,
-                         &prepare<C>, &launch_stage<C>, &launch_layout<C>, &launch_wavespeed<C>};
+    return DgKernelTable{C::N,       C::BX,          C::BY,         C::THREADS,      C::SMEM_BYTES,     C::SLOT,
+                         C::TXY,     C::TZ,          C::RELOAD ? 1 : 0, C::MINB, &prepare<C>, &launch_stage<C>,  &launch_traces<C>,
+                         &launch_layout<C>, &launch_wavespeed<C>};
 }
 
-// Variants per N (default first): Cfg<N, BX, BY, BZ, min blocks per SM, RELOAD, P, PP, OX, OY, OZ>.
-// DESIGN.md "brick shapes" and "shared-memory layout" explain the choices.
+// Variants per N (default first): Cfg<N, BX, BY, min blocks per SM, RELOAD, PP, OX, OY>.
+// DESIGN.md "column shapes" and "shared-memory layout" explain the choices.
 #if DG_N == 2
-using V0 = Cfg<2, 4, 4, 2, 6, 1, 9, 76, 1, 1, 2>;
-using V1 = Cfg<2, 4, 4, 2, 6, 0, 9, 76, 1, 1, 2>;
-using V2 = Cfg<2, 4, 4, 4, 3, 1, 8, 65, 1, 0, 0>;
-using V3 = Cfg<2, 4, 4, 4, 3, 0, 8, 65, 1, 0, 0>;
+using V0 = Cfg<2, 8, 8, 3, 0>;
+using V1 = Cfg<2, 4, 4, 6, 0>;
 #elif DG_N == 3
-using V0 = Cfg<3, 4, 4, 2, 2, 1, 12, 156, 3, 0, 0>;
-using V1 = Cfg<3, 2, 2, 2, 7, 0, 6, 38, 2, 0, 0>;
-using V2 = Cfg<3, 2, 2, 2, 7, 1, 6, 38, 2, 0, 0>;
-using V3 = Cfg<3, 4, 4, 2, 2, 0, 12, 156, 3, 0, 0>;
+using V0 = Cfg<3, 4, 4, 3, 0>;
+using V1 = Cfg<3, 2, 2, 6, 0>;
 #elif DG_N == 4
-using V0 = Cfg<4, 2, 2, 2, 3, 0, 9, 74, 1, 1, 2>;
-using V1 = Cfg<4, 2, 2, 2, 3, 1, 9, 74, 1, 1, 2>;
-using V2 = Cfg<4, 2, 2, 1, 6, 1, 8, 65, 3, 0, 0>;
-using V3 = Cfg<4, 2, 2, 1, 6, 0, 8, 65, 3, 0, 0>;
+using V0 = Cfg<4, 4, 2, 3, 0>;
+using V1 = Cfg<4, 2, 2, 5, 0>;
 #elif DG_N == 5
-using V0 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0>;
-using V1 = Cfg<5, 1, 2, 2, 4, 1, 0, 0, 0, 1, 0>;
-using V2 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0, 2, 2, 2>;
-using V3 = Cfg<5, 1, 2, 2, 4, 0, 0, 0, 0, 1, 0, 2, 1, 1>;
-using V4 = Cfg<5, 5, 1, 1, 3, 0, 0, 0, 4, 1, 0>;   // 125 lines on 128 threads
-using V5 = Cfg<5, 1, 2, 3, 3, 1, 0, 0, 0, 1, 0>;
-#define DG_MORE_VARIANTS make_table<V4>(), make_table<V5>(),
+using V0 = Cfg<5, 2, 2, 3, 0>;
+using V1 = Cfg<5, 2, 1, 5, 0>;
 #elif DG_N == 6
-using V0 = Cfg<6, 1, 1, 2, 4, 1, 6, 38, 1, 0, 0>;
-using V1 = Cfg<6, 1, 1, 2, 4, 0, 6, 38, 1, 0, 0>;
-using V2 = Cfg<6, 1, 2, 2, 2, 1, 6, 75, 0, 3, 0>;
-using V3 = Cfg<6, 1, 2, 2, 2, 0, 6, 75, 0, 3, 0>;
+using V0 = Cfg<6, 2, 1, 3, 0>;
+using V1 = Cfg<6, 2, 2, 2, 0>;
 #elif DG_N == 7
-using V0 = Cfg<7, 1, 1, 2, 3, 1, 7, 55, 1, 0, 0>;
-using V1 = Cfg<7, 1, 1, 2, 3, 0, 7, 55, 1, 0, 0>;
-using V2 = Cfg<7, 1, 1, 1, 6, 1, 7, 55, 1, 0, 0>;
-using V3 = Cfg<7, 1, 1, 1, 6, 0, 7, 55, 1, 0, 0>;
+using V0 = Cfg<7, 1, 1, 4, 0>;
+using V1 = Cfg<7, 2, 1, 2, 0>;
 #elif DG_N == 8
-using V0 = Cfg<8, 1, 1, 2, 2, 0, 8, 65, 1, 1, 0>;
-using V1 = Cfg<8, 1, 1, 2, 2, 1, 8, 65, 1, 1, 0>;
-using V2 = Cfg<8, 1, 1, 1, 4, 1, 8, 65, 1, 0, 0>;
-using V3 = Cfg<8, 1, 1, 1, 4, 0, 8, 65, 1, 0, 0>;
+using V0 = Cfg<8, 1, 1, 3, 0>;
+using V1 = Cfg<8, 1, 1, 3, 1>;
 #else
 #error "DG_N must be 2..8"
 #endif
 
-using VE = Cfg<DG_N, 1, 1, 1, 4, 1>;   // one element per block: always there (tiny and ragged meshes, tests)
+using VE = Cfg<DG_N, 1, 1, 2, 1>;   // one element per layer: always there (tiny and ragged meshes, tests)
 
-#ifndef DG_MORE_VARIANTS
-#define DG_MORE_VARIANTS
-#endif
-const DgKernelTable k_tables[] = {make_table<V0>(), make_table<V1>(), make_table<V2>(), make_table<V3>(),
-                                  DG_MORE_VARIANTS make_table<VE>()};
+const DgKernelTable k_tables[] = {make_table<V0>(), make_table<V1>(), make_table<VE>()};
 
 }  // namespace
 
