@@ -164,14 +164,14 @@ def run_reference(args, rank):
 # ----------------------------------------------------------------------------------------------
 # the CUDA path
 # ----------------------------------------------------------------------------------------------
-def time_workload(workload, K, W, device, dist, sampler_index=None, want_e2e=False, variant=None):
+def time_workload(workload, K, W, device, dist, sampler_index=None, want_e2e=False, variant=None, lz=0):
     import torch
     from paper_2006_15698_b200 import DG
     from paper_2006_15698_b200 import inputs as I
     c = I.CONFIGS[workload]
     p, ext, n = c["p"], c["extent"], (c["nx"], c["ny"], c["nz"])
     q = I.make_field(workload, xp=torch, device=device)
-    dg = DG(*n, p, GAMMA, ext, device=device, variant=variant)
+    dg = DG(*n, p, GAMMA, ext, device=device, variant=variant, brick=(0, 0, lz) if lz else None)
     dg.set_state(q)
     dt = I.cfl_dt(dg.max_wavespeed(), p, ext, n, 0.1)
     dof = n[0] * n[1] * n[2] * (p + 1) ** 3
@@ -262,7 +262,7 @@ def run_variant_sweep(args):
     peak, _ = measured_peaks()
     p = I.CONFIGS[args.workload]["p"]
     for v in range(load_library().dg_variant_count(p)):
-        r = time_workload(args.workload, args.steps, max(3, args.warmup), device, None, variant=v)
+        r = time_workload(args.workload, args.steps, max(3, args.warmup), device, None, variant=v, lz=args.lz)
         rate = r["dof"] * STAGES * args.steps / (r["ms"] * 1e-3)
         print(json.dumps({"workload": args.workload, "variant": v, "kernel": r["kernel"], "value": rate, "unit": UNIT,
                           "roofline_frac": rate * ALGO_BYTES_PER_DOF_STAGE / 1e9 / peak, "finite": r["finite"]}), flush=True)
@@ -349,6 +349,7 @@ def main():
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--lz", type=int, default=0, help="layers per chunk (tuning; 0 = library default)")
     ap.add_argument("--sweep-variants", action="store_true", help="time every compiled variant of --workload")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

@@ -83,33 +83,18 @@ void build_host_ops(int N, HostOps &o) {
     }
 }
 
-// Device tables: the weak-form volume operator and the lift weights with the inverse (diagonal) mass and
-// the constant geometric factor g_a = 2/h_a of each axis folded in.
-void build_device_ops(int N, const double g[3], DgOps &d) {
+// Device tables on the reference element: the weak-form volume operator and the lift weights with the
+// inverse (diagonal) mass folded in; the constant geometric factor 2/h_a of each axis
+// travels separately (DgStageArgs::scale).
+void build_ref_ops(int N, DgRefOps &d) {
     HostOps o;
     build_host_ops(N, o);
     std::memset(&d, 0, sizeof(d));
     for (int i = 0; i < N; ++i) {
         d.lp[i] = (double)o.lp[i];
-        d.lm[i] = (double)o.lm[i];
-        for (int a = 0; a < 3; ++a) {
-            const long double ga = (long double)g[a];
-            d.lpg[a][i] = (double)(0.5L * ga * o.lp[i] / o.w[i]);   // 1/2: the kernel's interface flux is 2 F*
-            d.lmg[a][i] = (double)(0.5L * ga * o.lm[i] / o.w[i]);
-            for (int q = 0; q < N; ++q) d.Dg[a][q][i] = (double)(ga * o.w[q] * o.D[q][i] / o.w[i]);
-        }
+        d.lq[i] = (double)(0.5L * o.lp[i] / o.w[i]);   // 1/2: the kernel's interface flux is 2 F*
+        for (int q = 0; q < N; ++q) d.D[q][i] = (double)(o.w[q] * o.D[q][i] / o.w[i]);
     }
-}
-
-// The same tables with the time step folded in: the stage kernel then accumulates dt * L(Q) directly.
-void scale_ops(const DgOps &in, double dt, DgOps &out) {
-    out = in;
-    for (int a = 0; a < 3; ++a)
-        for (int i = 0; i < DG_NMAX; ++i) {
-            out.lpg[a][i] = dt * in.lpg[a][i];
-            out.lmg[a][i] = dt * in.lmg[a][i];
-            for (int q = 0; q < DG_NMAX; ++q) out.Dg[a][q][i] = dt * in.Dg[a][q][i];
-        }
 }
 
 // Carpenter-Kennedy (5,4) 2N-storage Runge-Kutta, "LSERK45" (reading R9).
@@ -165,7 +150,7 @@ struct dg_ctx {
     int tcur;           // Txy[tcur], Tz[tcur] hold the traces of the current Q
     bool lam_valid;     // scal[0] holds the max wavespeed of the current Q (reduced by the last stage)
     int sms, blocks_per_sm;
-    DgOps ops;          // device operator tables of this mesh (travel in the kernel arguments)
+    double g[3];        // 2/h_a per axis
     bool bound, has_state;
     cudaStream_t stream;
     unsigned long long launches;
@@ -256,7 +241,7 @@ DgStageArgs stage_args(const dg_ctx *c, int mode) {
     a.gamma = c->gamma;
     a.gm1 = c->gamma - 1.0;
     a.mode = mode;
-    a.ops = c->ops;
+    for (int i = 0; i < 3; ++i) a.scale[i] = c->g[i];
     return a;
 }
 
@@ -287,10 +272,10 @@ int export_vector(dg_ctx *c, double *internal, double *out, int on_device, const
 
 // One LSERK45 step = 5 launches of the fused stage kernel; the last stage can reduce the max wavespeed
 // of the state it produces on the way (a9 fused: no extra sweep over the state).
-int enqueue_step(dg_ctx *c, const DgOps &scaled, bool want_lam) {
+int enqueue_step(dg_ctx *c, double dt, bool want_lam) {
     for (int s = 0; s < 5; ++s) {
         DgStageArgs a = stage_args(c, DG_MODE_STAGE);
-        a.ops = scaled;
+        for (int i = 0; i < 3; ++i) a.scale[i] = dt * c->g[i];
         a.rkA = (double)kRkA[s];
         a.rkB = (double)kRkB[s];
         a.want_lam = (want_lam && s == 4) ? 1 : 0;
@@ -448,9 +433,12 @@ int dg_bind(dg_ctx *c, void *ws, size_t bytes, void *stream) {
     }
     e = cudaMemsetAsync(c->scal, 0, 256, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "workspace memset");
-    const double g[3] = {2.0 / (c->extent[0] / c->nx), 2.0 / (c->extent[1] / c->ny), 2.0 / (c->extent[2] / c->nz)};
-    build_device_ops(c->N, g, c->ops);
-    e = c->kt->prepare(&c->blocks_per_sm);
+    c->g[0] = 2.0 / (c->extent[0] / c->nx);
+    c->g[1] = 2.0 / (c->extent[1] / c->ny);
+    c->g[2] = 2.0 / (c->extent[2] / c->nz);
+    DgRefOps ref;
+    build_ref_ops(c->N, ref);
+    e = c->kt->prepare(ref, &c->blocks_per_sm);
     if (e != cudaSuccess) return cuda_fail(c, e, "stage kernel setup");
     if (c->blocks_per_sm < 1) return fail(c, DG_ECUDA, "stage kernel does not fit on the GPU");
     c->bound = true;
@@ -479,10 +467,6 @@ int dg_set_state(dg_ctx *c, const double *q, int on_device) {
     a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
     a.nbx = c->nbx; a.nby = c->nby;
     a.lz = c->lz; a.nchunks = c->nchunks;
-    for (int i = 0; i < DG_NMAX; ++i) {
-        a.lp[i] = c->ops.lp[i];
-        a.lm[i] = c->ops.lm[i];
-    }
     cudaError_t e = c->kt->launch_traces(a, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "trace kernel");
     c->launches++;
@@ -511,10 +495,8 @@ int dg_rk_step(dg_ctx *c, double dt, int nsteps) {
     if (!c) return DG_EINVAL;
     if (nsteps < 0 || !std::isfinite(dt)) return fail(c, DG_EINVAL, "nsteps < 0 or dt not finite");
     if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_rk_step needs dg_bind and dg_set_state first");
-    DgOps scaled;
-    scale_ops(c->ops, dt, scaled);
     for (int step = 0; step < nsteps; ++step) {
-        const int rc = enqueue_step(c, scaled, false);
+        const int rc = enqueue_step(c, dt, false);
         if (rc != DG_OK) return rc;
     }
     return DG_OK;
@@ -534,9 +516,7 @@ int dg_rk_step_cfl(dg_ctx *c, double cfl, int nsteps, double *t_advanced, double
         if (rc != DG_OK) return rc;
         if (!(lam > 0.0) || !std::isfinite(lam)) return fail(c, DG_ESTATE, "max wavespeed %g is not positive and finite", lam);
         dt = cfl * hmin / ((2.0 * c->p + 1.0) * lam);
-        DgOps scaled;
-        scale_ops(c->ops, dt, scaled);
-        rc = enqueue_step(c, scaled, true);
+        rc = enqueue_step(c, dt, true);
         if (rc != DG_OK) return rc;
         t += dt;
     }

@@ -8,16 +8,16 @@
 #define DG_NV 5      // rho, rho u, rho v, rho w, rho E       (eq (2))
 #define DG_NMAX 8    // largest N = p+1 compiled
 
-// 1-D operators of the collocated Gauss-Legendre Lagrange basis, built on the
-// host in long double (dg_api.cu) with the constant geometric factor 2/h_a of each axis
-// folded in, rounded to double once.  In the Runge-Kutta stage kernel Dg, lpg and lmg
-// are additionally multiplied by the time step (dg_rk_step), so the kernel accumulates dt * L(Q).  They
-// travel inside the kernel arguments (constant bank; per context, so contexts with different meshes coexist).
-struct DgOps {
-    double Dg[3][DG_NMAX][DG_NMAX];     // Dg[a][q][i] = (2/h_a) w_q l_i'(xi_q) / w_i   (eq (5) 2nd term / mass)
-    double lpg[3][DG_NMAX];             // 1/2 (2/h_a) l_i(+1) / w_i     (lift / mass; the kernel forms 2 F*)
-    double lmg[3][DG_NMAX];             // 1/2 (2/h_a) l_i(-1) / w_i
-    double lp[DG_NMAX], lm[DG_NMAX];    // l_i(+1), l_i(-1)                             (face traces)
+// 1-D operators of the collocated Gauss-Legendre Lagrange basis on the reference element [-1,1]
+// (PAPER.md:72-80), built on the host in long double (dg_api.cu), rounded to double once.  They depend on
+// N = p+1 only, so every kernel translation unit keeps ONE copy in __constant__ memory (uploaded by
+// prepare()); the constant geometric factor 2/h_a of each axis and the time step travel
+// in DgStageArgs::scale and are applied when an axis' contribution is added to the Runge-Kutta register.
+// The nodes are symmetric: l_i(-1) = l_{N-1-i}(+1), so the "-" tables are the "+" tables read backwards.
+struct DgRefOps {
+    double D[DG_NMAX][DG_NMAX];   // D[q][i] = w_q l_i'(xi_q) / w_i        (eq (5) 2nd term / mass)
+    double lq[DG_NMAX];           // 1/2 l_i(+1) / w_i                     (lift / mass; the kernel forms 2 F*)
+    double lp[DG_NMAX];           // l_i(+1)                               (face traces)
 };
 
 #ifdef __CUDACC__
@@ -66,14 +66,13 @@ struct DgStageArgs {
     double rkA, rkB;      // stage coefficients; rkA == 0 means "do not read K" (stage 1)
     int mode;
     int want_lam;
-    DgOps ops;
+    double scale[3];      // 2/h_a per axis, times dt in stage mode: K accumulates dt * L(Q)
 };
 
 struct DgTraceArgs {
     const double *Q;
     double *Txy, *Tz;
     int nx, ny, nz, nbx, nby, lz, nchunks;
-    double lp[DG_NMAX], lm[DG_NMAX];
 };
 
 struct DgLayoutArgs {
@@ -100,7 +99,8 @@ struct DgKernelTable {
     long long tz;            // z face-trace doubles per chunk slot
     int reload;
     int minb;                // blocks per SM the kernel is compiled for (__launch_bounds__)
-    cudaError_t (*prepare)(int *blocks_per_sm);   // opt in to the shared memory size; resident blocks per SM
+    // upload the reference operators, opt in to the shared memory size; *blocks_per_sm = resident blocks per SM
+    cudaError_t (*prepare)(const DgRefOps &ref, int *blocks_per_sm);
     cudaError_t (*launch_stage)(const DgStageArgs &a, cudaStream_t s);
     cudaError_t (*launch_traces)(const DgTraceArgs &a, cudaStream_t s);
     cudaError_t (*launch_layout)(const DgLayoutArgs &a, int sms, cudaStream_t s);

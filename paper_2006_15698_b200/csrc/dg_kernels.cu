@@ -71,8 +71,6 @@ struct Cfg {
     static constexpr int TZ = 2 * DG_NV * CZ;                      // z trace doubles per chunk slot
     static constexpr bool MULTI = (BX > 1) || (BY > 1);
     static constexpr int LINEBUF = MULTI ? DG_NV * L : 0;          // T- / F* hand-over between elements of a layer
-    static constexpr int SMEM_DOUBLES = 3 * BUF + 2 * LINEBUF;
-    static constexpr int SMEM_BYTES = SMEM_DOUBLES * 8 + 64;       // + mbarriers
     static_assert(PP >= HP && (PP % 2) == 0, "plane pitch must be even and hold a plane");
     static_assert((BUF % 2) == 0 && (LINEBUF % 2) == 0, "buffers must stay 16-byte aligned");
 };
@@ -250,10 +248,29 @@ __device__ __forceinline__ bool line_inside(const Geo &g, int ext0, int ext1) {
     return g.t1 < ext0 * C::N && g.t2 < ext1 * C::N;
 }
 
+// Reference-element operators of this N (DgRefOps; uploaded by prepare()).  "-" side tables are the "+" side
+// tables read backwards (symmetric nodes).
+__constant__ DgRefOps c_ref;
+#define DG_LP(q) c_ref.lp[q]
+#define DG_LM(q) c_ref.lp[DG_N - 1 - (q)]
+#define DG_LQP(i) c_ref.lq[i]
+#define DG_LQM(i) c_ref.lq[DG_N - 1 - (i)]
+
+// What the compute warps need of the kernel arguments and the block's position, written to shared memory once
+// per block: layer_body() is a separate (not inlined) function and takes everything from here.
+struct BlockInfo {
+    const double *halo[4];     // Txy_old blocks of layer z0 this column reads: x low, x high, y low, y high
+    double *txy_out;           // this column's Txy_new slot of layer z0
+    const double *tz_lo, *tz_hi;
+    double *tz_out;
+    long long tstride;         // doubles between consecutive layers in Txy
+    double gamma, gm1, rkA, rkB, scale[3];
+    int ext0, ext1, readK, nl;
+};
+
 // PE for one of the axes x, y: traces of the Q in shared memory on the column boundary -> Tslot.
 template <class C, int AX>
-__device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta, const double *Qs, double *Tslot,
-                                                const double (&lp)[DG_NMAX], const double (&lm)[DG_NMAX]) {
+__device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta, const double *Qs, double *Tslot) {
     using A = Axis<C, AX>;
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE;
     const bool first = g.e == 0, last = g.e == exta - 1;
@@ -269,28 +286,34 @@ __device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta
 #pragma unroll
             for (int n = 0; n < NV; ++n) {
                 const double Qv = Q0[n * PLANE + q * A::S];
-                Tp[n] = fma(lp[q], Qv, Tp[n]);
-                Tm[n] = fma(lm[q], Qv, Tm[n]);
+                Tp[n] = fma(DG_LP(q), Qv, Tp[n]);
+                Tm[n] = fma(DG_LM(q), Qv, Tm[n]);
             }
 #pragma unroll
         for (int n = 0; n < NV; ++n) {
             dst[n * A::Ca] = Tm[n];
             dst[(NV + n) * A::Ca] = Tp[n];
         }
-    } else {
-        // one end only: the interpolation weights of the - end are those of the + end reversed
+    } else if (first) {
         double T[NV];
 #pragma unroll
         for (int n = 0; n < NV; ++n) T[n] = 0.0;
 #pragma unroll
-        for (int q = 0; q < N; ++q) {
-            const double w = first ? lm[q] : lp[q];
+        for (int q = 0; q < N; ++q)
 #pragma unroll
-            for (int n = 0; n < NV; ++n) T[n] = fma(w, Q0[n * PLANE + q * A::S], T[n]);
-        }
-        if (!first) dst += NV * A::Ca;
+            for (int n = 0; n < NV; ++n) T[n] = fma(DG_LM(q), Q0[n * PLANE + q * A::S], T[n]);
 #pragma unroll
         for (int n = 0; n < NV; ++n) dst[n * A::Ca] = T[n];
+    } else {
+        double T[NV];
+#pragma unroll
+        for (int n = 0; n < NV; ++n) T[n] = 0.0;
+#pragma unroll
+        for (int q = 0; q < N; ++q)
+#pragma unroll
+            for (int n = 0; n < NV; ++n) T[n] = fma(DG_LP(q), Q0[n * PLANE + q * A::S], T[n]);
+#pragma unroll
+        for (int n = 0; n < NV; ++n) dst[(NV + n) * A::Ca] = T[n];
     }
 }
 
@@ -311,19 +334,18 @@ __device__ __forceinline__ const double *halo_source(const double *T, int nbx, i
 // Order chosen for register pressure: the line's Q goes into registers once; the face traces and the two
 // interface fluxes come first (no accumulators alive yet); the accumulators then START from the lift term
 // and the volume term is added node by node.
-//   r_i = sum_q Dhat_iq F_q - (l_i(+1) F*_+ - l_i(-1) F*_-) (2/h_a)/w_i
+//   r_i = (2/h_a) [ sum_q Dhat_iq F_q - (l_i(+1) F*_+ - l_i(-1) F*_-)/w_i ]
 // Threads without a line of their own (`act` false: the tail of the last warp, lines in the padding of a ragged
-// column) run the arithmetic on a valid line all the same and only their stores are switched off: every
-// register is then defined on every path through the layer loop, which is what keeps the line's 10 N + 30
-// values from staying alive (and spilling) across the other two passes.
+// column) run the arithmetic on a valid line all the same and only their stores are switched off.
 template <class C, int AX, int MODE>
-__device__ __forceinline__ void xy_pass(const DgStageArgs &a, const Geo &g, bool act, int exta, const double *halo_lo,
+__device__ __forceinline__ void xy_pass(const BlockInfo *bi, const Geo &g, bool act, int exta, const double *halo_lo,
                                         const double *halo_hi, const double *Qs, double *KR, double *Tms, double *Fss,
-                                        bool readK, uint64_t *fullk, unsigned kparity) {
+                                        uint64_t *fullk, unsigned kparity) {
     using A = Axis<C, AX>;
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE, L = C::L, S = A::S, Ca = A::Ca;
     const bool first = g.e == 0, last = g.e == exta - 1;
     const int lb = g.e * Ca + g.c;   // slot of this line in the hand-over buffers
+    const double gamma = bi->gamma, gm1 = bi->gm1;
     // PH: the neighbour columns' traces this line touches, momentum slots rotated, HBM/L2 -> registers
     double Hlo[NV], Hhi[NV];
 #pragma unroll
@@ -351,8 +373,8 @@ __device__ __forceinline__ void xy_pass(const DgStageArgs &a, const Geo &g, bool
         for (int q = 0; q < N; ++q) {
             const double Qv = Q0[var_of_slot<C, AX>(s) * PLANE + q * S];
             if (!C::RELOAD) QL[s][q] = Qv;
-            Tp[s] = fma(a.ops.lp[q], Qv, Tp[s]);
-            Tm[s] = fma(a.ops.lm[q], Qv, Tm[s]);
+            Tp[s] = fma(DG_LP(q), Qv, Tp[s]);
+            Tm[s] = fma(DG_LM(q), Qv, Tm[s]);
         }
     }
     if (A::MULTI) {
@@ -369,27 +391,27 @@ __device__ __forceinline__ void xy_pass(const DgStageArgs &a, const Geo &g, bool
 #pragma unroll
         for (int n = 0; n < NV; ++n) Hhi[n] = Tms[n * L + lb + Ca];   // T- of the next element of this layer
     }
-    lax_friedrichs2(Tp, Hhi, 1.0, a.gamma, a.gm1, Fp);
+    lax_friedrichs2(Tp, Hhi, 1.0, gamma, gm1, Fp);
     if (A::MULTI) {
         if (act) {
 #pragma unroll
             for (int n = 0; n < NV; ++n) Fss[n * L + lb] = Fp[n];
         }
-        if (first) lax_friedrichs2(Tm, Hlo, -1.0, a.gamma, a.gm1, Fm);
+        if (first) lax_friedrichs2(Tm, Hlo, -1.0, gamma, gm1, Fm);
         bar_sync<C::NCOMP>(1);
         if (!first) {
 #pragma unroll
             for (int n = 0; n < NV; ++n) Fm[n] = Fss[n * L + lb - Ca];
         }
     } else {
-        lax_friedrichs2(Tm, Hlo, -1.0, a.gamma, a.gm1, Fm);
+        lax_friedrichs2(Tm, Hlo, -1.0, gamma, gm1, Fm);
     }
 
-    // ------------- PC: lift (2/h and 1/w folded into the tables) starts the accumulators -----------
+    // ------------- PC: lift (1/w folded into the table) starts the accumulators -----------------------
     double V[NV][N];
 #pragma unroll
     for (int i = 0; i < N; ++i) {
-        const double cp = a.ops.lpg[AX][i], cm = a.ops.lmg[AX][i];
+        const double cp = DG_LQP(i), cm = DG_LQM(i);
 #pragma unroll
         for (int n = 0; n < NV; ++n) V[n][i] = fma(cm, Fm[n], -cp * Fp[n]);
     }
@@ -400,11 +422,11 @@ __device__ __forceinline__ void xy_pass(const DgStageArgs &a, const Geo &g, bool
 #pragma unroll
         for (int s = 0; s < NV; ++s)
             Qn[s] = C::RELOAD ? Q0[var_of_slot<C, AX>(s) * PLANE + q * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : q];
-        euler_flux_normal(Qn, a.gm1, F, vel, pres, rinv);
+        euler_flux_normal(Qn, gm1, F, vel, pres, rinv);
 #pragma unroll
         for (int n = 0; n < NV; ++n)
 #pragma unroll
-            for (int i = 0; i < N; ++i) V[n][i] = fma(a.ops.Dg[AX][q][i], F[n], V[n][i]);
+            for (int i = 0; i < N; ++i) V[n][i] = fma(c_ref.D[q][i], F[n], V[n][i]);
     }
     // ------------- PD: Runge-Kutta accumulation on the staged K -----------------------------------------
     if (AX == 0) {
@@ -414,21 +436,22 @@ __device__ __forceinline__ void xy_pass(const DgStageArgs &a, const Geo &g, bool
     }
     if (act) {
         double *K0 = KR + g.base;
+        const double sc = bi->scale[AX];
         if (AX == 0) {
-            if (readK) {
-                const double rkA = a.rkA;
+            if (bi->readK) {
+                const double rkA = bi->rkA;
 #pragma unroll
                 for (int s = 0; s < NV; ++s)
 #pragma unroll
                     for (int i = 0; i < N; ++i) {
                         double *p = K0 + var_of_slot<C, AX>(s) * PLANE + i * S;
-                        *p = fma(rkA, *p, V[s][i]);
+                        *p = fma(rkA, *p, sc * V[s][i]);
                     }
             } else {
 #pragma unroll
                 for (int s = 0; s < NV; ++s)
 #pragma unroll
-                    for (int i = 0; i < N; ++i) K0[var_of_slot<C, AX>(s) * PLANE + i * S] = V[s][i];
+                    for (int i = 0; i < N; ++i) K0[var_of_slot<C, AX>(s) * PLANE + i * S] = sc * V[s][i];
             }
         } else {
 #pragma unroll
@@ -436,23 +459,24 @@ __device__ __forceinline__ void xy_pass(const DgStageArgs &a, const Geo &g, bool
 #pragma unroll
                 for (int i = 0; i < N; ++i) {
                     double *p = K0 + var_of_slot<C, AX>(s) * PLANE + i * S;
-                    *p += V[s][i];
+                    *p = fma(sc, V[s][i], *p);
                 }
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// the z pass of one layer: thread (gx, gy) owns the z line; the flux on the lower face is carried in Fm
+// the z pass of one layer: thread (gx, gy) owns the z line; the flux on the lower face of the layer is the one
+// this thread computed for the upper face of the previous layer, kept in FmS (shared memory, [5][L])
 // ------------------------------------------------------------------------------------------------
 template <class C, int MODE, bool LAM>
-__device__ __forceinline__ void z_pass(const DgStageArgs &a, const Geo &g, bool act, double *Qs, const double *Qnext,
-                                       const double *tz_lo, const double *tz_hi, double *tz_out, double *KR,
-                                       double (&Fm)[DG_NV], bool first_layer, bool last_layer, double &lam_best) {
+__device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l, bool act, double *Qs, const double *Qnext,
+                                       double *KR, double *FmS, bool first_layer, bool last_layer, double &lam_best) {
     constexpr int AX = 2;
     using A = Axis<C, AX>;
-    constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE, S = A::S, Ca = A::Ca;
-    double QL[C::RELOAD ? 1 : NV][C::RELOAD ? 1 : N], V[NV][N], Fp[NV];
+    constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE, S = A::S, Ca = A::Ca, L = C::L;
+    const double gamma = bi->gamma, gm1 = bi->gm1;
+    double QL[C::RELOAD ? 1 : NV][C::RELOAD ? 1 : N], V[NV][N], Fp[NV], Fm[NV];
     // PH: T- of the line above: from the next layer of the ring, or (top of the chunk) from HBM
     double Hhi[NV];
     if (!last_layer) {
@@ -461,10 +485,11 @@ __device__ __forceinline__ void z_pass(const DgStageArgs &a, const Geo &g, bool 
         for (int s = 0; s < NV; ++s) {
             double t = 0.0;
 #pragma unroll
-            for (int q = 0; q < N; ++q) t = fma(a.ops.lm[q], Q1[var_of_slot<C, AX>(s) * PLANE + q * S], t);
+            for (int q = 0; q < N; ++q) t = fma(DG_LM(q), Q1[var_of_slot<C, AX>(s) * PLANE + q * S], t);
             Hhi[s] = t;
         }
     } else {
+        const double *tz_hi = bi->tz_hi;
 #pragma unroll
         for (int s = 0; s < NV; ++s) Hhi[s] = __ldg(tz_hi + var_of_slot<C, AX>(s) * Ca + g.c);
     }
@@ -478,27 +503,35 @@ __device__ __forceinline__ void z_pass(const DgStageArgs &a, const Geo &g, bool 
         for (int q = 0; q < N; ++q) {
             const double Qv = Q0[var_of_slot<C, AX>(s) * PLANE + q * S];
             if (!C::RELOAD) QL[s][q] = Qv;
-            Tp[s] = fma(a.ops.lp[q], Qv, Tp[s]);
+            Tp[s] = fma(DG_LP(q), Qv, Tp[s]);
         }
     }
     // PB
     if (first_layer) {   // bottom of the chunk: own T- against T+ of the layer below (from HBM)
         double Tm[NV], Hlo[NV];
+        const double *tz_lo = bi->tz_lo;
 #pragma unroll
         for (int s = 0; s < NV; ++s) {
             double t = 0.0;
 #pragma unroll
-            for (int q = 0; q < N; ++q) t = fma(a.ops.lm[q], Q0[var_of_slot<C, AX>(s) * PLANE + q * S], t);
+            for (int q = 0; q < N; ++q) t = fma(DG_LM(q), Q0[var_of_slot<C, AX>(s) * PLANE + q * S], t);
             Tm[s] = t;
             Hlo[s] = __ldg(tz_lo + var_of_slot<C, AX>(s) * Ca + g.c);
         }
-        lax_friedrichs2(Tm, Hlo, -1.0, a.gamma, a.gm1, Fm);
+        lax_friedrichs2(Tm, Hlo, -1.0, gamma, gm1, Fm);
+    } else {
+#pragma unroll
+        for (int n = 0; n < NV; ++n) Fm[n] = FmS[n * L + l];
     }
-    lax_friedrichs2(Tp, Hhi, 1.0, a.gamma, a.gm1, Fp);
+    lax_friedrichs2(Tp, Hhi, 1.0, gamma, gm1, Fp);
+    if (!last_layer) {
+#pragma unroll
+        for (int n = 0; n < NV; ++n) FmS[n * L + l] = Fp[n];   // the next layer's lower face (same thread reads it)
+    }
     // PC
 #pragma unroll
     for (int i = 0; i < N; ++i) {
-        const double cp = a.ops.lpg[AX][i], cm = a.ops.lmg[AX][i];
+        const double cp = DG_LQP(i), cm = DG_LQM(i);
 #pragma unroll
         for (int n = 0; n < NV; ++n) V[n][i] = fma(cm, Fm[n], -cp * Fp[n]);
     }
@@ -509,29 +542,29 @@ __device__ __forceinline__ void z_pass(const DgStageArgs &a, const Geo &g, bool 
 #pragma unroll
         for (int s = 0; s < NV; ++s)
             Qn[s] = C::RELOAD ? Q0[var_of_slot<C, AX>(s) * PLANE + q * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : q];
-        euler_flux_normal(Qn, a.gm1, F, vel, pres, rinv);
+        euler_flux_normal(Qn, gm1, F, vel, pres, rinv);
 #pragma unroll
         for (int n = 0; n < NV; ++n)
 #pragma unroll
-            for (int i = 0; i < N; ++i) V[n][i] = fma(a.ops.Dg[AX][q][i], F[n], V[n][i]);
+            for (int i = 0; i < N; ++i) V[n][i] = fma(c_ref.D[q][i], F[n], V[n][i]);
     }
-#pragma unroll
-    for (int n = 0; n < NV; ++n) Fm[n] = Fp[n];   // the next layer's lower face
     bar_sync<C::NCOMP>(1);   // the y pass of every line is done with K (and, RELOAD, with Q)
     if (act) {
         // PD
         double *K0 = KR + g.base;
         double *Q0w = Qs + g.base;
+        const double sc = bi->scale[AX];
         if (MODE == DG_MODE_RESIDUAL) {
 #pragma unroll
             for (int s = 0; s < NV; ++s)
 #pragma unroll
                 for (int i = 0; i < N; ++i) {
                     double *p = K0 + var_of_slot<C, AX>(s) * PLANE + i * S;
-                    *p += V[s][i];
+                    *p = fma(sc, V[s][i], *p);
                 }
         } else {
-            const double rkB = a.rkB;
+            const double rkB = bi->rkB;
+            double *tz_out = bi->tz_out;
             double Qn[LAM ? NV : 1][N];
 #pragma unroll
             for (int s = 0; s < NV; ++s) {
@@ -539,7 +572,7 @@ __device__ __forceinline__ void z_pass(const DgStageArgs &a, const Geo &g, bool 
                 const int sq = LAM ? s : 0;
 #pragma unroll
                 for (int i = 0; i < N; ++i) {
-                    const double Kn = K0[n * PLANE + i * S] + V[s][i];
+                    const double Kn = fma(sc, V[s][i], K0[n * PLANE + i * S]);
                     const double Qold = C::RELOAD ? Q0w[n * PLANE + i * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : i];
                     Qn[sq][i] = fma(rkB, Kn, Qold);
                     K0[n * PLANE + i * S] = Kn;
@@ -549,13 +582,13 @@ __device__ __forceinline__ void z_pass(const DgStageArgs &a, const Geo &g, bool 
                 if (first_layer) {
                     double tm = 0.0;
 #pragma unroll
-                    for (int i = 0; i < N; ++i) tm = fma(a.ops.lm[i], Qn[sq][i], tm);
+                    for (int i = 0; i < N; ++i) tm = fma(DG_LM(i), Qn[sq][i], tm);
                     tz_out[n * Ca + g.c] = tm;
                 }
                 if (last_layer) {
                     double tp = 0.0;
 #pragma unroll
-                    for (int i = 0; i < N; ++i) tp = fma(a.ops.lp[i], Qn[sq][i], tp);
+                    for (int i = 0; i < N; ++i) tp = fma(DG_LP(i), Qn[sq][i], tp);
                     tz_out[(NV + n) * Ca + g.c] = tp;
                 }
             }
@@ -566,8 +599,8 @@ __device__ __forceinline__ void z_pass(const DgStageArgs &a, const Geo &g, bool 
                 for (int i = 0; i < N; ++i) {
                     const double rinv = 1.0 / Qn[0][i];
                     const double u = Qn[LAM ? 2 : 0][i] * rinv, v = Qn[LAM ? 3 : 0][i] * rinv, w = Qn[LAM ? 1 : 0][i] * rinv;
-                    const double pres = a.gm1 * (Qn[LAM ? 4 : 0][i] - 0.5 * Qn[0][i] * (u * u + v * v + w * w));
-                    const double sp = sqrt(u * u + v * v + w * w) + sqrt(a.gamma * pres * rinv);
+                    const double pres = gm1 * (Qn[LAM ? 4 : 0][i] - 0.5 * Qn[0][i] * (u * u + v * v + w * w));
+                    const double sp = sqrt(u * u + v * v + w * w) + sqrt(gamma * pres * rinv);
                     if (!(sp <= lam_best)) lam_best = sp;   // NaN sticks
                 }
             }
@@ -637,20 +670,72 @@ __device__ __forceinline__ void copy_warp(const DgStageArgs &a, int lane, int bx
 }
 
 // ------------------------------------------------------------------------------------------------
+// one layer of the sweep, as a function of its own
+// ------------------------------------------------------------------------------------------------
+// NOT inlined on purpose: inside the layer loop of the kernel ptxas treats the ~(N^2 + 2N) operator-table loads
+// as loop invariants, hoists them out, overflows the uniform register file and brings them back through local
+// memory (measured: 50 spill slots per DOF, 29 % of the stall samples).  As a function with no loop of its own
+// the body compiles as it did when a block owned one brick.  Everything it needs comes from shared memory.
+template <class C>
+struct Smem {
+    static constexpr int QB0 = 0, QB1 = C::BUF, KR = 2 * C::BUF, TMS = 3 * C::BUF, FSS = TMS + C::LINEBUF,
+                         FMS = FSS + C::LINEBUF, INFO = FMS + DG_NV * C::L, BARS = INFO + (int)((sizeof(BlockInfo) + 15) / 16 * 2),
+                         DOUBLES = BARS + 4;
+    static constexpr int BYTES = DOUBLES * 8;
+};
+
+template <class C, int MODE, bool LAM>
+__device__ __noinline__ double layer_body(int it, double lam_best) {
+    extern __shared__ __align__(128) double smem[];
+    using SM = Smem<C>;
+    constexpr int L = C::L;
+    const BlockInfo *bi = reinterpret_cast<const BlockInfo *>(smem + SM::INFO);
+    uint64_t *fullq = reinterpret_cast<uint64_t *>(smem + SM::BARS), *fullk = fullq + 2;
+    double *Qs = smem + ((it & 1) ? SM::QB1 : SM::QB0);
+    const double *Qnext = smem + ((it & 1) ? SM::QB0 : SM::QB1);
+    double *KR = smem + SM::KR, *Tms = smem + SM::TMS, *Fss = smem + SM::FSS, *FmS = smem + SM::FMS;
+    const int l = threadIdx.x, lx = min(l, L - 1);
+    const bool inL = l < L;
+    const int ext0 = bi->ext0, ext1 = bi->ext1;
+    const long long toff = (long long)it * bi->tstride;
+    mbar_wait(&fullq[it & 1], (it >> 1) & 1);
+    {
+        const Geo gx = make_geo<C, 0>(lx);
+        xy_pass<C, 0, MODE>(bi, gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, bi->halo[0] + toff, bi->halo[1] + toff, Qs,
+                            KR, Tms, Fss, fullk, it & 1);
+    }
+    {
+        const Geo gy = make_geo<C, 1>(lx);
+        xy_pass<C, 1, MODE>(bi, gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, bi->halo[2] + toff, bi->halo[3] + toff, Qs,
+                            KR, Tms, Fss, fullk, it & 1);
+    }
+    const bool last_layer = it + 1 == bi->nl;
+    if (!last_layer) mbar_wait(&fullq[(it + 1) & 1], ((it + 1) >> 1) & 1);
+    {
+        const Geo gz = make_geo<C, 2>(lx);
+        z_pass<C, MODE, LAM>(bi, gz, lx, inL && line_inside<C, 2>(gz, ext0, ext1), Qs, Qnext, KR, FmS, it == 0, last_layer,
+                             lam_best);
+    }
+    if (MODE == DG_MODE_STAGE) {
+        bar_sync<C::NCOMP>(1);   // the updated Q of the whole layer is in shared memory
+        double *Tslot = bi->txy_out + toff;
+        const Geo gx = make_geo<C, 0>(lx), gy = make_geo<C, 1>(lx);
+        boundary_traces<C, 0>(gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, Qs, Tslot);
+        boundary_traces<C, 1>(gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, Qs, Tslot);
+    }
+    fence_proxy_async();
+    bar_arrive<C::THREADS>(2);   // hand the layer to the copy warp
+    return lam_best;
+}
+
+// ------------------------------------------------------------------------------------------------
 // the fused stage kernel: block (bx, by, chunk) marches through layers z0 .. z0 + nl - 1 of column (bx, by)
 // ------------------------------------------------------------------------------------------------
 template <class C, int MODE, bool LAM>
 __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __grid_constant__ DgStageArgs a) {
-    constexpr int L = C::L;
     extern __shared__ __align__(128) double smem[];
-    double *Qb0 = smem;                    // ring of two layers of Q (old, then updated in place)
-    double *Qb1 = Qb0 + C::BUF;
-    double *KR = Qb1 + C::BUF;             // Runge-Kutta register of the layer, accumulated in place
-    double *Tms = KR + C::BUF;             // [5][L] T- of every line (right state of the line below)
-    double *Fss = Tms + C::LINEBUF;        // [5][L] F* at the + end of every line
-    uint64_t *bars = reinterpret_cast<uint64_t *>(Fss + C::LINEBUF);
-    uint64_t *fullq = bars, *fullk = bars + 2;
-
+    using SM = Smem<C>;
+    uint64_t *fullq = reinterpret_cast<uint64_t *>(smem + SM::BARS), *fullk = fullq + 2;
     const int tid = threadIdx.x;
     const int bxi = blockIdx.x, byi = blockIdx.y, chunk = blockIdx.z;
     const int z0 = chunk * a.lz;
@@ -661,71 +746,40 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
         mbar_init(&fullq[1], 1);
         mbar_init(fullk, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        BlockInfo *bi = reinterpret_cast<BlockInfo *>(smem + SM::INFO);
+        const size_t cstride = (size_t)a.nbx * a.nby, col = (size_t)byi * a.nbx + bxi;
+        bi->halo[0] = halo_source<C, 0>(a.Txy_old, a.nbx, a.nby, bxi, byi, z0, 0);
+        bi->halo[1] = halo_source<C, 0>(a.Txy_old, a.nbx, a.nby, bxi, byi, z0, 1);
+        bi->halo[2] = halo_source<C, 1>(a.Txy_old, a.nbx, a.nby, bxi, byi, z0, 0);
+        bi->halo[3] = halo_source<C, 1>(a.Txy_old, a.nbx, a.nby, bxi, byi, z0, 1);
+        bi->txy_out = a.Txy_new + ((size_t)z0 * cstride + col) * C::TXY;
+        // z traces at the ends of the chunk: T+ of the chunk below (its side 1), T- of the chunk above (its side 0)
+        const int clo = (chunk == 0) ? a.nchunks - 1 : chunk - 1, chi = (chunk + 1 == a.nchunks) ? 0 : chunk + 1;
+        bi->tz_lo = a.Tz_old + ((size_t)clo * cstride + col) * C::TZ + DG_NV * C::CZ;
+        bi->tz_hi = a.Tz_old + ((size_t)chi * cstride + col) * C::TZ;
+        bi->tz_out = a.Tz_new + ((size_t)chunk * cstride + col) * C::TZ;
+        bi->tstride = (long long)cstride * C::TXY;
+        bi->gamma = a.gamma;
+        bi->gm1 = a.gm1;
+        bi->rkA = a.rkA;
+        bi->rkB = a.rkB;
+        bi->scale[0] = a.scale[0];
+        bi->scale[1] = a.scale[1];
+        bi->scale[2] = a.scale[2];
+        bi->ext0 = min(C::BX, a.nx - bxi * C::BX);   // elements of this column per axis (ragged last column)
+        bi->ext1 = min(C::BY, a.ny - byi * C::BY);
+        bi->readK = readK ? 1 : 0;
+        bi->nl = nl;
     }
     __syncthreads();
     if (tid >= C::NCOMP) {
-        copy_warp<C, MODE>(a, tid - C::NCOMP, bxi, byi, z0, nl, readK, Qb0, Qb1, KR, fullq, fullk);
+        copy_warp<C, MODE>(a, tid - C::NCOMP, bxi, byi, z0, nl, readK, smem + SM::QB0, smem + SM::QB1, smem + SM::KR, fullq,
+                           fullk);
         return;
     }
-
-    const int l = tid;
-    const int ext0 = min(C::BX, a.nx - bxi * C::BX);   // elements of this column per axis (ragged last column)
-    const int ext1 = min(C::BY, a.ny - byi * C::BY);
-    const bool inL = l < L;
-    const size_t cstride = (size_t)a.nbx * a.nby;
-    const size_t col = (size_t)byi * a.nbx + bxi;
-
-    double Fm[DG_NV] = {0.0, 0.0, 0.0, 0.0, 0.0};
     double lam_best = 0.0;
 #pragma unroll 1
-    for (int it = 0; it < nl; ++it) {
-        const int ez = z0 + it;
-        double *Qs = (it & 1) ? Qb1 : Qb0;
-        const double *Qnext = (it & 1) ? Qb0 : Qb1;
-        // The geometry of a thread's three lines is recomputed per layer from an opaque copy of the line index:
-        // kept across the loop it would cost ~20 registers in the sections that need every one of them.
-        int lx = min(l, L - 1);
-        asm volatile("" : "+r"(lx));
-        mbar_wait(&fullq[it & 1], (it >> 1) & 1);
-        {
-            const Geo gx = make_geo<C, 0>(lx);
-            const bool actx = inL && line_inside<C, 0>(gx, ext0, ext1);
-            xy_pass<C, 0, MODE>(a, gx, actx, ext0, halo_source<C, 0>(a.Txy_old, a.nbx, a.nby, bxi, byi, ez, 0),
-                                halo_source<C, 0>(a.Txy_old, a.nbx, a.nby, bxi, byi, ez, 1), Qs, KR, Tms, Fss, readK,
-                                fullk, it & 1);
-        }
-        asm volatile("" : "+r"(lx));
-        {
-            const Geo gy = make_geo<C, 1>(lx);
-            const bool acty = inL && line_inside<C, 1>(gy, ext0, ext1);
-            xy_pass<C, 1, MODE>(a, gy, acty, ext1, halo_source<C, 1>(a.Txy_old, a.nbx, a.nby, bxi, byi, ez, 0),
-                                halo_source<C, 1>(a.Txy_old, a.nbx, a.nby, bxi, byi, ez, 1), Qs, KR, Tms, Fss, readK,
-                                fullk, it & 1);
-        }
-        asm volatile("" : "+r"(lx));
-        const bool last_layer = it + 1 == nl;
-        if (!last_layer) mbar_wait(&fullq[(it + 1) & 1], ((it + 1) >> 1) & 1);
-        {
-            // z traces at the ends of the chunk: T+ of the chunk below (its side 1), T- of the chunk above (its side 0)
-            const int clo = (chunk == 0) ? a.nchunks - 1 : chunk - 1, chi = (chunk + 1 == a.nchunks) ? 0 : chunk + 1;
-            const double *tz_lo = a.Tz_old + ((size_t)clo * cstride + col) * C::TZ + DG_NV * C::CZ;
-            const double *tz_hi = a.Tz_old + ((size_t)chi * cstride + col) * C::TZ;
-            double *tz_out = a.Tz_new + ((size_t)chunk * cstride + col) * C::TZ;
-            const Geo gz = make_geo<C, 2>(lx);
-            const bool actz = inL && line_inside<C, 2>(gz, ext0, ext1);
-            z_pass<C, MODE, LAM>(a, gz, actz, Qs, Qnext, tz_lo, tz_hi, tz_out, KR, Fm, it == 0, last_layer, lam_best);
-        }
-        if (MODE == DG_MODE_STAGE) {
-            bar_sync<C::NCOMP>(1);   // the updated Q of the whole layer is in shared memory
-            asm volatile("" : "+r"(lx));
-            double *Tslot = a.Txy_new + ((size_t)ez * cstride + col) * C::TXY;
-            const Geo gx = make_geo<C, 0>(lx), gy = make_geo<C, 1>(lx);
-            boundary_traces<C, 0>(gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, Qs, Tslot, a.ops.lp, a.ops.lm);
-            boundary_traces<C, 1>(gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, Qs, Tslot, a.ops.lp, a.ops.lm);
-        }
-        fence_proxy_async();
-        bar_arrive<C::THREADS>(2);   // hand the layer to the copy warp
-    }
+    for (int it = 0; it < nl; ++it) lam_best = layer_body<C, MODE, LAM>(it, lam_best);
     if (LAM) {
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {
@@ -756,8 +810,8 @@ __global__ void __launch_bounds__(C::NCOMP) dg_traces_kernel(const __grid_consta
     const int ext0 = min(C::BX, a.nx - bxi * C::BX), ext1 = min(C::BY, a.ny - byi * C::BY);
     const bool inL = tid < C::L;
     double *Tslot = a.Txy + slot * C::TXY;
-    boundary_traces<C, 0>(gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, smem, Tslot, a.lp, a.lm);
-    boundary_traces<C, 1>(gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, smem, Tslot, a.lp, a.lm);
+    boundary_traces<C, 0>(gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, smem, Tslot);
+    boundary_traces<C, 1>(gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, smem, Tslot);
     const int chunk = ez / a.lz;
     const bool zfirst = ez == chunk * a.lz, zlast = (ez + 1 == a.nz) || (ez + 1 == (chunk + 1) * a.lz);
     if ((zfirst || zlast) && inL && line_inside<C, 2>(gz, ext0, ext1)) {
@@ -768,8 +822,8 @@ __global__ void __launch_bounds__(C::NCOMP) dg_traces_kernel(const __grid_consta
 #pragma unroll
             for (int q = 0; q < N; ++q) {
                 const double Qv = smem[n * C::PLANE + gz.base + q * C::PP];
-                tp = fma(a.lp[q], Qv, tp);
-                tm = fma(a.lm[q], Qv, tm);
+                tp = fma(DG_LP(q), Qv, tp);
+                tm = fma(DG_LM(q), Qv, tm);
             }
             if (zfirst) dst[n * C::CZ] = tm;
             if (zlast) dst[(NV + n) * C::CZ] = tp;
@@ -848,10 +902,10 @@ __global__ void __launch_bounds__(256) dg_wavespeed_kernel(const DgWaveArgs a) {
 // host-side launchers, one table per variant
 // ------------------------------------------------------------------------------------------------
 template <class C>
-cudaError_t prepare(int *blocks_per_sm) {
-    cudaError_t err = cudaSuccess;
+cudaError_t prepare(const DgRefOps &ref, int *blocks_per_sm) {
+    cudaError_t err = cudaMemcpyToSymbol(c_ref, &ref, sizeof(DgRefOps));
     auto opt_in = [&](auto kernel) {
-        if (err == cudaSuccess) err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+        if (err == cudaSuccess) err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Smem<C>::BYTES);
     };
     opt_in(dg_stage_kernel<C, DG_MODE_STAGE, false>);
     opt_in(dg_stage_kernel<C, DG_MODE_STAGE, true>);
@@ -860,15 +914,15 @@ cudaError_t prepare(int *blocks_per_sm) {
         err = cudaFuncSetAttribute(dg_traces_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::BUF * 8);
     if (err != cudaSuccess) return err;
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, dg_stage_kernel<C, DG_MODE_STAGE, false>,
-                                                         C::THREADS, C::SMEM_BYTES);
+                                                         C::THREADS, Smem<C>::BYTES);
 }
 
 template <class C>
 cudaError_t launch_stage(const DgStageArgs &a, cudaStream_t s) {
     const dim3 grid((unsigned)a.nbx, (unsigned)a.nby, (unsigned)a.nchunks);
-    if (a.mode == DG_MODE_RESIDUAL) dg_stage_kernel<C, DG_MODE_RESIDUAL, false><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(a);
-    else if (a.want_lam) dg_stage_kernel<C, DG_MODE_STAGE, true><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(a);
-    else dg_stage_kernel<C, DG_MODE_STAGE, false><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(a);
+    if (a.mode == DG_MODE_RESIDUAL) dg_stage_kernel<C, DG_MODE_RESIDUAL, false><<<grid, C::THREADS, Smem<C>::BYTES, s>>>(a);
+    else if (a.want_lam) dg_stage_kernel<C, DG_MODE_STAGE, true><<<grid, C::THREADS, Smem<C>::BYTES, s>>>(a);
+    else dg_stage_kernel<C, DG_MODE_STAGE, false><<<grid, C::THREADS, Smem<C>::BYTES, s>>>(a);
     return cudaGetLastError();
 }
 
@@ -901,41 +955,35 @@ cudaError_t launch_wavespeed(const DgWaveArgs &a, int sms, cudaStream_t s) {
 
 template <class C>
 constexpr DgKernelTable make_table() {
-    return DgKernelTable{C::N,       C::BX,          C::BY,         C::THREADS,      C::SMEM_BYTES,     C::SLOT,
+    return DgKernelTable{C::N,       C::BX,          C::BY,         C::THREADS,      Smem<C>::BYTES,     C::SLOT,
                          C::TXY,     C::TZ,          C::RELOAD ? 1 : 0, C::MINB, &prepare<C>, &launch_stage<C>,  &launch_traces<C>,
                          &launch_layout<C>, &launch_wavespeed<C>};
 }
 
 // Variants per N (default first): Cfg<N, BX, BY, min blocks per SM, RELOAD, PP, OX, OY>.
 // DESIGN.md "column shapes" and "shared-memory layout" explain the choices.
+#define DG_T(...) make_table<Cfg<__VA_ARGS__>>()
 #if DG_N == 2
-using V0 = Cfg<2, 8, 8, 3, 0>;
-using V1 = Cfg<2, 4, 4, 6, 0>;
+#define DG_VARIANTS DG_T(2, 8, 8, 3, 0, 0, 3, 0), DG_T(2, 4, 4, 6, 0, 72, 3, 0), DG_T(2, 8, 8, 2, 0, 0, 3, 0)
 #elif DG_N == 3
-using V0 = Cfg<3, 4, 4, 3, 0>;
-using V1 = Cfg<3, 2, 2, 6, 0>;
+#define DG_VARIANTS DG_T(3, 4, 4, 3, 0, 0, 4, 4), DG_T(3, 2, 2, 6, 0, 0, 4, 0), DG_T(3, 4, 4, 2, 0, 0, 4, 4)
 #elif DG_N == 4
-using V0 = Cfg<4, 4, 2, 3, 0>;
-using V1 = Cfg<4, 2, 2, 5, 0>;
+#define DG_VARIANTS DG_T(4, 4, 2, 3, 0, 130, 3, 0), DG_T(4, 2, 2, 5, 0, 66, 1, 0), DG_T(4, 4, 2, 2, 0, 130, 3, 0)
 #elif DG_N == 5
-using V0 = Cfg<5, 2, 2, 3, 0>;
-using V1 = Cfg<5, 2, 1, 5, 0>;
+#define DG_VARIANTS DG_T(5, 2, 2, 3, 0, 106, 4, 0), DG_T(5, 2, 2, 2, 0, 106, 4, 0), DG_T(5, 2, 2, 3, 1, 106, 4, 0), \
+                    DG_T(5, 2, 2, 2, 1, 106, 4, 0), DG_T(5, 2, 1, 5, 0, 0, 4, 0), DG_T(5, 2, 1, 4, 1, 0, 4, 0)
 #elif DG_N == 6
-using V0 = Cfg<6, 2, 1, 3, 0>;
-using V1 = Cfg<6, 2, 2, 2, 0>;
+#define DG_VARIANTS DG_T(6, 2, 1, 3, 0, 76, 4, 0), DG_T(6, 2, 2, 2, 0, 148, 4, 4), DG_T(6, 2, 1, 3, 1, 76, 4, 0)
 #elif DG_N == 7
-using V0 = Cfg<7, 1, 1, 4, 0>;
-using V1 = Cfg<7, 2, 1, 2, 0>;
+#define DG_VARIANTS DG_T(7, 1, 1, 4, 0, 0, 0, 1), DG_T(7, 2, 1, 2, 0, 0, 4, 0), DG_T(7, 1, 1, 4, 1, 0, 0, 1)
 #elif DG_N == 8
-using V0 = Cfg<8, 1, 1, 3, 0>;
-using V1 = Cfg<8, 1, 1, 3, 1>;
+#define DG_VARIANTS DG_T(8, 1, 1, 3, 0, 66, 1, 1), DG_T(8, 1, 1, 3, 1, 66, 1, 1), DG_T(8, 1, 1, 2, 0, 66, 1, 1)
 #else
 #error "DG_N must be 2..8"
 #endif
 
-using VE = Cfg<DG_N, 1, 1, 2, 1>;   // one element per layer: always there (tiny and ragged meshes, tests)
-
-const DgKernelTable k_tables[] = {make_table<V0>(), make_table<V1>(), make_table<VE>()};
+// last: one element per layer, always there (tiny and ragged meshes, tests)
+const DgKernelTable k_tables[] = {DG_VARIANTS, DG_T(DG_N, 1, 1, 2, 1)};
 
 }  // namespace
 
