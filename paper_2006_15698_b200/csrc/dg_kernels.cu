@@ -263,7 +263,9 @@ struct BlockInfo {
     double *txy_out;           // this column's Txy_new slot of layer z0
     const double *tz_lo, *tz_hi;
     double *tz_out;
+    const double *kslot;       // this column's K slot of layer z0 (L2 prefetch only)
     long long tstride;         // doubles between consecutive layers in Txy
+    long long kstride;         // ... in Q and K
     double gamma, gm1, rkA, rkB, scale[3];
     int ext0, ext1, readK, nl;
 };
@@ -649,12 +651,9 @@ __device__ __forceinline__ void copy_warp(const DgStageArgs &a, int lane, int bx
     else if (lane == 0) mbar_arrive(fullk);
     if (nl > 1) copy_in<C>(Qb1, a.Q + (slot0 + lstride) * C::SLOT, &fullq[1], lane);
     prefetch_halo(z0);
-    if (nl > 1) prefetch_halo(z0 + 1);
     for (int it = 0; it < nl; ++it) {
         double *Qcur = (it & 1) ? Qb1 : Qb0;
         const size_t slot = slot0 + (size_t)it * lstride;
-        if (lane == 4 && readK && it + 2 < nl) l2_prefetch(a.K + (slot + 2 * lstride) * C::SLOT, C::NPL * C::HP * 8);
-        if (it + 2 < nl) prefetch_halo(z0 + it + 2);
         bar_sync<C::THREADS>(2);                                     // the compute warps are done with layer `it`
         copy_out<C>(a.K + slot * C::SLOT, KR, lane);
         if (MODE == DG_MODE_STAGE) copy_out<C>(a.Q + slot * C::SLOT, Qcur, lane);
@@ -710,6 +709,13 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
                             KR, Tms, Fss, fullk, it & 1);
     }
     const bool last_layer = it + 1 == bi->nl;
+    // Ask L2 for what the NEXT layer reads with a short lead (about a third of a layer): its K slot, which the
+    // copy warp can only fetch once this layer's K has left shared memory, and the neighbour columns' traces.
+    // Asked for earlier, L2 has evicted them again by the time they are used (measured: +25 % DRAM reads).
+    if (!last_layer && l < 5) {
+        if (l < 4) l2_prefetch(bi->halo[l] + toff + bi->tstride, DG_NV * (l < 2 ? C::CX : C::CY) * 8);
+        else if (bi->readK) l2_prefetch(bi->kslot + (long long)(it + 1) * bi->kstride, C::NPL * C::HP * 8);
+    }
     if (!last_layer) mbar_wait(&fullq[(it + 1) & 1], ((it + 1) >> 1) & 1);
     {
         const Geo gz = make_geo<C, 2>(lx);
@@ -759,6 +765,8 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
         bi->tz_hi = a.Tz_old + ((size_t)chi * cstride + col) * C::TZ;
         bi->tz_out = a.Tz_new + ((size_t)chunk * cstride + col) * C::TZ;
         bi->tstride = (long long)cstride * C::TXY;
+        bi->kslot = a.K + ((size_t)z0 * cstride + col) * C::SLOT;
+        bi->kstride = (long long)cstride * C::SLOT;
         bi->gamma = a.gamma;
         bi->gm1 = a.gm1;
         bi->rkA = a.rkA;
