@@ -263,7 +263,7 @@ struct BlockInfo {
     double *txy_out;           // this column's Txy_new slot of layer z0
     const double *tz_lo, *tz_hi;
     double *tz_out;
-    const double *kslot;       // this column's K slot of layer z0 (L2 prefetch only)
+    double *kslot;             // this column's K slot of layer z0
     long long tstride;         // doubles between consecutive layers in Txy
     long long kstride;         // ... in Q and K
     double gamma, gm1, rkA, rkB, scale[3];
@@ -432,7 +432,7 @@ __device__ __forceinline__ void xy_pass(const BlockInfo *bi, const Geo &g, bool 
     }
     // ------------- PD: Runge-Kutta accumulation on the staged K -----------------------------------------
     if (AX == 0) {
-        mbar_wait(fullk, kparity);     // the copy warp has read the previous K out and this layer's K has landed
+        if (bi->readK) mbar_wait(fullk, kparity);   // this layer's K has landed in KR
     } else if (!A::MULTI) {
         bar_sync<C::NCOMP>(1);         // the x pass of every line is done (with MULTI the two barriers above said so)
     }
@@ -473,7 +473,8 @@ __device__ __forceinline__ void xy_pass(const BlockInfo *bi, const Geo &g, bool 
 // ------------------------------------------------------------------------------------------------
 template <class C, int MODE, bool LAM>
 __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l, bool act, double *Qs, const double *Qnext,
-                                       double *KR, double *FmS, bool first_layer, bool last_layer, double &lam_best) {
+                                       const double *KR, double *FmS, double *Kg, bool first_layer, bool last_layer,
+                                       double &lam_best) {
     constexpr int AX = 2;
     using A = Axis<C, AX>;
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE, S = A::S, Ca = A::Ca, L = C::L;
@@ -552,8 +553,10 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
     }
     bar_sync<C::NCOMP>(1);   // the y pass of every line is done with K (and, RELOAD, with Q)
     if (act) {
-        // PD
-        double *K0 = KR + g.base;
+        // PD: the updated K (or R) goes straight to HBM from the z lines (coalesced across the lanes, streaming),
+        // so that KR is free for the next layer's K as soon as every line has read it
+        const double *K0 = KR + g.base;
+        double *Kline = Kg + g.base;
         double *Q0w = Qs + g.base;
         const double sc = bi->scale[AX];
         if (MODE == DG_MODE_RESIDUAL) {
@@ -561,8 +564,8 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
             for (int s = 0; s < NV; ++s)
 #pragma unroll
                 for (int i = 0; i < N; ++i) {
-                    double *p = K0 + var_of_slot<C, AX>(s) * PLANE + i * S;
-                    *p = fma(sc, V[s][i], *p);
+                    const int n = var_of_slot<C, AX>(s);
+                    __stcs(Kline + (n * N + i) * C::HP, fma(sc, V[s][i], K0[n * PLANE + i * S]));
                 }
         } else {
             const double rkB = bi->rkB;
@@ -577,7 +580,7 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
                     const double Kn = fma(sc, V[s][i], K0[n * PLANE + i * S]);
                     const double Qold = C::RELOAD ? Q0w[n * PLANE + i * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : i];
                     Qn[sq][i] = fma(rkB, Kn, Qold);
-                    K0[n * PLANE + i * S] = Kn;
+                    __stcs(Kline + (n * N + i) * C::HP, Kn);
                     Q0w[n * PLANE + i * S] = Qn[sq][i];
                 }
                 // PE for the z faces: traces of the updated Q, only at the two ends of the chunk
@@ -641,28 +644,21 @@ __device__ __forceinline__ void copy_warp(const DgStageArgs &a, int lane, int bx
                                           double *Qb0, double *Qb1, double *KR, uint64_t *fullq, uint64_t *fullk) {
     const size_t lstride = (size_t)a.nbx * a.nby;                    // slots per layer
     const size_t slot0 = (size_t)z0 * lstride + (size_t)byi * a.nbx + bxi;
-    // L2 prefetch of the neighbour columns' traces of a layer (4 blocks of 5 Ca doubles)
-    auto prefetch_halo = [&](int ez) {
-        if (lane < 2) l2_prefetch(halo_source<C, 0>(a.Txy_old, a.nbx, a.nby, bxi, byi, ez, lane), DG_NV * C::CX * 8);
-        else if (lane < 4) l2_prefetch(halo_source<C, 1>(a.Txy_old, a.nbx, a.nby, bxi, byi, ez, lane - 2), DG_NV * C::CY * 8);
-    };
     copy_in<C>(Qb0, a.Q + slot0 * C::SLOT, &fullq[0], lane);
-    if (readK) copy_in<C>(KR, a.K + slot0 * C::SLOT, fullk, lane);
-    else if (lane == 0) mbar_arrive(fullk);
+    if (readK) copy_in<C>(KR, a.K + slot0 * C::SLOT, fullk, lane);   // later layers: issued by the compute warps
     if (nl > 1) copy_in<C>(Qb1, a.Q + (slot0 + lstride) * C::SLOT, &fullq[1], lane);
-    prefetch_halo(z0);
+    // L2 prefetch of the neighbour columns' traces of the first layer (4 blocks of 5 Ca doubles)
+    if (lane < 2) l2_prefetch(halo_source<C, 0>(a.Txy_old, a.nbx, a.nby, bxi, byi, z0, lane), DG_NV * C::CX * 8);
+    else if (lane < 4) l2_prefetch(halo_source<C, 1>(a.Txy_old, a.nbx, a.nby, bxi, byi, z0, lane - 2), DG_NV * C::CY * 8);
     for (int it = 0; it < nl; ++it) {
         double *Qcur = (it & 1) ? Qb1 : Qb0;
         const size_t slot = slot0 + (size_t)it * lstride;
         bar_sync<C::THREADS>(2);                                     // the compute warps are done with layer `it`
-        copy_out<C>(a.K + slot * C::SLOT, KR, lane);
-        if (MODE == DG_MODE_STAGE) copy_out<C>(a.Q + slot * C::SLOT, Qcur, lane);
-        bulk_commit();
-        bulk_wait_read();                                            // shared memory has been read out
-        __syncwarp();
-        if (it + 1 < nl) {
-            if (readK) copy_in<C>(KR, a.K + (slot + lstride) * C::SLOT, fullk, lane);
-            else if (lane == 0) mbar_arrive(fullk);
+        if (MODE == DG_MODE_STAGE) {
+            copy_out<C>(a.Q + slot * C::SLOT, Qcur, lane);
+            bulk_commit();
+            bulk_wait_read();                                        // shared memory has been read out
+            __syncwarp();
         }
         if (it + 2 < nl) copy_in<C>(Qcur, a.Q + (slot + 2 * lstride) * C::SLOT, &fullq[it & 1], lane);
     }
@@ -719,11 +715,13 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
     if (!last_layer) mbar_wait(&fullq[(it + 1) & 1], ((it + 1) >> 1) & 1);
     {
         const Geo gz = make_geo<C, 2>(lx);
-        z_pass<C, MODE, LAM>(bi, gz, lx, inL && line_inside<C, 2>(gz, ext0, ext1), Qs, Qnext, KR, FmS, it == 0, last_layer,
-                             lam_best);
+        z_pass<C, MODE, LAM>(bi, gz, lx, inL && line_inside<C, 2>(gz, ext0, ext1), Qs, Qnext, KR, FmS,
+                             bi->kslot + (long long)it * bi->kstride, it == 0, last_layer, lam_best);
     }
+    bar_sync<C::NCOMP>(1);   // the updated Q of the whole layer is in shared memory; every line has read KR
     if (MODE == DG_MODE_STAGE) {
-        bar_sync<C::NCOMP>(1);   // the updated Q of the whole layer is in shared memory
+        // the next layer's K can come in now (needed at the end of its x pass)
+        if (l < 32 && bi->readK && !last_layer) copy_in<C>(KR, bi->kslot + (long long)(it + 1) * bi->kstride, fullk, l);
         double *Tslot = bi->txy_out + toff;
         const Geo gx = make_geo<C, 0>(lx), gy = make_geo<C, 1>(lx);
         boundary_traces<C, 0>(gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, Qs, Tslot);
