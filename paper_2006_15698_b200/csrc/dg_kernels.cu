@@ -55,11 +55,13 @@ struct Cfg {
     static constexpr bool RELOAD = RELOAD_ != 0;
     static constexpr int GX = BX * N, GY = BY * N;                 // nodes of a layer per axis (z: N)
     static constexpr int NODES = GX * GY * N;
-    static constexpr int HP = (GX * GY + 1) & ~1;                  // HBM pitch of one (gy,gx) plane, doubles (even)
+    // pitch of one (gy,gx) plane, doubles, in HBM AND in shared memory (a layer is ONE bulk copy): even, and
+    // padded by PP_ - GX GY where that removes shared-memory bank conflicts at a few per cent more traffic
+    static constexpr int HP = PP_ ? PP_ : ((GX * GY + 1) & ~1);
     static constexpr int NPL = DG_NV * N;                          // planes per slot
     static constexpr int SLOT = (NPL * HP + 15) & ~15;             // doubles per layer slot in Q, K (128-byte multiple)
     static constexpr int P = GX;                                   // shared-memory row pitch (dense)
-    static constexpr int PP = PP_ ? PP_ : HP;                      // shared-memory plane pitch
+    static constexpr int PP = HP;                                  // shared-memory plane pitch
     static constexpr int PLANE = N * PP;                           // shared doubles per variable
     static constexpr int BUF = DG_NV * PLANE;                      // shared doubles per layer buffer
     static constexpr int OX = OX_, OY = OY_;
@@ -616,27 +618,17 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
 // ------------------------------------------------------------------------------------------------
 // the copy warp: every byte of Q and K between HBM and shared memory moves here, by the TMA engine
 // ------------------------------------------------------------------------------------------------
+// A layer slot is one contiguous block on both sides: one bulk copy each way, issued by one lane.
 template <class C>
 __device__ __forceinline__ void copy_in(double *sdst, const double *gsrc, uint64_t *bar, int lane) {
     constexpr unsigned BYTES = C::NPL * C::HP * 8;
-    if (C::PP == C::HP) {
-        if (lane == 0) {
-            mbar_expect_tx(bar, BYTES);
-            bulk_load(sdst, gsrc, BYTES, bar);
-        }
-    } else {
-        if (lane == 0) mbar_expect_tx(bar, BYTES);
-        __syncwarp();
-        for (int pl = lane; pl < C::NPL; pl += 32) bulk_load(sdst + pl * C::PP, gsrc + pl * C::HP, C::HP * 8, bar);
-    }
+    if (lane != 0) return;
+    mbar_expect_tx(bar, BYTES);
+    bulk_load(sdst, gsrc, BYTES, bar);
 }
 template <class C>
 __device__ __forceinline__ void copy_out(double *gdst, const double *ssrc, int lane) {
-    if (C::PP == C::HP) {
-        if (lane == 0) bulk_store(gdst, ssrc, C::NPL * C::HP * 8);
-    } else {
-        for (int pl = lane; pl < C::NPL; pl += 32) bulk_store(gdst + pl * C::HP, ssrc + pl * C::PP, C::HP * 8);
-    }
+    if (lane == 0) bulk_store(gdst, ssrc, C::NPL * C::HP * 8);
 }
 
 template <class C, int MODE>
@@ -970,20 +962,19 @@ constexpr DgKernelTable make_table() {
 // DESIGN.md "column shapes" and "shared-memory layout" explain the choices.
 #define DG_T(...) make_table<Cfg<__VA_ARGS__>>()
 #if DG_N == 2
-#define DG_VARIANTS DG_T(2, 8, 8, 3, 0, 0, 3, 0), DG_T(2, 4, 4, 6, 0, 72, 3, 0), DG_T(2, 8, 8, 2, 0, 0, 3, 0)
+#define DG_VARIANTS DG_T(2, 8, 8, 3, 0, 0, 3, 0), DG_T(2, 4, 4, 6, 0, 0, 3, 0), DG_T(2, 8, 8, 3, 1, 0, 3, 0), DG_T(2, 8, 4, 4, 1, 0, 3, 0)
 #elif DG_N == 3
-#define DG_VARIANTS DG_T(3, 4, 4, 3, 0, 0, 4, 4), DG_T(3, 2, 2, 6, 0, 0, 4, 0), DG_T(3, 4, 4, 2, 0, 0, 4, 4)
+#define DG_VARIANTS DG_T(3, 4, 4, 3, 0, 0, 4, 4), DG_T(3, 2, 2, 6, 0, 0, 4, 0), DG_T(3, 4, 4, 3, 1, 0, 4, 4), DG_T(3, 4, 2, 4, 1, 0, 4, 4)
 #elif DG_N == 4
-#define DG_VARIANTS DG_T(4, 4, 2, 3, 0, 130, 3, 0), DG_T(4, 2, 2, 5, 0, 66, 1, 0), DG_T(4, 4, 2, 2, 0, 130, 3, 0)
+#define DG_VARIANTS DG_T(4, 4, 2, 3, 1, 130, 3, 0), DG_T(4, 2, 2, 5, 1, 66, 1, 0), DG_T(4, 4, 2, 3, 0, 130, 3, 0), DG_T(4, 2, 2, 5, 0, 66, 1, 0)
 #elif DG_N == 5
-#define DG_VARIANTS DG_T(5, 2, 2, 3, 0, 106, 4, 0), DG_T(5, 2, 2, 2, 0, 106, 4, 0), DG_T(5, 2, 2, 3, 1, 106, 4, 0), \
-                    DG_T(5, 2, 2, 2, 1, 106, 4, 0), DG_T(5, 2, 1, 5, 0, 0, 4, 0), DG_T(5, 2, 1, 4, 1, 0, 4, 0)
+#define DG_VARIANTS DG_T(5, 2, 2, 3, 1, 0, 4, 5), DG_T(5, 2, 2, 3, 0, 0, 4, 5), DG_T(5, 2, 1, 6, 1, 0, 4, 0), DG_T(5, 2, 1, 4, 1, 0, 4, 0)
 #elif DG_N == 6
-#define DG_VARIANTS DG_T(6, 2, 1, 3, 0, 76, 4, 0), DG_T(6, 2, 2, 2, 0, 148, 4, 4), DG_T(6, 2, 1, 3, 1, 76, 4, 0)
+#define DG_VARIANTS DG_T(6, 2, 1, 3, 1, 0, 4, 0), DG_T(6, 2, 2, 2, 1, 148, 4, 4), DG_T(6, 2, 1, 3, 0, 0, 4, 0), DG_T(6, 1, 1, 6, 1, 0, 0, 0)
 #elif DG_N == 7
-#define DG_VARIANTS DG_T(7, 1, 1, 4, 0, 0, 0, 1), DG_T(7, 2, 1, 2, 0, 0, 4, 0), DG_T(7, 1, 1, 4, 1, 0, 0, 1)
+#define DG_VARIANTS DG_T(7, 1, 1, 4, 1, 0, 0, 1), DG_T(7, 2, 1, 2, 1, 0, 4, 0), DG_T(7, 1, 1, 4, 0, 0, 0, 1), DG_T(7, 1, 1, 5, 1, 0, 0, 1)
 #elif DG_N == 8
-#define DG_VARIANTS DG_T(8, 1, 1, 3, 0, 66, 1, 1), DG_T(8, 1, 1, 3, 1, 66, 1, 1), DG_T(8, 1, 1, 2, 0, 66, 1, 1)
+#define DG_VARIANTS DG_T(8, 1, 1, 3, 1, 66, 1, 1), DG_T(8, 1, 1, 3, 0, 66, 1, 1), DG_T(8, 1, 1, 2, 0, 66, 1, 1), DG_T(8, 2, 1, 1, 0, 130, 1, 0)
 #else
 #error "DG_N must be 2..8"
 #endif
