@@ -962,19 +962,23 @@ constexpr DgKernelTable make_table() {
 // DESIGN.md "column shapes" and "shared-memory layout" explain the choices.
 #define DG_T(...) make_table<Cfg<__VA_ARGS__>>()
 #if DG_N == 2
-#define DG_VARIANTS DG_T(2, 8, 8, 3, 0, 0, 3, 0), DG_T(2, 4, 4, 6, 0, 0, 3, 0), DG_T(2, 8, 8, 3, 1, 0, 3, 0), DG_T(2, 8, 4, 4, 1, 0, 3, 0)
+#define DG_VARIANTS DG_T(2, 9, 8, 2, 1, 290, 0, 0), DG_T(2, 8, 4, 3, 0, 0, 3, 0), DG_T(2, 4, 4, 6, 0, 0, 3, 0), DG_T(2, 8, 8, 2, 0, 0, 3, 0), \
+                    DG_T(2, 9, 8, 2, 0, 290, 0, 0), DG_T(2, 9, 9, 2, 1, 0, 0, 0)
 #elif DG_N == 3
-#define DG_VARIANTS DG_T(3, 4, 4, 3, 0, 0, 4, 4), DG_T(3, 2, 2, 6, 0, 0, 4, 0), DG_T(3, 4, 4, 3, 1, 0, 4, 4), DG_T(3, 4, 2, 4, 1, 0, 4, 4)
+#define DG_VARIANTS DG_T(3, 4, 4, 2, 0, 0, 4, 4), DG_T(3, 6, 3, 2, 0, 0, 4, 0), DG_T(3, 4, 4, 3, 1, 0, 4, 4), DG_T(3, 4, 2, 4, 1, 0, 4, 0), \
+                    DG_T(3, 6, 6, 1, 0, 0, 4, 0), DG_T(3, 6, 4, 2, 0, 0, 4, 0)
 #elif DG_N == 4
-#define DG_VARIANTS DG_T(4, 4, 2, 3, 1, 130, 3, 0), DG_T(4, 2, 2, 5, 1, 66, 1, 0), DG_T(4, 4, 2, 3, 0, 130, 3, 0), DG_T(4, 2, 2, 5, 0, 66, 1, 0)
+#define DG_VARIANTS DG_T(4, 2, 2, 4, 0, 66, 1, 0), DG_T(4, 2, 2, 5, 1, 66, 1, 0), DG_T(4, 4, 2, 2, 0, 130, 3, 0), DG_T(4, 4, 2, 3, 1, 130, 3, 0), \
+                    DG_T(4, 2, 2, 3, 0, 66, 1, 0)
 #elif DG_N == 5
-#define DG_VARIANTS DG_T(5, 2, 2, 3, 1, 0, 4, 5), DG_T(5, 2, 2, 3, 0, 0, 4, 5), DG_T(5, 2, 1, 6, 1, 0, 4, 0), DG_T(5, 2, 1, 4, 1, 0, 4, 0)
+#define DG_VARIANTS DG_T(5, 2, 3, 2, 0, 154, 4, 0), DG_T(5, 3, 2, 2, 0, 0, 4, 0), DG_T(5, 2, 2, 3, 1, 106, 4, 0), DG_T(5, 2, 2, 3, 1, 0, 4, 5)
 #elif DG_N == 6
-#define DG_VARIANTS DG_T(6, 2, 1, 3, 1, 0, 4, 0), DG_T(6, 2, 2, 2, 1, 148, 4, 4), DG_T(6, 2, 1, 3, 0, 0, 4, 0), DG_T(6, 1, 1, 6, 1, 0, 0, 0)
+#define DG_VARIANTS DG_T(6, 2, 1, 3, 0, 0, 4, 0), DG_T(6, 2, 1, 3, 1, 0, 4, 0), DG_T(6, 3, 1, 2, 0, 114, 2, 0), DG_T(6, 1, 3, 2, 0, 118, 0, 0), \
+                    DG_T(6, 1, 1, 5, 1, 0, 0, 0), DG_T(6, 1, 1, 4, 0, 0, 0, 0)
 #elif DG_N == 7
-#define DG_VARIANTS DG_T(7, 1, 1, 4, 1, 0, 0, 1), DG_T(7, 2, 1, 2, 1, 0, 4, 0), DG_T(7, 1, 1, 4, 0, 0, 0, 1), DG_T(7, 1, 1, 5, 1, 0, 0, 1)
+#define DG_VARIANTS DG_T(7, 2, 1, 2, 1, 0, 4, 0), DG_T(7, 1, 1, 4, 1, 0, 0, 1), DG_T(7, 1, 1, 4, 0, 0, 0, 1), DG_T(7, 1, 1, 3, 0, 0, 0, 1)
 #elif DG_N == 8
-#define DG_VARIANTS DG_T(8, 1, 1, 3, 1, 66, 1, 1), DG_T(8, 1, 1, 3, 0, 66, 1, 1), DG_T(8, 1, 1, 2, 0, 66, 1, 1), DG_T(8, 2, 1, 1, 0, 130, 1, 0)
+#define DG_VARIANTS DG_T(8, 1, 1, 3, 1, 66, 1, 1), DG_T(8, 1, 1, 3, 0, 66, 1, 1), DG_T(8, 2, 1, 1, 0, 130, 1, 0), DG_T(8, 1, 2, 1, 0, 130, 1, 1)
 #else
 #error "DG_N must be 2..8"
 #endif
