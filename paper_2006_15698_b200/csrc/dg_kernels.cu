@@ -72,7 +72,7 @@ struct Cfg {
     static constexpr int TXY = 2 * DG_NV * (CX + CY);              // x/y trace doubles per layer slot
     static constexpr int TZ = 2 * DG_NV * CZ;                      // z trace doubles per chunk slot
     static constexpr bool MULTI = (BX > 1) || (BY > 1);
-    static constexpr int LINEBUF = MULTI ? DG_NV * L : 0;          // T- / F* hand-over between elements of a layer
+    static constexpr int LINEBUF = MULTI ? ((DG_NV * L + 1) & ~1) : 0;   // T- / F* hand-over between elements of a layer
     static_assert(PP >= HP && (PP % 2) == 0, "plane pitch must be even and hold a plane");
     static_assert((BUF % 2) == 0 && (LINEBUF % 2) == 0, "buffers must stay 16-byte aligned");
 };
@@ -666,7 +666,7 @@ __device__ __forceinline__ void copy_warp(const DgStageArgs &a, int lane, int bx
 template <class C>
 struct Smem {
     static constexpr int QB0 = 0, QB1 = C::BUF, KR = 2 * C::BUF, TMS = 3 * C::BUF, FSS = TMS + C::LINEBUF,
-                         FMS = FSS + C::LINEBUF, INFO = FMS + DG_NV * C::L, BARS = INFO + (int)((sizeof(BlockInfo) + 15) / 16 * 2),
+                         FMS = FSS + C::LINEBUF, INFO = FMS + ((DG_NV * C::L + 1) & ~1), BARS = INFO + (int)((sizeof(BlockInfo) + 15) / 16 * 2),
                          DOUBLES = BARS + 4;
     static constexpr int BYTES = DOUBLES * 8;
 };
@@ -963,15 +963,16 @@ constexpr DgKernelTable make_table() {
 #define DG_T(...) make_table<Cfg<__VA_ARGS__>>()
 #if DG_N == 2
 #define DG_VARIANTS DG_T(2, 9, 8, 2, 1, 290, 0, 0), DG_T(2, 8, 4, 3, 0, 0, 3, 0), DG_T(2, 4, 4, 6, 0, 0, 3, 0), DG_T(2, 8, 8, 2, 0, 0, 3, 0), \
-                    DG_T(2, 9, 8, 2, 0, 290, 0, 0), DG_T(2, 9, 9, 2, 1, 0, 0, 0)
+                    DG_T(2, 9, 7, 2, 1, 258, 3, 0), DG_T(2, 9, 7, 3, 1, 258, 3, 0)
 #elif DG_N == 3
 #define DG_VARIANTS DG_T(3, 4, 4, 2, 0, 0, 4, 4), DG_T(3, 6, 3, 2, 0, 0, 4, 0), DG_T(3, 4, 4, 3, 1, 0, 4, 4), DG_T(3, 4, 2, 4, 1, 0, 4, 0), \
-                    DG_T(3, 6, 6, 1, 0, 0, 4, 0), DG_T(3, 6, 4, 2, 0, 0, 4, 0)
+                    DG_T(3, 6, 4, 2, 0, 0, 4, 0), DG_T(3, 2, 7, 3, 1, 134, 4, 0), DG_T(3, 2, 7, 3, 0, 134, 4, 0)
 #elif DG_N == 4
 #define DG_VARIANTS DG_T(4, 2, 2, 4, 0, 66, 1, 0), DG_T(4, 2, 2, 5, 1, 66, 1, 0), DG_T(4, 4, 2, 2, 0, 130, 3, 0), DG_T(4, 4, 2, 3, 1, 130, 3, 0), \
                     DG_T(4, 2, 2, 3, 0, 66, 1, 0)
 #elif DG_N == 5
-#define DG_VARIANTS DG_T(5, 2, 3, 2, 0, 154, 4, 0), DG_T(5, 3, 2, 2, 0, 0, 4, 0), DG_T(5, 2, 2, 3, 1, 106, 4, 0), DG_T(5, 2, 2, 3, 1, 0, 4, 5)
+#define DG_VARIANTS DG_T(5, 2, 3, 2, 0, 154, 4, 0), DG_T(5, 3, 2, 2, 0, 0, 4, 0), DG_T(5, 2, 2, 3, 1, 106, 4, 0), DG_T(5, 5, 1, 2, 0, 0, 4, 0), \
+                    DG_T(5, 5, 1, 2, 1, 0, 4, 0), DG_T(5, 1, 5, 2, 0, 138, 0, 1)
 #elif DG_N == 6
 #define DG_VARIANTS DG_T(6, 2, 1, 3, 0, 0, 4, 0), DG_T(6, 2, 1, 3, 1, 0, 4, 0), DG_T(6, 3, 1, 2, 0, 114, 2, 0), DG_T(6, 1, 3, 2, 0, 118, 0, 0), \
                     DG_T(6, 1, 1, 5, 1, 0, 0, 0), DG_T(6, 1, 1, 4, 0, 0, 0, 0)
