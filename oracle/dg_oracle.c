@@ -515,7 +515,7 @@ int oracle_max_wavespeed(int nx, int ny, int nz, int p, double gamma, const doub
         const real u = Q1 * oneOrho, v = Q2 * oneOrho, w = Q3 * oneOrho;
         const real pr = d.gm1 * (Q4 - (real)0.5 * Q0 * (u * u + v * v + w * w));
         const real s = R_SQRT(u * u + v * v + w * w) + R_SQRT(d.gamma * pr * oneOrho);
-        if (s > best) best = s;
+        if (s > best || s != s) best = s;   /* NaN sticks: no limiter, non-physical states propagate (R15) */
     }
     *lam = (double)best;
     return 0;

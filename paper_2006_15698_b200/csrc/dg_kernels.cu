@@ -608,7 +608,7 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
                     const double u = Qn[LAM ? 2 : 0][i] * rinv, v = Qn[LAM ? 3 : 0][i] * rinv, w = Qn[LAM ? 1 : 0][i] * rinv;
                     const double pres = gm1 * (Qn[LAM ? 4 : 0][i] - 0.5 * Qn[0][i] * (u * u + v * v + w * w));
                     const double sp = sqrt(u * u + v * v + w * w) + sqrt(gamma * pres * rinv);
-                    if (!(sp <= lam_best)) lam_best = sp;   // NaN sticks
+                    if (sp > lam_best || sp != sp) lam_best = sp;   // NaN sticks
                 }
             }
         }
@@ -782,7 +782,7 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {
             const double o = __shfl_xor_sync(0xffffffffu, lam_best, off);
-            if (!(o <= lam_best)) lam_best = o;
+            if (o > lam_best || o != o) lam_best = o;
         }
         if ((tid & 31) == 0) atomicMax(a.lam_bits, (unsigned long long)__double_as_longlong(lam_best));
     }
@@ -886,12 +886,12 @@ __global__ void __launch_bounds__(256) dg_wavespeed_kernel(const DgWaveArgs a) {
         const double u = Q1 * rinv, v = Q2 * rinv, w = Q3 * rinv;
         const double pres = a.gm1 * (Q4 - 0.5 * Q0 * (u * u + v * v + w * w));
         const double s = sqrt(u * u + v * v + w * w) + sqrt(a.gamma * pres * rinv);
-        if (!(s <= best)) best = s;   // NaN sticks
+        if (s > best || s != s) best = s;   // NaN sticks
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
         const double o = __shfl_xor_sync(0xffffffffu, best, off);
-        if (!(o <= best)) best = o;
+        if (o > best || o != o) best = o;
     }
     if ((threadIdx.x & 31) == 0) atomicMax(a.lam_bits, (unsigned long long)__double_as_longlong(best));
 }

@@ -141,6 +141,31 @@ def test_max_wavespeed_matches_definition():
     assert abs(ORC.max_wavespeed(q, 3, G) - ref) < 1e-14 * ref
 
 
+def test_max_wavespeed_closed_forms_uniform_spike_and_nan():
+    """Pins oracle_max_wavespeed by numbers written out by hand (the rule itself is DESIGN.md reading R10: the
+    paper has no CFL rule).  Uniform state rho = 1.25, u = (0.3, -0.4, 1.2), p = 1.75, gamma = 7/5:
+    |u| = sqrt(0.09 + 0.16 + 1.44) = 1.3 and c = sqrt(1.4 * 1.75 / 1.25) = sqrt(1.96) = 1.4, so lam = 2.7.
+    One spiked node rho = 1, u = (0.6, 0.8, 0), p = 3.15: |u| = 1, c = sqrt(1.4 * 3.15) = sqrt(4.41) = 2.1,
+    lam = 3.1, wherever the node sits (pins the max-reduction, first / middle / last node)."""
+    nx, ny, nz, p = 3, 2, 2, 2
+    q = I.uniform_state(nx, ny, nz, p, rho=1.25, vel=(0.3, -0.4, 1.2), pres=1.75, gamma=1.4)
+    assert abs(ORC.max_wavespeed(q, p, 1.4) - 2.7) < 4e-15
+    spike = I.uniform_state(1, 1, 1, 0, rho=1.0, vel=(0.6, 0.8, 0.0), pres=3.15, gamma=1.4).reshape(5)
+    flat = q.reshape(-1, 5)
+    for node in (0, flat.shape[0] // 2 + 3, flat.shape[0] - 1):
+        qs = q.copy()
+        qs.reshape(-1, 5)[node] = spike
+        assert abs(ORC.max_wavespeed(qs, p, 1.4) - 3.1) < 4e-15, node
+    # a velocity spike below the maximum must not win, a transposed momentum component must not matter
+    qs = q.copy()
+    qs.reshape(-1, 5)[7] = I.uniform_state(1, 1, 1, 0, rho=1.25, vel=(1.2, 0.3, -0.4), pres=1.75, gamma=1.4).reshape(5)
+    assert abs(ORC.max_wavespeed(qs, p, 1.4) - 2.7) < 4e-15
+    # negative pressure: the square root is NaN and it propagates (no limiter, reading R15)
+    qs = q.copy()
+    qs.reshape(-1, 5)[11, 4] = 0.1
+    assert np.isnan(ORC.max_wavespeed(qs, p, 1.4))
+
+
 def test_invalid_arguments_are_rejected():
     q = I.make_field("cfg1")
     with pytest.raises(ValueError):
