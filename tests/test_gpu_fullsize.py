@@ -43,7 +43,8 @@ def take_box(t, lo, size):
     return t.index_select(0, iz).index_select(1, iy).index_select(2, ix).cpu().numpy()
 
 
-def sampled_parity(cfg, boxes_res, boxes_rk, tol_res=1e-11, tol_rk=1e-11, cfl=0.1):
+def sampled_parity(cfg, boxes_res, boxes_rk, tol_res=1e-11, tol_rk=1e-11, cfl=0.1, allowed_res=(), allowed_rk=(),
+                   always_arbiter=False, reports=None):
     c = I.CONFIGS[cfg]
     p, ext, n = c["p"], c["extent"], (c["nx"], c["ny"], c["nz"])
     q = I.make_field(cfg, xp=torch, device="cuda")
@@ -63,7 +64,9 @@ def sampled_parity(cfg, boxes_res, boxes_rk, tol_res=1e-11, tol_rk=1e-11, cfl=0.
         r_gpu = take_box(r, lo, size)
         inner = (slice(1, -1),) * 3
         rep = assert_parity(r_gpu[inner], r_orc[inner], lambda: ARB.residual(qb, p, G, sub_ext)[inner], tol_res,
-                            (cfg, "residual", lo))
+                            (cfg, "residual", lo), allowed=allowed_res, always_arbiter=always_arbiter)
+        if reports is not None:
+            reports.append((cfg, "residual", lo, size, rep))
         worst["residual"] = max(worst.get("residual", 0.0), rep["strict_rel_max"])
         worst.setdefault("residual_arbiter_vars", set()).update(rep["arbiter_vars"])
     del r
@@ -76,7 +79,9 @@ def sampled_parity(cfg, boxes_res, boxes_rk, tol_res=1e-11, tol_rk=1e-11, cfl=0.
         q_gpu = take_box(q, lo, size)
         inner = (slice(5, -5),) * 3
         rep = assert_parity(q_gpu[inner], q_orc[inner], lambda: ARB.rk_step(qb, p, G, sub_ext, dt, 1)[inner], tol_rk,
-                            (cfg, "rk step", lo))
+                            (cfg, "rk step", lo), allowed=allowed_rk, always_arbiter=always_arbiter)
+        if reports is not None:
+            reports.append((cfg, "1 RK step", lo, size, rep))
         worst["rk_step"] = max(worst.get("rk_step", 0.0), rep["strict_rel_max"])
         worst.setdefault("rk_arbiter_vars", set()).update(rep["arbiter_vars"])
     assert abs(lam - max(ORC.max_wavespeed(qb, p, G) for qb in q_boxes)) < 0.2 * lam   # same field, sampled
@@ -86,10 +91,21 @@ def sampled_parity(cfg, boxes_res, boxes_rk, tol_res=1e-11, tol_rk=1e-11, cfl=0.
     return worst
 
 
+# Which variables may pass through the arbiter clause (oracle/parity.py).  At full size the residual of every
+# variable is a cancellation residue of terms 1e4-1e5 times larger (2/h is 100-700 and the fields are smooth), so
+# the fp64 ORACLE's own error against its long-double build is 1e-11..1e-9 of the result there (eta/s column of
+# profiles/r02_parity_report.md): no fp64 evaluation can meet 1e-11 of the result, and the GPU is held to
+# g <= 4 eta instead (measured: g/eta <= 1.3).  After a Runge-Kutta step only rho w of the Taylor-Green fields
+# (identically zero initially) is such a residue.
+RES_ALLOWED = ("rho", "rho u", "rho v", "rho w", "rho E")
+RK_ALLOWED_TGV = ("rho w",)
+
+
 def test_cfg3_taylor_green_64cubed_p4_full_size():
     boxes_res = [((0, 0, 0), (4, 4, 4)), ((62, 62, 62), (4, 5, 6)), ((30, 17, 5), (6, 4, 4))]
-    boxes_rk = [((59, 60, 61), (12, 12, 12))]
-    print(sampled_parity("cfg3", boxes_res, boxes_rk))
+    # Runge-Kutta step: a box across the periodic corner, one on the seams of the default 2x3 columns, one inside
+    boxes_rk = [((59, 60, 61), (12, 12, 12)), ((25, 19, 7), (12, 12, 12))]
+    print(sampled_parity("cfg3", boxes_res, boxes_rk, allowed_res=RES_ALLOWED, allowed_rk=RK_ALLOWED_TGV))
 
 
 @pytest.mark.parametrize("p", range(1, 8))
@@ -97,7 +113,7 @@ def test_cfg4_order_sweep_full_size(p):
     n = I.cfg4_elems_per_side(p)
     boxes_res = [((n - 3, n - 2, n - 3), (6, 5, 6)), ((n // 2, 1, n // 3), (4, 4, 4))]
     boxes_rk = [((n - 6, n - 6, n - 6), (12, 12, 12))]
-    print(sampled_parity(f"cfg4_p{p}", boxes_res, boxes_rk))
+    print(sampled_parity(f"cfg4_p{p}", boxes_res, boxes_rk, allowed_res=RES_ALLOWED, allowed_rk=()))
 
 
 def test_cfg5_taylor_green_96cubed_p7_full_size():
@@ -107,4 +123,4 @@ def test_cfg5_taylor_green_96cubed_p7_full_size():
         pytest.skip("needs a 180 GB device")
     boxes_res = [((94, 94, 94), (4, 4, 4)), ((40, 3, 77), (4, 4, 4))]
     boxes_rk = [((90, 91, 92), (12, 12, 12))]
-    print(sampled_parity("cfg5", boxes_res, boxes_rk))
+    print(sampled_parity("cfg5", boxes_res, boxes_rk, allowed_res=RES_ALLOWED, allowed_rk=RK_ALLOWED_TGV))

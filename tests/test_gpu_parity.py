@@ -136,12 +136,12 @@ def test_cfg2_vortex_residual_and_100_steps():
     dg = DG(*n, p, G, ext)
     dg.set_state(q0)
     # rho w of the z-invariant vortex is identically zero: its residual is rounding residue (arbiter clause)
-    rep = assert_parity(dg.residual(), ORC.residual(q0, p, G, ext), lambda: ARB.residual(q0, p, G, ext), TOL_RES, "cfg2 residual")
-    assert rep["arbiter_vars"] in ([], ["rho w"]), rep
+    rep = assert_parity(dg.residual(), ORC.residual(q0, p, G, ext), lambda: ARB.residual(q0, p, G, ext), TOL_RES, "cfg2 residual",
+                        allowed=["rho w"])
     dt = I.cfl_dt(ORC.max_wavespeed(q0, p, G), p, ext, n, 0.1)
     q = dg.rk_step(dt, 100).get_state()
-    rep = assert_parity(q, ORC.rk_step(q0, p, G, ext, dt, 100), lambda: ARB.rk_step(q0, p, G, ext, dt, 100), TOL_RK100, "cfg2 100 steps")
-    assert rep["arbiter_vars"] in ([], ["rho w"]), rep
+    rep = assert_parity(q, ORC.rk_step(q0, p, G, ext, dt, 100), lambda: ARB.rk_step(q0, p, G, ext, dt, 100), TOL_RK100, "cfg2 100 steps",
+                        allowed=["rho w"])
     # and the solution is the translated vortex to discretisation accuracy
     exact = I.isentropic_vortex(*n, p, ext, t=100 * dt)
     assert np.abs(q[..., 0] - exact[..., 0]).max() < 5e-3
@@ -161,10 +161,14 @@ def test_100_steps_reduced_grids_of_cfg3_cfg4_cfg5(p):
         dt = I.cfl_dt(ORC.max_wavespeed(q0, p, G), p, ext, (n, n, n), 0.1)
         dg = DG(n, n, n, p, G, ext)
         r = dg.set_state(q0).residual()
-        assert_parity(r, ORC.residual(q0, p, G, ext), lambda: ARB.residual(q0, p, G, ext), TOL_RES, (p, field, "residual"))
+        # Taylor-Green at Mach 0.1: the mass and energy residuals are cancellation residues (div u = 0) and rho w
+        # starts identically zero; the Fourier-mode field has no such variable
+        tgv = field == "taylor_green"
+        assert_parity(r, ORC.residual(q0, p, G, ext), lambda: ARB.residual(q0, p, G, ext), TOL_RES, (p, field, "residual"),
+                      allowed=("rho", "rho u", "rho v", "rho w", "rho E") if tgv else ())
         q = dg.rk_step(dt, 100).get_state()
         assert_parity(q, ORC.rk_step(q0, p, G, ext, dt, 100), lambda: ARB.rk_step(q0, p, G, ext, dt, 100), TOL_RK100,
-                      (p, field, "100 steps"))
+                      (p, field, "100 steps"), allowed=("rho w",) if tgv else ())
         dg.close()
 
 
@@ -178,6 +182,48 @@ def test_rk_step_composes_and_zero_steps_is_identity():
     c = dg.set_state(q0).rk_step(1e-3, 1).rk_step(1e-3, 2).get_state()
     assert np.array_equal(b, c)
     assert dg.launch_count > 0
+    dg.close()
+
+
+def test_rk_step_cfl_matches_oracle_loop_and_fused_wavespeed():
+    """dg_rk_step_cfl: every step takes dt = cfl min(h) / ((2p+1) lam_max(Q)) (reading R10) with lam_max
+    reduced on the device by the last stage of the previous step.  Against the oracle driven by the same rule."""
+    for p, shape, ext in ((1, (5, 4, 3), (1.0, 0.9, 0.5)), (3, (4, 4, 3), (1.0, 1.0, 0.8)), (4, (3, 2, 4), (0.7, 0.5, 1.0))):
+        q0 = rough_field(*shape, p, ext, seed=5)
+        dg = DG(*shape, p, G, ext)
+        t_gpu, dt_last = dg.set_state(q0).rk_step_cfl(0.1, 4)
+        q_gpu = dg.get_state()
+        q, t = q0, 0.0
+        for _ in range(4):
+            dt = I.cfl_dt(ORC.max_wavespeed(q, p, G), p, ext, shape, 0.1)
+            q = ORC.rk_step(q, p, G, ext, dt, 1)
+            t += dt
+        assert abs(t_gpu - t) <= 1e-13 * t and abs(dt_last - dt) <= 1e-13 * dt, (p, t_gpu, t)
+        assert relerr(q_gpu, q) < 1e-12, (p, relerr(q_gpu, q))
+        # the wavespeed the last stage reduced on the way == the oracle's of the final state (8-byte read-back)
+        launches = dg.launch_count
+        lam = dg.max_wavespeed()
+        assert dg.launch_count == launches                     # no reduction kernel ran
+        assert abs(lam - ORC.max_wavespeed(q_gpu, p, G)) <= 4e-16 * lam
+        # after a plain rk_step the cached value is stale and the reduction kernel runs again
+        dg.rk_step(1e-4, 1)
+        lam2 = dg.max_wavespeed()
+        assert dg.launch_count == launches + 6
+        assert abs(lam2 - ORC.max_wavespeed(dg.get_state(), p, G)) <= 4e-16 * lam2
+        dg.close()
+
+
+def test_max_wavespeed_propagates_nan():
+    """A node with negative pressure: the wavespeed is NaN (no limiter, reading R15), in the stand-alone
+    reduction and in the one fused into the last stage; dg_rk_step_cfl then refuses to step (DG_ESTATE)."""
+    p, shape, ext = 2, (4, 3, 2), (1.0, 1.0, 1.0)
+    q = rough_field(*shape, p, ext, seed=9)
+    q[1, 2, 3, 0, 1, 2, 4] = 1e-3                              # rho E far below the kinetic energy
+    dg = DG(*shape, p, G, ext)
+    assert np.isnan(dg.set_state(q).max_wavespeed())
+    assert np.isnan(ORC.max_wavespeed(q, p, G))
+    with pytest.raises(DGError):
+        dg.rk_step_cfl(0.1, 1)
     dg.close()
 
 

@@ -39,11 +39,22 @@ def test_cancellation_clause_accepts_a_reordered_fp64_evaluation_and_rejects_rea
         ok, rep = compare(bad, r, arb, 1e-11)
         assert not ok, (n, rep)
     try:
-        assert_parity(other * (1 + 1e-10), r, lambda: arb, 1e-11, "scaled")
+        assert_parity(other * (1 + 1e-10), r, lambda: arb, 1e-11, "scaled", allowed=["rho w"])
     except AssertionError:
         pass
     else:
         raise AssertionError("a 1e-10 relative scaling must fail the 1e-11 parity test")
+    # the clause is only open to the variables the caller names
+    assert_parity(other, r, lambda: arb, 1e-11, "strong form", allowed=["rho w"])
+    try:
+        assert_parity(other, r, lambda: arb, 1e-11, "strong form, nothing allowed")
+    except AssertionError:
+        pass
+    else:
+        raise AssertionError("rho w needs the arbiter clause and was not allowed to use it")
+    # and the report carries the numbers for every variable once the arbiter has been evaluated
+    rep = assert_parity(other, r, arb, 1e-11, "report", allowed=["rho w"], always_arbiter=True)
+    assert all(row["g_over_eta"] is not None or row["oracle_own_error"] == 0.0 for row in rep["rows"])
 
 
 def test_strict_metric_without_arbiter():
