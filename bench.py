@@ -14,6 +14,12 @@ p = 1..7 sweep of config 4 ("p_sweep", skip with --no-sweep).
 Prints ONE JSON line (rank 0).  Timing: CUDA events on the stream the kernels are launched on,
 after W >= 3 warm-up steps, barrier + synchronize on both sides, max over ranks.  The working set
 (>= 2.6 GB per stage) is far larger than the 126 MB L2, so no flush is needed between iterations.
+
+Besides the contract's keys the line carries: `sustained` (the same workload for >= 300 steps, i.e. under
+the board's power cap), `cfg5` (the largest single-GPU case, 10 steps), `p_sweep` (config 4, p = 1..7),
+`adaptive_dt` (dg_rk_step_cfl: CFL time step from the device-side max-wavespeed reduction every step),
+`roofline` (HBM: 152 algorithmic bytes per DOF and stage against the measured copy bandwidth) and
+`roofline_fp64` (algorithmic flops against the FP64 FMA rate measured by a microbenchmark in the same run).
 """
 import argparse
 import json
@@ -28,7 +34,15 @@ sys.path.insert(0, ROOT)
 METRIC = "DOF-updates/s per RK stage"
 UNIT = "DOF-updates/s"
 STAGES = 5
-ALGO_BYTES_PER_DOF_STAGE = 152.0   # read Q,K + write Q,K = 4 x 40 B, stage 1 does not read K
+ALGO_BYTES_PER_DOF_STAGE = 152.0   # read Q,K + write Q,K = 4 x 40 B, stage 1 does not read K;
+                                   # the kernel also skips the dead K store of stage 5 and moves 144
+
+
+def algo_flops_per_dof(p):
+    """Algorithmic flops per DOF and stage: 178 + 30 N + 225 / N (volume 38 + 30 N from
+    PAPER.md:135, traces 60, lift 60, 3 N^2 unique face nodes x 75, Runge-Kutta 20)."""
+    N = p + 1
+    return 178.0 + 30.0 * N + 225.0 / N
 GAMMA = 1.4
 
 
@@ -47,7 +61,7 @@ def ncu_traffic(workload):
         with open(path) as f:
             entry = json.load(f).get(workload)
         if entry:
-            return entry.get("dram_bytes_per_launch")
+            return entry
     return None
 
 
@@ -119,30 +133,55 @@ def physical_gpu_index(local_rank):
 # ----------------------------------------------------------------------------------------------
 # the oracle on the host cores: cpu_baseline leg and --impl reference
 # ----------------------------------------------------------------------------------------------
-def oracle_sample(workload, target_seconds=10.0, fixed_steps=None):
-    """Time the CPU oracle (as it stands) on a bounded sub-box of the workload's field."""
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_sample(workload, target_seconds=10.0, fixed_steps=None, build="omp", nodes=4.0e5):
+    """Time the CPU oracle (as it stands: an unoptimised checker, NOT a tuned CPU DG code) on a bounded sample of
+    the workload: the workload's own field formula and extent on a reduced periodic mesh of about `nodes` nodes
+    (out of cache), so the sample is smooth and exactly periodic like the workload itself."""
+    import numpy as np
     from oracle import Oracle
     from paper_2006_15698_b200 import inputs as I
-    c = I.CONFIGS[workload]
+    c = dict(I.CONFIGS[workload])
     p, ext = c["p"], c["extent"]
-    ne = max(2, min(c["nx"], int(round((4.0e5 / (p + 1) ** 3) ** (1.0 / 3.0)))))   # ~4e5 nodes, out of cache
-    box = ((0, ne), (0, ne), (0, ne))
-    q = I.make_field(workload, box=box)
-    sub_ext = tuple(ext[a] * ne / (c["nx"], c["ny"], c["nz"])[a] for a in range(3))
-    orc = Oracle("omp")
-    dt = I.cfl_dt(orc.max_wavespeed(q, p, GAMMA), p, sub_ext, (ne, ne, ne), 0.1)
+    ne = max(2, min(c["nx"], int(round((nodes / (p + 1) ** 3) ** (1.0 / 3.0)))))
+    c.update(nx=ne, ny=ne, nz=ne)
+    q = I.make_field(c)
+    orc = Oracle(build)
+    dt = I.cfl_dt(orc.max_wavespeed(q, p, GAMMA), p, ext, (ne, ne, ne), 0.1)
     dof = ne ** 3 * (p + 1) ** 3
     t0 = time.perf_counter()
-    orc.rk_step(q, p, GAMMA, sub_ext, dt, 1)
+    orc.rk_step(q, p, GAMMA, ext, dt, 1)
     t1 = time.perf_counter() - t0
     steps = fixed_steps if fixed_steps is not None else max(1, min(50, int(round(target_seconds / max(t1, 1e-6)))))
     t0 = time.perf_counter()
-    orc.rk_step(q, p, GAMMA, sub_ext, dt, steps)
+    out = orc.rk_step(q, p, GAMMA, ext, dt, steps)
     t = time.perf_counter() - t0
     return {"value": dof * STAGES * steps / t, "unit": UNIT, "cores": orc.threads, "kind": "oracle",
-            "sample": f"{ne}^3-element sub-box of {workload} (p={p}, {dof} nodes), {steps} LSERK45 steps, "
-                      f"oracle/dg_oracle.c OpenMP-over-elements build, {t:.1f} s",
-            "seconds_per_step": t / steps, "dof": dof}
+            "sample": f"{workload}'s field on a reduced periodic {ne}^3-element mesh (p={p}, {dof} nodes), {steps} LSERK45 "
+                      f"steps, oracle/dg_oracle.c ({'OpenMP over elements' if 'omp' in build else 'single thread'}), {t:.1f} s; "
+                      "the oracle is a plain checker, not a tuned CPU DG code",
+            "seconds_per_step": t / steps, "dof": dof, "finite": bool(np.isfinite(out).all()), "cpu_model": cpu_model()}
+
+
+def oracle_per_p():
+    """SURVEY.md 8(d) "oracle timing": per p = 1..7 (config 4's field), single thread and OpenMP, bounded."""
+    rows = []
+    for p in range(1, 8):
+        one = oracle_sample(f"cfg4_p{p}", fixed_steps=1, build="fp64", nodes=2.0e5)
+        omp = oracle_sample(f"cfg4_p{p}", fixed_steps=2, build="omp", nodes=4.0e5)
+        rows.append({"p": p, "single_thread": one["value"], "omp": omp["value"], "omp_threads": omp["cores"],
+                     "dof_single": one["dof"], "dof_omp": omp["dof"]})
+    return rows
 
 
 def run_reference(args, rank):
@@ -155,7 +194,7 @@ def run_reference(args, rank):
             "steps": K, "warmup": W, "ms_per_step": 1e3 * samp["seconds_per_step"], "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"{args.workload} (bounded sample: {samp['sample']})"},
-            "cpu_baseline": {k: samp[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "cpu_baseline": {k: samp[k] for k in ("value", "unit", "cores", "kind", "sample", "finite", "cpu_model")},
             "e2e": {"value": samp["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -204,11 +243,11 @@ def time_workload(workload, K, W, device, dist, sampler_index=None, want_e2e=Fal
 
     if want_e2e:
         # second device-timed number: the max-wavespeed reduction (CFL time step) executed before every step
-        steps_a = min(K, 10)
+        steps_a = min(K, 20)
+        dg.rk_step_cfl(0.1, 2)
         barrier()
         t0 = time.perf_counter()
-        for _ in range(steps_a):
-            dg.rk_step(I.cfl_dt(dg.max_wavespeed(), p, ext, n, 0.1), 1)      # max_wavespeed synchronises
+        dg.rk_step_cfl(0.1, steps_a)      # per step: 8-byte read-back of the wavespeed the last stage reduced
         torch.cuda.synchronize(device)
         out["adaptive_dt"] = {"seconds": time.perf_counter() - t0, "steps": steps_a}
         # end to end through the public API with HOST buffers: every step copies the state in from
@@ -280,11 +319,20 @@ def run_ours(args, rank, world, local_rank):
     device = torch.device(f"cuda:{local_rank}")
     torch.cuda.set_device(device)
     K, W = args.steps, max(3, args.warmup)
-    main = time_workload(args.workload, K, W, device, dist, physical_gpu_index(local_rank), want_e2e=True)
+    main = time_workload(args.workload, K, W, device, dist, physical_gpu_index(local_rank), want_e2e=True, lz=args.lz,
+                         variant=args.variant)
 
     ms = reduce_max(main["ms"], dist, device)
     e2e_s = reduce_max(main["e2e"]["seconds"], dist, device)
-    sweep = []
+    sweep, sustained, big, fp64 = [], None, None, None
+    if world == 1 and not args.no_extras:
+        # the same workload for >= 300 steps: the board reaches its power cap after ~0.3 s and holds lower clocks
+        sustained = time_workload(args.workload, max(300, K), W, device, None, physical_gpu_index(local_rank), lz=args.lz,
+                                  variant=args.variant)
+        from paper_2006_15698_b200.binding import fp64_peak
+        fp64 = fp64_peak(device)
+        if args.workload != "cfg5" and torch.cuda.mem_get_info(device)[1] >= 150 * 2 ** 30:
+            big = time_workload("cfg5", 10, 3, device, None, physical_gpu_index(local_rank))
     if not args.no_sweep and world == 1:
         for p in range(1, 8):
             s = time_workload(f"cfg4_p{p}", 20, 3, device, None)
@@ -301,9 +349,23 @@ def run_ours(args, rank, world, local_rank):
     value = whole_job_rate(dof, K, ms, world)
     launch_s = ms * 1e-3 / main["launches"]                       # the step IS 5 stage-kernel launches
     achieved = ALGO_BYTES_PER_DOF_STAGE * dof / launch_s / 1e9
+
+    def traffic_of(workload, n_dof):
+        entry = ncu_traffic(workload)
+        if not entry:
+            return None, None
+        return entry.get("dram_bytes_per_launch"), entry
+
+    def frac_of(rate):
+        return rate * ALGO_BYTES_PER_DOF_STAGE / 1e9 / peak
+
     for s in sweep:
-        s["roofline_frac"] = s["value"] * ALGO_BYTES_PER_DOF_STAGE / 1e9 / peak
+        s["roofline_frac"] = frac_of(s["value"])
+        t, _ = traffic_of(f"cfg4_p{s['p']}", s["dof"])
+        s["traffic"] = t
+        s["traffic_over_algorithmic"] = None if t is None else t / (ALGO_BYTES_PER_DOF_STAGE * s["dof"])
     e2e = main["e2e"]
+    traffic, traffic_entry = traffic_of(args.workload, dof)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -321,20 +383,46 @@ def run_ours(args, rank, world, local_rank):
                      "frac": achieved / peak, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": ALGO_BYTES_PER_DOF_STAGE * dof,
                      "avg_launch_ms": launch_s * 1e3, "frac_of_8TBs_nominal": achieved / 8000.0,
-                     "traffic": ncu_traffic(args.workload), "traffic_unit": "DRAM bytes per launch (ncu, profiles/)"},
+                     "traffic": traffic,
+                     "traffic_unit": "DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full)",
+                     "traffic_static": True,
+                     "traffic_source": None if traffic_entry is None else traffic_entry.get("source")},
         "e2e": {"value": whole_job_rate(dof, e2e["steps"], e2e_s * 1e3, world), "unit": UNIT,
                 "h2d_bytes_per_step": e2e["bytes_each_way"], "d2h_bytes_per_step": e2e["bytes_each_way"],
                 "steps": e2e["steps"], "api": "DG.set_state(pinned host) -> DG.rk_step(dt,1) -> DG.get_state(pinned host)"},
         "adaptive_dt": {"value": whole_job_rate(dof, main["adaptive_dt"]["steps"], main["adaptive_dt"]["seconds"] * 1e3, world),
                         "unit": UNIT, "steps": main["adaptive_dt"]["steps"],
-                        "what": "dg_max_wavespeed (device reduction + 8-byte read-back) before every step, dt = CFL rule"},
+                        "what": "dg_rk_step_cfl: dt = CFL rule from the max wavespeed the last stage of the previous step "
+                                "reduced on the device (8-byte read-back per step), wall clock"},
         "p_sweep": sweep,
         "context": "paper: 1.13e9 DOF-updates/s per V100 (kernels only, derived from Table II, PAPER.md:264-269); "
                    "another machine, not a target",
     }
+    if sustained is not None:
+        s_rate = sustained["dof"] * STAGES * sustained["launches"] / 5 / (sustained["ms"] * 1e-3)
+        line["sustained"] = {"value": s_rate, "unit": UNIT, "steps": sustained["launches"] // 5, "roofline_frac": frac_of(s_rate),
+                             "clocks": sustained["clocks"],
+                             "nj_per_dof_update": None if not sustained["clocks"] or not sustained["clocks"].get("power_w")
+                             else 1e9 * sustained["clocks"]["power_w"] / s_rate}
+    if big is not None:
+        b_rate = big["dof"] * STAGES * 10 / (big["ms"] * 1e-3)
+        t, _ = traffic_of("cfg5", big["dof"])
+        line["cfg5"] = {"value": b_rate, "unit": UNIT, "steps": 10, "dof": big["dof"], "roofline_frac": frac_of(b_rate),
+                        "brick": big["kernel"], "finite": big["finite"], "clocks": big["clocks"], "traffic": t}
+    if fp64 is not None:
+        flops = algo_flops_per_dof(main["p"]) * value
+        line["roofline_fp64"] = {"bound": "fp64", "achieved": flops / 1e12, "peak": 2.0 * fp64 / 1e12, "unit": "TFLOP/s",
+                                 "frac": flops / (2.0 * fp64),
+                                 "peak_source": "measured in this run: dg_fp64_peak (8 independent DFMA chains per thread, "
+                                                "8 blocks of 256 threads per SM), 2 flop per FMA",
+                                 "algorithmic_flop_per_dof_stage": algo_flops_per_dof(main["p"]),
+                                 "note": "flop count of SURVEY.md 8(d); executed FP64 instructions per DOF: profiles/"}
     if not args.no_cpu and world == 1:
         cb = oracle_sample(args.workload, target_seconds=10.0)
-        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample", "finite", "cpu_model")}
+        one = oracle_sample(args.workload, fixed_steps=1, build="fp64", nodes=2.0e5)
+        line["cpu_baseline"]["single_thread"] = {"value": one["value"], "sample": one["sample"]}
+        line["cpu_baseline"]["per_p"] = oracle_per_p()
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
@@ -349,6 +437,8 @@ def main():
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the sustained run, cfg5 and the FP64 microbenchmark")
+    ap.add_argument("--variant", type=int, default=None, help="stage-kernel variant index (tuning; default: library's choice)")
     ap.add_argument("--lz", type=int, default=0, help="layers per chunk (tuning; 0 = library default)")
     ap.add_argument("--sweep-variants", action="store_true", help="time every compiled variant of --workload")
     args = ap.parse_args()

@@ -34,6 +34,8 @@ SYMBOLS = {
     "dg_kernel_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_longlong)]),
     "dg_selftest_fastmath": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t,
                                             ctypes.c_void_p]),
+    "dg_fp64_peak": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p,
+                                    ctypes.POINTER(ctypes.c_ulonglong)]),
     "dg_destroy": (ctypes.c_int, [ctypes.c_void_p]),
     "dg_last_error": (ctypes.c_char_p, [ctypes.c_void_p]),
 }
@@ -51,6 +53,31 @@ def selftest_fastmath(x):
     if rc != 0:
         raise DGError(rc, "dg_selftest_fastmath")
     return r, q
+
+
+def fp64_peak(device="cuda:0", iters=2048, repeats=5):
+    """Measured FP64 FMA rate of the device (thread-level FMA/s) from the library's microbenchmark kernel
+    (dg_fp64_peak), timed with CUDA events on the current stream; best of `repeats`."""
+    import torch
+    lib = load_library()
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        blocks = sms * 8
+        out = torch.empty(blocks * 256, dtype=torch.float64, device=dev)
+        stream = torch.cuda.current_stream(dev)
+        count = ctypes.c_ulonglong(0)
+        best = 0.0
+        for _ in range(repeats + 1):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            rc = lib.dg_fp64_peak(out.data_ptr(), blocks, iters, stream.cuda_stream, ctypes.byref(count))
+            e1.record(stream)
+            if rc != 0:
+                raise DGError(rc, "dg_fp64_peak")
+            torch.cuda.synchronize(dev)
+            best = max(best, count.value / (e0.elapsed_time(e1) * 1e-3))
+    return best
 
 
 class DGError(RuntimeError):

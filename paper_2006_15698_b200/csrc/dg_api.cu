@@ -122,6 +122,19 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 }  // namespace
 
+// FP64 peak microbenchmark (test/bench entry dg_fp64_peak): 8 independent DFMA chains per thread, 4096 deep.
+__global__ void __launch_bounds__(256) dg_fp64_peak_kernel(double *out, int iters, double a, double b) {
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+            x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+        }
+    }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+}
+
 __global__ void dg_fastmath_kernel(const double *x, double *r, double *q, size_t n) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) {
@@ -279,6 +292,7 @@ int enqueue_step(dg_ctx *c, double dt, bool want_lam) {
         a.rkA = (double)kRkA[s];
         a.rkB = (double)kRkB[s];
         a.want_lam = (want_lam && s == 4) ? 1 : 0;
+        a.store_k = (s == 4) ? 0 : 1;
         if (a.want_lam) {
             cudaError_t e = cudaMemsetAsync(c->scal, 0, 8, c->stream);
             if (e != cudaSuccess) return cuda_fail(c, e, "memset");
@@ -559,6 +573,13 @@ int dg_selftest_fastmath(const double *x, double *r, double *q, size_t n, void *
     if (!x || !r || !q) return DG_EINVAL;
     if (n == 0) return DG_OK;
     dg_fastmath_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(x, r, q, n);
+    return cudaGetLastError() == cudaSuccess ? DG_OK : DG_ECUDA;
+}
+
+int dg_fp64_peak(double *out, int blocks, int iters, void *stream, unsigned long long *fma_count) {
+    if (!out || blocks < 1 || iters < 1) return DG_EINVAL;
+    dg_fp64_peak_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(out, iters, 0.999999, 1e-6);
+    if (fma_count) *fma_count = (unsigned long long)blocks * 256ull * (unsigned long long)iters * 128ull;
     return cudaGetLastError() == cudaSuccess ? DG_OK : DG_ECUDA;
 }
 

@@ -66,6 +66,7 @@ struct DgStageArgs {
     double rkA, rkB;      // stage coefficients; rkA == 0 means "do not read K" (stage 1)
     int mode;
     int want_lam;
+    int store_k;          // 0 in the last stage of a step: K is dead then (the next stage 1 has A = 0) and is not written
     double scale[3];      // 2/h_a per axis, times dt in stage mode: K accumulates dt * L(Q)
 };
 

@@ -269,7 +269,7 @@ struct BlockInfo {
     long long tstride;         // doubles between consecutive layers in Txy
     long long kstride;         // ... in Q and K
     double gamma, gm1, rkA, rkB, scale[3];
-    int ext0, ext1, readK, nl;
+    int ext0, ext1, readK, storeK, nl;
 };
 
 // PE for one of the axes x, y: traces of the Q in shared memory on the column boundary -> Tslot.
@@ -571,6 +571,7 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
                 }
         } else {
             const double rkB = bi->rkB;
+            const bool storeK = bi->storeK != 0;
             double *tz_out = bi->tz_out;
             double Qn[LAM ? NV : 1][N];
 #pragma unroll
@@ -582,7 +583,7 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
                     const double Kn = fma(sc, V[s][i], K0[n * PLANE + i * S]);
                     const double Qold = C::RELOAD ? Q0w[n * PLANE + i * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : i];
                     Qn[sq][i] = fma(rkB, Kn, Qold);
-                    __stcs(Kline + (n * N + i) * C::HP, Kn);
+                    if (storeK) __stcs(Kline + (n * N + i) * C::HP, Kn);
                     Q0w[n * PLANE + i * S] = Qn[sq][i];
                 }
                 // PE for the z faces: traces of the updated Q, only at the two ends of the chunk
@@ -767,6 +768,7 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
         bi->ext0 = min(C::BX, a.nx - bxi * C::BX);   // elements of this column per axis (ragged last column)
         bi->ext1 = min(C::BY, a.ny - byi * C::BY);
         bi->readK = readK ? 1 : 0;
+        bi->storeK = a.store_k;
         bi->nl = nl;
     }
     __syncthreads();
@@ -965,8 +967,8 @@ constexpr DgKernelTable make_table() {
 #define DG_VARIANTS DG_T(2, 9, 8, 2, 1, 290, 0, 0), DG_T(2, 8, 4, 3, 0, 0, 3, 0), DG_T(2, 4, 4, 6, 0, 0, 3, 0), DG_T(2, 8, 8, 2, 0, 0, 3, 0), \
                     DG_T(2, 9, 7, 2, 1, 258, 3, 0), DG_T(2, 9, 7, 3, 1, 258, 3, 0)
 #elif DG_N == 3
-#define DG_VARIANTS DG_T(3, 4, 4, 2, 0, 0, 4, 4), DG_T(3, 6, 3, 2, 0, 0, 4, 0), DG_T(3, 4, 4, 3, 1, 0, 4, 4), DG_T(3, 4, 2, 4, 1, 0, 4, 0), \
-                    DG_T(3, 6, 4, 2, 0, 0, 4, 0), DG_T(3, 2, 7, 3, 1, 134, 4, 0), DG_T(3, 2, 7, 3, 0, 134, 4, 0)
+#define DG_VARIANTS DG_T(3, 6, 4, 2, 0, 0, 4, 0), DG_T(3, 4, 4, 2, 0, 0, 4, 4), DG_T(3, 2, 7, 3, 0, 134, 4, 0), DG_T(3, 6, 3, 2, 0, 0, 4, 0), \
+                    DG_T(3, 4, 4, 3, 1, 0, 4, 4), DG_T(3, 4, 2, 4, 1, 0, 4, 0)
 #elif DG_N == 4
 #define DG_VARIANTS DG_T(4, 2, 2, 4, 0, 66, 1, 0), DG_T(4, 2, 2, 5, 1, 66, 1, 0), DG_T(4, 4, 2, 2, 0, 130, 3, 0), DG_T(4, 4, 2, 3, 1, 130, 3, 0), \
                     DG_T(4, 2, 2, 3, 0, 66, 1, 0)
@@ -974,7 +976,7 @@ constexpr DgKernelTable make_table() {
 #define DG_VARIANTS DG_T(5, 2, 3, 2, 0, 154, 4, 0), DG_T(5, 3, 2, 2, 0, 0, 4, 0), DG_T(5, 2, 2, 3, 1, 106, 4, 0), DG_T(5, 5, 1, 2, 0, 0, 4, 0), \
                     DG_T(5, 5, 1, 2, 1, 0, 4, 0), DG_T(5, 1, 5, 2, 0, 138, 0, 1)
 #elif DG_N == 6
-#define DG_VARIANTS DG_T(6, 2, 1, 3, 0, 0, 4, 0), DG_T(6, 2, 1, 3, 1, 0, 4, 0), DG_T(6, 3, 1, 2, 0, 114, 2, 0), DG_T(6, 1, 3, 2, 0, 118, 0, 0), \
+#define DG_VARIANTS DG_T(6, 1, 3, 2, 0, 118, 0, 0), DG_T(6, 3, 1, 2, 0, 114, 2, 0), DG_T(6, 2, 1, 3, 0, 0, 4, 0), DG_T(6, 2, 1, 3, 1, 0, 4, 0), \
                     DG_T(6, 1, 1, 5, 1, 0, 0, 0), DG_T(6, 1, 1, 4, 0, 0, 0, 0)
 #elif DG_N == 7
 #define DG_VARIANTS DG_T(7, 2, 1, 2, 1, 0, 4, 0), DG_T(7, 1, 1, 4, 1, 0, 0, 1), DG_T(7, 1, 1, 4, 0, 0, 0, 1), DG_T(7, 1, 1, 3, 0, 0, 0, 1)

@@ -17,7 +17,7 @@ def declared_symbols():
     names = set()
     for header in HEADERS:
         text = re.sub(r"/\*.*?\*/", "", open(header).read(), flags=re.S)
-        names |= set(re.findall(r"\b(dg_[a-z_]+)\s*\(", text))
+        names |= set(re.findall(r"\b(dg_[a-z0-9_]+)\s*\(", text))
     return sorted(names)
 
 
