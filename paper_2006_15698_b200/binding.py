@@ -117,7 +117,7 @@ class DG:
     """One mesh + one state vector on the GPU.  Arrays are float64, shape (nz,ny,nx,N,N,N,5)."""
 
     def __init__(self, nx, ny, nz, p, gamma=1.4, extent=(1.0, 1.0, 1.0), device="cuda:0", brick=None, bind=True,
-                 variant=None):
+                 variant=None, poison=False):
         self.lib = load_library()
         self.nx, self.ny, self.nz, self.p, self.N = nx, ny, nz, p, p + 1
         self.gamma, self.extent = float(gamma), tuple(float(e) for e in extent)
@@ -136,14 +136,16 @@ class DG:
         self.device = None
         self._torch = None
         if bind:
-            self.bind(device)
+            self.bind(device, poison=poison)
 
     # -- plumbing -------------------------------------------------------------------------------
     def _check(self, rc):
         if rc != 0:
             raise DGError(rc, self.lib.dg_last_error(self._h).decode())
 
-    def bind(self, device="cuda:0", stream=None):
+    def bind(self, device="cuda:0", stream=None, poison=False):
+        """Allocate the workspace and hand it to the library.  poison=True fills it with 0xFF bytes (NaN as doubles)
+        first: a test aid that makes any read of memory the library has not written show up in the results."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2006_15698_b200 needs a CUDA device; there is no CPU fallback")
@@ -152,6 +154,8 @@ class DG:
         nbytes = self.lib.dg_workspace_bytes(self._h)
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            if poison:
+                self.workspace.fill_(255)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             self._check(self.lib.dg_bind(self._h, self.workspace.data_ptr(), nbytes, self.stream.cuda_stream))
 

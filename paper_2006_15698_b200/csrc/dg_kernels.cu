@@ -146,11 +146,14 @@ __device__ __forceinline__ void euler_flux_normal(const double (&Q)[DG_NV], doub
     // 1/2 rho |u|^2 = 1/2 |rho u|^2 / rho
     const double m2 = fma(Q[3], Q[3], fma(Q[2], Q[2], Q[1] * Q[1]));
     pres = gm1 * fma(-0.5, m2 * oneOrho, Q[4]);
+    // Products rounded on their own (never contracted into a later add): the interface flux below adds the
+    // fluxes of the two sides, and a product fused into that sum on one side only would make the two blocks
+    // that share a face compute fluxes that differ in the last bit.
     F[0] = Q[1];                                    // rho u_a
     F[1] = fma(Q[1], vel, pres);
-    F[2] = Q[2] * vel;
-    F[3] = Q[3] * vel;
-    F[4] = (Q[4] + pres) * vel;
+    F[2] = __dmul_rn(Q[2], vel);
+    F[3] = __dmul_rn(Q[3], vel);
+    F[4] = __dmul_rn(Q[4] + pres, vel);
 }
 
 // Local Lax-Friedrichs flux (reading R3), rotated slots as above, returned DOUBLED
@@ -167,7 +170,7 @@ __device__ __forceinline__ void lax_friedrichs2(const double (&Qown)[DG_NV], con
     const double lamb = fabs(ub) + sqrt_pos(gamma * pb * rb);
     const double sl = sgn * ((lama > lamb) ? lama : lamb);
 #pragma unroll
-    for (int n = 0; n < DG_NV; ++n) Fs[n] = fma(-sl, Qoth[n] - Qown[n], Fa[n] + Fb[n]);
+    for (int n = 0; n < DG_NV; ++n) Fs[n] = fma(-sl, Qoth[n] - Qown[n], __dadd_rn(Fa[n], Fb[n]));
 }
 
 // ------------------------------------------------------------------------------------------------

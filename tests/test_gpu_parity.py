@@ -227,6 +227,37 @@ def test_max_wavespeed_propagates_nan():
     dg.close()
 
 
+@pytest.mark.parametrize("p", range(1, 8))
+def test_poisoned_workspace_and_run_to_run_determinism(p):
+    """compute-sanitizer is closed on this GPU pool (its runs have left GPUs needing a reset), so the two things
+    its initcheck and racecheck tools would look for are tested directly, for every compiled variant, on a mesh
+    that is ragged against every column shape and has several chunks of layers:
+    (1) the workspace is filled with NaN before dg_bind: any read of a trace, K or padding entry the library has
+        not written would turn up as NaN or as a parity failure;
+    (2) the same residual + 3 steps, run three times, must agree bit for bit (a shared-memory or trace-buffer race
+        between warps or blocks shows as run-to-run differences)."""
+    nx, ny, nz, ext = 5, 7, 6, (1.0, 1.4, 1.2)
+    q = rough_field(nx, ny, nz, p, ext, seed=21)
+    r_orc = ORC.residual(q, p, G, ext)
+    dt = I.cfl_dt(ORC.max_wavespeed(q, p, G), p, ext, (nx, ny, nz), 0.1)
+    q_orc = ORC.rk_step(q, p, G, ext, dt, 3)
+    for v in variants(p):
+        outs = []
+        for rep in range(3):
+            dg = DG(nx, ny, nz, p, G, ext, variant=v, brick=(0, 0, 2 + rep % 2), poison=True)
+            r = dg.set_state(q).residual()
+            q3 = dg.rk_step(dt, 3).get_state()
+            lam = dg.max_wavespeed()
+            dg.close()
+            assert np.isfinite(r).all() and np.isfinite(q3).all() and np.isfinite(lam), (p, v)
+            assert relerr(r, r_orc) < TOL_RES and relerr(q3, q_orc) < 1e-12, (p, v, relerr(r, r_orc), relerr(q3, q_orc))
+            outs.append((r, q3))
+        # repetitions 0 and 2 use the same chunk length: bitwise equal; repetition 1 (other chunk length) too,
+        # because a face flux does not depend on which block computes it
+        for r, q3 in outs[1:]:
+            assert np.array_equal(r, outs[0][0]) and np.array_equal(q3, outs[0][1]), (p, v)
+
+
 def test_fast_math():
     """The kernels' branch-free reciprocal / square root (csrc/dg_internal.h) against IEEE division and
     sqrt on the CPU: at most 2 units in the last place over 14 decades of positive normal arguments."""
