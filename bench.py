@@ -276,6 +276,66 @@ def time_workload(workload, K, W, device, dist, sampler_index=None, want_e2e=Fal
     return out
 
 
+def per_kernel_breakdown(workload, steps, device):
+    """the paper's Table II layout for this implementation: volume, surface and
+    update-project kernels launched one by one (dg_split_*), each timed with CUDA events on the launching stream, next
+    to the fused step on the same state.  Flop counts per DOF and evaluation: volume 38 + 30 N,
+    surface 120 + 225 / N (traces, Lax-Friedrichs at 3 N^2 unique face nodes, lift: SURVEY.md 8(d)), update 20."""
+    import torch
+    from paper_2006_15698_b200 import DG
+    from paper_2006_15698_b200 import inputs as I
+    c = I.CONFIGS[workload]
+    p, ext, n = c["p"], c["extent"], (c["nx"], c["ny"], c["nz"])
+    N = p + 1
+    q = I.make_field(workload, xp=torch, device=device)
+    dg = DG(*n, p, GAMMA, ext, device=device)
+    dg.set_state(q)
+    dt = I.cfl_dt(dg.max_wavespeed(), p, ext, n, 0.1)
+    dof = n[0] * n[1] * n[2] * N ** 3
+    stream = torch.cuda.current_stream(device)
+    dg.rk_step_split(dt, 2)
+    torch.cuda.synchronize(device)
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(steps * STAGES)]
+    l0 = dg.launch_count
+    for s in range(steps * STAGES):
+        ev[s][0].record(stream)
+        dg.split_volume()
+        ev[s][1].record(stream)
+        dg.split_surface()
+        ev[s][2].record(stream)
+        dg.split_update(dt, s % STAGES)
+        ev[s][3].record(stream)
+    torch.cuda.synchronize(device)
+    launches = dg.launch_count - l0
+    t = [sum(e[i].elapsed_time(e[i + 1]) for e in ev) * 1e-3 for i in range(3)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dg.rk_step(dt, 2)
+    e0.record(stream)
+    dg.rk_step(dt, steps)
+    e1.record(stream)
+    torch.cuda.synchronize(device)
+    fused = e0.elapsed_time(e1) * 1e-3
+    finite = bool(torch.isfinite(dg.get_state(q)).all().item())
+    dg.close()
+    del q
+    torch.cuda.empty_cache()
+    evals = steps * STAGES
+    flop = {"volume": 38.0 + 30.0 * N, "surface": 120.0 + 225.0 / N, "update_project": 20.0}
+    rows = {}
+    for name, sec in zip(("volume", "surface", "update_project"), t):
+        rows[name] = {"seconds": sec, "dof_per_s": dof * evals / sec, "tflops": flop[name] * dof * evals / sec / 1e12,
+                      "flop_per_dof": flop[name]}
+    total = sum(t)
+    return {"workload": f"{workload}: {list(n)} elements, p={p}, {dof} nodes", "steps": steps, "kernels": rows,
+            "split_total_seconds": total, "split_dof_updates_per_s": dof * evals / total,
+            "fused_seconds": fused, "fused_dof_updates_per_s": dof * evals / fused, "launches": launches, "finite": finite,
+            "note": "update_project = K, Q update over the whole vectors + the face-trace kernel; the surface kernel evaluates "
+                    "every face from both sides; flop rates use the algorithmic counts of PAPER.md:135 / SURVEY.md 8(d)",
+            "paper_table2_per_v100": {"volume_dof_per_s": 6.35e9, "surface_dof_per_s": 5.23e9,
+                                      "update_project_dof_per_s": 1.87e9,
+                                      "source": "derived from PAPER.md:264-269 (3,072 V100, 100 steps); another machine"}}
+
+
 def reduce_max(x, dist, device):
     """Max over ranks of a per-rank time (replicas: the slowest replica sets the whole-job rate)."""
     if dist is None:
@@ -333,6 +393,9 @@ def run_ours(args, rank, world, local_rank):
         fp64 = fp64_peak(device)
         if args.workload != "cfg5" and torch.cuda.mem_get_info(device)[1] >= 150 * 2 ** 30:
             big = time_workload("cfg5", 10, 3, device, None, physical_gpu_index(local_rank))
+    per_kernel = None
+    if world == 1 and not args.no_extras:
+        per_kernel = per_kernel_breakdown("table2_p6", 10, device)
     if not args.no_sweep and world == 1:
         for p in range(1, 8):
             s = time_workload(f"cfg4_p{p}", 20, 3, device, None)
@@ -409,6 +472,8 @@ def run_ours(args, rank, world, local_rank):
         t, _ = traffic_of("cfg5", big["dof"])
         line["cfg5"] = {"value": b_rate, "unit": UNIT, "steps": 10, "dof": big["dof"], "roofline_frac": frac_of(b_rate),
                         "brick": big["kernel"], "finite": big["finite"], "clocks": big["clocks"], "traffic": t}
+    if per_kernel is not None:
+        line["per_kernel"] = per_kernel
     if fp64 is not None:
         flops = algo_flops_per_dof(main["p"]) * value
         line["roofline_fp64"] = {"bound": "fp64", "achieved": flops / 1e12, "peak": 2.0 * fp64 / 1e12, "unit": "TFLOP/s",

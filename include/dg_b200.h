@@ -121,6 +121,22 @@ int dg_rk_step(dg_ctx *ctx, double dt, int nsteps);
  * NULL).  DG_ESTATE if the wavespeed is not positive and finite. */
 int dg_rk_step_cfl(dg_ctx *ctx, double cfl, int nsteps, double *t_advanced, double *dt_last);
 
+/* Paper-shaped per-kernel mode (Table II): the same spatial residual and stage
+ * update as dg_rk_step, run as the paper's three kernels so that their times can be measured one by one (the fused
+ * path is the product; this mode exists for the breakdown and is parity-tested against the oracle's terms).
+ *   dg_split_volume : R  = volume term of the current state (eq (5) 2nd term / mass; "overwrites R")
+ *   dg_split_surface: R -= lift of the local Lax-Friedrichs interface fluxes (eq (5) 3rd term / mass)
+ *   dg_split_update : K = A_s K + dt R; Q = Q + B_s K for stage s = 0..4 of LSERK45, then the face traces of the new
+ *                     state ("update-project")
+ * After volume + surface R = dQ/dt = L(Q) as dg_residual returns it.  R lives in the library's staging vector: do
+ * not interleave host-pointer dg_set_state / dg_get_state / dg_residual calls between volume and update.  All three
+ * are enqueued on the stream without synchronisation.  dg_split_get_r copies R out in canonical layout (host or
+ * device pointer; the host variant overwrites the Runge-Kutta register, which is dead between steps). */
+int dg_split_volume(dg_ctx *ctx);
+int dg_split_surface(dg_ctx *ctx);
+int dg_split_update(dg_ctx *ctx, double dt, int stage);
+int dg_split_get_r(dg_ctx *ctx, double *r_out, int on_device);
+
 /* Copy the current state out in canonical layout.  Synchronises when q_out is a host pointer. */
 int dg_get_state(dg_ctx *ctx, double *q_out, int on_device);
 

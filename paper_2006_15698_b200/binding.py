@@ -29,6 +29,10 @@ SYMBOLS = {
     "dg_rk_step": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int]),
     "dg_rk_step_cfl": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int, _DP, _DP]),
     "dg_get_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
+    "dg_split_volume": (ctypes.c_int, [ctypes.c_void_p]),
+    "dg_split_surface": (ctypes.c_int, [ctypes.c_void_p]),
+    "dg_split_update": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int]),
+    "dg_split_get_r": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
     "dg_nodes": (ctypes.c_int, [ctypes.c_void_p, _DP, _DP]),
     "dg_launch_count": (ctypes.c_ulonglong, [ctypes.c_void_p]),
     "dg_kernel_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_longlong)]),
@@ -229,6 +233,37 @@ class DG:
         with self._torch.cuda.device(self.device):
             self._check(self.lib.dg_rk_step_cfl(self._h, float(cfl), int(nsteps), ctypes.byref(t), ctypes.byref(dt)))
         return t.value, dt.value
+
+    # -- paper-shaped per-kernel mode (Table II breakdown) ------------------------------------------
+    def split_volume(self):
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.dg_split_volume(self._h))
+        return self
+
+    def split_surface(self):
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.dg_split_surface(self._h))
+        return self
+
+    def split_update(self, dt, stage):
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.dg_split_update(self._h, float(dt), int(stage)))
+        return self
+
+    def split_r(self, out=None):
+        if out is None:
+            out = np.empty(self.shape)
+        ptr, dev, _ = self._ptr(out, True)
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.dg_split_get_r(self._h, ptr, dev))
+        return out
+
+    def rk_step_split(self, dt, nsteps=1):
+        """nsteps LSERK45 steps as 5 x (volume, surface, update-project) launches."""
+        for _ in range(int(nsteps)):
+            for stage in range(5):
+                self.split_volume().split_surface().split_update(dt, stage)
+        return self
 
     def get_state(self, out=None):
         if out is None:

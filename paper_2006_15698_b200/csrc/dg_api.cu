@@ -135,6 +135,17 @@ __global__ void __launch_bounds__(256) dg_fp64_peak_kernel(double *out, int iter
     out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
 }
 
+// "Update" half of the paper's update-project kernel: K = A K + dt R, Q = Q + B K over the internal
+// vectors (padding included: it stays zero); the "project" half is the face-trace kernel launched right after.
+__global__ void __launch_bounds__(256) dg_split_update_kernel(double *Q, double *K, const double *R, size_t n, double rkA,
+                                                              double rkB, double dt) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const double k = (rkA == 0.0) ? dt * R[i] : fma(rkA, K[i], dt * R[i]);
+        K[i] = k;
+        Q[i] = fma(rkB, k, Q[i]);
+    }
+}
+
 __global__ void dg_fastmath_kernel(const double *x, double *r, double *q, size_t n) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) {
@@ -228,7 +239,7 @@ Carve carve(const dg_ctx *c) {
     size_t off = 0;
     v.q = off;    off += align_up(c->int_len * 8 + 16, 256);   // +16: the L2 prefetch rounds out to 16-byte granules
     v.k = off;    off += align_up(c->int_len * 8 + 16, 256);
-    v.s = off;    off += align_up(c->state_len * 8, 256);
+    v.s = off;    off += align_up((c->int_len > c->state_len ? c->int_len : c->state_len) * 8, 256);   // staging / split-mode R
     v.txy0 = off; off += align_up(c->txy_len * 8 + 16, 256);
     v.txy1 = off; off += align_up(c->txy_len * 8 + 16, 256);
     v.tz0 = off;  off += align_up(c->tz_len * 8, 256);
@@ -304,6 +315,36 @@ int enqueue_step(dg_ctx *c, double dt, bool want_lam) {
     }
     c->lam_valid = want_lam;
     return DG_OK;
+}
+
+// face traces of the current Q into buffer 0 (after dg_set_state and after a split-mode update)
+int refresh_traces(dg_ctx *c) {
+    c->tcur = 0;
+    DgTraceArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.Q = c->Q;
+    a.Txy = c->Txy[0];
+    a.Tz = c->Tz[0];
+    a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
+    a.nbx = c->nbx; a.nby = c->nby;
+    a.lz = c->lz; a.nchunks = c->nchunks;
+    cudaError_t e = c->kt->launch_traces(a, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "trace kernel");
+    c->launches++;
+    return DG_OK;
+}
+
+DgSplitArgs split_args(const dg_ctx *c) {
+    DgSplitArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.Q = c->Q;
+    a.R = c->S;
+    a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
+    a.nbx = c->nbx; a.nby = c->nby;
+    a.gamma = c->gamma;
+    a.gm1 = c->gamma - 1.0;
+    for (int i = 0; i < 3; ++i) a.scale[i] = c->g[i];
+    return a;
 }
 
 int read_lam(dg_ctx *c, double *lam_host) {
@@ -471,19 +512,8 @@ int dg_set_state(dg_ctx *c, const double *q, int on_device) {
     }
     int rc = launch_layout(c, c->Q, const_cast<double *>(src), 1);
     if (rc != DG_OK) return rc;
-    // traces of the new state into buffer 0
-    c->tcur = 0;
-    DgTraceArgs a;
-    std::memset(&a, 0, sizeof(a));
-    a.Q = c->Q;
-    a.Txy = c->Txy[0];
-    a.Tz = c->Tz[0];
-    a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
-    a.nbx = c->nbx; a.nby = c->nby;
-    a.lz = c->lz; a.nchunks = c->nchunks;
-    cudaError_t e = c->kt->launch_traces(a, c->stream);
-    if (e != cudaSuccess) return cuda_fail(c, e, "trace kernel");
-    c->launches++;
+    rc = refresh_traces(c);
+    if (rc != DG_OK) return rc;
     c->has_state = true;
     c->lam_valid = false;
     return DG_OK;
@@ -536,6 +566,51 @@ int dg_rk_step_cfl(dg_ctx *c, double cfl, int nsteps, double *t_advanced, double
     }
     if (t_advanced) *t_advanced = t;
     if (dt_last) *dt_last = dt;
+    return DG_OK;
+}
+
+int dg_split_volume(dg_ctx *c) {
+    if (!c) return DG_EINVAL;
+    if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_split_volume needs dg_bind and dg_set_state first");
+    cudaError_t e = c->kt->launch_split_volume(split_args(c), c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "volume kernel");
+    c->launches++;
+    return DG_OK;
+}
+
+int dg_split_surface(dg_ctx *c) {
+    if (!c) return DG_EINVAL;
+    if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_split_surface needs dg_bind and dg_set_state first");
+    cudaError_t e = c->kt->launch_split_surface(split_args(c), c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "surface kernel");
+    c->launches++;
+    return DG_OK;
+}
+
+int dg_split_update(dg_ctx *c, double dt, int stage) {
+    if (!c) return DG_EINVAL;
+    if (stage < 0 || stage > 4 || !std::isfinite(dt)) return fail(c, DG_EINVAL, "stage outside 0..4 or dt not finite");
+    if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_split_update needs dg_bind and dg_set_state first");
+    const size_t want = (c->int_len + 255) / 256, cap = (size_t)(c->sms > 0 ? c->sms : 1) * 16u;
+    dg_split_update_kernel<<<(unsigned)(want < cap ? want : cap), 256, 0, c->stream>>>(
+        c->Q, c->K, c->S, c->int_len, (double)kRkA[stage], (double)kRkB[stage], dt);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, "update kernel");
+    c->launches++;
+    c->lam_valid = false;
+    return refresh_traces(c);   // "project": face traces of the updated state, so that the fused path can go on
+}
+
+int dg_split_get_r(dg_ctx *c, double *r_out, int on_device) {
+    if (!c || !r_out) return c ? fail(c, DG_EINVAL, "null pointer") : DG_EINVAL;
+    if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_split_get_r needs dg_bind and dg_set_state first");
+    if (on_device) return launch_layout(c, c->S, r_out, 0);
+    // host: R lives in the staging vector itself, so the canonical copy goes through the K array (dead between steps)
+    int rc = launch_layout(c, c->S, c->K, 0);
+    if (rc != DG_OK) return rc;
+    cudaError_t e = cudaMemcpyAsync(r_out, c->K, c->state_len * 8, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "device->host copy of the residual");
     return DG_OK;
 }
 

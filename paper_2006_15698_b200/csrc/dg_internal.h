@@ -76,6 +76,15 @@ struct DgTraceArgs {
     int nx, ny, nz, nbx, nby, lz, nchunks;
 };
 
+// Arguments of the paper-shaped per-kernel mode (Table II): volume and surface kernels.
+struct DgSplitArgs {
+    const double *Q;
+    double *R;            // residual accumulator, internal layout (volume kernel overwrites it, surface kernel adds)
+    int nx, ny, nz, nbx, nby;
+    double gamma, gm1;
+    double scale[3];      // 2/h_a per axis
+};
+
 struct DgLayoutArgs {
     double *internal;
     double *canonical;      // [e][k][j][i][n]
@@ -104,6 +113,8 @@ struct DgKernelTable {
     cudaError_t (*prepare)(const DgRefOps &ref, int *blocks_per_sm);
     cudaError_t (*launch_stage)(const DgStageArgs &a, cudaStream_t s);
     cudaError_t (*launch_traces)(const DgTraceArgs &a, cudaStream_t s);
+    cudaError_t (*launch_split_volume)(const DgSplitArgs &a, cudaStream_t s);
+    cudaError_t (*launch_split_surface)(const DgSplitArgs &a, cudaStream_t s);
     cudaError_t (*launch_layout)(const DgLayoutArgs &a, int sms, cudaStream_t s);
     cudaError_t (*launch_wavespeed)(const DgWaveArgs &a, int sms, cudaStream_t s);
 };

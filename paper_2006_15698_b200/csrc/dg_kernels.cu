@@ -30,6 +30,8 @@
 
 #include <stdint.h>
 
+#include <type_traits>
+
 #ifndef DG_N
 #error "compile with -DDG_N=<p+1>"
 #endif
@@ -835,6 +837,150 @@ __global__ void __launch_bounds__(C::NCOMP) dg_traces_kernel(const __grid_consta
 }
 
 // ------------------------------------------------------------------------------------------------
+// paper-shaped per-kernel mode (Table II): the volume kernel (K1) and the
+// surface kernel (K2) as launches of their own over the same layout; one block per layer slot, one thread per
+// node line and axis.  Not the hot path: it exists to print the paper's per-kernel breakdown next to the fused
+// step and is parity-tested against the oracle's volume and surface terms.
+// ------------------------------------------------------------------------------------------------
+template <class C>
+__device__ __forceinline__ void stage_layer_in(double *smem_dst, const double *gsrc, int tid) {
+    for (int idx = tid; idx < C::NPL * C::HP; idx += C::NCOMP) smem_dst[idx] = gsrc[idx];
+}
+
+// R <- sum over the axes of (2/h_a) sum_q Dhat_iq F^a_q   (eq (5) 2nd term / mass; overwrites R like the listing)
+template <class C>
+__global__ void __launch_bounds__(C::NCOMP) dg_split_volume_kernel(const __grid_constant__ DgSplitArgs a) {
+    constexpr int NV = DG_NV, N = C::N, PLANE = C::PLANE;
+    extern __shared__ __align__(128) double smem[];
+    double *Qs = smem, *Rs = smem + C::BUF;
+    const int tid = threadIdx.x, bxi = blockIdx.x, byi = blockIdx.y, ez = blockIdx.z;
+    const size_t slot = ((size_t)ez * a.nby + byi) * a.nbx + bxi;
+    stage_layer_in<C>(Qs, a.Q + slot * C::SLOT, tid);
+    __syncthreads();
+    const int ext0 = min(C::BX, a.nx - bxi * C::BX), ext1 = min(C::BY, a.ny - byi * C::BY);
+    const int lx = min(tid, C::L - 1);
+    const bool inL = tid < C::L;
+    auto axis = [&](auto AXT) {
+        constexpr int AX = decltype(AXT)::value;
+        using A = Axis<C, AX>;
+        const Geo g = make_geo<C, AX>(lx);
+        const bool act = inL && line_inside<C, AX>(g, ext0, ext1);
+        double V[NV][N];
+#pragma unroll
+        for (int q = 0; q < N; ++q) {
+            double Qn[NV], F[NV], vel, pres, rinv;
+#pragma unroll
+            for (int s = 0; s < NV; ++s) Qn[s] = Qs[g.base + var_of_slot<C, AX>(s) * PLANE + q * A::S];
+            euler_flux_normal(Qn, a.gm1, F, vel, pres, rinv);
+#pragma unroll
+            for (int n = 0; n < NV; ++n)
+#pragma unroll
+                for (int i = 0; i < N; ++i) V[n][i] = (q == 0) ? c_ref.D[q][i] * F[n] : fma(c_ref.D[q][i], F[n], V[n][i]);
+        }
+        if (act) {
+#pragma unroll
+            for (int s = 0; s < NV; ++s)
+#pragma unroll
+                for (int i = 0; i < N; ++i) {
+                    double *p = Rs + g.base + var_of_slot<C, AX>(s) * PLANE + i * A::S;
+                    *p = (AX == 0) ? a.scale[AX] * V[s][i] : fma(a.scale[AX], V[s][i], *p);
+                }
+        }
+        __syncthreads();
+    };
+    axis(std::integral_constant<int, 0>{});
+    axis(std::integral_constant<int, 1>{});
+    axis(std::integral_constant<int, 2>{});
+    double *dst = a.R + slot * C::SLOT;
+    for (int idx = tid; idx < C::NPL * C::HP; idx += C::NCOMP) dst[idx] = Rs[idx];
+}
+
+// Trace of the line through node (j, k transverse) of element (ex, ey, ez) along axis AX, at its + or - end,
+// read from the state in HBM (any element of the mesh; periodic wrap by the caller), slots rotated for AX.
+template <class C, int AX>
+__device__ __forceinline__ void global_line_trace(const DgSplitArgs &a, int ex, int ey, int ez, int t1, int t2, bool plus,
+                                                  double (&T)[DG_NV]) {
+    constexpr int N = C::N;
+    const int bxi = ex / C::BX, byi = ey / C::BY;
+    const int lx = ex - bxi * C::BX, ly = ey - byi * C::BY;
+    const double *src = a.Q + (((size_t)ez * a.nby + byi) * a.nbx + bxi) * C::SLOT;
+    // (t1, t2) are node indices INSIDE the element here: x lines (j, k), y lines (i, k), z lines (i, j)
+    int base, stride;
+    if (AX == 0) { base = t2 * C::HP + (ly * N + t1) * C::GX + lx * N; stride = 1; }
+    else if (AX == 1) { base = t2 * C::HP + (ly * N) * C::GX + lx * N + t1; stride = C::GX; }
+    else { base = (ly * N + t2) * C::GX + lx * N + t1; stride = C::HP; }
+#pragma unroll
+    for (int s = 0; s < DG_NV; ++s) {
+        double t = 0.0;
+        const double *p = src + var_of_slot<C, AX>(s) * (N * C::HP) + base;
+#pragma unroll
+        for (int q = 0; q < N; ++q) t = fma(plus ? DG_LP(q) : DG_LM(q), __ldg(p + q * stride), t);
+        T[s] = t;
+    }
+}
+
+// R += -(2/h_a) (l_i(+1) F*_+ - l_i(-1) F*_-)/w_i for the three axes: every line evaluates the local Lax-Friedrichs
+// flux at both of its ends from its own traces and the two neighbour elements' (eq (5) 3rd term / mass)
+template <class C>
+__global__ void __launch_bounds__(C::NCOMP) dg_split_surface_kernel(const __grid_constant__ DgSplitArgs a) {
+    constexpr int NV = DG_NV, N = C::N, PLANE = C::PLANE;
+    extern __shared__ __align__(128) double smem[];
+    double *Qs = smem, *Rs = smem + C::BUF;
+    const int tid = threadIdx.x, bxi = blockIdx.x, byi = blockIdx.y, ez = blockIdx.z;
+    const size_t slot = ((size_t)ez * a.nby + byi) * a.nbx + bxi;
+    stage_layer_in<C>(Qs, a.Q + slot * C::SLOT, tid);
+    stage_layer_in<C>(Rs, a.R + slot * C::SLOT, tid);
+    __syncthreads();
+    const int ext0 = min(C::BX, a.nx - bxi * C::BX), ext1 = min(C::BY, a.ny - byi * C::BY);
+    const int lx = min(tid, C::L - 1);
+    const bool inL = tid < C::L;
+    auto axis = [&](auto AXT) {
+        constexpr int AX = decltype(AXT)::value;
+        using A = Axis<C, AX>;
+        const Geo g = make_geo<C, AX>(lx);
+        const bool act = inL && line_inside<C, AX>(g, ext0, ext1);
+        if (act) {
+            double Tp[NV], Tm[NV], Hlo[NV], Hhi[NV], Fp[NV], Fm[NV];
+#pragma unroll
+            for (int s = 0; s < NV; ++s) {
+                Tp[s] = Tm[s] = 0.0;
+#pragma unroll
+                for (int q = 0; q < N; ++q) {
+                    const double Qv = Qs[g.base + var_of_slot<C, AX>(s) * PLANE + q * A::S];
+                    Tp[s] = fma(DG_LP(q), Qv, Tp[s]);
+                    Tm[s] = fma(DG_LM(q), Qv, Tm[s]);
+                }
+            }
+            // this line's element and its two neighbours along AX (periodic), node indices in the element
+            int ex = bxi * C::BX, ey = byi * C::BY, e2 = ez, n1, n2;
+            if (AX == 0) { ex += g.e; ey += g.t1 / N; n1 = g.t1 % N; n2 = g.t2; }
+            else if (AX == 1) { ey += g.e; ex += g.t1 / N; n1 = g.t1 % N; n2 = g.t2; }
+            else { ex += g.t1 / N; ey += g.t2 / N; n1 = g.t1 % N; n2 = g.t2 % N; }
+            const int na = (AX == 0) ? a.nx : (AX == 1) ? a.ny : a.nz;
+            const int ea = (AX == 0) ? ex : (AX == 1) ? ey : e2;
+            const int up = (ea + 1 == na) ? 0 : ea + 1, dn = (ea == 0) ? na - 1 : ea - 1;
+            global_line_trace<C, AX>(a, AX == 0 ? up : ex, AX == 1 ? up : ey, AX == 2 ? up : e2, n1, n2, false, Hhi);
+            global_line_trace<C, AX>(a, AX == 0 ? dn : ex, AX == 1 ? dn : ey, AX == 2 ? dn : e2, n1, n2, true, Hlo);
+            lax_friedrichs2(Tp, Hhi, 1.0, a.gamma, a.gm1, Fp);
+            lax_friedrichs2(Tm, Hlo, -1.0, a.gamma, a.gm1, Fm);
+#pragma unroll
+            for (int s = 0; s < NV; ++s)
+#pragma unroll
+                for (int i = 0; i < N; ++i) {
+                    double *p = Rs + g.base + var_of_slot<C, AX>(s) * PLANE + i * A::S;
+                    *p = fma(a.scale[AX], fma(DG_LQM(i), Fm[s], -DG_LQP(i) * Fp[s]), *p);
+                }
+        }
+        __syncthreads();
+    };
+    axis(std::integral_constant<int, 0>{});
+    axis(std::integral_constant<int, 1>{});
+    axis(std::integral_constant<int, 2>{});
+    double *dst = a.R + slot * C::SLOT;
+    for (int idx = tid; idx < C::NPL * C::HP; idx += C::NCOMP) dst[idx] = Rs[idx];
+}
+
+// ------------------------------------------------------------------------------------------------
 // layout conversion canonical [e][k][j][i][n] <-> internal [slot][n][k][HP: gy, gx]
 // one thread per node; canonical side reads/writes 40 contiguous bytes per thread
 // ------------------------------------------------------------------------------------------------
@@ -915,6 +1061,10 @@ cudaError_t prepare(const DgRefOps &ref, int *blocks_per_sm) {
     opt_in(dg_stage_kernel<C, DG_MODE_RESIDUAL, false>);
     if (err == cudaSuccess)
         err = cudaFuncSetAttribute(dg_traces_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::BUF * 8);
+    if (err == cudaSuccess)
+        err = cudaFuncSetAttribute(dg_split_volume_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * C::BUF * 8);
+    if (err == cudaSuccess)
+        err = cudaFuncSetAttribute(dg_split_surface_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * C::BUF * 8);
     if (err != cudaSuccess) return err;
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, dg_stage_kernel<C, DG_MODE_STAGE, false>,
                                                          C::THREADS, Smem<C>::BYTES);
@@ -933,6 +1083,20 @@ template <class C>
 cudaError_t launch_traces(const DgTraceArgs &a, cudaStream_t s) {
     const dim3 grid((unsigned)a.nbx, (unsigned)a.nby, (unsigned)a.nz);
     dg_traces_kernel<C><<<grid, C::NCOMP, C::BUF * 8, s>>>(a);
+    return cudaGetLastError();
+}
+
+template <class C>
+cudaError_t launch_split_volume(const DgSplitArgs &a, cudaStream_t s) {
+    const dim3 grid((unsigned)a.nbx, (unsigned)a.nby, (unsigned)a.nz);
+    dg_split_volume_kernel<C><<<grid, C::NCOMP, 2 * C::BUF * 8, s>>>(a);
+    return cudaGetLastError();
+}
+
+template <class C>
+cudaError_t launch_split_surface(const DgSplitArgs &a, cudaStream_t s) {
+    const dim3 grid((unsigned)a.nbx, (unsigned)a.nby, (unsigned)a.nz);
+    dg_split_surface_kernel<C><<<grid, C::NCOMP, 2 * C::BUF * 8, s>>>(a);
     return cudaGetLastError();
 }
 
@@ -959,7 +1123,7 @@ cudaError_t launch_wavespeed(const DgWaveArgs &a, int sms, cudaStream_t s) {
 template <class C>
 constexpr DgKernelTable make_table() {
     return DgKernelTable{C::N,       C::BX,          C::BY,         C::THREADS,      Smem<C>::BYTES,     C::SLOT,
-                         C::TXY,     C::TZ,          C::RELOAD ? 1 : 0, C::MINB, &prepare<C>, &launch_stage<C>,  &launch_traces<C>,
+                         C::TXY,     C::TZ,          C::RELOAD ? 1 : 0, C::MINB, &prepare<C>, &launch_stage<C>,  &launch_traces<C>, &launch_split_volume<C>, &launch_split_surface<C>,
                          &launch_layout<C>, &launch_wavespeed<C>};
 }
 
