@@ -95,6 +95,20 @@ void build_ref_ops(int N, DgRefOps &d) {
         d.lq[i] = (double)(0.5L * o.lp[i] / o.w[i]);   // 1/2: the kernel's interface flux is 2 F*
         for (int q = 0; q < N; ++q) d.D[q][i] = (double)(o.w[q] * o.D[q][i] / o.w[i]);
     }
+    // even-odd form (see DgRefOps): Dhat[i][q] = w_q D[q][i] / w_i in long double, then the half sums / differences
+    const int H = N / 2, mid = N / 2;
+    auto Dhat = [&](int i, int q) { return o.w[q] * o.D[q][i] / o.w[i]; };
+    auto lq = [&](int i) { return 0.5L * o.lp[i] / o.w[i]; };
+    for (int q = 0; q < H; ++q) {
+        for (int i = 0; i < H; ++i) d.Pe[q][i] = (double)(0.5L * (Dhat(i, q) + Dhat(i, N - 1 - q)));
+        for (int i = 0; i < H + (N & 1); ++i) d.Po[q][i] = (double)(0.5L * (Dhat(i, q) - Dhat(i, N - 1 - q)));
+    }
+    for (int i = 0; i < H; ++i) {
+        d.Dm[i] = (N & 1) ? (double)Dhat(i, mid) : 0.0;
+        d.ls[i] = (double)(0.5L * (lq(i) + lq(N - 1 - i)));
+        d.la[i] = (double)(0.5L * (lq(N - 1 - i) - lq(i)));
+    }
+    if (N & 1) d.ls[mid] = (double)lq(mid);
 }
 
 // Carpenter-Kennedy (5,4) 2N-storage Runge-Kutta, "LSERK45" (reading R9).

@@ -18,6 +18,15 @@ struct DgRefOps {
     double D[DG_NMAX][DG_NMAX];   // D[q][i] = w_q l_i'(xi_q) / w_i        (eq (5) 2nd term / mass)
     double lq[DG_NMAX];           // 1/2 l_i(+1) / w_i                     (lift / mass; the kernel forms 2 F*)
     double lp[DG_NMAX];           // l_i(+1)                               (face traces)
+    // Even-odd form of the same operators (symmetric nodes: Dhat is centro-antisymmetric, Dhat[N-1-i][N-1-q] = -Dhat[i][q]),
+    // H = N/2, q' = N-1-q, i' = N-1-i; the kernels use it for N >= 5 (N^2/2 + 2N instead of N^2 + 2N operations per line
+    // and variable for derivative + lift):
+    //   r_i = a_i + s_i, r_i' = s_i - a_i,  a_i = sum_{q<H} Pe[q][i] (F_q + F_q') (+ Dm[i] F_mid),  s_i = sum_{q<H} Po[q][i] (F_q - F_q')
+    double Pe[DG_NMAX / 2][DG_NMAX / 2];       // 1/2 (Dhat[i][q] + Dhat[i][q'])
+    double Po[DG_NMAX / 2][DG_NMAX / 2 + 1];   // 1/2 (Dhat[i][q] - Dhat[i][q']), i up to the middle node
+    double Dm[DG_NMAX / 2];                    // Dhat[i][mid] (odd N)
+    double ls[DG_NMAX / 2 + 1];                // lift, even part: 1/2 (lq[i] + lq[i']) (middle node: lq[mid]); multiplies (F*_- - F*_+)
+    double la[DG_NMAX / 2];                    // lift, odd part:  1/2 (lq[i'] - lq[i]);                        multiplies (F*_- + F*_+)
 };
 
 #ifdef __CUDACC__

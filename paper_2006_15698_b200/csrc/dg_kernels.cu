@@ -337,6 +337,81 @@ __device__ __forceinline__ const double *halo_source(const double *T, int nbx, i
     return T + nbr * C::TXY + A::TBASE + (side == 0 ? DG_NV * A::Ca : 0);
 }
 
+// PC + PA for one line: V_i = sum_q Dhat_iq F_q - (l_i(+1) 2F*_+ - l_i(-1) 2F*_-)/(2 w_i), F_q the pointwise Euler flux
+// of the line's node q (loadQ(q, Qn) delivers its state, slots rotated).  N >= 5: even-odd form (DgRefOps): the
+// nodes are taken in mirror pairs, half-size operators act on the sum and the difference of the pair's fluxes.
+template <class C, class LoadQ>
+__device__ __forceinline__ void lift_and_volume(LoadQ loadQ, double gm1, const double (&Fm)[DG_NV], const double (&Fp)[DG_NV],
+                                                double (&V)[DG_NV][C::N]) {
+    constexpr int N = C::N, NV = DG_NV;
+    if constexpr (N < 5) {
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            const double cp = DG_LQP(i), cm = DG_LQM(i);
+#pragma unroll
+            for (int n = 0; n < NV; ++n) V[n][i] = fma(cm, Fm[n], -cp * Fp[n]);
+        }
+#pragma unroll
+        for (int q = 0; q < N; ++q) {
+            double Qn[NV], F[NV], vel, pres, rinv;
+            loadQ(q, Qn);
+            euler_flux_normal(Qn, gm1, F, vel, pres, rinv);
+#pragma unroll
+            for (int n = 0; n < NV; ++n)
+#pragma unroll
+                for (int i = 0; i < N; ++i) V[n][i] = fma(c_ref.D[q][i], F[n], V[n][i]);
+        }
+    } else {
+        constexpr int H = N / 2, ODD = N & 1, MID = N / 2;
+        double A[NV][H], S[NV][H + ODD];
+        // lift: L_i + L_i' = (lq_i + lq_i')(F*_- - F*_+),  L_i - L_i' = (lq_i' - lq_i)(F*_- + F*_+)   (halved in the tables)
+#pragma unroll
+        for (int n = 0; n < NV; ++n) {
+            const double fd = Fm[n] - Fp[n], fs = Fm[n] + Fp[n];
+#pragma unroll
+            for (int i = 0; i < H; ++i) {
+                S[n][i] = c_ref.ls[i] * fd;
+                A[n][i] = c_ref.la[i] * fs;
+            }
+            if (ODD) S[n][ODD ? MID : 0] = c_ref.ls[MID] * fd;
+        }
+#pragma unroll
+        for (int q = 0; q < H; ++q) {
+            double Qa[NV], Qb[NV], Fa[NV], Fb[NV], vel, pres, rinv;
+            loadQ(q, Qa);
+            loadQ(N - 1 - q, Qb);
+            euler_flux_normal(Qa, gm1, Fa, vel, pres, rinv);
+            euler_flux_normal(Qb, gm1, Fb, vel, pres, rinv);
+#pragma unroll
+            for (int n = 0; n < NV; ++n) {
+                const double fe = Fa[n] + Fb[n], fo = Fa[n] - Fb[n];
+#pragma unroll
+                for (int i = 0; i < H; ++i) A[n][i] = fma(c_ref.Pe[q][i], fe, A[n][i]);
+#pragma unroll
+                for (int i = 0; i < H + ODD; ++i) S[n][i] = fma(c_ref.Po[q][i], fo, S[n][i]);
+            }
+        }
+        if (ODD) {
+            double Qc[NV], Fc[NV], vel, pres, rinv;
+            loadQ(MID, Qc);
+            euler_flux_normal(Qc, gm1, Fc, vel, pres, rinv);
+#pragma unroll
+            for (int n = 0; n < NV; ++n)
+#pragma unroll
+                for (int i = 0; i < H; ++i) A[n][i] = fma(c_ref.Dm[i], Fc[n], A[n][i]);
+        }
+#pragma unroll
+        for (int n = 0; n < NV; ++n) {
+#pragma unroll
+            for (int i = 0; i < H; ++i) {
+                V[n][i] = S[n][i] + A[n][i];
+                V[n][N - 1 - i] = S[n][i] - A[n][i];
+            }
+            if (ODD) V[n][MID] = S[n][ODD ? MID : 0];
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // the x and y passes of one layer
 // ------------------------------------------------------------------------------------------------
@@ -416,27 +491,15 @@ __device__ __forceinline__ void xy_pass(const BlockInfo *bi, const Geo &g, bool 
         lax_friedrichs2(Tm, Hlo, -1.0, gamma, gm1, Fm);
     }
 
-    // ------------- PC: lift (1/w folded into the table) starts the accumulators -----------------------
+    // ------------- PC + PA: lift, pointwise flux and sum-factorised derivative -------------------------------
     double V[NV][N];
+    lift_and_volume<C>(
+        [&](int q, double(&Qn)[NV]) {
 #pragma unroll
-    for (int i = 0; i < N; ++i) {
-        const double cp = DG_LQP(i), cm = DG_LQM(i);
-#pragma unroll
-        for (int n = 0; n < NV; ++n) V[n][i] = fma(cm, Fm[n], -cp * Fp[n]);
-    }
-    // ------------- PA: pointwise flux and sum-factorised derivative --------------------------------
-#pragma unroll
-    for (int q = 0; q < N; ++q) {
-        double Qn[NV], F[NV], vel, pres, rinv;
-#pragma unroll
-        for (int s = 0; s < NV; ++s)
-            Qn[s] = C::RELOAD ? Q0[var_of_slot<C, AX>(s) * PLANE + q * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : q];
-        euler_flux_normal(Qn, gm1, F, vel, pres, rinv);
-#pragma unroll
-        for (int n = 0; n < NV; ++n)
-#pragma unroll
-            for (int i = 0; i < N; ++i) V[n][i] = fma(c_ref.D[q][i], F[n], V[n][i]);
-    }
+            for (int s = 0; s < NV; ++s)
+                Qn[s] = C::RELOAD ? Q0[var_of_slot<C, AX>(s) * PLANE + q * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : q];
+        },
+        gm1, Fm, Fp, V);
     // ------------- PD: Runge-Kutta accumulation on the staged K -----------------------------------------
     if (AX == 0) {
         if (bi->readK) mbar_wait(fullk, kparity);   // this layer's K has landed in KR
@@ -538,26 +601,14 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
 #pragma unroll
         for (int n = 0; n < NV; ++n) FmS[n * L + l] = Fp[n];   // the next layer's lower face (same thread reads it)
     }
-    // PC
+    // PC + PA
+    lift_and_volume<C>(
+        [&](int q, double(&Qn)[NV]) {
 #pragma unroll
-    for (int i = 0; i < N; ++i) {
-        const double cp = DG_LQP(i), cm = DG_LQM(i);
-#pragma unroll
-        for (int n = 0; n < NV; ++n) V[n][i] = fma(cm, Fm[n], -cp * Fp[n]);
-    }
-    // PA
-#pragma unroll
-    for (int q = 0; q < N; ++q) {
-        double Qn[NV], F[NV], vel, pres, rinv;
-#pragma unroll
-        for (int s = 0; s < NV; ++s)
-            Qn[s] = C::RELOAD ? Q0[var_of_slot<C, AX>(s) * PLANE + q * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : q];
-        euler_flux_normal(Qn, gm1, F, vel, pres, rinv);
-#pragma unroll
-        for (int n = 0; n < NV; ++n)
-#pragma unroll
-            for (int i = 0; i < N; ++i) V[n][i] = fma(c_ref.D[q][i], F[n], V[n][i]);
-    }
+            for (int s = 0; s < NV; ++s)
+                Qn[s] = C::RELOAD ? Q0[var_of_slot<C, AX>(s) * PLANE + q * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : q];
+        },
+        gm1, Fm, Fp, V);
     bar_sync<C::NCOMP>(1);   // the y pass of every line is done with K (and, RELOAD, with Q)
     if (act) {
         // PD: the updated K (or R) goes straight to HBM from the z lines (coalesced across the lanes, streaming),
