@@ -30,6 +30,9 @@ def _load(variant):
         for f in (lib.oracle_volume_term, lib.oracle_surface_term, lib.oracle_residual):
             f.argtypes = mesh + [_DP, _DP]
         lib.oracle_rk_step.argtypes = mesh + [_DP, ctypes.c_double, ctypes.c_int]
+        _IP = ctypes.POINTER(ctypes.c_int)
+        lib.oracle_residual_bc.argtypes = mesh + [_IP, _DP, _DP, _DP]
+        lib.oracle_rk_step_bc.argtypes = mesh + [_IP, _DP, _DP, ctypes.c_double, ctypes.c_int]
         lib.oracle_max_wavespeed.argtypes = [ctypes.c_int] * 4 + [ctypes.c_double, _DP, _DP]
         _LIBS[name] = lib
     return _LIBS[name]
@@ -110,6 +113,30 @@ class Oracle:
         ext = np.asarray(extent, dtype=np.float64)
         _check(self.lib.oracle_rk_step(nx, ny, nz, p, float(gamma), _p(ext), _p(q), float(dt), int(nsteps)),
                "rk_step")
+        return q
+
+    @staticmethod
+    def _bc(bc, qinf):
+        b = (ctypes.c_int * 6)(*[int(v) for v in bc])
+        qi = np.ascontiguousarray(qinf if qinf is not None else np.zeros(5), dtype=np.float64)
+        return b, qi
+
+    def residual_bc(self, q, p, gamma, extent, bc, qinf=None):
+        """dQ/dt with non-periodic faces: bc = (x-, x+, y-, y+, z-, z+), 0 periodic, 1 slip wall, 2 far field."""
+        q, nx, ny, nz = self._mesh(q, p)
+        ext = np.asarray(extent, dtype=np.float64)
+        b, qi = self._bc(bc, qinf)
+        r = np.empty_like(q)
+        _check(self.lib.oracle_residual_bc(nx, ny, nz, p, float(gamma), _p(ext), b, _p(qi), _p(q), _p(r)), "residual_bc")
+        return r
+
+    def rk_step_bc(self, q, p, gamma, extent, bc, qinf, dt, nsteps):
+        q, nx, ny, nz = self._mesh(q, p)
+        q = q.copy()
+        ext = np.asarray(extent, dtype=np.float64)
+        b, qi = self._bc(bc, qinf)
+        _check(self.lib.oracle_rk_step_bc(nx, ny, nz, p, float(gamma), _p(ext), b, _p(qi), _p(q), float(dt), int(nsteps)),
+               "rk_step_bc")
         return q
 
     def max_wavespeed(self, q, p, gamma):

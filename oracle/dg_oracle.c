@@ -167,6 +167,10 @@ typedef struct {
     real g[3];              /* 2/h_a: constant geometric factor per axis  PAPER.md:31, 143 (`vgeo`) */
     real Dhat[NMAX * NMAX]; /* Dhat[i*N+q] = w_q l_i'(xi_q) / w_i */
     real lp[NMAX], lm[NMAX], w[NMAX];
+    /* boundary condition of the six domain faces x-, x+, y-, y+, z-, z+ (reading R19; the paper's benchmark is
+     * periodic, and gives no other condition): 0 periodic, 1 slip wall, 2 far field (state qinf) */
+    int bc[6];
+    real qinf[NV];
 } disc;
 
 static int disc_init(disc *d, int nx, int ny, int nz, int p, double gamma,
@@ -191,7 +195,32 @@ static int disc_init(disc *d, int nx, int ny, int nz, int p, double gamma,
         d->w[i] = (real)w[i];
         for (int q = 0; q < N; ++q) d->Dhat[i * N + q] = (real)(w[q] * D[q * N + i] / w[i]);
     }
+    for (int f = 0; f < 6; ++f) d->bc[f] = 0;
+    for (int n = 0; n < NV; ++n) d->qinf[n] = 0;
     return 0;
+}
+
+/* Non-periodic faces.  Periodicity is a property of an axis: both of its faces or neither. */
+static int disc_set_bc(disc *d, const int bc[6], const double qinf[NV]) {
+    if (!bc) return 0;
+    for (int a = 0; a < 3; ++a) {
+        const int lo = bc[2 * a], hi = bc[2 * a + 1];
+        if (lo < 0 || lo > 2 || hi < 0 || hi > 2 || ((lo == 0) != (hi == 0))) return 1;
+        if ((lo == 2 || hi == 2) && !qinf) return 1;
+        d->bc[2 * a] = lo;
+        d->bc[2 * a + 1] = hi;
+    }
+    if (qinf)
+        for (int n = 0; n < NV; ++n) d->qinf[n] = (real)qinf[n];
+    return 0;
+}
+
+/* Exterior (ghost) state of a boundary face from the interior trace Q (reading R19): slip wall = the interior state
+ * with the face-normal momentum component negated (zero mass flux through the wall by symmetry of the interface flux);
+ * far field = the prescribed state. */
+static void ghost_state(const disc *d, int kind, int axis, const real Q[NV], real G[NV]) {
+    for (int n = 0; n < NV; ++n) G[n] = (kind == 2) ? d->qinf[n] : Q[n];
+    if (kind == 1) G[1 + axis] = -Q[1 + axis];
 }
 
 /* canonical index of variable 0 at node (i,j,k) of element e */
@@ -327,7 +356,10 @@ static void surface_term(const disc *d, const real *q, real *S) {
                 }
     }
 
-    /* step 3: interface flux at the + face of every element along every axis */
+    /* step 3: interface flux at the + face of every element along every axis; on a non-periodic axis the + face of
+     * the last element takes the ghost state as right state, and the - face of the first element (ghost state on the
+     * left) goes to the extra array Flo[axis][face slot of the boundary element] */
+    real *Flo = (real *)malloc(sizeof(real) * d->nelem * per_elem);   /* only boundary elements' entries are used */
 #ifdef _OPENMP
 #pragma omp parallel for
 #endif
@@ -337,12 +369,20 @@ static void surface_term(const disc *d, const real *q, real *S) {
         const int ey = (int)((e / (size_t)d->nx) % (size_t)d->ny);
         const int ez = (int)(e / ((size_t)d->nx * d->ny));
         for (int a = 0; a < 3; ++a) {
+            const int ea = (a == 0) ? ex : (a == 1) ? ey : ez;
+            const int na = (a == 0) ? d->nx : (a == 1) ? d->ny : d->nz;
             const size_t en = (a == 0)   ? eidx(d, (ex + 1) % d->nx, ey, ez)
                               : (a == 1) ? eidx(d, ex, (ey + 1) % d->ny, ez)
                                          : eidx(d, ex, ey, (ez + 1) % d->nz);
+            const int bhi = (ea == na - 1) ? d->bc[2 * a + 1] : 0, blo = (ea == 0) ? d->bc[2 * a] : 0;
             for (size_t f = 0; f < nf; ++f) {
                 const real *QL = Tp + e * per_elem + (a * nf + f) * NV;
                 const real *QR = Tm + en * per_elem + (a * nf + f) * NV;
+                real ghost[NV];
+                if (bhi) {
+                    ghost_state(d, bhi, a, QL, ghost);
+                    QR = ghost;
+                }
                 real *Fst = Fs + e * per_elem + (a * nf + f) * NV;
                 real FL[NV], FR[NV], uL, uR, cL, cR;
                 euler_flux(d, QL, a, FL, &uL, &cL);
@@ -352,6 +392,19 @@ static void surface_term(const disc *d, const real *q, real *S) {
                 const real lam = (lamL > lamR) ? lamL : lamR;
                 for (int n = 0; n < NV; ++n)
                     Fst[n] = (real)0.5 * (FL[n] + FR[n]) - (real)0.5 * lam * (QR[n] - QL[n]);
+                if (blo) {   /* - face of a first element: left state = ghost of the own T-, right state = own T- */
+                    const real *Qr = Tm + e * per_elem + (a * nf + f) * NV;
+                    real Ql[NV];
+                    ghost_state(d, blo, a, Qr, Ql);
+                    real *Fb = Flo + e * per_elem + (a * nf + f) * NV;
+                    euler_flux(d, Ql, a, FL, &uL, &cL);
+                    euler_flux(d, Qr, a, FR, &uR, &cR);
+                    const real lamL2 = R_FABS(uL) + cL;
+                    const real lamR2 = R_FABS(uR) + cR;
+                    const real lam2 = (lamL2 > lamR2) ? lamL2 : lamR2;
+                    for (int n = 0; n < NV; ++n)
+                        Fb[n] = (real)0.5 * (FL[n] + FR[n]) - (real)0.5 * lam2 * (Qr[n] - Ql[n]);
+                }
             }
         }
     }
@@ -368,6 +421,7 @@ static void surface_term(const disc *d, const real *q, real *S) {
         const size_t em[3] = {eidx(d, (ex + d->nx - 1) % d->nx, ey, ez),
                               eidx(d, ex, (ey + d->ny - 1) % d->ny, ez),
                               eidx(d, ex, ey, (ez + d->nz - 1) % d->nz)};
+        const int at_lo[3] = {ex == 0 && d->bc[0], ey == 0 && d->bc[2], ez == 0 && d->bc[4]};
         for (int k = 0; k < N; ++k)
             for (int j = 0; j < N; ++j)
                 for (int i = 0; i < N; ++i) {
@@ -378,7 +432,8 @@ static void surface_term(const disc *d, const real *q, real *S) {
                         real acc = 0;
                         for (int a = 0; a < 3; ++a) {
                             const real Fplus = Fs[e * per_elem + (a * nf + f[a]) * NV + n];
-                            const real Fminus = Fs[em[a] * per_elem + (a * nf + f[a]) * NV + n];
+                            const real Fminus = at_lo[a] ? Flo[e * per_elem + (a * nf + f[a]) * NV + n]
+                                                         : Fs[em[a] * per_elem + (a * nf + f[a]) * NV + n];
                             acc += d->g[a] *
                                    ((d->lp[s[a]] * Fplus - d->lm[s[a]] * Fminus) / d->w[s[a]]);
                         }
@@ -386,6 +441,7 @@ static void surface_term(const disc *d, const real *q, real *S) {
                     }
                 }
     }
+    free(Flo);
     free(Tp);
     free(Tm);
     free(Fs);
@@ -410,9 +466,9 @@ static void to_double(const real *y, double *x, size_t len) {
 }
 
 static int run_term(int which, int nx, int ny, int nz, int p, double gamma,
-                    const double extent[3], const double *q, double *r) {
+                    const double extent[3], const int bc[6], const double qinf[NV], const double *q, double *r) {
     disc d;
-    if (!q || !r || disc_init(&d, nx, ny, nz, p, gamma, extent)) return 1;
+    if (!q || !r || disc_init(&d, nx, ny, nz, p, gamma, extent) || disc_set_bc(&d, bc, qinf)) return 1;
     const size_t len = d.nelem * d.nnode * NV;
     real *qq = to_real(q, len);
     real *rr = (real *)malloc(sizeof(real) * len);
@@ -431,15 +487,19 @@ static int run_term(int which, int nx, int ny, int nz, int p, double gamma,
 
 int oracle_volume_term(int nx, int ny, int nz, int p, double gamma, const double extent[3],
                        const double *q, double *r) {
-    return run_term(0, nx, ny, nz, p, gamma, extent, q, r);
+    return run_term(0, nx, ny, nz, p, gamma, extent, NULL, NULL, q, r);
 }
 int oracle_surface_term(int nx, int ny, int nz, int p, double gamma, const double extent[3],
                         const double *q, double *r) {
-    return run_term(1, nx, ny, nz, p, gamma, extent, q, r);
+    return run_term(1, nx, ny, nz, p, gamma, extent, NULL, NULL, q, r);
 }
 int oracle_residual(int nx, int ny, int nz, int p, double gamma, const double extent[3],
                     const double *q, double *r) {
-    return run_term(2, nx, ny, nz, p, gamma, extent, q, r);
+    return run_term(2, nx, ny, nz, p, gamma, extent, NULL, NULL, q, r);
+}
+int oracle_residual_bc(int nx, int ny, int nz, int p, double gamma, const double extent[3], const int bc[6],
+                       const double qinf[5], const double *q, double *r) {
+    return run_term(2, nx, ny, nz, p, gamma, extent, bc, qinf, q, r);
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -470,8 +530,13 @@ void oracle_lserk45(double A[5], double B[5]) {
 
 int oracle_rk_step(int nx, int ny, int nz, int p, double gamma, const double extent[3],
                    double *q, double dt, int nsteps) {
+    return oracle_rk_step_bc(nx, ny, nz, p, gamma, extent, NULL, NULL, q, dt, nsteps);
+}
+
+int oracle_rk_step_bc(int nx, int ny, int nz, int p, double gamma, const double extent[3], const int bc[6],
+                      const double qinf[5], double *q, double dt, int nsteps) {
     disc d;
-    if (!q || nsteps < 0 || disc_init(&d, nx, ny, nz, p, gamma, extent)) return 1;
+    if (!q || nsteps < 0 || disc_init(&d, nx, ny, nz, p, gamma, extent) || disc_set_bc(&d, bc, qinf)) return 1;
     const size_t len = d.nelem * d.nnode * NV;
     real *Q = to_real(q, len);
     real *K = (real *)malloc(sizeof(real) * len);

@@ -58,6 +58,15 @@ int oracle_residual(int nx, int ny, int nz, int p, double gamma, const double ex
 int oracle_rk_step(int nx, int ny, int nz, int p, double gamma, const double extent[3],
                    double *q, double dt, int nsteps);
 
+/* The same two with non-periodic domain faces (the paper gives no boundary condition, PAPER.md:126
+ * "periodic domain": DESIGN.md reading R19).  bc[6] = condition of the faces x-, x+, y-, y+, z-, z+: 0 periodic (both
+ * faces of an axis or neither), 1 slip wall (exterior state = interior trace with the normal momentum negated),
+ * 2 far field (exterior state = qinf[5], conserved variables).  bc == NULL means periodic everywhere. */
+int oracle_residual_bc(int nx, int ny, int nz, int p, double gamma, const double extent[3], const int bc[6],
+                       const double qinf[5], const double *q, double *r);
+int oracle_rk_step_bc(int nx, int ny, int nz, int p, double gamma, const double extent[3], const int bc[6],
+                      const double qinf[5], double *q, double dt, int nsteps);
+
 /* lam = max over nodes of sqrt(u^2+v^2+w^2) + c   (reading R10). */
 int oracle_max_wavespeed(int nx, int ny, int nz, int p, double gamma, const double *q,
                          double *lam);
