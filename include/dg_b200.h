@@ -71,6 +71,19 @@ int dg_create(dg_ctx **out, int nx, int ny, int nz, int p, double gamma, const d
  * sizes, so it is refused after dg_bind (DG_ESTATE). */
 int dg_set_brick(dg_ctx *ctx, int bx, int by, int lz);
 
+/* Boundary conditions of the six domain faces, bc = {x-, x+, y-, y+, z-, z+}.  The paper's
+ * benchmark is periodic and gives no other condition; these are DESIGN.md reading R19:
+ *   DG_BC_PERIODIC : the neighbour across the face is the element at the other end of the axis (default; an axis is
+ *                    periodic on both of its faces or on neither, DG_EINVAL otherwise)
+ *   DG_BC_WALL     : slip wall; the exterior state of the Lax-Friedrichs flux is the interior trace with
+ *                    its face-normal momentum negated
+ *   DG_BC_FARFIELD : the exterior state is q_inf[5] = (rho, rho u, rho v, rho w, rho E), a host array copied by the call
+ *                    (may be NULL when no face is a far field)
+ * May be called at any time between dg_create and dg_destroy; takes effect with the next dg_residual / dg_rk_step.
+ * dg_split_surface supports periodic faces only (DG_EUNSUPPORTED otherwise). */
+enum { DG_BC_PERIODIC = 0, DG_BC_WALL = 1, DG_BC_FARFIELD = 2 };
+int dg_set_boundary(dg_ctx *ctx, const int bc[6], const double q_inf[5]);
+
 /* Number of stage-kernel variants (column shape x shared-memory layout x residency) compiled into the
  * library for degree p; 0 when p is outside 1..7.  dg_create picks the first variant whose columns
  * pad the mesh by less than 4 % (variants are listed fastest first). */

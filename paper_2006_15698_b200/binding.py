@@ -18,6 +18,7 @@ SYMBOLS = {
     "dg_create": (ctypes.c_int, [ctypes.POINTER(ctypes.c_void_p), ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                  ctypes.c_int, ctypes.c_double, _DP]),
     "dg_set_brick": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
+    "dg_set_boundary": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), _DP]),
     "dg_variant_count": (ctypes.c_int, [ctypes.c_int]),
     "dg_set_variant": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
     "dg_state_len": (ctypes.c_size_t, [ctypes.c_void_p]),
@@ -162,6 +163,13 @@ class DG:
                 self.workspace.fill_(255)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             self._check(self.lib.dg_bind(self._h, self.workspace.data_ptr(), nbytes, self.stream.cuda_stream))
+
+    def set_boundary(self, bc, q_inf=None):
+        """bc = (x-, x+, y-, y+, z-, z+): 0 periodic, 1 slip wall, 2 far field with exterior state q_inf (5 doubles)."""
+        b = (ctypes.c_int * 6)(*[int(v) for v in bc])
+        qi = None if q_inf is None else (ctypes.c_double * 5)(*[float(v) for v in q_inf])
+        self._check(self.lib.dg_set_boundary(self._h, b, qi))
+        return self
 
     @property
     def state_len(self):

@@ -189,6 +189,8 @@ struct dg_ctx {
     bool lam_valid;     // scal[0] holds the max wavespeed of the current Q (reduced by the last stage)
     int sms, blocks_per_sm;
     double g[3];        // 2/h_a per axis
+    int bc[6];          // boundary condition per domain face (dg_set_boundary), 0 = periodic
+    double qinf[DG_NV];
     bool bound, has_state;
     cudaStream_t stream;
     unsigned long long launches;
@@ -280,6 +282,8 @@ DgStageArgs stage_args(const dg_ctx *c, int mode) {
     a.gm1 = c->gamma - 1.0;
     a.mode = mode;
     for (int i = 0; i < 3; ++i) a.scale[i] = c->g[i];
+    for (int i = 0; i < 6; ++i) a.bc[i] = c->bc[i];
+    for (int i = 0; i < DG_NV; ++i) a.qinf[i] = c->qinf[i];
     return a;
 }
 
@@ -446,6 +450,26 @@ int dg_set_brick(dg_ctx *c, int bx, int by, int lz) {
     return fail(c, DG_EUNSUPPORTED, "column %dx%d is not compiled for p=%d", bx, by, c->p);
 }
 
+int dg_set_boundary(dg_ctx *c, const int bc[6], const double q_inf[5]) {
+    if (!c || !bc) return c ? fail(c, DG_EINVAL, "null boundary array") : DG_EINVAL;
+    bool far = false;
+    for (int a = 0; a < 3; ++a) {
+        const int lo = bc[2 * a], hi = bc[2 * a + 1];
+        if (lo < 0 || lo > 2 || hi < 0 || hi > 2) return fail(c, DG_EINVAL, "boundary condition outside 0..2");
+        if ((lo == DG_BC_PERIODIC) != (hi == DG_BC_PERIODIC))
+            return fail(c, DG_EINVAL, "an axis is periodic on both of its faces or on neither");
+        far = far || lo == DG_BC_FARFIELD || hi == DG_BC_FARFIELD;
+    }
+    if (far) {
+        if (!q_inf) return fail(c, DG_EINVAL, "a far-field face needs the far-field state");
+        for (int n = 0; n < DG_NV; ++n)
+            if (!std::isfinite(q_inf[n])) return fail(c, DG_EINVAL, "far-field state is not finite");
+    }
+    for (int f = 0; f < 6; ++f) c->bc[f] = bc[f];
+    for (int n = 0; n < DG_NV; ++n) c->qinf[n] = q_inf ? q_inf[n] : 0.0;
+    return DG_OK;
+}
+
 int dg_variant_count(int p) {
     int count = 0;
     if (p < 1 || p > 7) return 0;
@@ -595,6 +619,8 @@ int dg_split_volume(dg_ctx *c) {
 int dg_split_surface(dg_ctx *c) {
     if (!c) return DG_EINVAL;
     if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_split_surface needs dg_bind and dg_set_state first");
+    for (int f = 0; f < 6; ++f)
+        if (c->bc[f]) return fail(c, DG_EUNSUPPORTED, "the per-kernel mode is periodic only");
     cudaError_t e = c->kt->launch_split_surface(split_args(c), c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "surface kernel");
     c->launches++;

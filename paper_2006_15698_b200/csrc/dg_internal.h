@@ -77,6 +77,8 @@ struct DgStageArgs {
     int want_lam;
     int store_k;          // 0 in the last stage of a step: K is dead then (the next stage 1 has A = 0) and is not written
     double scale[3];      // 2/h_a per axis, times dt in stage mode: K accumulates dt * L(Q)
+    int bc[6];            // domain faces x-, x+, y-, y+, z-, z+: 0 periodic, 1 slip wall, 2 far field (R19)
+    double qinf[DG_NV];   // far-field state (conserved variables)
 };
 
 struct DgTraceArgs {

@@ -275,6 +275,9 @@ struct BlockInfo {
     long long kstride;         // ... in Q and K
     double gamma, gm1, rkA, rkB, scale[3];
     int ext0, ext1, readK, storeK, nl;
+    int bc[6];                 // boundary condition of this block's x-, x+, y-, y+, z-, z+ side if it lies on a non-periodic
+                               // domain face (1 slip wall, 2 far field), else 0
+    double qinf[DG_NV];
 };
 
 // PE for one of the axes x, y: traces of the Q in shared memory on the column boundary -> Tslot.
@@ -335,6 +338,15 @@ __device__ __forceinline__ const double *halo_source(const double *T, int nbx, i
     else by = (side == 0) ? ((by == 0) ? nby - 1 : by - 1) : ((by + 1 == nby) ? 0 : by + 1);
     const size_t nbr = (size_t)bx + (size_t)nbx * ((size_t)by + (size_t)nby * ez);
     return T + nbr * C::TXY + A::TBASE + (side == 0 ? DG_NV * A::Ca : 0);
+}
+
+// Exterior (ghost) state of a non-periodic domain face from the interior trace T, momentum slots rotated for AX
+// (reading R19): slip wall = T with the normal momentum (slot 1) negated; far field = the prescribed state.
+template <class C, int AX>
+__device__ __forceinline__ void ghost_state(int kind, const double (&T)[DG_NV], const double *qinf, double (&G)[DG_NV]) {
+#pragma unroll
+    for (int s = 0; s < DG_NV; ++s) G[s] = (kind == 2) ? qinf[var_of_slot<C, AX>(s)] : T[s];
+    if (kind == 1) G[1] = -T[1];
 }
 
 // PC + PA for one line: V_i = sum_q Dhat_iq F_q - (l_i(+1) 2F*_+ - l_i(-1) 2F*_-)/(2 w_i), F_q the pointwise Euler flux
@@ -461,6 +473,12 @@ __device__ __forceinline__ void xy_pass(const BlockInfo *bi, const Geo &g, bool 
             Tm[s] = fma(DG_LM(q), Qv, Tm[s]);
         }
     }
+    // non-periodic domain faces: the neighbour's trace is the ghost state of the own one
+    {
+        const int blo = bi->bc[2 * AX], bhi = bi->bc[2 * AX + 1];
+        if (blo && first) ghost_state<C, AX>(blo, Tm, bi->qinf, Hlo);
+        if (bhi && last) ghost_state<C, AX>(bhi, Tp, bi->qinf, Hhi);
+    }
     if (A::MULTI) {
         if (act) {
 #pragma unroll
@@ -579,6 +597,7 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
             Tp[s] = fma(DG_LP(q), Qv, Tp[s]);
         }
     }
+    if (last_layer && bi->bc[5]) ghost_state<C, AX>(bi->bc[5], Tp, bi->qinf, Hhi);   // non-periodic top of the domain
     // PB
     if (first_layer) {   // bottom of the chunk: own T- against T+ of the layer below (from HBM)
         double Tm[NV], Hlo[NV];
@@ -591,6 +610,7 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
             Tm[s] = t;
             Hlo[s] = __ldg(tz_lo + var_of_slot<C, AX>(s) * Ca + g.c);
         }
+        if (bi->bc[4]) ghost_state<C, AX>(bi->bc[4], Tm, bi->qinf, Hlo);   // non-periodic bottom of the domain
         lax_friedrichs2(Tm, Hlo, -1.0, gamma, gm1, Fm);
     } else {
 #pragma unroll
@@ -825,6 +845,13 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
         bi->ext1 = min(C::BY, a.ny - byi * C::BY);
         bi->readK = readK ? 1 : 0;
         bi->storeK = a.store_k;
+        bi->bc[0] = (bxi == 0) ? a.bc[0] : 0;
+        bi->bc[1] = (bxi + 1 == a.nbx) ? a.bc[1] : 0;
+        bi->bc[2] = (byi == 0) ? a.bc[2] : 0;
+        bi->bc[3] = (byi + 1 == a.nby) ? a.bc[3] : 0;
+        bi->bc[4] = (chunk == 0) ? a.bc[4] : 0;
+        bi->bc[5] = (chunk + 1 == a.nchunks) ? a.bc[5] : 0;
+        for (int n = 0; n < DG_NV; ++n) bi->qinf[n] = a.qinf[n];
         bi->nl = nl;
     }
     __syncthreads();
