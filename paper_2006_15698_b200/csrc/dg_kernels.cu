@@ -433,7 +433,7 @@ __device__ __forceinline__ void lift_and_volume(LoadQ loadQ, double gm1, const d
 //   r_i = (2/h_a) [ sum_q Dhat_iq F_q - (l_i(+1) F*_+ - l_i(-1) F*_-)/w_i ]
 // Threads without a line of their own (`act` false: the tail of the last warp, lines in the padding of a ragged
 // column) run the arithmetic on a valid line all the same and only their stores are switched off.
-template <class C, int AX, int MODE>
+template <class C, int AX, int MODE, bool BC>
 __device__ __forceinline__ void xy_pass(const BlockInfo *bi, const Geo &g, bool act, int exta, const double *halo_lo,
                                         const double *halo_hi, const double *Qs, double *KR, double *Tms, double *Fss,
                                         uint64_t *fullk, unsigned kparity) {
@@ -473,8 +473,8 @@ __device__ __forceinline__ void xy_pass(const BlockInfo *bi, const Geo &g, bool 
             Tm[s] = fma(DG_LM(q), Qv, Tm[s]);
         }
     }
-    // non-periodic domain faces: the neighbour's trace is the ghost state of the own one
-    {
+    // non-periodic domain faces (BC instances only): the neighbour's trace is the ghost state of the own one
+    if (BC) {
         const int blo = bi->bc[2 * AX], bhi = bi->bc[2 * AX + 1];
         if (blo && first) ghost_state<C, AX>(blo, Tm, bi->qinf, Hlo);
         if (bhi && last) ghost_state<C, AX>(bhi, Tp, bi->qinf, Hhi);
@@ -559,7 +559,7 @@ __device__ __forceinline__ void xy_pass(const BlockInfo *bi, const Geo &g, bool 
 // the z pass of one layer: thread (gx, gy) owns the z line; the flux on the lower face of the layer is the one
 // this thread computed for the upper face of the previous layer, kept in FmS (shared memory, [5][L])
 // ------------------------------------------------------------------------------------------------
-template <class C, int MODE, bool LAM>
+template <class C, int MODE, bool LAM, bool BC>
 __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l, bool act, double *Qs, const double *Qnext,
                                        const double *KR, double *FmS, double *Kg, bool first_layer, bool last_layer,
                                        double &lam_best) {
@@ -597,7 +597,7 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
             Tp[s] = fma(DG_LP(q), Qv, Tp[s]);
         }
     }
-    if (last_layer && bi->bc[5]) ghost_state<C, AX>(bi->bc[5], Tp, bi->qinf, Hhi);   // non-periodic top of the domain
+    if (BC && last_layer && bi->bc[5]) ghost_state<C, AX>(bi->bc[5], Tp, bi->qinf, Hhi);   // non-periodic top of the domain
     // PB
     if (first_layer) {   // bottom of the chunk: own T- against T+ of the layer below (from HBM)
         double Tm[NV], Hlo[NV];
@@ -610,7 +610,7 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
             Tm[s] = t;
             Hlo[s] = __ldg(tz_lo + var_of_slot<C, AX>(s) * Ca + g.c);
         }
-        if (bi->bc[4]) ghost_state<C, AX>(bi->bc[4], Tm, bi->qinf, Hlo);   // non-periodic bottom of the domain
+        if (BC && bi->bc[4]) ghost_state<C, AX>(bi->bc[4], Tm, bi->qinf, Hlo);   // non-periodic bottom of the domain
         lax_friedrichs2(Tm, Hlo, -1.0, gamma, gm1, Fm);
     } else {
 #pragma unroll
@@ -748,7 +748,7 @@ struct Smem {
     static constexpr int BYTES = DOUBLES * 8;
 };
 
-template <class C, int MODE, bool LAM>
+template <class C, int MODE, bool LAM, bool BC>
 __device__ __noinline__ double layer_body(int it, double lam_best) {
     extern __shared__ __align__(128) double smem[];
     using SM = Smem<C>;
@@ -765,12 +765,12 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
     mbar_wait(&fullq[it & 1], (it >> 1) & 1);
     {
         const Geo gx = make_geo<C, 0>(lx);
-        xy_pass<C, 0, MODE>(bi, gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, bi->halo[0] + toff, bi->halo[1] + toff, Qs,
+        xy_pass<C, 0, MODE, BC>(bi, gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, bi->halo[0] + toff, bi->halo[1] + toff, Qs,
                             KR, Tms, Fss, fullk, it & 1);
     }
     {
         const Geo gy = make_geo<C, 1>(lx);
-        xy_pass<C, 1, MODE>(bi, gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, bi->halo[2] + toff, bi->halo[3] + toff, Qs,
+        xy_pass<C, 1, MODE, BC>(bi, gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, bi->halo[2] + toff, bi->halo[3] + toff, Qs,
                             KR, Tms, Fss, fullk, it & 1);
     }
     const bool last_layer = it + 1 == bi->nl;
@@ -784,7 +784,7 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
     if (!last_layer) mbar_wait(&fullq[(it + 1) & 1], ((it + 1) >> 1) & 1);
     {
         const Geo gz = make_geo<C, 2>(lx);
-        z_pass<C, MODE, LAM>(bi, gz, lx, inL && line_inside<C, 2>(gz, ext0, ext1), Qs, Qnext, KR, FmS,
+        z_pass<C, MODE, LAM, BC>(bi, gz, lx, inL && line_inside<C, 2>(gz, ext0, ext1), Qs, Qnext, KR, FmS,
                              bi->kslot + (long long)it * bi->kstride, it == 0, last_layer, lam_best);
     }
     bar_sync<C::NCOMP>(1);   // the updated Q of the whole layer is in shared memory; every line has read KR
@@ -804,7 +804,8 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
 // ------------------------------------------------------------------------------------------------
 // the fused stage kernel: block (bx, by, chunk) marches through layers z0 .. z0 + nl - 1 of column (bx, by)
 // ------------------------------------------------------------------------------------------------
-template <class C, int MODE, bool LAM>
+// BC = false: every domain face periodic (the paper's benchmark; no boundary code in the instance).
+template <class C, int MODE, bool LAM, bool BC>
 __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __grid_constant__ DgStageArgs a) {
     extern __shared__ __align__(128) double smem[];
     using SM = Smem<C>;
@@ -862,7 +863,7 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
     }
     double lam_best = 0.0;
 #pragma unroll 1
-    for (int it = 0; it < nl; ++it) lam_best = layer_body<C, MODE, LAM>(it, lam_best);
+    for (int it = 0; it < nl; ++it) lam_best = layer_body<C, MODE, LAM, BC>(it, lam_best);
     if (LAM) {
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {
@@ -1134,9 +1135,12 @@ cudaError_t prepare(const DgRefOps &ref, int *blocks_per_sm) {
     auto opt_in = [&](auto kernel) {
         if (err == cudaSuccess) err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Smem<C>::BYTES);
     };
-    opt_in(dg_stage_kernel<C, DG_MODE_STAGE, false>);
-    opt_in(dg_stage_kernel<C, DG_MODE_STAGE, true>);
-    opt_in(dg_stage_kernel<C, DG_MODE_RESIDUAL, false>);
+    opt_in(dg_stage_kernel<C, DG_MODE_STAGE, false, false>);
+    opt_in(dg_stage_kernel<C, DG_MODE_STAGE, true, false>);
+    opt_in(dg_stage_kernel<C, DG_MODE_RESIDUAL, false, false>);
+    opt_in(dg_stage_kernel<C, DG_MODE_STAGE, false, true>);
+    opt_in(dg_stage_kernel<C, DG_MODE_STAGE, true, true>);
+    opt_in(dg_stage_kernel<C, DG_MODE_RESIDUAL, false, true>);
     if (err == cudaSuccess)
         err = cudaFuncSetAttribute(dg_traces_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::BUF * 8);
     if (err == cudaSuccess)
@@ -1144,16 +1148,25 @@ cudaError_t prepare(const DgRefOps &ref, int *blocks_per_sm) {
     if (err == cudaSuccess)
         err = cudaFuncSetAttribute(dg_split_surface_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * C::BUF * 8);
     if (err != cudaSuccess) return err;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, dg_stage_kernel<C, DG_MODE_STAGE, false>,
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, dg_stage_kernel<C, DG_MODE_STAGE, false, false>,
                                                          C::THREADS, Smem<C>::BYTES);
 }
 
 template <class C>
 cudaError_t launch_stage(const DgStageArgs &a, cudaStream_t s) {
     const dim3 grid((unsigned)a.nbx, (unsigned)a.nby, (unsigned)a.nchunks);
-    if (a.mode == DG_MODE_RESIDUAL) dg_stage_kernel<C, DG_MODE_RESIDUAL, false><<<grid, C::THREADS, Smem<C>::BYTES, s>>>(a);
-    else if (a.want_lam) dg_stage_kernel<C, DG_MODE_STAGE, true><<<grid, C::THREADS, Smem<C>::BYTES, s>>>(a);
-    else dg_stage_kernel<C, DG_MODE_STAGE, false><<<grid, C::THREADS, Smem<C>::BYTES, s>>>(a);
+    const bool bc = a.bc[0] || a.bc[1] || a.bc[2] || a.bc[3] || a.bc[4] || a.bc[5];
+    const size_t sm = Smem<C>::BYTES;
+    if (a.mode == DG_MODE_RESIDUAL) {
+        if (bc) dg_stage_kernel<C, DG_MODE_RESIDUAL, false, true><<<grid, C::THREADS, sm, s>>>(a);
+        else dg_stage_kernel<C, DG_MODE_RESIDUAL, false, false><<<grid, C::THREADS, sm, s>>>(a);
+    } else if (a.want_lam) {
+        if (bc) dg_stage_kernel<C, DG_MODE_STAGE, true, true><<<grid, C::THREADS, sm, s>>>(a);
+        else dg_stage_kernel<C, DG_MODE_STAGE, true, false><<<grid, C::THREADS, sm, s>>>(a);
+    } else {
+        if (bc) dg_stage_kernel<C, DG_MODE_STAGE, false, true><<<grid, C::THREADS, sm, s>>>(a);
+        else dg_stage_kernel<C, DG_MODE_STAGE, false, false><<<grid, C::THREADS, sm, s>>>(a);
+    }
     return cudaGetLastError();
 }
 
