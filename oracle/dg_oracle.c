@@ -24,7 +24,8 @@
  *
  * Parity unpinned BY THE PAPER (fixed by DESIGN.md readings, pinned only by consistency,
  * conservation and convergence): the exact Lax-Friedrichs variant (R3), the CFL rule (R10),
- * the element ordering (R13).
+ * the element ordering (R13), the wall / far-field ghost states of non-periodic faces (R19: the
+ * paper's domain is periodic; pinned by the mirror-image equivalence with the periodic path).
  *
  * Floating-point form: products and sums are evaluated in the
  * order written below, q ascending; build with -ffp-contract=off so the compiler fuses nothing.
