@@ -128,10 +128,11 @@ int dg_rk_step(dg_ctx *ctx, double dt, int nsteps);
 
 /* nsteps >= 0 LSERK45 steps, each with its own time step from the CFL rule of reading R10,
  *     dt = cfl * min(hx,hy,hz) / ((2p+1) * lam_max(Q at the start of the step)),
- * lam_max reduced on the device by the last stage of the previous step (no extra sweep over the
- * state; one 8-byte read-back and stream synchronisation per step).  cfl > 0.  On return
- * *t_advanced = sum of the time steps taken and *dt_last = the last one (host pointers, either may be
- * NULL).  DG_ESTATE if the wavespeed is not positive and finite. */
+ * formed ON THE DEVICE: lam_max is reduced by the last stage of the previous step (no extra sweep over the state)
+ * and the next step's kernels read it from device memory, so the steps are enqueued without a host round trip.
+ * One read-back at the start checks the wavespeed of the current state (DG_ESTATE if not positive and finite,
+ * nothing stepped) and one at the end returns *t_advanced = sum of the time steps taken and *dt_last = the last
+ * one (host pointers, either may be NULL; DG_ESTATE if the state went non-physical on the way).  cfl > 0. */
 int dg_rk_step_cfl(dg_ctx *ctx, double cfl, int nsteps, double *t_advanced, double *dt_last);
 
 /* Paper-shaped per-kernel mode (Table II): the same spatial residual and stage

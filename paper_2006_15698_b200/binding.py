@@ -211,9 +211,24 @@ class DG:
             raise ValueError("output array is read-only")
         return ctypes.c_void_p(a.ctypes.data), 0, a
 
+    def _order_before(self, dev):
+        """Device tensors may have been produced on torch's current stream: make the bound stream wait for it
+        (include/dg_b200.h: the library orders its work on the stream given to dg_bind only)."""
+        if dev:
+            cur = self._torch.cuda.current_stream(self.device)
+            if cur != self.stream:
+                self.stream.wait_stream(cur)
+
+    def _order_after(self, dev):
+        if dev:
+            cur = self._torch.cuda.current_stream(self.device)
+            if cur != self.stream:
+                cur.wait_stream(self.stream)
+
     # -- the six calls of north_star (+ max wavespeed) ---------------------------------------------
     def set_state(self, q):
         ptr, dev, keep = self._ptr(q, False)
+        self._order_before(dev)
         with self._torch.cuda.device(self.device):
             self._check(self.lib.dg_set_state(self._h, ptr, dev))
         if dev == 0 and isinstance(keep, self._torch.Tensor) and keep.is_pinned():
@@ -225,8 +240,10 @@ class DG:
         if out is None:
             out = np.empty(self.shape)
         ptr, dev, _ = self._ptr(out, True)
+        self._order_before(dev)
         with self._torch.cuda.device(self.device):
             self._check(self.lib.dg_residual(self._h, ptr, dev))
+        self._order_after(dev)
         return out
 
     def rk_step(self, dt, nsteps=1):
@@ -277,8 +294,10 @@ class DG:
         if out is None:
             out = np.empty(self.shape)
         ptr, dev, _ = self._ptr(out, True)
+        self._order_before(dev)
         with self._torch.cuda.device(self.device):
             self._check(self.lib.dg_get_state(self._h, ptr, dev))
+        self._order_after(dev)
         return out
 
     def max_wavespeed(self):

@@ -186,7 +186,8 @@ struct dg_ctx {
     double *Q, *K, *S, *Txy[2], *Tz[2];
     unsigned long long *scal;
     int tcur;           // Txy[tcur], Tz[tcur] hold the traces of the current Q
-    bool lam_valid;     // scal[0] holds the max wavespeed of the current Q (reduced by the last stage)
+    bool lam_valid;     // scal[lcur] holds the max wavespeed of the current Q (reduced by the last stage)
+    int lcur;           // scal[0..1]: two wavespeed slots (one read, one written by a CFL step); scal[2..3]: time advanced, last dt
     int sms, blocks_per_sm;
     double g[3];        // 2/h_a per axis
     int bc[6];          // boundary condition per domain face (dg_set_boundary), 0 = periodic
@@ -312,26 +313,34 @@ int export_vector(dg_ctx *c, double *internal, double *out, int on_device, const
     return DG_OK;
 }
 
-// One LSERK45 step = 5 launches of the fused stage kernel; the last stage can reduce the max wavespeed
-// of the state it produces on the way (a9 fused: no extra sweep over the state).
-int enqueue_step(dg_ctx *c, double dt, bool want_lam) {
+// One LSERK45 step = 5 launches of the fused stage kernel.  cfl_factor > 0: the time step is formed on the device from
+// the wavespeed in scal[lcur] and the last stage reduces the wavespeed of the state it produces into the other slot
+// (a9 fused: no extra sweep over the state, no host round trip).
+int enqueue_step(dg_ctx *c, double dt, double cfl_factor) {
+    const bool cfl = cfl_factor > 0.0;
+    unsigned long long *lam_in = c->scal + c->lcur, *lam_out = c->scal + (1 - c->lcur);
+    if (cfl) {
+        cudaError_t e = cudaMemsetAsync(lam_out, 0, 8, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "memset");
+    }
     for (int s = 0; s < 5; ++s) {
         DgStageArgs a = stage_args(c, DG_MODE_STAGE);
-        for (int i = 0; i < 3; ++i) a.scale[i] = dt * c->g[i];
+        for (int i = 0; i < 3; ++i) a.scale[i] = cfl ? c->g[i] : dt * c->g[i];
         a.rkA = (double)kRkA[s];
         a.rkB = (double)kRkB[s];
-        a.want_lam = (want_lam && s == 4) ? 1 : 0;
+        a.want_lam = (cfl && s == 4) ? 1 : 0;
         a.store_k = (s == 4) ? 0 : 1;
-        if (a.want_lam) {
-            cudaError_t e = cudaMemsetAsync(c->scal, 0, 8, c->stream);
-            if (e != cudaSuccess) return cuda_fail(c, e, "memset");
-        }
+        a.lam_in = cfl ? lam_in : nullptr;
+        a.cfl_factor = cfl_factor;
+        a.t_acc = (cfl && s == 0) ? reinterpret_cast<double *>(c->scal + 2) : nullptr;
+        a.lam_bits = lam_out;
         cudaError_t e = c->kt->launch_stage(a, c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "stage kernel");
         c->launches++;
         c->tcur = 1 - c->tcur;
     }
-    c->lam_valid = want_lam;
+    if (cfl) c->lcur = 1 - c->lcur;
+    c->lam_valid = cfl;
     return DG_OK;
 }
 
@@ -365,23 +374,29 @@ DgSplitArgs split_args(const dg_ctx *c) {
     return a;
 }
 
+// the max wavespeed of the current state is in scal[lcur] (enqueued; reduction kernel only if no stage left it there)
+int ensure_lam(dg_ctx *c) {
+    if (c->lam_valid) return DG_OK;
+    cudaError_t e = cudaMemsetAsync(c->scal + c->lcur, 0, 8, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "memset");
+    DgWaveArgs a;
+    a.Q = c->Q;
+    a.lam_bits = c->scal + c->lcur;
+    a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
+    a.nbx = c->nbx; a.nby = c->nby;
+    a.gamma = c->gamma;
+    a.gm1 = c->gamma - 1.0;
+    e = c->kt->launch_wavespeed(a, c->sms, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "wavespeed kernel");
+    c->launches++;
+    c->lam_valid = true;
+    return DG_OK;
+}
+
 int read_lam(dg_ctx *c, double *lam_host) {
-    if (!c->lam_valid) {
-        cudaError_t e = cudaMemsetAsync(c->scal, 0, 8, c->stream);
-        if (e != cudaSuccess) return cuda_fail(c, e, "memset");
-        DgWaveArgs a;
-        a.Q = c->Q;
-        a.lam_bits = c->scal;
-        a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
-        a.nbx = c->nbx; a.nby = c->nby;
-        a.gamma = c->gamma;
-        a.gm1 = c->gamma - 1.0;
-        e = c->kt->launch_wavespeed(a, c->sms, c->stream);
-        if (e != cudaSuccess) return cuda_fail(c, e, "wavespeed kernel");
-        c->launches++;
-        c->lam_valid = true;
-    }
-    cudaError_t e = cudaMemcpyAsync(lam_host, c->scal, 8, cudaMemcpyDeviceToHost, c->stream);
+    const int rc = ensure_lam(c);
+    if (rc != DG_OK) return rc;
+    cudaError_t e = cudaMemcpyAsync(lam_host, c->scal + c->lcur, 8, cudaMemcpyDeviceToHost, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "device->host copy");
     e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "synchronise");
@@ -578,7 +593,7 @@ int dg_rk_step(dg_ctx *c, double dt, int nsteps) {
     if (nsteps < 0 || !std::isfinite(dt)) return fail(c, DG_EINVAL, "nsteps < 0 or dt not finite");
     if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_rk_step needs dg_bind and dg_set_state first");
     for (int step = 0; step < nsteps; ++step) {
-        const int rc = enqueue_step(c, dt, false);
+        const int rc = enqueue_step(c, dt, 0.0);
         if (rc != DG_OK) return rc;
     }
     return DG_OK;
@@ -591,19 +606,28 @@ int dg_rk_step_cfl(dg_ctx *c, double cfl, int nsteps, double *t_advanced, double
     double hmin = c->extent[0] / c->nx;
     if (c->extent[1] / c->ny < hmin) hmin = c->extent[1] / c->ny;
     if (c->extent[2] / c->nz < hmin) hmin = c->extent[2] / c->nz;
-    double t = 0.0, dt = 0.0;
-    for (int step = 0; step < nsteps; ++step) {
-        double lam = 0.0;
-        int rc = read_lam(c, &lam);   // 8-byte read-back; reduced by the previous step's last stage
-        if (rc != DG_OK) return rc;
-        if (!(lam > 0.0) || !std::isfinite(lam)) return fail(c, DG_ESTATE, "max wavespeed %g is not positive and finite", lam);
-        dt = cfl * hmin / ((2.0 * c->p + 1.0) * lam);
-        rc = enqueue_step(c, dt, true);
-        if (rc != DG_OK) return rc;
-        t += dt;
+    // the wavespeed of the state the call starts from is checked on the host (one read-back per call) ...
+    double lam = 0.0;
+    int rc = read_lam(c, &lam);
+    if (rc != DG_OK) return rc;
+    if (!(lam > 0.0) || !std::isfinite(lam)) return fail(c, DG_ESTATE, "max wavespeed %g is not positive and finite", lam);
+    double out[2] = {0.0, 0.0};
+    if (nsteps > 0) {
+        // ... every step then forms its dt on the device from the wavespeed the step before reduced
+        const double cfl_factor = cfl * hmin / (2.0 * c->p + 1.0);
+        cudaError_t e = cudaMemsetAsync(c->scal + 2, 0, 16, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "memset");
+        for (int step = 0; step < nsteps; ++step) {
+            rc = enqueue_step(c, 0.0, cfl_factor);
+            if (rc != DG_OK) return rc;
+        }
+        e = cudaMemcpyAsync(out, c->scal + 2, 16, cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "read-back of the time advanced");
     }
-    if (t_advanced) *t_advanced = t;
-    if (dt_last) *dt_last = dt;
+    if (t_advanced) *t_advanced = out[0];
+    if (dt_last) *dt_last = out[1];
+    if (!std::isfinite(out[0])) return fail(c, DG_ESTATE, "the state became non-physical during the steps (time advanced %g)", out[0]);
     return DG_OK;
 }
 

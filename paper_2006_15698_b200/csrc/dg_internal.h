@@ -77,6 +77,12 @@ struct DgStageArgs {
     int want_lam;
     int store_k;          // 0 in the last stage of a step: K is dead then (the next stage 1 has A = 0) and is not written
     double scale[3];      // 2/h_a per axis, times dt in stage mode: K accumulates dt * L(Q)
+    // CFL stepping (dg_rk_step_cfl): when lam_in is set the time step is formed ON THE DEVICE, dt = cfl_factor / lam
+    // with lam the max wavespeed the previous step's last stage left in *lam_in, and multiplies `scale`; the first
+    // block of a step's first stage adds dt to t_acc[0] and stores it in t_acc[1].  No host round trip per step.
+    const unsigned long long *lam_in;
+    double cfl_factor;    // cfl * min(h) / (2p + 1)
+    double *t_acc;
     int bc[6];            // domain faces x-, x+, y-, y+, z-, z+: 0 periodic, 1 slip wall, 2 far field (R19)
     double qinf[DG_NV];   // far-field state (conserved variables)
 };

@@ -19,8 +19,9 @@
 //       r_i = sum_q Dhat_iq F_q - (l_i(+1) F*_+ - l_i(-1) F*_-) (2/h_a)/w_i       (eq (5) 3rd and 2nd term)
 //   PA  pointwise Euler flux (eq (2)-(3)) at the line's N nodes and the sum-factorised
 //       derivative (the contraction of listing lines 220-237), all in registers
-//   PD  LSERK45 accumulated in place on the staged K:  x: K = A K + r_x,  y: K += r_y,
-//       z: K += r_z, Q += B K, both left in shared memory for the copy warp; or R itself in residual mode
+//   PD  LSERK45 accumulated in place on the staged K:  x: K = A K + s_x r_x,  y: K += s_y r_y,
+//       z: K += s_z r_z (s_a = dt 2/h_a), written straight to HBM from the z lines; Q += B K left in shared memory
+//       for the copy warp; or R itself in residual mode
 //   PE  x / y face traces of the UPDATED Q on the column boundary, written to the other trace buffer
 // so that Q and K are read once and written once per stage and no block ever needs another block's nodal
 // values: neighbours meet only through the double-buffered column-boundary traces.
@@ -56,7 +57,6 @@ struct Cfg {
     // it in 10 N registers across the interface fluxes
     static constexpr bool RELOAD = RELOAD_ != 0;
     static constexpr int GX = BX * N, GY = BY * N;                 // nodes of a layer per axis (z: N)
-    static constexpr int NODES = GX * GY * N;
     // pitch of one (gy,gx) plane, doubles, in HBM AND in shared memory (a layer is ONE bulk copy): even, and
     // padded by PP_ - GX GY where that removes shared-memory bank conflicts at a few per cent more traffic
     static constexpr int HP = PP_ ? PP_ : ((GX * GY + 1) & ~1);
@@ -677,14 +677,18 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
                 }
             }
             if (LAM) {
-                // max wavespeed of the updated state (reading R10), IEEE division and square root;
-                // slots are (rho, rho w, rho u, rho v, rho E): the speed does not care about the rotation
+                // max wavespeed of the updated state (reading R10) with the kernels' own reciprocal and
+                // square root (a few ulp; the IEEE routines' slow paths cost 4 % of a step here); slots are
+                // (rho, rho w, rho u, rho v, rho E): the speed does not care about the rotation.  A negative
+                // density or pressure still gives NaN (the seeds of rcp / rsqrt propagate it).
 #pragma unroll
                 for (int i = 0; i < N; ++i) {
-                    const double rinv = 1.0 / Qn[0][i];
-                    const double u = Qn[LAM ? 2 : 0][i] * rinv, v = Qn[LAM ? 3 : 0][i] * rinv, w = Qn[LAM ? 1 : 0][i] * rinv;
-                    const double pres = gm1 * (Qn[LAM ? 4 : 0][i] - 0.5 * Qn[0][i] * (u * u + v * v + w * w));
-                    const double sp = sqrt(u * u + v * v + w * w) + sqrt(gamma * pres * rinv);
+                    const double rinv = rcp_pos(Qn[0][i]);
+                    const double m2 = fma(Qn[LAM ? 3 : 0][i], Qn[LAM ? 3 : 0][i],
+                                          fma(Qn[LAM ? 2 : 0][i], Qn[LAM ? 2 : 0][i], Qn[LAM ? 1 : 0][i] * Qn[LAM ? 1 : 0][i]));
+                    const double pres = gm1 * fma(-0.5, m2 * rinv, Qn[LAM ? 4 : 0][i]);
+                    const double um = (m2 > 1e-280) ? sqrt_pos(m2) * rinv : 0.0;   // fluid at rest: the seed of 0 is inf
+                    const double sp = um + sqrt_pos(gamma * pres * rinv);
                     if (sp > lam_best || sp != sp) lam_best = sp;   // NaN sticks
                 }
             }
@@ -839,9 +843,17 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
         bi->gm1 = a.gm1;
         bi->rkA = a.rkA;
         bi->rkB = a.rkB;
-        bi->scale[0] = a.scale[0];
-        bi->scale[1] = a.scale[1];
-        bi->scale[2] = a.scale[2];
+        double dtf = 1.0;
+        if (a.lam_in) {   // CFL time step from the wavespeed reduced on the device (reading R10)
+            dtf = a.cfl_factor / __longlong_as_double((long long)*a.lam_in);
+            if (a.t_acc && bxi == 0 && byi == 0 && chunk == 0) {
+                a.t_acc[0] += dtf;
+                a.t_acc[1] = dtf;
+            }
+        }
+        bi->scale[0] = a.scale[0] * dtf;
+        bi->scale[1] = a.scale[1] * dtf;
+        bi->scale[2] = a.scale[2] * dtf;
         bi->ext0 = min(C::BX, a.nx - bxi * C::BX);   // elements of this column per axis (ragged last column)
         bi->ext1 = min(C::BY, a.ny - byi * C::BY);
         bi->readK = readK ? 1 : 0;

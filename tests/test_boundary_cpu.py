@@ -93,3 +93,18 @@ def test_calls_before_bind_are_refused_and_brick_knob():
     assert lib.dg_bind(h, None, 0, None) == 1
     assert lib.dg_launch_count(h) == 0
     lib.dg_destroy(h)
+
+
+def test_set_boundary_validates_its_arguments():
+    lib, h, rc = _create(4, 4, 4, 2)
+    IA, DA = ctypes.c_int * 6, ctypes.c_double * 5
+    lib.dg_set_boundary.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)]
+    assert lib.dg_set_boundary(h, IA(0, 0, 0, 0, 0, 0), None) == 0
+    assert lib.dg_set_boundary(h, IA(1, 1, 0, 0, 1, 1), None) == 0                     # walls need no state
+    assert lib.dg_set_boundary(h, IA(1, 0, 0, 0, 0, 0), None) == 1                     # periodic on one face only
+    assert lib.dg_set_boundary(h, IA(3, 3, 0, 0, 0, 0), None) == 1
+    assert lib.dg_set_boundary(h, IA(2, 2, 0, 0, 0, 0), None) == 1                     # far field without a state
+    assert lib.dg_set_boundary(h, IA(2, 2, 0, 0, 0, 0), DA(1.0, 0.1, 0.0, 0.0, float("nan"))) == 1
+    assert lib.dg_set_boundary(h, IA(2, 1, 0, 0, 0, 0), DA(1.0, 0.1, 0.0, 0.0, 2.5)) == 0
+    assert lib.dg_set_boundary(h, None, None) == 1
+    lib.dg_destroy(h)

@@ -204,13 +204,23 @@ def test_rk_step_cfl_matches_oracle_loop_and_fused_wavespeed():
         launches = dg.launch_count
         lam = dg.max_wavespeed()
         assert dg.launch_count == launches                     # no reduction kernel ran
-        assert abs(lam - ORC.max_wavespeed(q_gpu, p, G)) <= 4e-16 * lam
+        assert abs(lam - ORC.max_wavespeed(q_gpu, p, G)) <= 2e-15 * lam     # fused: the kernels' own rcp / sqrt (<= 2 ulp each)
         # after a plain rk_step the cached value is stale and the reduction kernel runs again
         dg.rk_step(1e-4, 1)
         lam2 = dg.max_wavespeed()
         assert dg.launch_count == launches + 6
         assert abs(lam2 - ORC.max_wavespeed(dg.get_state(), p, G)) <= 4e-16 * lam2
         dg.close()
+
+
+def test_fused_wavespeed_of_a_fluid_at_rest():
+    """Zero velocity everywhere (the reciprocal-square-root seed of 0 is inf): the fused reduction must return c."""
+    n, p, ext = (4, 4, 4), 2, (1.0, 1.0, 1.0)
+    q = I.uniform_state(*n, p, rho=1.25, vel=(0.0, 0.0, 0.0), pres=1.75, gamma=G)
+    dg = DG(*n, p, G, ext)
+    dg.set_state(q).rk_step_cfl(0.1, 2)
+    assert abs(dg.max_wavespeed() - 1.4) < 1e-14                # sqrt(1.4 * 1.75 / 1.25) = 1.4, state stays uniform
+    dg.close()
 
 
 def test_max_wavespeed_propagates_nan():
