@@ -378,6 +378,71 @@ def run_variant_sweep(args):
                           "roofline_frac": rate * ALGO_BYTES_PER_DOF_STAGE / 1e9 / peak, "finite": r["finite"]}), flush=True)
 
 
+def run_decomposed(args, rank, world, local_rank):
+    """--decomposed: ONE mesh cut into `world` blocks, one rank per GPU, face traces exchanged over
+    NCCL after every stage (paper_2006_15698_b200/decomposed.py).  Strong scaling: total work fixed.  Not the default
+    (north_star / SURVEY.md 8(e): replicas only) and, this round, run on hardware with one GPU only (world = 1: no
+    messages); the multi-rank data path is tested with several contexts in one process (tests/test_gpu_halo.py)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2006_15698_b200 import inputs as I
+    from paper_2006_15698_b200.decomposed import DistributedDG
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    device = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(device)
+    c = I.CONFIGS[args.workload]
+    p, ext, n = c["p"], c["extent"], (c["nx"], c["ny"], c["nz"])
+    procs = [1, 1, 1]
+    w, a = world, 2
+    while w > 1:                                  # factor the rank count over z, y, x in turn
+        for f in (2, 3, 5, 7):
+            if w % f == 0:
+                procs[a] *= f
+                w //= f
+                a = (a - 1) % 3
+                break
+        else:
+            procs[a] *= w
+            w = 1
+    local = None if world > 1 else (lambda r, s, v: None)
+    dd = DistributedDG(n, p, GAMMA, ext, tuple(procs), rank, device=device, exchange=local,
+                       reduce_max=None if world > 1 else (lambda x: x))
+    box = dd.box
+    dd.set_state(I.make_field(args.workload, box=box, xp=torch, device=device))
+    dt = I.cfl_dt(dd.max_wavespeed(), p, ext, n, 0.1)
+    K, W = args.steps, max(3, args.warmup)
+    dd.rk_step(dt, W)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize(device)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stream = torch.cuda.current_stream(device)
+    e0.record(stream)
+    dd.rk_step(dt, K)
+    e1.record(stream)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize(device)
+    ms = reduce_max(e0.elapsed_time(e1), dist if world > 1 else None, device)
+    dof = n[0] * n[1] * n[2] * (p + 1) ** 3
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        value = dof * STAGES * K / (ms * 1e-3)
+        print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+                          "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                          "dtype": "f64", "data": "synthetic",
+                          "config": {"workload": f"{args.workload}: {list(n)} elements, p={p}, ONE mesh in {procs} blocks, "
+                                                 "face traces exchanged after every stage", "parallelism": f"block decomposition {procs}"},
+                          "gpu_launches": dd.dg.launch_count,
+                          "roofline": {"bound": "hbm", "achieved": ALGO_BYTES_PER_DOF_STAGE * dof * STAGES * K / (ms * 1e-3) / 1e9 / world,
+                                       "peak": peak, "unit": "GB/s per GPU", "frac": value * ALGO_BYTES_PER_DOF_STAGE / 1e9 / peak / world,
+                                       "peak_source": peak_src, "traffic": None}}), flush=True)
+    dd.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     if not torch.cuda.is_available():
@@ -516,6 +581,8 @@ def main():
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--decomposed", action="store_true",
+                    help="one mesh cut into one block per GPU with halo exchange (strong scaling) instead of replicas")
     ap.add_argument("--no-extras", action="store_true", help="skip the sustained run, cfg5 and the FP64 microbenchmark")
     ap.add_argument("--variant", type=int, default=None, help="stage-kernel variant index (tuning; default: library's choice)")
     ap.add_argument("--lz", type=int, default=0, help="layers per chunk (tuning; 0 = library default)")
@@ -528,6 +595,8 @@ def main():
         run_variant_sweep(args)
     elif args.impl == "reference":
         run_reference(args, rank)
+    elif args.decomposed:
+        run_decomposed(args, rank, world, local_rank)
     else:
         run_ours(args, rank, world, local_rank)
 

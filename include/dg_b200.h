@@ -79,9 +79,13 @@ int dg_set_brick(dg_ctx *ctx, int bx, int by, int lz);
  *                    its face-normal momentum negated
  *   DG_BC_FARFIELD : the exterior state is q_inf[5] = (rho, rho u, rho v, rho w, rho E), a host array copied by the call
  *                    (may be NULL when no face is a far field)
+ *   DG_BC_HALO     : the elements beyond the face belong to ANOTHER context (block decomposition of a larger mesh over
+ *                    several GPUs; nearest-neighbour coupling only); their face
+ *                    traces are read from the buffer given to dg_set_halo, which the caller fills from the
+ *                    neighbour's dg_halo_export before every stage (see below)
  * May be called at any time between dg_create and dg_destroy; takes effect with the next dg_residual / dg_rk_step.
  * dg_split_surface supports periodic faces only (DG_EUNSUPPORTED otherwise). */
-enum { DG_BC_PERIODIC = 0, DG_BC_WALL = 1, DG_BC_FARFIELD = 2 };
+enum { DG_BC_PERIODIC = 0, DG_BC_WALL = 1, DG_BC_FARFIELD = 2, DG_BC_HALO = 3 };
 int dg_set_boundary(dg_ctx *ctx, const int bc[6], const double q_inf[5]);
 
 /* Number of stage-kernel variants (column shape x shared-memory layout x residency) compiled into the
@@ -134,6 +138,33 @@ int dg_rk_step(dg_ctx *ctx, double dt, int nsteps);
  * nothing stepped) and one at the end returns *t_advanced = sum of the time steps taken and *dt_last = the last
  * one (host pointers, either may be NULL; DG_ESTATE if the state went non-physical on the way).  cfl > 0. */
 int dg_rk_step_cfl(dg_ctx *ctx, double cfl, int nsteps, double *t_advanced, double *dt_last);
+
+/* Block decomposition over several contexts / GPUs (one exchange of face
+ * data per Runge-Kutta stage).  The library does no communication itself: it exports and imports face traces, the
+ * caller moves them (NCCL / peer copies between GPUs, plain copies between contexts of one GPU).  All contexts of a
+ * decomposition must use the same p, the same column shape (variant) and, across a shared face, the same number of
+ * elements in the two transverse directions.
+ *   dg_halo_len(ctx, f)      doubles in the trace buffer of domain face f = 0..5 (x-, x+, y-, y+, z-, z+)
+ *   dg_halo_export(ctx, f, dst_dev)  gathers the face traces of the CURRENT state on face f (the T- of the first /
+ *                            T+ of the last elements along the axis) into the DEVICE buffer dst_dev,
+ *                            enqueued on the stream; this is what the neighbour across f needs
+ *   dg_set_halo(ctx, f, halo_dev)    the DEVICE buffer (dg_halo_len doubles, caller-owned, must stay valid) from which
+ *                            the kernels read the traces of the elements beyond face f when its condition is
+ *                            DG_BC_HALO: the export of the opposite face of the neighbour context; it must hold
+ *                            the neighbour's traces of the current state whenever dg_residual / dg_rk_stage runs
+ *   dg_rk_stage(ctx, dt, s)  ONE stage s = 0..4 of the LSERK45 step (dg_rk_step = stages 0..4 in a row), so that the
+ *                            caller can exchange the faces between stages: export -> move -> next stage.
+ * The interface flux of a shared face is evaluated by both contexts, bit-identically, so a decomposed run reproduces
+ * the single-context run bit for bit (tests/test_gpu_halo.py).  dg_rk_step_cfl is refused with halo faces (the CFL
+ * wavespeed is a maximum over all contexts: reduce dg_max_wavespeed across them and use dg_rk_stage). */
+/* Before dg_bind: element sizes h = {hx, hy, hz} given directly instead of extent / n (a block of a decomposed mesh
+ * must use the SAME doubles as its neighbours; extent * n_local / n_global divided by n_local again can differ in
+ * the last bit).  DG_ESTATE after dg_bind. */
+int dg_set_spacing(dg_ctx *ctx, const double h[3]);
+size_t dg_halo_len(const dg_ctx *ctx, int face);
+int dg_halo_export(dg_ctx *ctx, int face, double *dst_dev);
+int dg_set_halo(dg_ctx *ctx, int face, const double *halo_dev);
+int dg_rk_stage(dg_ctx *ctx, double dt, int stage);
 
 /* Paper-shaped per-kernel mode (Table II): the same spatial residual and stage
  * update as dg_rk_step, run as the paper's three kernels so that their times can be measured one by one (the fused

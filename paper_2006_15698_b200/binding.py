@@ -28,6 +28,11 @@ SYMBOLS = {
     "dg_residual": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
     "dg_max_wavespeed": (ctypes.c_int, [ctypes.c_void_p, _DP]),
     "dg_rk_step": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int]),
+    "dg_rk_stage": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int]),
+    "dg_set_spacing": (ctypes.c_int, [ctypes.c_void_p, _DP]),
+    "dg_halo_len": (ctypes.c_size_t, [ctypes.c_void_p, ctypes.c_int]),
+    "dg_halo_export": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]),
+    "dg_set_halo": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]),
     "dg_rk_step_cfl": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int, _DP, _DP]),
     "dg_get_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
     "dg_split_volume": (ctypes.c_int, [ctypes.c_void_p]),
@@ -122,7 +127,7 @@ class DG:
     """One mesh + one state vector on the GPU.  Arrays are float64, shape (nz,ny,nx,N,N,N,5)."""
 
     def __init__(self, nx, ny, nz, p, gamma=1.4, extent=(1.0, 1.0, 1.0), device="cuda:0", brick=None, bind=True,
-                 variant=None, poison=False):
+                 variant=None, poison=False, spacing=None):
         self.lib = load_library()
         self.nx, self.ny, self.nz, self.p, self.N = nx, ny, nz, p, p + 1
         self.gamma, self.extent = float(gamma), tuple(float(e) for e in extent)
@@ -137,6 +142,8 @@ class DG:
             self._check(self.lib.dg_set_brick(self._h, *brick))
         if variant is not None:
             self._check(self.lib.dg_set_variant(self._h, int(variant)))
+        if spacing is not None:
+            self._check(self.lib.dg_set_spacing(self._h, (ctypes.c_double * 3)(*[float(v) for v in spacing])))
         self.workspace = None
         self.device = None
         self._torch = None
@@ -258,6 +265,35 @@ class DG:
         with self._torch.cuda.device(self.device):
             self._check(self.lib.dg_rk_step_cfl(self._h, float(cfl), int(nsteps), ctypes.byref(t), ctypes.byref(dt)))
         return t.value, dt.value
+
+    # -- block decomposition over several contexts / GPUs: face export / import, stage by stage ----------
+    def rk_stage(self, dt, stage):
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.dg_rk_stage(self._h, float(dt), int(stage)))
+        return self
+
+    def halo_len(self, face):
+        return self.lib.dg_halo_len(self._h, int(face))
+
+    def halo_export(self, face, out=None):
+        """Face traces of the current state on domain face `face` into a float64 cuda tensor (what the neighbour needs)."""
+        torch = self._torch
+        if out is None:
+            out = torch.empty(self.halo_len(face), dtype=torch.float64, device=self.device)
+        assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == self.halo_len(face)
+        self._order_before(1)
+        with torch.cuda.device(self.device):
+            self._check(self.lib.dg_halo_export(self._h, int(face), out.data_ptr()))
+        self._order_after(1)
+        return out
+
+    def set_halo(self, face, buf):
+        """`buf`: float64 cuda tensor of halo_len(face) doubles the caller keeps alive and fills before every stage."""
+        assert buf.is_cuda and buf.dtype == self._torch.float64 and buf.is_contiguous() and buf.numel() == self.halo_len(face)
+        self._halo_keep = getattr(self, "_halo_keep", {})
+        self._halo_keep[int(face)] = buf
+        self._check(self.lib.dg_set_halo(self._h, int(face), buf.data_ptr()))
+        return self
 
     # -- paper-shaped per-kernel mode (Table II breakdown) ------------------------------------------
     def split_volume(self):

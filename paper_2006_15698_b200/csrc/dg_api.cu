@@ -160,6 +160,17 @@ __global__ void __launch_bounds__(256) dg_split_update_kernel(double *Q, double 
     }
 }
 
+// Gathers the runs src[o * outer_stride + i * inner_stride + 0 .. run) into a dense buffer (dg_halo_export).
+__global__ void __launch_bounds__(256) dg_pack_kernel(double *dst, const double *src, long long n_outer, long long outer_stride,
+                                                      long long n_inner, long long inner_stride, int run) {
+    const long long total = n_outer * n_inner * run;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+        const long long blk = idx / run, r = idx - blk * run;
+        const long long o = blk / n_inner, i = blk - o * n_inner;
+        dst[idx] = src[o * outer_stride + i * inner_stride + r];
+    }
+}
+
 __global__ void dg_fastmath_kernel(const double *x, double *r, double *q, size_t n) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) {
@@ -172,6 +183,7 @@ struct dg_ctx {
     int nx, ny, nz, p, N;
     double gamma;
     double extent[3];
+    double h[3];        // element size per axis (extent / n unless dg_set_spacing gave it)
     const DgKernelTable *kt;
     int variant;
     int nbx, nby;       // columns of bx x by elements
@@ -191,6 +203,7 @@ struct dg_ctx {
     int sms, blocks_per_sm;
     double g[3];        // 2/h_a per axis
     int bc[6];          // boundary condition per domain face (dg_set_boundary), 0 = periodic
+    const double *halo[6];   // DG_BC_HALO faces: the caller's device buffer with the neighbour context's traces
     double qinf[DG_NV];
     bool bound, has_state;
     cudaStream_t stream;
@@ -283,7 +296,10 @@ DgStageArgs stage_args(const dg_ctx *c, int mode) {
     a.gm1 = c->gamma - 1.0;
     a.mode = mode;
     for (int i = 0; i < 3; ++i) a.scale[i] = c->g[i];
-    for (int i = 0; i < 6; ++i) a.bc[i] = c->bc[i];
+    for (int i = 0; i < 6; ++i) {
+        a.bc[i] = (c->bc[i] == DG_BC_HALO) ? 0 : c->bc[i];
+        a.halo_ext[i] = (c->bc[i] == DG_BC_HALO) ? c->halo[i] : nullptr;
+    }
     for (int i = 0; i < DG_NV; ++i) a.qinf[i] = c->qinf[i];
     return a;
 }
@@ -316,28 +332,42 @@ int export_vector(dg_ctx *c, double *internal, double *out, int on_device, const
 // One LSERK45 step = 5 launches of the fused stage kernel.  cfl_factor > 0: the time step is formed on the device from
 // the wavespeed in scal[lcur] and the last stage reduces the wavespeed of the state it produces into the other slot
 // (a9 fused: no extra sweep over the state, no host round trip).
+int check_halos(dg_ctx *c) {
+    for (int f = 0; f < 6; ++f)
+        if (c->bc[f] == DG_BC_HALO && !c->halo[f]) return fail(c, DG_ESTATE, "face %d is a halo face but dg_set_halo was not called", f);
+    return DG_OK;
+}
+
+int enqueue_stage(dg_ctx *c, int s, double dt, double cfl_factor) {
+    const bool cfl = cfl_factor > 0.0;
+    DgStageArgs a = stage_args(c, DG_MODE_STAGE);
+    for (int i = 0; i < 3; ++i) a.scale[i] = cfl ? c->g[i] : dt * c->g[i];
+    a.rkA = (double)kRkA[s];
+    a.rkB = (double)kRkB[s];
+    a.want_lam = (cfl && s == 4) ? 1 : 0;
+    a.store_k = (s == 4) ? 0 : 1;
+    a.lam_in = cfl ? c->scal + c->lcur : nullptr;
+    a.cfl_factor = cfl_factor;
+    a.t_acc = (cfl && s == 0) ? reinterpret_cast<double *>(c->scal + 2) : nullptr;
+    a.lam_bits = c->scal + (1 - c->lcur);
+    cudaError_t e = c->kt->launch_stage(a, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "stage kernel");
+    c->launches++;
+    c->tcur = 1 - c->tcur;
+    return DG_OK;
+}
+
 int enqueue_step(dg_ctx *c, double dt, double cfl_factor) {
     const bool cfl = cfl_factor > 0.0;
-    unsigned long long *lam_in = c->scal + c->lcur, *lam_out = c->scal + (1 - c->lcur);
+    int rc = check_halos(c);
+    if (rc != DG_OK) return rc;
     if (cfl) {
-        cudaError_t e = cudaMemsetAsync(lam_out, 0, 8, c->stream);
+        cudaError_t e = cudaMemsetAsync(c->scal + (1 - c->lcur), 0, 8, c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "memset");
     }
     for (int s = 0; s < 5; ++s) {
-        DgStageArgs a = stage_args(c, DG_MODE_STAGE);
-        for (int i = 0; i < 3; ++i) a.scale[i] = cfl ? c->g[i] : dt * c->g[i];
-        a.rkA = (double)kRkA[s];
-        a.rkB = (double)kRkB[s];
-        a.want_lam = (cfl && s == 4) ? 1 : 0;
-        a.store_k = (s == 4) ? 0 : 1;
-        a.lam_in = cfl ? lam_in : nullptr;
-        a.cfl_factor = cfl_factor;
-        a.t_acc = (cfl && s == 0) ? reinterpret_cast<double *>(c->scal + 2) : nullptr;
-        a.lam_bits = lam_out;
-        cudaError_t e = c->kt->launch_stage(a, c->stream);
-        if (e != cudaSuccess) return cuda_fail(c, e, "stage kernel");
-        c->launches++;
-        c->tcur = 1 - c->tcur;
+        rc = enqueue_stage(c, s, dt, cfl_factor);
+        if (rc != DG_OK) return rc;
     }
     if (cfl) c->lcur = 1 - c->lcur;
     c->lam_valid = cfl;
@@ -423,6 +453,9 @@ int dg_create(dg_ctx **out, int nx, int ny, int nz, int p, double gamma, const d
     c->nx = nx; c->ny = ny; c->nz = nz; c->p = p; c->N = p + 1;
     c->gamma = gamma;
     for (int a = 0; a < 3; ++a) c->extent[a] = extent[a];
+    c->h[0] = extent[0] / nx;
+    c->h[1] = extent[1] / ny;
+    c->h[2] = extent[2] / nz;
     c->state_len = (size_t)nx * ny * nz * (size_t)(c->N * c->N * c->N) * DG_NV;
     // default variant: the first compiled column shape that wastes < 4 % of its nodes on padding of ragged
     // columns (they are listed fastest first), else the one that wastes least
@@ -470,7 +503,7 @@ int dg_set_boundary(dg_ctx *c, const int bc[6], const double q_inf[5]) {
     bool far = false;
     for (int a = 0; a < 3; ++a) {
         const int lo = bc[2 * a], hi = bc[2 * a + 1];
-        if (lo < 0 || lo > 2 || hi < 0 || hi > 2) return fail(c, DG_EINVAL, "boundary condition outside 0..2");
+        if (lo < 0 || lo > 3 || hi < 0 || hi > 3) return fail(c, DG_EINVAL, "boundary condition outside 0..3");
         if ((lo == DG_BC_PERIODIC) != (hi == DG_BC_PERIODIC))
             return fail(c, DG_EINVAL, "an axis is periodic on both of its faces or on neither");
         far = far || lo == DG_BC_FARFIELD || hi == DG_BC_FARFIELD;
@@ -541,9 +574,7 @@ int dg_bind(dg_ctx *c, void *ws, size_t bytes, void *stream) {
     }
     e = cudaMemsetAsync(c->scal, 0, 256, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "workspace memset");
-    c->g[0] = 2.0 / (c->extent[0] / c->nx);
-    c->g[1] = 2.0 / (c->extent[1] / c->ny);
-    c->g[2] = 2.0 / (c->extent[2] / c->nz);
+    for (int a = 0; a < 3; ++a) c->g[a] = 2.0 / c->h[a];
     DgRefOps ref;
     build_ref_ops(c->N, ref);
     e = c->kt->prepare(ref, &c->blocks_per_sm);
@@ -575,6 +606,8 @@ int dg_set_state(dg_ctx *c, const double *q, int on_device) {
 int dg_residual(dg_ctx *c, double *r_out, int on_device) {
     if (!c || !r_out) return c ? fail(c, DG_EINVAL, "null residual pointer") : DG_EINVAL;
     if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_residual needs dg_bind and dg_set_state first");
+    const int hrc = check_halos(c);
+    if (hrc != DG_OK) return hrc;
     DgStageArgs a = stage_args(c, DG_MODE_RESIDUAL);
     cudaError_t e = c->kt->launch_stage(a, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "residual kernel");
@@ -599,13 +632,80 @@ int dg_rk_step(dg_ctx *c, double dt, int nsteps) {
     return DG_OK;
 }
 
+int dg_rk_stage(dg_ctx *c, double dt, int stage) {
+    if (!c) return DG_EINVAL;
+    if (stage < 0 || stage > 4 || !std::isfinite(dt)) return fail(c, DG_EINVAL, "stage outside 0..4 or dt not finite");
+    if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_rk_stage needs dg_bind and dg_set_state first");
+    int rc = check_halos(c);
+    if (rc != DG_OK) return rc;
+    c->lam_valid = false;
+    return enqueue_stage(c, stage, dt, 0.0);
+}
+
+int dg_set_spacing(dg_ctx *c, const double h[3]) {
+    if (!c || !h) return c ? fail(c, DG_EINVAL, "null spacing") : DG_EINVAL;
+    if (c->bound) return fail(c, DG_ESTATE, "dg_set_spacing after dg_bind");
+    for (int a = 0; a < 3; ++a)
+        if (!(h[a] > 0.0) || !std::isfinite(h[a])) return fail(c, DG_EINVAL, "element size must be positive and finite");
+    const int n[3] = {c->nx, c->ny, c->nz};
+    for (int a = 0; a < 3; ++a) {
+        c->h[a] = h[a];
+        c->extent[a] = h[a] * n[a];
+    }
+    return DG_OK;
+}
+
+int dg_set_halo(dg_ctx *c, int face, const double *halo_dev) {
+    if (!c || face < 0 || face > 5) return c ? fail(c, DG_EINVAL, "face outside 0..5") : DG_EINVAL;
+    c->halo[face] = halo_dev;
+    return DG_OK;
+}
+
+size_t dg_halo_len(const dg_ctx *c, int face) {
+    if (!c || face < 0 || face > 5) return 0;
+    if (face < 2) return (size_t)c->nz * c->nby * DG_NV * c->kt->cx;
+    if (face < 4) return (size_t)c->nz * c->nbx * DG_NV * c->kt->cy;
+    return (size_t)c->nby * c->nbx * DG_NV * c->kt->cz;
+}
+
+int dg_halo_export(dg_ctx *c, int face, double *dst_dev) {
+    if (!c || !dst_dev || face < 0 || face > 5) return c ? fail(c, DG_EINVAL, "bad face or null buffer") : DG_EINVAL;
+    if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_halo_export needs dg_bind and dg_set_state first");
+    const long long txy = c->kt->txy, tz = c->kt->tz, cx = c->kt->cx, cy = c->kt->cy, cz = c->kt->cz;
+    const long long nbx = c->nbx, nby = c->nby, nz = c->nz;
+    const double *src;
+    long long n_outer, outer_stride, n_inner, inner_stride;
+    int run;
+    if (face < 2) {          // T- of the first / T+ of the last column along x, every (ez, by)
+        src = c->Txy[c->tcur] + (face == 0 ? 0 : (nbx - 1) * txy + DG_NV * cx);
+        n_outer = 1; outer_stride = 0; n_inner = nz * nby; inner_stride = nbx * txy; run = (int)(DG_NV * cx);
+    } else if (face < 4) {   // ... along y, every (ez, bx)
+        src = c->Txy[c->tcur] + 2 * DG_NV * cx + (face == 2 ? 0 : (nby - 1) * nbx * txy + DG_NV * cy);
+        n_outer = nz; outer_stride = nby * nbx * txy; n_inner = nbx; inner_stride = txy; run = (int)(DG_NV * cy);
+    } else {                 // T- of the first / T+ of the last layer, every column
+        src = c->Tz[c->tcur] + (face == 4 ? 0 : ((long long)c->nchunks - 1) * nby * nbx * tz + DG_NV * cz);
+        n_outer = 1; outer_stride = 0; n_inner = nby * nbx; inner_stride = tz; run = (int)(DG_NV * cz);
+    }
+    const long long total = n_outer * n_inner * run;
+    const long long want = (total + 255) / 256, cap = (long long)(c->sms > 0 ? c->sms : 1) * 16;
+    dg_pack_kernel<<<(unsigned)(want < cap ? (want ? want : 1) : cap), 256, 0, c->stream>>>(dst_dev, src, n_outer, outer_stride,
+                                                                                       n_inner, inner_stride, run);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, "pack kernel");
+    c->launches++;
+    return DG_OK;
+}
+
 int dg_rk_step_cfl(dg_ctx *c, double cfl, int nsteps, double *t_advanced, double *dt_last) {
     if (!c) return DG_EINVAL;
     if (nsteps < 0 || !(cfl > 0.0) || !std::isfinite(cfl)) return fail(c, DG_EINVAL, "nsteps < 0 or cfl not positive");
     if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_rk_step_cfl needs dg_bind and dg_set_state first");
-    double hmin = c->extent[0] / c->nx;
-    if (c->extent[1] / c->ny < hmin) hmin = c->extent[1] / c->ny;
-    if (c->extent[2] / c->nz < hmin) hmin = c->extent[2] / c->nz;
+    for (int f = 0; f < 6; ++f)
+        if (c->bc[f] == DG_BC_HALO)
+            return fail(c, DG_EUNSUPPORTED, "with halo faces the wavespeed is a maximum over all contexts: use dg_max_wavespeed + dg_rk_stage");
+    double hmin = c->h[0];
+    if (c->h[1] < hmin) hmin = c->h[1];
+    if (c->h[2] < hmin) hmin = c->h[2];
     // the wavespeed of the state the call starts from is checked on the host (one read-back per call) ...
     double lam = 0.0;
     int rc = read_lam(c, &lam);

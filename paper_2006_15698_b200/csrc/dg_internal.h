@@ -83,6 +83,10 @@ struct DgStageArgs {
     const unsigned long long *lam_in;
     double cfl_factor;    // cfl * min(h) / (2p + 1)
     double *t_acc;
+    // Faces whose neighbour lives in ANOTHER context (block decomposition over GPUs): the traces of
+    // the elements beyond domain face f come from the caller's buffer halo_ext[f] (null: none), laid out like the
+    // neighbour's export (dg_halo_export): x faces [ez][by][5][CX], y faces [ez][bx][5][CY], z faces [by][bx][5][CZ]
+    const double *halo_ext[6];
     int bc[6];            // domain faces x-, x+, y-, y+, z-, z+: 0 periodic, 1 slip wall, 2 far field (R19)
     double qinf[DG_NV];   // far-field state (conserved variables)
 };
@@ -124,6 +128,7 @@ struct DgKernelTable {
     long long slot;          // doubles per layer slot in Q/K
     long long txy;           // x/y face-trace doubles per layer slot
     long long tz;            // z face-trace doubles per chunk slot
+    int cx, cy, cz;          // face nodes of a layer slot's x side, y side, and of a column's z side
     int reload;
     int minb;                // blocks per SM the kernel is compiled for (__launch_bounds__)
     // upload the reference operators, opt in to the shared memory size; *blocks_per_sm = resident blocks per SM

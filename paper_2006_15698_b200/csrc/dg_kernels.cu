@@ -272,6 +272,7 @@ struct BlockInfo {
     double *tz_out;
     double *kslot;             // this column's K slot of layer z0
     long long tstride;         // doubles between consecutive layers in Txy
+    long long hstride[4];      // ... in the four blocks of halo[] (Txy, or an external halo buffer)
     long long kstride;         // ... in Q and K
     double gamma, gm1, rkA, rkB, scale[3];
     int ext0, ext1, readK, storeK, nl;
@@ -713,16 +714,15 @@ __device__ __forceinline__ void copy_out(double *gdst, const double *ssrc, int l
 }
 
 template <class C, int MODE>
-__device__ __forceinline__ void copy_warp(const DgStageArgs &a, int lane, int bxi, int byi, int z0, int nl, bool readK,
-                                          double *Qb0, double *Qb1, double *KR, uint64_t *fullq, uint64_t *fullk) {
+__device__ __forceinline__ void copy_warp(const DgStageArgs &a, const BlockInfo *bi, int lane, int bxi, int byi, int z0, int nl,
+                                          bool readK, double *Qb0, double *Qb1, double *KR, uint64_t *fullq, uint64_t *fullk) {
     const size_t lstride = (size_t)a.nbx * a.nby;                    // slots per layer
     const size_t slot0 = (size_t)z0 * lstride + (size_t)byi * a.nbx + bxi;
     copy_in<C>(Qb0, a.Q + slot0 * C::SLOT, &fullq[0], lane);
     if (readK) copy_in<C>(KR, a.K + slot0 * C::SLOT, fullk, lane);   // later layers: issued by the compute warps
     if (nl > 1) copy_in<C>(Qb1, a.Q + (slot0 + lstride) * C::SLOT, &fullq[1], lane);
     // L2 prefetch of the neighbour columns' traces of the first layer (4 blocks of 5 Ca doubles)
-    if (lane < 2) l2_prefetch(halo_source<C, 0>(a.Txy_old, a.nbx, a.nby, bxi, byi, z0, lane), DG_NV * C::CX * 8);
-    else if (lane < 4) l2_prefetch(halo_source<C, 1>(a.Txy_old, a.nbx, a.nby, bxi, byi, z0, lane - 2), DG_NV * C::CY * 8);
+    if (lane < 4) l2_prefetch(bi->halo[lane], DG_NV * (lane < 2 ? C::CX : C::CY) * 8);
     for (int it = 0; it < nl; ++it) {
         double *Qcur = (it & 1) ? Qb1 : Qb0;
         const size_t slot = slot0 + (size_t)it * lstride;
@@ -769,12 +769,14 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
     mbar_wait(&fullq[it & 1], (it >> 1) & 1);
     {
         const Geo gx = make_geo<C, 0>(lx);
-        xy_pass<C, 0, MODE, BC>(bi, gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, bi->halo[0] + toff, bi->halo[1] + toff, Qs,
+        xy_pass<C, 0, MODE, BC>(bi, gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, bi->halo[0] + it * bi->hstride[0],
+                                bi->halo[1] + it * bi->hstride[1], Qs,
                             KR, Tms, Fss, fullk, it & 1);
     }
     {
         const Geo gy = make_geo<C, 1>(lx);
-        xy_pass<C, 1, MODE, BC>(bi, gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, bi->halo[2] + toff, bi->halo[3] + toff, Qs,
+        xy_pass<C, 1, MODE, BC>(bi, gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, bi->halo[2] + it * bi->hstride[2],
+                                bi->halo[3] + it * bi->hstride[3], Qs,
                             KR, Tms, Fss, fullk, it & 1);
     }
     const bool last_layer = it + 1 == bi->nl;
@@ -782,7 +784,7 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
     // copy warp can only fetch once this layer's K has left shared memory, and the neighbour columns' traces.
     // Asked for earlier, L2 has evicted them again by the time they are used (measured: +25 % DRAM reads).
     if (!last_layer && l < 5) {
-        if (l < 4) l2_prefetch(bi->halo[l] + toff + bi->tstride, DG_NV * (l < 2 ? C::CX : C::CY) * 8);
+        if (l < 4) l2_prefetch(bi->halo[l] + (it + 1) * bi->hstride[l], DG_NV * (l < 2 ? C::CX : C::CY) * 8);
         else if (bi->readK) l2_prefetch(bi->kslot + (long long)(it + 1) * bi->kstride, C::NPL * C::HP * 8);
     }
     if (!last_layer) mbar_wait(&fullq[(it + 1) & 1], ((it + 1) >> 1) & 1);
@@ -826,15 +828,24 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         BlockInfo *bi = reinterpret_cast<BlockInfo *>(smem + SM::INFO);
         const size_t cstride = (size_t)a.nbx * a.nby, col = (size_t)byi * a.nbx + bxi;
+        // neighbour columns' traces: the periodic neighbour's Txy block, or (block decomposition over GPUs) the
+        // caller's halo buffer of that domain face
         bi->halo[0] = halo_source<C, 0>(a.Txy_old, a.nbx, a.nby, bxi, byi, z0, 0);
         bi->halo[1] = halo_source<C, 0>(a.Txy_old, a.nbx, a.nby, bxi, byi, z0, 1);
         bi->halo[2] = halo_source<C, 1>(a.Txy_old, a.nbx, a.nby, bxi, byi, z0, 0);
         bi->halo[3] = halo_source<C, 1>(a.Txy_old, a.nbx, a.nby, bxi, byi, z0, 1);
+        for (int f = 0; f < 4; ++f) bi->hstride[f] = (long long)cstride * C::TXY;
+        if (a.halo_ext[0] && bxi == 0) { bi->halo[0] = a.halo_ext[0] + ((size_t)z0 * a.nby + byi) * (DG_NV * C::CX); bi->hstride[0] = (long long)a.nby * (DG_NV * C::CX); }
+        if (a.halo_ext[1] && bxi + 1 == a.nbx) { bi->halo[1] = a.halo_ext[1] + ((size_t)z0 * a.nby + byi) * (DG_NV * C::CX); bi->hstride[1] = (long long)a.nby * (DG_NV * C::CX); }
+        if (a.halo_ext[2] && byi == 0) { bi->halo[2] = a.halo_ext[2] + ((size_t)z0 * a.nbx + bxi) * (DG_NV * C::CY); bi->hstride[2] = (long long)a.nbx * (DG_NV * C::CY); }
+        if (a.halo_ext[3] && byi + 1 == a.nby) { bi->halo[3] = a.halo_ext[3] + ((size_t)z0 * a.nbx + bxi) * (DG_NV * C::CY); bi->hstride[3] = (long long)a.nbx * (DG_NV * C::CY); }
         bi->txy_out = a.Txy_new + ((size_t)z0 * cstride + col) * C::TXY;
         // z traces at the ends of the chunk: T+ of the chunk below (its side 1), T- of the chunk above (its side 0)
         const int clo = (chunk == 0) ? a.nchunks - 1 : chunk - 1, chi = (chunk + 1 == a.nchunks) ? 0 : chunk + 1;
         bi->tz_lo = a.Tz_old + ((size_t)clo * cstride + col) * C::TZ + DG_NV * C::CZ;
         bi->tz_hi = a.Tz_old + ((size_t)chi * cstride + col) * C::TZ;
+        if (a.halo_ext[4] && chunk == 0) bi->tz_lo = a.halo_ext[4] + col * (DG_NV * C::CZ);
+        if (a.halo_ext[5] && chunk + 1 == a.nchunks) bi->tz_hi = a.halo_ext[5] + col * (DG_NV * C::CZ);
         bi->tz_out = a.Tz_new + ((size_t)chunk * cstride + col) * C::TZ;
         bi->tstride = (long long)cstride * C::TXY;
         bi->kslot = a.K + ((size_t)z0 * cstride + col) * C::SLOT;
@@ -869,7 +880,7 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
     }
     __syncthreads();
     if (tid >= C::NCOMP) {
-        copy_warp<C, MODE>(a, tid - C::NCOMP, bxi, byi, z0, nl, readK, smem + SM::QB0, smem + SM::QB1, smem + SM::KR, fullq,
+        copy_warp<C, MODE>(a, reinterpret_cast<const BlockInfo *>(smem + SM::INFO), tid - C::NCOMP, bxi, byi, z0, nl, readK, smem + SM::QB0, smem + SM::QB1, smem + SM::KR, fullq,
                            fullk);
         return;
     }
@@ -1226,7 +1237,7 @@ cudaError_t launch_wavespeed(const DgWaveArgs &a, int sms, cudaStream_t s) {
 template <class C>
 constexpr DgKernelTable make_table() {
     return DgKernelTable{C::N,       C::BX,          C::BY,         C::THREADS,      Smem<C>::BYTES,     C::SLOT,
-                         C::TXY,     C::TZ,          C::RELOAD ? 1 : 0, C::MINB, &prepare<C>, &launch_stage<C>,  &launch_traces<C>, &launch_split_volume<C>, &launch_split_surface<C>,
+                         C::TXY,     C::TZ,          C::CX, C::CY, C::CZ, C::RELOAD ? 1 : 0, C::MINB, &prepare<C>, &launch_stage<C>,  &launch_traces<C>, &launch_split_volume<C>, &launch_split_surface<C>,
                          &launch_layout<C>, &launch_wavespeed<C>};
 }
 

@@ -1,0 +1,279 @@
+"""Block decomposition of one mesh over several contexts / GPUs.
+
+The paper's coarse-grain parallelism is an MPI mesh decomposition with one exchange of face data per Runge-Kutta
+stage.  Here: one process per GPU, `torch.distributed` (NCCL over NVLink / NVSwitch) for the plumbing, and the
+library's face export / import (dg_halo_export, dg_set_halo, dg_rk_stage in include/dg_b200.h) for the data: a rank's
+context treats the faces it shares with other ranks as DG_BC_HALO faces, exports the traces of its own boundary
+elements after every stage and receives the neighbours' straight into the buffers its kernels read.  All arithmetic
+stays in the CUDA kernels; this module is argument marshalling and message plumbing only.
+
+`Decomposition` is pure host logic (no torch, no GPU): who owns which elements, who is whose neighbour across which
+face, in which order messages are posted.  `DistributedDG` is one rank's part of the mesh.  The exchange itself is a
+callable, so that the tests can run several ranks' contexts inside one process on one GPU (copies instead of messages).
+"""
+PERIODIC, WALL, FARFIELD, HALO = 0, 1, 2, 3
+FACES = ("x-", "x+", "y-", "y+", "z-", "z+")
+
+
+def _split(n, parts):
+    """Element ranges of `parts` contiguous pieces of 0..n, sizes differing by at most one."""
+    base, extra = divmod(n, parts)
+    out, lo = [], 0
+    for i in range(parts):
+        hi = lo + base + (1 if i < extra else 0)
+        out.append((lo, hi))
+        lo = hi
+    return out
+
+
+class Decomposition:
+    """procs = (px, py, pz) ranks along x, y, z; rank = cx + px * (cy + py * cz).  bc = the GLOBAL domain's conditions
+    (x-, x+, y-, y+, z-, z+), values as in include/dg_b200.h."""
+
+    def __init__(self, n, procs, bc=(PERIODIC,) * 6):
+        self.n = tuple(int(v) for v in n)
+        self.procs = tuple(int(v) for v in procs)
+        self.bc = tuple(int(v) for v in bc)
+        if any(p < 1 for p in self.procs) or any(p > m for p, m in zip(self.procs, self.n)):
+            raise ValueError("every rank needs at least one element along every axis")
+        for a in range(3):
+            if (self.bc[2 * a] == PERIODIC) != (self.bc[2 * a + 1] == PERIODIC):
+                raise ValueError("an axis is periodic on both of its faces or on neither")
+        self.size = self.procs[0] * self.procs[1] * self.procs[2]
+        self.ranges = [_split(self.n[a], self.procs[a]) for a in range(3)]
+
+    def coords(self, rank):
+        px, py, _ = self.procs
+        return (rank % px, (rank // px) % py, rank // (px * py))
+
+    def rank_of(self, c):
+        px, py, _ = self.procs
+        return c[0] + px * (c[1] + py * c[2])
+
+    def local_box(self, rank):
+        """((x0, x1), (y0, y1), (z0, z1)): the rank's element ranges in the global mesh."""
+        c = self.coords(rank)
+        return tuple(self.ranges[a][c[a]] for a in range(3))
+
+    def local_n(self, rank):
+        return tuple(hi - lo for lo, hi in self.local_box(rank))
+
+    def neighbour(self, rank, face):
+        """Rank owning the elements beyond `face` of `rank`, or None on a non-periodic domain face.  With one rank
+        along a periodic axis the neighbour is the rank itself (the context then simply stays periodic there)."""
+        a, side = face // 2, face % 2
+        c = list(self.coords(rank))
+        c[a] += 1 if side else -1
+        if c[a] < 0 or c[a] >= self.procs[a]:
+            if self.bc[face] != PERIODIC:
+                return None
+            c[a] %= self.procs[a]
+        return self.rank_of(c)
+
+    def local_bc(self, rank):
+        """Boundary conditions of the rank's context: HALO where another rank is the neighbour."""
+        out = []
+        for f in range(6):
+            nb = self.neighbour(rank, f)
+            if nb is None:
+                out.append(self.bc[f])
+            elif nb == rank:
+                out.append(PERIODIC)
+            else:
+                out.append(HALO)
+        return tuple(out)
+
+    def sends(self, rank):
+        """[(face, neighbour)] in the order this rank posts its sends: face order.  The export of face f feeds the
+        neighbour's face f ^ 1."""
+        return [(f, nb) for f in range(6) for nb in [self.neighbour(rank, f)] if nb is not None and nb != rank]
+
+    def recvs(self, rank):
+        """[(my face, neighbour)] in the order this rank posts its receives: for every peer, the order in which THAT
+        peer posts its sends to me (point-to-point messages between two ranks match in posting order)."""
+        out = []
+        for peer in range(self.size):
+            if peer == rank:
+                continue
+            for f, nb in self.sends(peer):
+                if nb == rank:
+                    out.append((f ^ 1, peer))
+        return out
+
+
+def choose_variant(dec, p, shapes):
+    """One column shape for ALL ranks (neighbours must agree on the face-trace layout): the first compiled variant
+    (they are listed fastest first) that pads no rank's local mesh by 4 % or more, else the one that pads least.
+    shapes = [(bx, by)] of the compiled variants of degree p."""
+    worst = []
+    for bx, by in shapes:
+        w = 0.0
+        for r in range(dec.size):
+            nx, ny, _ = dec.local_n(r)
+            padded = (-(-nx // bx) * bx) * (-(-ny // by) * by)
+            w = max(w, padded / float(nx * ny) - 1.0)
+        worst.append(w)
+    for v, w in enumerate(worst):
+        if w < 0.04:
+            return v
+    return min(range(len(shapes)), key=lambda v: worst[v])
+
+
+def variant_shapes(p):
+    """(bx, by) of every stage-kernel variant compiled for degree p."""
+    from .binding import DG, load_library
+    out = []
+    for v in range(load_library().dg_variant_count(p)):
+        probe = DG(8, 8, 8, p, bind=False, variant=v)
+        info = probe.kernel_info()
+        out.append((info["bx"], info["by"]))
+        probe.close()
+    return out
+
+
+def exchange_torch_distributed(dist):
+    """Face exchange over torch.distributed point-to-point operations (NCCL: GPU buffers over NVLink)."""
+    def run(rank, sends, recvs):
+        ops = [dist.P2POp(dist.isend, buf, peer, tag=face) for face, peer, buf in sends]
+        ops += [dist.P2POp(dist.irecv, buf, peer, tag=face ^ 1) for face, peer, buf in recvs]
+        if ops:
+            for req in dist.batch_isend_irecv(ops):
+                req.wait()
+    return run
+
+
+class DistributedDG:
+    """One rank's block of a decomposed mesh.  `q` arrays are the rank's LOCAL canonical arrays
+    (nz_l, ny_l, nx_l, N, N, N, 5); `exchange(rank, sends, recvs)` moves [(face, peer, tensor)] lists (default:
+    torch.distributed); `reduce_max(x)` returns the maximum of a float over all ranks (default: all_reduce)."""
+
+    def __init__(self, n, p, gamma, extent, procs, rank, bc=(PERIODIC,) * 6, q_inf=None, device="cuda:0", exchange=None,
+                 reduce_max=None, variant=None):
+        import torch
+        from .binding import DG
+        self.dec = Decomposition(n, procs, bc)
+        self.rank, self.p = int(rank), int(p)
+        self.box = self.dec.local_box(self.rank)
+        nl = self.dec.local_n(self.rank)
+        ext_l = tuple(extent[a] * nl[a] / float(self.dec.n[a]) for a in range(3))
+        if variant is None:
+            variant = choose_variant(self.dec, p, variant_shapes(p))
+        # the element sizes are those of the GLOBAL mesh, the same doubles on every rank
+        self.dg = DG(*nl, p, gamma, ext_l, device=device, variant=variant,
+                     spacing=tuple(extent[a] / float(self.dec.n[a]) for a in range(3)))
+        self.local_bc = self.dec.local_bc(self.rank)
+        self.dg.set_boundary(self.local_bc, q_inf)
+        dev = self.dg.device
+        self._send = [(f, nb, torch.empty(self.dg.halo_len(f), dtype=torch.float64, device=dev)) for f, nb in self.dec.sends(self.rank)]
+        self._recv = [(f, nb, torch.empty(self.dg.halo_len(f), dtype=torch.float64, device=dev)) for f, nb in self.dec.recvs(self.rank)]
+        for f, _, buf in self._recv:
+            self.dg.set_halo(f, buf)
+        if exchange is None or reduce_max is None:
+            import torch.distributed as dist
+            if exchange is None:
+                exchange = exchange_torch_distributed(dist)
+            if reduce_max is None:
+                def reduce_max(x):
+                    t = torch.tensor([x], dtype=torch.float64, device=dev)
+                    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                    return float(t.item())
+        self._exchange, self._reduce_max = exchange, reduce_max
+
+    # the two halves of an exchange are separate so that a single process can drive several ranks (tests)
+    def export_faces(self):
+        for f, _, buf in self._send:
+            self.dg.halo_export(f, buf)
+        return self._send
+
+    def exchange(self):
+        if not self._send and not self._recv:
+            return
+        self.export_faces()
+        self.dg.stream.synchronize()                 # the messages read buffers written on the library's stream
+        self._exchange(self.rank, self._send, self._recv)
+
+    def set_state(self, q_local):
+        self.dg.set_state(q_local)
+        self.exchange()
+        return self
+
+    def residual(self, out=None):
+        return self.dg.residual(out)
+
+    def max_wavespeed(self):
+        return self._reduce_max(self.dg.max_wavespeed())
+
+    def rk_step(self, dt, nsteps=1):
+        for _ in range(int(nsteps)):
+            for stage in range(5):
+                self.dg.rk_stage(dt, stage)
+                self.exchange()
+        return self
+
+    def rk_step_cfl(self, cfl, nsteps=1, h_min=None):
+        """dt = cfl h_min / ((2p+1) lam) with lam the maximum wavespeed over ALL ranks, before every step."""
+        t = 0.0
+        for _ in range(int(nsteps)):
+            dt = cfl * h_min / ((2 * self.p + 1) * self.max_wavespeed())
+            self.rk_step(dt, 1)
+            t += dt
+        return t
+
+    def get_state(self, out=None):
+        return self.dg.get_state(out)
+
+    def close(self):
+        self.dg.close()
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# several ranks' contexts inside ONE process on one GPU (tests; no messages, no kernels waiting on one another:
+# every rank's stage is an ordinary launch, the faces move by device copies in between)
+# ------------------------------------------------------------------------------------------------------------------
+def exchange_in_process(ranks):
+    """ranks: list of DistributedDG indexed by rank, all in this process."""
+    exports = {}
+    for r in ranks:
+        for f, _, buf in r.export_faces():
+            exports[(r.rank, f)] = buf
+    for r in ranks:
+        for f, peer, buf in r._recv:
+            buf.copy_(exports[(peer, f ^ 1)])
+
+
+def make_in_process(n, p, gamma, extent, procs, bc=(PERIODIC,) * 6, q_inf=None, device="cuda:0", variant=None):
+    dec = Decomposition(n, procs, bc)
+    if variant is None:
+        variant = choose_variant(dec, p, variant_shapes(p))
+    nothing = lambda rank, sends, recvs: None
+    return [DistributedDG(n, p, gamma, extent, procs, r, bc, q_inf, device, exchange=nothing, reduce_max=lambda x: x,
+                          variant=variant) for r in range(dec.size)]
+
+
+def set_state_in_process(ranks, q_global):
+    """q_global: the global canonical array (nz, ny, nx, N, N, N, 5); every rank takes its block."""
+    import numpy as np
+    for r in ranks:
+        (x0, x1), (y0, y1), (z0, z1) = r.box
+        r.dg.set_state(np.ascontiguousarray(q_global[z0:z1, y0:y1, x0:x1]))
+    exchange_in_process(ranks)
+
+
+def rk_step_in_process(ranks, dt, nsteps=1):
+    for _ in range(int(nsteps)):
+        for stage in range(5):
+            for r in ranks:
+                r.dg.rk_stage(dt, stage)
+            exchange_in_process(ranks)
+
+
+def gather_in_process(ranks, what="state"):
+    """Global canonical array assembled from the ranks' blocks (what = "state" or "residual")."""
+    import numpy as np
+    dec = ranks[0].dec
+    N = ranks[0].p + 1
+    out = np.empty((dec.n[2], dec.n[1], dec.n[0], N, N, N, 5))
+    for r in ranks:
+        (x0, x1), (y0, y1), (z0, z1) = r.box
+        out[z0:z1, y0:y1, x0:x1] = r.dg.get_state() if what == "state" else r.dg.residual()
+    return out

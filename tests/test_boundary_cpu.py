@@ -102,7 +102,10 @@ def test_set_boundary_validates_its_arguments():
     assert lib.dg_set_boundary(h, IA(0, 0, 0, 0, 0, 0), None) == 0
     assert lib.dg_set_boundary(h, IA(1, 1, 0, 0, 1, 1), None) == 0                     # walls need no state
     assert lib.dg_set_boundary(h, IA(1, 0, 0, 0, 0, 0), None) == 1                     # periodic on one face only
-    assert lib.dg_set_boundary(h, IA(3, 3, 0, 0, 0, 0), None) == 1
+    assert lib.dg_set_boundary(h, IA(4, 4, 0, 0, 0, 0), None) == 1
+    assert lib.dg_set_boundary(h, IA(3, 1, 0, 0, 3, 3), None) == 0                     # halo faces (other contexts)
+    assert lib.dg_halo_len(h, 0) == lib.dg_halo_len(h, 1) > 0 and lib.dg_halo_len(h, 6) == 0
+    assert lib.dg_set_halo(h, 7, None) == 1
     assert lib.dg_set_boundary(h, IA(2, 2, 0, 0, 0, 0), None) == 1                     # far field without a state
     assert lib.dg_set_boundary(h, IA(2, 2, 0, 0, 0, 0), DA(1.0, 0.1, 0.0, 0.0, float("nan"))) == 1
     assert lib.dg_set_boundary(h, IA(2, 1, 0, 0, 0, 0), DA(1.0, 0.1, 0.0, 0.0, 2.5)) == 0

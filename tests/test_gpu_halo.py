@@ -1,0 +1,74 @@
+"""Block decomposition over several contexts: the ranks' contexts run inside one process on the one
+GPU this box has, faces move by device copies between the stages (no kernel waits on another).  The decomposed run must
+reproduce the single-context run BIT FOR BIT (a shared face's interface flux is evaluated by both sides, bit-identically)
+and match the oracle of the whole mesh."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import Oracle                                    # noqa: E402
+from oracle.parity import relerr                             # noqa: E402
+from paper_2006_15698_b200 import DG                         # noqa: E402
+from paper_2006_15698_b200 import decomposed as D            # noqa: E402
+from paper_2006_15698_b200 import inputs as I                # noqa: E402
+
+G = 1.4
+ORC = Oracle("omp")
+
+
+def rough_field(nx, ny, nz, p, extent, seed=11):
+    return I.density_wave(nx, ny, nz, p, extent, vel=(0.5, -0.3, 0.2), noise=5e-2, seed=seed, waves=(1, 2, 1))
+
+
+@pytest.mark.parametrize("procs", [(2, 1, 1), (1, 2, 1), (1, 1, 2), (2, 2, 2), (3, 1, 2)])
+@pytest.mark.parametrize("p", [1, 3, 4])
+def test_decomposed_run_equals_the_single_context_run_bit_for_bit(procs, p):
+    n, ext = (7, 6, 5), (1.0, 0.9, 0.8)                        # uneven blocks, ragged columns
+    q = rough_field(*n, p, ext)
+    dt = I.cfl_dt(ORC.max_wavespeed(q, p, G), p, ext, n, 0.1)
+    ranks = D.make_in_process(n, p, G, ext, procs)
+    variant = ranks[0].dg.kernel_info()["variant"]
+    single = DG(*n, p, G, ext, variant=variant)
+    D.set_state_in_process(ranks, q)
+    single.set_state(q)
+    r_dec, r_one = D.gather_in_process(ranks, "residual"), single.residual()
+    assert np.array_equal(r_dec, r_one), relerr(r_dec, r_one)
+    assert relerr(r_dec, ORC.residual(q, p, G, ext)) < 1e-11
+    D.rk_step_in_process(ranks, dt, 3)
+    q_dec, q_one = D.gather_in_process(ranks), single.rk_step(dt, 3).get_state()
+    assert np.array_equal(q_dec, q_one), relerr(q_dec, q_one)
+    assert relerr(q_dec, ORC.rk_step(q, p, G, ext, dt, 3)) < 1e-12
+    lam = max(r.max_wavespeed() for r in ranks)
+    assert abs(lam - ORC.max_wavespeed(q_dec, p, G)) <= 4e-16 * lam
+    for r in ranks:
+        r.close()
+    single.close()
+
+
+def test_decomposition_with_walls_and_far_field():
+    n, p, ext = (6, 5, 4), 2, (1.0, 1.0, 0.7)
+    bc = (D.WALL, D.FARFIELD, D.PERIODIC, D.PERIODIC, D.WALL, D.WALL)
+    qinf = I.uniform_state(1, 1, 1, 0, rho=1.05, vel=(0.45, -0.25, 0.15), pres=1.1, gamma=G).reshape(5)
+    q = rough_field(*n, p, ext, seed=4)
+    dt = I.cfl_dt(ORC.max_wavespeed(q, p, G), p, ext, n, 0.1)
+    ranks = D.make_in_process(n, p, G, ext, (2, 2, 2), bc, qinf)
+    assert ranks[0].local_bc == (D.WALL, D.HALO, D.HALO, D.HALO, D.WALL, D.HALO)
+    D.set_state_in_process(ranks, q)
+    assert relerr(D.gather_in_process(ranks, "residual"), ORC.residual_bc(q, p, G, ext, bc, qinf)) < 1e-11
+    D.rk_step_in_process(ranks, dt, 2)
+    assert relerr(D.gather_in_process(ranks), ORC.rk_step_bc(q, p, G, ext, bc, qinf, dt, 2)) < 1e-12
+    for r in ranks:
+        r.close()
+
+
+def test_halo_faces_need_their_buffers_and_refuse_the_device_side_cfl_step():
+    from paper_2006_15698_b200 import DGError
+    dg = DG(4, 4, 4, 1).set_boundary((D.HALO, D.HALO, 0, 0, 0, 0))
+    dg.set_state(rough_field(4, 4, 4, 1, (1.0,) * 3))
+    with pytest.raises(DGError):
+        dg.rk_step(1e-3, 1)                                    # dg_set_halo not called
+    with pytest.raises(DGError):
+        dg.rk_step_cfl(0.1, 1)                                 # the wavespeed would be this context's only
+    dg.close()
