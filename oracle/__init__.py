@@ -34,6 +34,11 @@ def _load(variant):
         lib.oracle_residual_bc.argtypes = mesh + [_IP, _DP, _DP, _DP]
         lib.oracle_rk_step_bc.argtypes = mesh + [_IP, _DP, _DP, ctypes.c_double, ctypes.c_int]
         lib.oracle_max_wavespeed.argtypes = [ctypes.c_int] * 4 + [ctypes.c_double, _DP, _DP]
+        lib.oracle_gradient.argtypes = [ctypes.c_int] * 4 + [_DP, ctypes.c_int, _DP, _DP]
+        visc = mesh + [ctypes.c_double, ctypes.c_double]
+        lib.oracle_viscous_term.argtypes = visc + [_DP, _DP]
+        lib.oracle_residual_ns.argtypes = visc + [_DP, _DP]
+        lib.oracle_rk_step_ns.argtypes = visc + [_DP, ctypes.c_double, ctypes.c_int]
         _LIBS[name] = lib
     return _LIBS[name]
 
@@ -144,3 +149,34 @@ class Oracle:
         lam = np.zeros(1)
         _check(self.lib.oracle_max_wavespeed(nx, ny, nz, p, float(gamma), _p(q), _p(lam)), "max_wavespeed")
         return float(lam[0])
+
+    # ---- viscous (Navier-Stokes) terms, SURVEY.md 8(f)-4 (reading R20) ----
+    def gradient(self, q, p, extent, axis):
+        """BR1 gradient d_axis Q of the five conserved variables (central interface value)."""
+        q, nx, ny, nz = self._mesh(q, p)
+        ext = np.asarray(extent, dtype=np.float64)
+        s = np.empty_like(q)
+        _check(self.lib.oracle_gradient(nx, ny, nz, p, _p(ext), int(axis), _p(q), _p(s)), "gradient")
+        return s
+
+    def _visc(self, fn, q, p, gamma, extent, mu, prandtl):
+        q, nx, ny, nz = self._mesh(q, p)
+        ext = np.asarray(extent, dtype=np.float64)
+        r = np.empty_like(q)
+        _check(fn(nx, ny, nz, p, float(gamma), _p(ext), float(mu), float(prandtl), _p(q), _p(r)), "viscous term")
+        return r
+
+    def viscous_term(self, q, p, gamma, extent, mu, prandtl):
+        """div Fv(Q, grad Q): the viscous part of dQ/dt."""
+        return self._visc(self.lib.oracle_viscous_term, q, p, gamma, extent, mu, prandtl)
+
+    def residual_ns(self, q, p, gamma, extent, mu, prandtl):
+        return self._visc(self.lib.oracle_residual_ns, q, p, gamma, extent, mu, prandtl)
+
+    def rk_step_ns(self, q, p, gamma, extent, mu, prandtl, dt, nsteps):
+        q, nx, ny, nz = self._mesh(q, p)
+        q = q.copy()
+        ext = np.asarray(extent, dtype=np.float64)
+        _check(self.lib.oracle_rk_step_ns(nx, ny, nz, p, float(gamma), _p(ext), float(mu), float(prandtl), _p(q),
+                                          float(dt), int(nsteps)), "rk_step_ns")
+        return q

@@ -564,6 +564,213 @@ int oracle_rk_step_bc(int nx, int ny, int nz, int p, double gamma, const double 
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Viscous (Navier-Stokes) terms -- SURVEY.md 8(f)-4.  The paper only names them ("the viscous
+ * formulation" of the CPU code; its GPU port and its equations (2)-(5) are inviscid), so everything here is
+ * DESIGN.md reading R20 and PARITY IS UNPINNED BY THE PAPER:
+ *   dQ/dt = L(Q) + div Fv(Q, grad Q),   Fv_a = (0, tau_a1, tau_a2, tau_a3, u_b tau_ab + kappa d_a(p/rho)),
+ *   tau_ab = mu (d_a u_b + d_b u_a - 2/3 delta_ab d_c u_c),   kappa = mu gamma / (Pr (gamma-1))
+ *   (constant dynamic viscosity mu, Stokes hypothesis, Fourier conduction with constant Prandtl number, ideal gas:
+ *   kappa d(p/rho) = (mu c_p / Pr) dT), discretised by the first Bassi-Rebay scheme (BR1) with the basis of eq (4)-(7):
+ *   step v1  S_a = d_a Q, the same weak form as eq (5) with the CENTRAL interface value Q* = (Q_L + Q_R)/2:
+ *            S_a = (2/h_a) [ (l(+1) Q*_+ - l(-1) Q*_-)/w - sum_q Dhat_sq Q_q ]      (one call of central_weak_derivative)
+ *   step v2  pointwise: velocity and p/rho gradients from S by the quotient rule, then Fv_a at every node
+ *   step v3  div Fv = sum_a central_weak_derivative(Fv_a, a): nodal Fv_a interpolated to the faces, central flux
+ * Periodic meshes only.  Pinned in tests/test_oracle_viscous.py by: the dense-matrix restatement with explicit
+ * quadrature; exact derivatives of polynomials on elements away from the periodic wrap; closed-form div Fv of a
+ * shear wave, a dilatation wave and a conduction wave (pin 4/3, the off-diagonal stress and kappa) with p-th order
+ * convergence; discrete conservation; axis permutation.
+ * ---------------------------------------------------------------------------------------- */
+/* out (+)= (2/h_a) [ (l_s(+1) G*_+ - l_s(-1) G*_-)/w_s - sum_q Dhat_sq G_q ] along axis a for the nodal field G
+ * (canonical layout, NV components), G*_+ = (T+ of the element + T- of its upper neighbour)/2, G*_- likewise below. */
+static void central_weak_derivative(const disc *d, const real *G, int a, real *out, int accumulate) {
+    const int N = d->N;
+    const size_t nf = (size_t)N * N, per_elem = nf * NV;
+    real *Tp = (real *)malloc(sizeof(real) * d->nelem * per_elem);
+    real *Tm = (real *)malloc(sizeof(real) * d->nelem * per_elem);
+    real *Gs = (real *)malloc(sizeof(real) * d->nelem * per_elem);   /* G* at the + face of every element */
+#ifdef _OPENMP
+#pragma omp parallel for
+#endif
+    for (long long el = 0; el < (long long)d->nelem; ++el) {
+        const size_t e = (size_t)el;
+        for (int t2 = 0; t2 < N; ++t2)
+            for (int t1 = 0; t1 < N; ++t1)
+                for (int n = 0; n < NV; ++n) {
+                    real sp = 0, sm = 0;
+                    for (int s = 0; s < N; ++s) {
+                        int i = 0, j = 0, k = 0;
+                        node_of_line(a, s, t1, t2, &i, &j, &k);
+                        const real v = G[qidx(d, e, i, j, k) + n];
+                        sp += d->lp[s] * v;
+                        sm += d->lm[s] * v;
+                    }
+                    Tp[e * per_elem + ((size_t)t2 * N + t1) * NV + n] = sp;
+                    Tm[e * per_elem + ((size_t)t2 * N + t1) * NV + n] = sm;
+                }
+    }
+#ifdef _OPENMP
+#pragma omp parallel for
+#endif
+    for (long long el = 0; el < (long long)d->nelem; ++el) {
+        const size_t e = (size_t)el;
+        const int ex = (int)(e % (size_t)d->nx), ey = (int)((e / (size_t)d->nx) % (size_t)d->ny),
+                  ez = (int)(e / ((size_t)d->nx * d->ny));
+        const size_t en = (a == 0)   ? eidx(d, (ex + 1) % d->nx, ey, ez)
+                          : (a == 1) ? eidx(d, ex, (ey + 1) % d->ny, ez)
+                                     : eidx(d, ex, ey, (ez + 1) % d->nz);
+        for (size_t f = 0; f < per_elem; ++f) Gs[e * per_elem + f] = (real)0.5 * (Tp[e * per_elem + f] + Tm[en * per_elem + f]);
+    }
+#ifdef _OPENMP
+#pragma omp parallel for
+#endif
+    for (long long el = 0; el < (long long)d->nelem; ++el) {
+        const size_t e = (size_t)el;
+        const int ex = (int)(e % (size_t)d->nx), ey = (int)((e / (size_t)d->nx) % (size_t)d->ny),
+                  ez = (int)(e / ((size_t)d->nx * d->ny));
+        const size_t em = (a == 0)   ? eidx(d, (ex + d->nx - 1) % d->nx, ey, ez)
+                          : (a == 1) ? eidx(d, ex, (ey + d->ny - 1) % d->ny, ez)
+                                     : eidx(d, ex, ey, (ez + d->nz - 1) % d->nz);
+        for (int t2 = 0; t2 < N; ++t2)
+            for (int t1 = 0; t1 < N; ++t1)
+                for (int s = 0; s < N; ++s) {
+                    int i = 0, j = 0, k = 0;
+                    node_of_line(a, s, t1, t2, &i, &j, &k);
+                    real *o = out + qidx(d, e, i, j, k);
+                    for (int n = 0; n < NV; ++n) {
+                        real vol = 0;
+                        for (int qp = 0; qp < N; ++qp) {
+                            int iq = 0, jq = 0, kq = 0;
+                            node_of_line(a, qp, t1, t2, &iq, &jq, &kq);
+                            vol += d->Dhat[s * N + qp] * G[qidx(d, e, iq, jq, kq) + n];
+                        }
+                        const real Gplus = Gs[e * per_elem + ((size_t)t2 * N + t1) * NV + n];
+                        const real Gminus = Gs[em * per_elem + ((size_t)t2 * N + t1) * NV + n];
+                        const real val = d->g[a] * ((d->lp[s] * Gplus - d->lm[s] * Gminus) / d->w[s] - vol);
+                        o[n] = accumulate ? o[n] + val : val;
+                    }
+                }
+    }
+    free(Tp);
+    free(Tm);
+    free(Gs);
+}
+
+/* step v2: Fv_a (a = 0,1,2) at one node from Q and S_a = d_a Q (quotient rule for the velocity and p/rho gradients) */
+static void viscous_flux(const disc *d, real mu, real kappa, const real Q[NV], const real *S[3], real Fv[3][NV]) {
+    const real oneOrho = (real)1 / Q[0];
+    const real u[3] = {Q[1] * oneOrho, Q[2] * oneOrho, Q[3] * oneOrho};
+    const real E = Q[4] * oneOrho;
+    real du[3][3], dT[3];   /* du[a][b] = d_a u_b;  dT[a] = d_a (p/rho) */
+    for (int a = 0; a < 3; ++a) {
+        for (int b = 0; b < 3; ++b) du[a][b] = (S[a][1 + b] - u[b] * S[a][0]) * oneOrho;
+        const real dE = (S[a][4] - E * S[a][0]) * oneOrho;
+        dT[a] = d->gm1 * (dE - (u[0] * du[a][0] + u[1] * du[a][1] + u[2] * du[a][2]));
+    }
+    const real divu = du[0][0] + du[1][1] + du[2][2];
+    for (int a = 0; a < 3; ++a) {
+        real tau[3];
+        for (int b = 0; b < 3; ++b) tau[b] = mu * (du[a][b] + du[b][a]);
+        tau[a] = tau[a] - mu * ((real)2 / (real)3) * divu;
+        Fv[a][0] = 0;
+        Fv[a][1] = tau[0];
+        Fv[a][2] = tau[1];
+        Fv[a][3] = tau[2];
+        Fv[a][4] = (u[0] * tau[0] + u[1] * tau[1] + u[2] * tau[2]) + kappa * dT[a];
+    }
+}
+
+/* rv = div Fv(Q, grad Q) in `real`, whole mesh; S0..S2 are scratch vectors of the state's length */
+static void viscous_term_real(const disc *d, real mu, real prandtl, const real *q, real *rv, real *S0, real *S1, real *S2) {
+    const size_t nodes = d->nelem * d->nnode;
+    const real kappa = mu * d->gamma / (prandtl * d->gm1);
+    real *S[3] = {S0, S1, S2};
+    for (int a = 0; a < 3; ++a) central_weak_derivative(d, q, a, S[a], 0);   /* step v1 */
+#ifdef _OPENMP
+#pragma omp parallel for
+#endif
+    for (long long mm = 0; mm < (long long)nodes; ++mm) {                     /* step v2, in place: S_a <- Fv_a */
+        const size_t m = (size_t)mm;
+        const real *Sn[3] = {S0 + m * NV, S1 + m * NV, S2 + m * NV};
+        real Fv[3][NV];
+        viscous_flux(d, mu, kappa, q + m * NV, Sn, Fv);
+        for (int a = 0; a < 3; ++a)
+            for (int n = 0; n < NV; ++n) S[a][m * NV + n] = Fv[a][n];
+    }
+    for (int a = 0; a < 3; ++a) central_weak_derivative(d, S[a], a, rv, a > 0);   /* step v3 */
+}
+
+static int viscous_args_ok(double mu, double prandtl) { return mu >= 0.0 && prandtl > 0.0; }
+
+int oracle_gradient(int nx, int ny, int nz, int p, const double extent[3], int axis, const double *q, double *s) {
+    disc d;
+    if (!q || !s || axis < 0 || axis > 2 || disc_init(&d, nx, ny, nz, p, 1.4, extent)) return 1;
+    const size_t len = d.nelem * d.nnode * NV;
+    real *qq = to_real(q, len), *ss = (real *)malloc(sizeof(real) * len);
+    central_weak_derivative(&d, qq, axis, ss, 0);
+    to_double(ss, s, len);
+    free(qq);
+    free(ss);
+    return 0;
+}
+
+int oracle_viscous_term(int nx, int ny, int nz, int p, double gamma, const double extent[3], double mu, double prandtl,
+                        const double *q, double *r) {
+    disc d;
+    if (!q || !r || !viscous_args_ok(mu, prandtl) || disc_init(&d, nx, ny, nz, p, gamma, extent)) return 1;
+    const size_t len = d.nelem * d.nnode * NV;
+    real *qq = to_real(q, len);
+    real *buf = (real *)malloc(sizeof(real) * 4 * len);
+    viscous_term_real(&d, (real)mu, (real)prandtl, qq, buf, buf + len, buf + 2 * len, buf + 3 * len);
+    to_double(buf, r, len);
+    free(qq);
+    free(buf);
+    return 0;
+}
+
+int oracle_residual_ns(int nx, int ny, int nz, int p, double gamma, const double extent[3], double mu, double prandtl,
+                       const double *q, double *r) {
+    disc d;
+    if (!q || !r || !viscous_args_ok(mu, prandtl) || disc_init(&d, nx, ny, nz, p, gamma, extent)) return 1;
+    const size_t len = d.nelem * d.nnode * NV;
+    real *qq = to_real(q, len);
+    real *buf = (real *)malloc(sizeof(real) * 5 * len);
+    residual_real(&d, qq, buf, buf + len);
+    viscous_term_real(&d, (real)mu, (real)prandtl, qq, buf + len, buf + 2 * len, buf + 3 * len, buf + 4 * len);
+    for (size_t m = 0; m < len; ++m) buf[m] = buf[m] + buf[len + m];
+    to_double(buf, r, len);
+    free(qq);
+    free(buf);
+    return 0;
+}
+
+int oracle_rk_step_ns(int nx, int ny, int nz, int p, double gamma, const double extent[3], double mu, double prandtl,
+                      double *q, double dt, int nsteps) {
+    disc d;
+    if (!q || nsteps < 0 || !viscous_args_ok(mu, prandtl) || disc_init(&d, nx, ny, nz, p, gamma, extent)) return 1;
+    const size_t len = d.nelem * d.nnode * NV;
+    real *Q = to_real(q, len);
+    real *buf = (real *)malloc(sizeof(real) * 6 * len);
+    real *K = buf, *R = buf + len, *Rv = buf + 2 * len;
+    const real h = (real)dt;
+    for (int step = 0; step < nsteps; ++step) {
+        for (size_t m = 0; m < len; ++m) K[m] = 0;
+        for (int s = 0; s < 5; ++s) {
+            const real A = (real)RK_A[s], B = (real)RK_B[s];
+            residual_real(&d, Q, R, Rv);
+            viscous_term_real(&d, (real)mu, (real)prandtl, Q, Rv, buf + 3 * len, buf + 4 * len, buf + 5 * len);
+            for (size_t m = 0; m < len; ++m) {
+                K[m] = A * K[m] + h * (R[m] + Rv[m]);
+                Q[m] = Q[m] + B * K[m];
+            }
+        }
+    }
+    to_double(Q, q, len);
+    free(Q);
+    free(buf);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
  * step 6: max wavespeed  lam = max_nodes ( sqrt(u^2+v^2+w^2) + sqrt(gamma p / rho) )
  * (not in the paper; R10.  dt = CFL min(h_a) / ((2p+1) lam) is formed by the caller.)
  * ---------------------------------------------------------------------------------------- */

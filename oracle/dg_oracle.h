@@ -67,6 +67,21 @@ int oracle_residual_bc(int nx, int ny, int nz, int p, double gamma, const double
 int oracle_rk_step_bc(int nx, int ny, int nz, int p, double gamma, const double extent[3], const int bc[6],
                       const double qinf[5], double *q, double dt, int nsteps);
 
+/* Viscous (Navier-Stokes) terms, SURVEY.md 8(f)-4.  The paper names them only and prints no equations:
+ * DESIGN.md reading R20, PARITY UNPINNED BY THE PAPER.  Constant dynamic viscosity mu >= 0, Stokes hypothesis, Fourier
+ * conduction with constant Prandtl number, first Bassi-Rebay scheme (central interface values for Q and for the viscous
+ * flux) in the basis of eq (4)-(7); periodic meshes only.
+ *   oracle_gradient:     s = d_axis Q, the BR1 gradient of the five conserved variables (canonical layout)
+ *   oracle_viscous_term: r = div Fv(Q, grad Q),  Fv_a = (0, tau_a1, tau_a2, tau_a3, u_b tau_ab + mu gamma/(Pr (gamma-1)) d_a(p/rho))
+ *   oracle_residual_ns:  r = L(Q) + div Fv;  oracle_rk_step_ns: LSERK45 steps of dQ/dt = L(Q) + div Fv */
+int oracle_gradient(int nx, int ny, int nz, int p, const double extent[3], int axis, const double *q, double *s);
+int oracle_viscous_term(int nx, int ny, int nz, int p, double gamma, const double extent[3], double mu, double prandtl,
+                        const double *q, double *r);
+int oracle_residual_ns(int nx, int ny, int nz, int p, double gamma, const double extent[3], double mu, double prandtl,
+                       const double *q, double *r);
+int oracle_rk_step_ns(int nx, int ny, int nz, int p, double gamma, const double extent[3], double mu, double prandtl,
+                      double *q, double dt, int nsteps);
+
 /* lam = max over nodes of sqrt(u^2+v^2+w^2) + c   (reading R10). */
 int oracle_max_wavespeed(int nx, int ny, int nz, int p, double gamma, const double *q,
                          double *lam);
