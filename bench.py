@@ -347,6 +347,75 @@ def per_kernel_breakdown(workload, steps, device):
                                       "source": "derived from PAPER.md:264-269 (3,072 V100, 100 steps); another machine"}}
 
 
+VISC_BYTES_PER_DOF = 800.0   # unfused viscous path, per evaluation: 3 gradients (read Q, write S_a: 240), pointwise flux
+                             # (read Q + S, write Fv: 280), 3 divergences (read Fv_a, read + write R: 360); DESIGN.md 6.6
+
+
+def navier_stokes_leg(workload, steps, device, mu=1e-3, prandtl=0.72):
+    """LSERK45 steps of dQ/dt = L(Q) + div Fv (dg_rk_step_ns: per-kernel mode + the seven viscous
+    kernels), timed with CUDA events on the launching stream; the viscous kernels on their own; the oracle's
+    rk_step_ns on a reduced mesh of the same field beside it."""
+    import torch
+    from paper_2006_15698_b200 import DG
+    from paper_2006_15698_b200 import inputs as I
+    c = I.CONFIGS[workload]
+    p, ext, n = c["p"], c["extent"], (c["nx"], c["ny"], c["nz"])
+    N = p + 1
+    q = I.make_field(workload, xp=torch, device=device)
+    dg = DG(*n, p, GAMMA, ext, device=device, viscosity=(mu, prandtl))
+    dg.set_state(q)
+    dt = I.cfl_dt(dg.max_wavespeed(), p, ext, n, 0.1)
+    dof = n[0] * n[1] * n[2] * N ** 3
+    stream = torch.cuda.current_stream(device)
+    dg.rk_step_ns(dt, 1)
+    torch.cuda.synchronize(device)
+    e = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    l0 = dg.launch_count
+    e[0].record(stream)
+    dg.rk_step_ns(dt, steps)
+    e[1].record(stream)
+    l1 = dg.launch_count
+    dg.split_volume().split_surface()
+    e[2].record(stream)
+    for _ in range(steps * STAGES):
+        dg.split_viscous()
+    e[3].record(stream)
+    torch.cuda.synchronize(device)
+    total, visc = e[0].elapsed_time(e[1]) * 1e-3, e[2].elapsed_time(e[3]) * 1e-3
+    finite = bool(torch.isfinite(dg.get_state(q)).all().item())
+    dg.close()
+    del q
+    torch.cuda.empty_cache()
+    evals = steps * STAGES
+    peak, _ = measured_peaks()
+    out = {"workload": f"{workload}: {list(n)} periodic elements, p={p}, {dof} nodes, mu={mu}, Pr={prandtl}",
+           "steps": steps, "value": dof * evals / total, "unit": UNIT, "seconds": total, "launches": l1 - l0,
+           "viscous_kernels": {"seconds": visc, "dof_per_s": dof * evals / visc, "launches_per_evaluation": 7,
+                               "roofline": {"bound": "hbm", "achieved": VISC_BYTES_PER_DOF * dof * evals / visc / 1e9,
+                                            "peak": peak, "unit": "GB/s",
+                                            "frac": VISC_BYTES_PER_DOF * dof * evals / visc / 1e9 / peak,
+                                            "algorithmic_bytes_per_dof": VISC_BYTES_PER_DOF}},
+           "finite": finite,
+           "note": "not fused: per-kernel mode (volume, surface, update-project) + three gradient kernels, the pointwise "
+                   "viscous flux, three divergence kernels per stage; reading R20 (the paper prints no viscous equations)"}
+    try:
+        import numpy as np
+        from oracle import Oracle
+        orc = Oracle("omp")
+        m = 12
+        small = dict(c, nx=m, ny=m, nz=m, extent=tuple(ext[a] * m / n[a] for a in range(3)))
+        qs = I.make_field(small)
+        t0 = time.perf_counter()
+        qo = orc.rk_step_ns(qs, p, GAMMA, small["extent"], mu, prandtl, dt, 1)
+        sec = time.perf_counter() - t0
+        out["cpu_baseline"] = {"value": m ** 3 * N ** 3 * STAGES / sec, "unit": UNIT, "cores": orc.threads, "kind": "oracle",
+                               "sample": f"1 LSERK45 Navier-Stokes step of the same field on a periodic {m}^3-element box, "
+                                         f"oracle_rk_step_ns (OpenMP), {sec:.1f} s", "finite": bool(np.isfinite(qo).all())}
+    except Exception as ex:   # the oracle is a reported baseline only
+        out["cpu_baseline"] = {"error": repr(ex)}
+    return out
+
+
 def reduce_max(x, dist, device):
     """Max over ranks of a per-rank time (replicas: the slowest replica sets the whole-job rate)."""
     if dist is None:
@@ -460,7 +529,7 @@ def run_ours(args, rank, world, local_rank):
 
     ms = reduce_max(main["ms"], dist, device)
     e2e_s = reduce_max(main["e2e"]["seconds"], dist, device)
-    sweep, sustained, big, fp64, per_kernel = [], None, None, None, None
+    sweep, sustained, big, fp64, per_kernel, ns = [], None, None, None, None, None
     # order: the short legs first (burst clocks, like the main leg), then the long ones that heat the board up
     if not args.no_sweep and world == 1:
         for p in range(1, 8):
@@ -473,6 +542,7 @@ def run_ours(args, rank, world, local_rank):
         from paper_2006_15698_b200.binding import fp64_peak
         fp64 = fp64_peak(device)
         per_kernel = per_kernel_breakdown("table2_p6", 10, device)
+        ns = navier_stokes_leg("table2_p6", 4, device)
         # the same workload for >= 300 steps: the board reaches its power cap after ~0.3 s and holds lower clocks
         sustained = time_workload(args.workload, max(300, K), W, device, None, physical_gpu_index(local_rank), lz=args.lz,
                                   variant=args.variant)
@@ -553,6 +623,8 @@ def run_ours(args, rank, world, local_rank):
                         "brick": big["kernel"], "finite": big["finite"], "clocks": big["clocks"], "traffic": t}
     if per_kernel is not None:
         line["per_kernel"] = per_kernel
+    if ns is not None:
+        line["navier_stokes"] = ns
     if fp64 is not None:
         flops = algo_flops_per_dof(main["p"]) * value
         line["roofline_fp64"] = {"bound": "fp64", "achieved": flops / 1e12, "peak": 2.0 * fp64 / 1e12, "unit": "TFLOP/s",

@@ -182,6 +182,26 @@ int dg_split_surface(dg_ctx *ctx);
 int dg_split_update(dg_ctx *ctx, double dt, int stage);
 int dg_split_get_r(dg_ctx *ctx, double *r_out, int on_device);
 
+/* Viscous (Navier-Stokes) terms, SURVEY.md 8(f)-4.  The paper names "the viscous formulation" of its CPU code
+ * and prints no viscous equations; the formulation is DESIGN.md reading R20:
+ *     dQ/dt = L(Q) + div Fv(Q, grad Q),  Fv_a = (0, tau_a1, tau_a2, tau_a3, u_b tau_ab + mu gamma/(Pr (gamma-1)) d_a(p/rho)),
+ *     tau_ab = mu (d_a u_b + d_b u_a - 2/3 delta_ab d_c u_c)
+ * (constant dynamic viscosity mu, Stokes hypothesis, Fourier conduction with constant Prandtl number Pr, ideal gas),
+ * discretised in the basis of eq (4)-(7) by the first Bassi-Rebay scheme: the gradient of the conserved variables and
+ * the divergence of the nodal viscous flux both use the weak form of eq (5) with the central interface value.
+ * Periodic meshes only (DG_EUNSUPPORTED otherwise).  Runs as kernels of its own on top of the per-kernel mode, not
+ * in the fused stage kernel.
+ *   dg_set_viscosity : before dg_bind (three more state-sized vectors in the workspace when mu > 0; DG_ESTATE after);
+ *                      mu >= 0, prandtl > 0 (DG_EINVAL otherwise); mu = 0 switches the terms off
+ *   dg_split_viscous : R += div Fv of the current state (after dg_split_volume + dg_split_surface R = L(Q) + div Fv);
+ *                      seven kernels: three gradients, the pointwise viscous flux, three divergences
+ *   dg_rk_step_ns    : nsteps LSERK45 steps of fixed dt of dQ/dt = L(Q) + div Fv
+ *                      (per stage: dg_split_volume, dg_split_surface, dg_split_viscous, dg_split_update)
+ * All enqueued on the stream without synchronisation. */
+int dg_set_viscosity(dg_ctx *ctx, double mu, double prandtl);
+int dg_split_viscous(dg_ctx *ctx);
+int dg_rk_step_ns(dg_ctx *ctx, double dt, int nsteps);
+
 /* Copy the current state out in canonical layout.  Synchronises when q_out is a host pointer. */
 int dg_get_state(dg_ctx *ctx, double *q_out, int on_device);
 

@@ -39,6 +39,9 @@ SYMBOLS = {
     "dg_split_surface": (ctypes.c_int, [ctypes.c_void_p]),
     "dg_split_update": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int]),
     "dg_split_get_r": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
+    "dg_set_viscosity": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_double]),
+    "dg_split_viscous": (ctypes.c_int, [ctypes.c_void_p]),
+    "dg_rk_step_ns": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int]),
     "dg_nodes": (ctypes.c_int, [ctypes.c_void_p, _DP, _DP]),
     "dg_launch_count": (ctypes.c_ulonglong, [ctypes.c_void_p]),
     "dg_kernel_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_longlong)]),
@@ -127,7 +130,7 @@ class DG:
     """One mesh + one state vector on the GPU.  Arrays are float64, shape (nz,ny,nx,N,N,N,5)."""
 
     def __init__(self, nx, ny, nz, p, gamma=1.4, extent=(1.0, 1.0, 1.0), device="cuda:0", brick=None, bind=True,
-                 variant=None, poison=False, spacing=None):
+                 variant=None, poison=False, spacing=None, viscosity=None):
         self.lib = load_library()
         self.nx, self.ny, self.nz, self.p, self.N = nx, ny, nz, p, p + 1
         self.gamma, self.extent = float(gamma), tuple(float(e) for e in extent)
@@ -144,6 +147,8 @@ class DG:
             self._check(self.lib.dg_set_variant(self._h, int(variant)))
         if spacing is not None:
             self._check(self.lib.dg_set_spacing(self._h, (ctypes.c_double * 3)(*[float(v) for v in spacing])))
+        if viscosity is not None:     # (mu, Prandtl number): Navier-Stokes terms, dg_split_viscous / dg_rk_step_ns
+            self._check(self.lib.dg_set_viscosity(self._h, float(viscosity[0]), float(viscosity[1])))
         self.workspace = None
         self.device = None
         self._torch = None
@@ -318,6 +323,22 @@ class DG:
         with self._torch.cuda.device(self.device):
             self._check(self.lib.dg_split_get_r(self._h, ptr, dev))
         return out
+
+    # -- viscous (Navier-Stokes) terms, SURVEY.md 8(f)-4 ---------------------------------------------
+    def split_viscous(self):
+        """R += div Fv(Q, grad Q) (after split_volume + split_surface: R = L(Q) + div Fv)."""
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.dg_split_viscous(self._h))
+        return self
+
+    def residual_ns(self, out=None):
+        """dQ/dt = L(Q) + div Fv of the current state (volume, surface and viscous kernels, then the copy out)."""
+        return self.split_volume().split_surface().split_viscous().split_r(out)
+
+    def rk_step_ns(self, dt, nsteps=1):
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.dg_rk_step_ns(self._h, float(dt), int(nsteps)))
+        return self
 
     def rk_step_split(self, dt, nsteps=1):
         """nsteps LSERK45 steps as 5 x (volume, surface, update-project) launches."""

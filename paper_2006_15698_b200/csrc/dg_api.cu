@@ -196,6 +196,8 @@ struct dg_ctx {
     size_t tz_len;      // doubles per z trace buffer
     // borrowed workspace
     double *Q, *K, *S, *Txy[2], *Tz[2];
+    double *V[3];       // viscous terms enabled (dg_set_viscosity): gradient / viscous-flux vectors, internal layout
+    double mu, prandtl; // dynamic viscosity (0 = inviscid, no V vectors) and Prandtl number (reading R20)
     unsigned long long *scal;
     int tcur;           // Txy[tcur], Tz[tcur] hold the traces of the current Q
     bool lam_valid;     // scal[lcur] holds the max wavespeed of the current Q (reduced by the last stage)
@@ -262,7 +264,7 @@ void set_layout(dg_ctx *c, int variant, const DgKernelTable *kt) {
 }
 
 struct Carve {
-    size_t q, k, s, txy0, txy1, tz0, tz1, scal, total;
+    size_t q, k, s, txy0, txy1, tz0, tz1, scal, v[3], total;
 };
 Carve carve(const dg_ctx *c) {
     Carve v;
@@ -275,6 +277,10 @@ Carve carve(const dg_ctx *c) {
     v.tz0 = off;  off += align_up(c->tz_len * 8, 256);
     v.tz1 = off;  off += align_up(c->tz_len * 8, 256);
     v.scal = off; off += 256;
+    for (int a = 0; a < 3; ++a) {
+        v.v[a] = off;
+        if (c->mu > 0.0) off += align_up(c->int_len * 8, 256);
+    }
     v.total = off;
     return v;
 }
@@ -554,6 +560,7 @@ int dg_bind(dg_ctx *c, void *ws, size_t bytes, void *stream) {
     c->Tz[0] = (double *)(base + v.tz0);
     c->Tz[1] = (double *)(base + v.tz1);
     c->scal = (unsigned long long *)(base + v.scal);
+    for (int a = 0; a < 3; ++a) c->V[a] = (c->mu > 0.0) ? (double *)(base + v.v[a]) : nullptr;
     c->stream = (cudaStream_t)stream;
     c->tcur = 0;
     c->has_state = false;
@@ -763,6 +770,73 @@ int dg_split_update(dg_ctx *c, double dt, int stage) {
     c->launches++;
     c->lam_valid = false;
     return refresh_traces(c);   // "project": face traces of the updated state, so that the fused path can go on
+}
+
+// Viscous (Navier-Stokes) terms, SURVEY.md 8(f)-4 (reading R20; the paper names them only).
+int dg_set_viscosity(dg_ctx *c, double mu, double prandtl) {
+    if (!c) return DG_EINVAL;
+    if (c->bound) return fail(c, DG_ESTATE, "dg_set_viscosity after dg_bind (it changes the workspace size)");
+    if (!(mu >= 0.0) || !std::isfinite(mu) || !(prandtl > 0.0) || !std::isfinite(prandtl))
+        return fail(c, DG_EINVAL, "need mu >= 0 and Prandtl number > 0");
+    c->mu = mu;
+    c->prandtl = prandtl;
+    return DG_OK;
+}
+
+int dg_split_viscous(dg_ctx *c) {
+    if (!c) return DG_EINVAL;
+    if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_split_viscous needs dg_bind and dg_set_state first");
+    if (!(c->mu > 0.0)) return fail(c, DG_ESTATE, "no viscosity set (dg_set_viscosity before dg_bind)");
+    for (int f = 0; f < 6; ++f)
+        if (c->bc[f]) return fail(c, DG_EUNSUPPORTED, "the viscous terms are periodic only");
+    DgViscArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.Q = c->Q;
+    a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
+    a.nbx = c->nbx; a.nby = c->nby;
+    a.gm1 = c->gamma - 1.0;
+    a.mu = c->mu;
+    a.kappa = c->mu * c->gamma / (c->prandtl * (c->gamma - 1.0));
+    for (int d = 0; d < 3; ++d) a.S[d] = c->V[d];
+    cudaError_t e = cudaSuccess;
+    for (int d = 0; d < 3 && e == cudaSuccess; ++d) {   // step v1: S_d = d_d Q
+        a.G = c->Q;
+        a.out = c->V[d];
+        a.axis = d;
+        a.accumulate = 0;
+        a.scale = c->g[d];
+        e = c->kt->launch_cwd(a, c->stream);
+        c->launches++;
+    }
+    if (e == cudaSuccess) {                              // step v2: Fv_d over S_d, pointwise
+        e = c->kt->launch_viscflux(a, c->sms, c->stream);
+        c->launches++;
+    }
+    for (int d = 0; d < 3 && e == cudaSuccess; ++d) {   // step v3: R += d_d Fv_d
+        a.G = c->V[d];
+        a.out = c->S;
+        a.axis = d;
+        a.accumulate = 1;
+        a.scale = c->g[d];
+        e = c->kt->launch_cwd(a, c->stream);
+        c->launches++;
+    }
+    if (e != cudaSuccess) return cuda_fail(c, e, "viscous kernels");
+    return DG_OK;
+}
+
+int dg_rk_step_ns(dg_ctx *c, double dt, int nsteps) {
+    if (!c) return DG_EINVAL;
+    if (nsteps < 0 || !std::isfinite(dt)) return fail(c, DG_EINVAL, "nsteps < 0 or dt not finite");
+    for (int step = 0; step < nsteps; ++step)
+        for (int s = 0; s < 5; ++s) {
+            int rc = dg_split_volume(c);
+            if (rc == DG_OK) rc = dg_split_surface(c);
+            if (rc == DG_OK) rc = dg_split_viscous(c);
+            if (rc == DG_OK) rc = dg_split_update(c, dt, s);
+            if (rc != DG_OK) return rc;
+        }
+    return DG_OK;
 }
 
 int dg_split_get_r(dg_ctx *c, double *r_out, int on_device) {

@@ -1022,12 +1022,12 @@ __global__ void __launch_bounds__(C::NCOMP) dg_split_volume_kernel(const __grid_
 // Trace of the line through node (j, k transverse) of element (ex, ey, ez) along axis AX, at its + or - end,
 // read from the state in HBM (any element of the mesh; periodic wrap by the caller), slots rotated for AX.
 template <class C, int AX>
-__device__ __forceinline__ void global_line_trace(const DgSplitArgs &a, int ex, int ey, int ez, int t1, int t2, bool plus,
-                                                  double (&T)[DG_NV]) {
+__device__ __forceinline__ void global_line_trace_of(const double *field, int nbx, int nby, int ex, int ey, int ez, int t1, int t2,
+                                                     bool plus, double (&T)[DG_NV]) {
     constexpr int N = C::N;
     const int bxi = ex / C::BX, byi = ey / C::BY;
     const int lx = ex - bxi * C::BX, ly = ey - byi * C::BY;
-    const double *src = a.Q + (((size_t)ez * a.nby + byi) * a.nbx + bxi) * C::SLOT;
+    const double *src = field + (((size_t)ez * nby + byi) * nbx + bxi) * C::SLOT;
     // (t1, t2) are node indices INSIDE the element here: x lines (j, k), y lines (i, k), z lines (i, j)
     int base, stride;
     if (AX == 0) { base = t2 * C::HP + (ly * N + t1) * C::GX + lx * N; stride = 1; }
@@ -1041,6 +1041,12 @@ __device__ __forceinline__ void global_line_trace(const DgSplitArgs &a, int ex, 
         for (int q = 0; q < N; ++q) t = fma(plus ? DG_LP(q) : DG_LM(q), __ldg(p + q * stride), t);
         T[s] = t;
     }
+}
+
+template <class C, int AX>
+__device__ __forceinline__ void global_line_trace(const DgSplitArgs &a, int ex, int ey, int ez, int t1, int t2, bool plus,
+                                                  double (&T)[DG_NV]) {
+    global_line_trace_of<C, AX>(a.Q, a.nbx, a.nby, ex, ey, ez, t1, t2, plus, T);
 }
 
 // R += -(2/h_a) (l_i(+1) F*_+ - l_i(-1) F*_-)/w_i for the three axes: every line evaluates the local Lax-Friedrichs
@@ -1102,6 +1108,123 @@ __global__ void __launch_bounds__(C::NCOMP) dg_split_surface_kernel(const __grid
     axis(std::integral_constant<int, 2>{});
     double *dst = a.R + slot * C::SLOT;
     for (int idx = tid; idx < C::NPL * C::HP; idx += C::NCOMP) dst[idx] = Rs[idx];
+}
+
+// ------------------------------------------------------------------------------------------------
+// viscous (Navier-Stokes) terms, SURVEY.md 8(f)-4.  The paper names them only and prints no equations:
+// DESIGN.md reading R20 -- constant viscosity, Stokes hypothesis, Fourier conduction with constant Prandtl number,
+// first Bassi-Rebay scheme in the basis of eq (4)-(7), periodic meshes.  Run as kernels of their own on top of the
+// per-kernel mode (not the fused hot path):
+//   dg_cwd_kernel       out (+)= (2/h_a) [ (l_i(+1) G*_+ - l_i(-1) G*_-)/w_i - sum_q Dhat_iq G_q ] along one axis, with the
+//                       CENTRAL interface value G* = (G_L + G_R)/2: the weak form of eq (5) for d_a G.  Applied to Q it
+//                       gives the gradient S_a, applied to the nodal viscous flux Fv_a it gives div Fv.
+//   dg_viscflux_kernel  pointwise: velocity and p/rho gradients from S by the quotient rule, Fv_a over S_a in place
+// ------------------------------------------------------------------------------------------------
+template <class C>
+__device__ __forceinline__ size_t internal_offset(size_t node, int nx, int ny, int nbx, int nby);
+
+template <class C, int AX>
+__device__ __forceinline__ void cwd_axis(const DgViscArgs &a, const double *Gs, int tid, int bxi, int byi, int ez, size_t slot) {
+    using A = Axis<C, AX>;
+    constexpr int NV = DG_NV, N = C::N, PLANE = C::PLANE;
+    const int ext0 = min(C::BX, a.nx - bxi * C::BX), ext1 = min(C::BY, a.ny - byi * C::BY);
+    if (tid >= C::L) return;
+    const Geo g = make_geo<C, AX>(tid);
+    if (!line_inside<C, AX>(g, ext0, ext1)) return;
+    double Gl[NV][N], Tp[NV], Tm[NV], Hlo[NV], Hhi[NV];
+#pragma unroll
+    for (int n = 0; n < NV; ++n) {
+        Tp[n] = Tm[n] = 0.0;
+#pragma unroll
+        for (int q = 0; q < N; ++q) {
+            const double v = Gs[g.base + n * PLANE + q * A::S];
+            Gl[n][q] = v;
+            Tp[n] = fma(DG_LP(q), v, Tp[n]);
+            Tm[n] = fma(DG_LM(q), v, Tm[n]);
+        }
+    }
+    // this line's element and its two neighbours along AX (periodic), node indices in the element
+    int ex = bxi * C::BX, ey = byi * C::BY, n1, n2;
+    if (AX == 0) { ex += g.e; ey += g.t1 / N; n1 = g.t1 % N; n2 = g.t2; }
+    else if (AX == 1) { ey += g.e; ex += g.t1 / N; n1 = g.t1 % N; n2 = g.t2; }
+    else { ex += g.t1 / N; ey += g.t2 / N; n1 = g.t1 % N; n2 = g.t2 % N; }
+    const int na = (AX == 0) ? a.nx : (AX == 1) ? a.ny : a.nz;
+    const int ea = (AX == 0) ? ex : (AX == 1) ? ey : ez;
+    const int up = (ea + 1 == na) ? 0 : ea + 1, dn = (ea == 0) ? na - 1 : ea - 1;
+    // identity slots here (no momentum rotation): global_line_trace_of returns slot s = variable var_of_slot(s)
+    double Ru[NV], Rd[NV];
+    global_line_trace_of<C, AX>(a.G, a.nbx, a.nby, AX == 0 ? up : ex, AX == 1 ? up : ey, AX == 2 ? up : ez, n1, n2, false, Ru);
+    global_line_trace_of<C, AX>(a.G, a.nbx, a.nby, AX == 0 ? dn : ex, AX == 1 ? dn : ey, AX == 2 ? dn : ez, n1, n2, true, Rd);
+#pragma unroll
+    for (int s = 0; s < NV; ++s) {
+        Hhi[var_of_slot<C, AX>(s)] = Ru[s];
+        Hlo[var_of_slot<C, AX>(s)] = Rd[s];
+    }
+    double *o = a.out + slot * C::SLOT + g.base;
+#pragma unroll
+    for (int n = 0; n < NV; ++n) {
+        const double sp = Tp[n] + Hhi[n], sm = Hlo[n] + Tm[n];   // 2 G*_+, 2 G*_-; c_ref.lq carries the 1/2 and 1/w
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            double v = fma(DG_LQP(i), sp, -DG_LQM(i) * sm);
+#pragma unroll
+            for (int q = 0; q < N; ++q) v = fma(-c_ref.D[q][i], Gl[n][q], v);
+            double *dst = o + n * PLANE + i * A::S;
+            *dst = a.accumulate ? fma(a.scale, v, *dst) : a.scale * v;
+        }
+    }
+}
+
+template <class C>
+__global__ void __launch_bounds__(C::NCOMP) dg_cwd_kernel(const __grid_constant__ DgViscArgs a) {
+    extern __shared__ __align__(128) double smem[];
+    const int tid = threadIdx.x, bxi = blockIdx.x, byi = blockIdx.y, ez = blockIdx.z;
+    const size_t slot = ((size_t)ez * a.nby + byi) * a.nbx + bxi;
+    stage_layer_in<C>(smem, a.G + slot * C::SLOT, tid);
+    __syncthreads();
+    if (a.axis == 0) cwd_axis<C, 0>(a, smem, tid, bxi, byi, ez, slot);
+    else if (a.axis == 1) cwd_axis<C, 1>(a, smem, tid, bxi, byi, ez, slot);
+    else cwd_axis<C, 2>(a, smem, tid, bxi, byi, ez, slot);
+}
+
+template <class C>
+__global__ void __launch_bounds__(256) dg_viscflux_kernel(const DgViscArgs a) {
+    constexpr size_t VS = (size_t)C::N * C::HP;   // doubles per variable inside a slot
+    const size_t total = (size_t)a.nx * a.ny * a.nz * (C::N * C::N * C::N);
+    for (size_t node = (size_t)blockIdx.x * blockDim.x + threadIdx.x; node < total; node += (size_t)gridDim.x * blockDim.x) {
+        const size_t io = internal_offset<C>(node, a.nx, a.ny, a.nbx, a.nby);
+        double Q[DG_NV], S[3][DG_NV];
+#pragma unroll
+        for (int n = 0; n < DG_NV; ++n) {
+            Q[n] = a.Q[io + n * VS];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) S[d][n] = a.S[d][io + n * VS];
+        }
+        const double rinv = 1.0 / Q[0];
+        const double u[3] = {Q[1] * rinv, Q[2] * rinv, Q[3] * rinv};
+        const double E = Q[4] * rinv;
+        double du[3][3], dT[3];   // du[d][b] = d_d u_b, dT[d] = d_d (p/rho)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+#pragma unroll
+            for (int b = 0; b < 3; ++b) du[d][b] = (S[d][1 + b] - u[b] * S[d][0]) * rinv;
+            const double dE = (S[d][4] - E * S[d][0]) * rinv;
+            dT[d] = a.gm1 * (dE - (u[0] * du[d][0] + u[1] * du[d][1] + u[2] * du[d][2]));
+        }
+        const double divu = du[0][0] + du[1][1] + du[2][2];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            double tau[3];
+#pragma unroll
+            for (int b = 0; b < 3; ++b) tau[b] = a.mu * (du[d][b] + du[b][d]);
+            tau[d] -= a.mu * (2.0 / 3.0) * divu;
+            a.S[d][io] = 0.0;
+            a.S[d][io + VS] = tau[0];
+            a.S[d][io + 2 * VS] = tau[1];
+            a.S[d][io + 3 * VS] = tau[2];
+            a.S[d][io + 4 * VS] = (u[0] * tau[0] + u[1] * tau[1] + u[2] * tau[2]) + a.kappa * dT[d];
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1192,6 +1315,8 @@ cudaError_t prepare(const DgRefOps &ref, int *blocks_per_sm) {
         err = cudaFuncSetAttribute(dg_split_volume_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * C::BUF * 8);
     if (err == cudaSuccess)
         err = cudaFuncSetAttribute(dg_split_surface_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * C::BUF * 8);
+    if (err == cudaSuccess)
+        err = cudaFuncSetAttribute(dg_cwd_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::BUF * 8);
     if (err != cudaSuccess) return err;
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, dg_stage_kernel<C, DG_MODE_STAGE, false, false>,
                                                          C::THREADS, Smem<C>::BYTES);
@@ -1236,6 +1361,13 @@ cudaError_t launch_split_surface(const DgSplitArgs &a, cudaStream_t s) {
     return cudaGetLastError();
 }
 
+template <class C>
+cudaError_t launch_cwd(const DgViscArgs &a, cudaStream_t s) {
+    const dim3 grid((unsigned)a.nbx, (unsigned)a.nby, (unsigned)a.nz);
+    dg_cwd_kernel<C><<<grid, C::NCOMP, C::BUF * 8, s>>>(a);
+    return cudaGetLastError();
+}
+
 inline unsigned flat_grid(size_t total, int sms) {
     const size_t want = (total + 255) / 256;
     const size_t cap = (size_t)(sms > 0 ? sms : 1) * 16u;   // grid-stride: a few blocks per SM
@@ -1257,10 +1389,17 @@ cudaError_t launch_wavespeed(const DgWaveArgs &a, int sms, cudaStream_t s) {
 }
 
 template <class C>
+cudaError_t launch_viscflux(const DgViscArgs &a, int sms, cudaStream_t s) {
+    const size_t total = (size_t)a.nx * a.ny * a.nz * (C::N * C::N * C::N);
+    dg_viscflux_kernel<C><<<flat_grid(total, sms), 256, 0, s>>>(a);
+    return cudaGetLastError();
+}
+
+template <class C>
 constexpr DgKernelTable make_table() {
     return DgKernelTable{C::N,       C::BX,          C::BY,         C::THREADS,      Smem<C>::BYTES,     C::SLOT,
                          C::TXY,     C::TZ,          C::CX, C::CY, C::CZ, C::RELOAD ? 1 : 0, C::MINB, &prepare<C>, &launch_stage<C>,  &launch_traces<C>, &launch_split_volume<C>, &launch_split_surface<C>,
-                         &launch_layout<C>, &launch_wavespeed<C>};
+                         &launch_layout<C>, &launch_wavespeed<C>, &launch_cwd<C>, &launch_viscflux<C>};
 }
 
 // Variants per N (default first): Cfg<N, BX, BY, min blocks per SM, RELOAD, PP, OX, OY>.
