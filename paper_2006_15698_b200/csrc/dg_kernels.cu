@@ -740,9 +740,8 @@ __device__ __forceinline__ void copy_warp(const DgStageArgs &a, const BlockInfo 
                                           bool readK, double *Qb0, double *Qb1, double *KR, uint64_t *fullq, uint64_t *fullk) {
     const size_t lstride = (size_t)a.nbx * a.nby;                    // slots per layer
     const size_t slot0 = (size_t)z0 * lstride + (size_t)byi * a.nbx + bxi;
-    copy_in<C>(Qb0, a.Q + slot0 * C::SLOT, &fullq[0], lane);
-    if (readK) copy_in<C>(KR, a.K + slot0 * C::SLOT, fullk, lane);   // later layers: issued by the compute warps
-    if (nl > 1) copy_in<C>(Qb1, a.Q + (slot0 + lstride) * C::SLOT, &fullq[1], lane);
+    // (the loads of the first two Q layers and of the first K layer were issued in the kernel's prologue; the K
+    // loads of later layers are issued by the compute warps)
     // L2 prefetch of the neighbour columns' traces of the first layer (4 blocks of 5 Ca doubles)
     if (lane < 4) l2_prefetch(bi->halo[lane], DG_NV * (lane < 2 ? C::CX : C::CY) * 8);
     for (int it = 0; it < nl; ++it) {
@@ -843,11 +842,20 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
     const int z0 = chunk * a.lz;
     const int nl = min(a.lz, a.nz - z0);
     const bool readK = (MODE == DG_MODE_STAGE) && (a.rkA != 0.0);
-    if (tid == 0) {
+    if (tid == C::NCOMP) {
+        // the copy warp's first lane sets the mbarriers up and sends the first bulk loads off at once, while thread 0
+        // fills BlockInfo: the loads' latency overlaps the block's prologue
         mbar_init(&fullq[0], 1);
         mbar_init(&fullq[1], 1);
         mbar_init(fullk, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        const size_t lstride = (size_t)a.nbx * a.nby;
+        const size_t slot0 = (size_t)z0 * lstride + (size_t)byi * a.nbx + bxi;
+        copy_in<C>(smem + SM::QB0, a.Q + slot0 * C::SLOT, &fullq[0], 0);
+        if (readK) copy_in<C>(smem + SM::KR, a.K + slot0 * C::SLOT, fullk, 0);
+        if (nl > 1) copy_in<C>(smem + SM::QB1, a.Q + (slot0 + lstride) * C::SLOT, &fullq[1], 0);
+    }
+    if (tid == 0) {
         BlockInfo *bi = reinterpret_cast<BlockInfo *>(smem + SM::INFO);
         const size_t cstride = (size_t)a.nbx * a.nby, col = (size_t)byi * a.nbx + bxi;
         // neighbour columns' traces: the periodic neighbour's Txy block, or (block decomposition over GPUs) the

@@ -87,3 +87,37 @@ def test_viscous_errors():
     a, b = DG(3, 3, 3, 2, G, bind=False), DG(3, 3, 3, 2, G, viscosity=(0.0, 0.7), bind=False)
     c = DG(3, 3, 3, 2, G, viscosity=(0.1, 0.7), bind=False)
     assert a.workspace_bytes == b.workspace_bytes < c.workspace_bytes
+
+
+def test_navier_stokes_full_size_sampled():
+    """bench.py's Navier-Stokes workload (table2_p6: 40^3 elements, p = 6, 22 M nodes), sampled as in
+    tests/test_gpu_fullsize.py: the viscous stencil reaches two elements (gradient, then divergence), so the periodic
+    oracle on a sub-box reproduces the full mesh 2 elements (residual) or 10 elements (one 5-stage step) inside it."""
+    from oracle.parity import assert_parity
+    from test_gpu_fullsize import take_box, RES_ALLOWED
+    arb = Oracle("ld_omp")
+    cfg, mu, pr = "table2_p6", 1e-3, 0.72
+    c = I.CONFIGS[cfg]
+    p, ext, n = c["p"], c["extent"], (c["nx"], c["ny"], c["nz"])
+    h = [ext[a] / n[a] for a in range(3)]
+    q = I.make_field(cfg, xp=torch, device="cuda")
+    dg = DG(*n, p, G, ext, viscosity=(mu, pr)).set_state(q)
+    dt = I.cfl_dt(dg.max_wavespeed(), p, ext, n, 0.1)
+    r = dg.residual_ns(torch.empty_like(q))
+    for lo, size in [((37, 38, 36), (6, 6, 7)), ((11, 20, 3), (6, 6, 6))]:       # across the periodic corner; inside
+        sub_ext = tuple(h[a] * size[a] for a in range(3))
+        qb = take_box(q, lo, size)
+        inner = (slice(2, -2),) * 3
+        # full size: every variable's residual is a cancellation residue (tests/test_gpu_fullsize.py, RES_ALLOWED)
+        assert_parity(take_box(r, lo, size)[inner], ORC.residual_ns(qb, p, G, sub_ext, mu, pr)[inner],
+                      lambda: arb.residual_ns(qb, p, G, sub_ext, mu, pr)[inner], 1e-11, (cfg, "residual_ns", lo),
+                      allowed=RES_ALLOWED)
+    del r
+    lo, size = (30, 29, 31), (22, 22, 22)
+    qb = take_box(q, lo, size)
+    dg.rk_step_ns(dt, 1).get_state(q)
+    sub_ext = tuple(h[a] * size[a] for a in range(3))
+    inner = (slice(10, -10),) * 3
+    assert_parity(take_box(q, lo, size)[inner], ORC.rk_step_ns(qb, p, G, sub_ext, mu, pr, dt, 1)[inner],
+                  lambda: arb.rk_step_ns(qb, p, G, sub_ext, mu, pr, dt, 1)[inner], 1e-11, (cfg, "rk_step_ns", lo), allowed=())
+    dg.close()
