@@ -476,7 +476,7 @@ def run_decomposed(args, rank, world, local_rank):
             w = 1
     local = None if world > 1 else (lambda r, s, v: None)
     dd = DistributedDG(n, p, GAMMA, ext, tuple(procs), rank, device=device, exchange=local,
-                       reduce_max=None if world > 1 else (lambda x: x))
+                       reduce_max=None if world > 1 else (lambda x: x), push=bool(args.push) and world > 1)
     box = dd.box
     dd.set_state(I.make_field(args.workload, box=box, xp=torch, device=device))
     dt = I.cfl_dt(dd.max_wavespeed(), p, ext, n, 0.1)
@@ -502,7 +502,9 @@ def run_decomposed(args, rank, world, local_rank):
                           "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
                           "dtype": "f64", "data": "synthetic",
                           "config": {"workload": f"{args.workload}: {list(n)} elements, p={p}, ONE mesh in {procs} blocks, "
-                                                 "face traces exchanged after every stage", "parallelism": f"block decomposition {procs}"},
+                                                 + ("face traces stored by the stage kernel straight into the neighbours' buffers (CUDA IPC / NVLink), "
+                                                    "one barrier per stage" if (args.push and world > 1) else "face traces exchanged after every stage"),
+                                     "parallelism": f"block decomposition {procs}"},
                           "gpu_launches": dd.dg.launch_count,
                           "roofline": {"bound": "hbm", "achieved": ALGO_BYTES_PER_DOF_STAGE * dof * STAGES * K / (ms * 1e-3) / 1e9 / world,
                                        "peak": peak, "unit": "GB/s per GPU", "frac": value * ALGO_BYTES_PER_DOF_STAGE / 1e9 / peak / world,
@@ -655,6 +657,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--decomposed", action="store_true",
                     help="one mesh cut into one block per GPU with halo exchange (strong scaling) instead of replicas")
+    ap.add_argument("--push", action="store_true",
+                    help="with --decomposed: push mode (dg_set_halo_push; the stage kernel stores the faces into the neighbours' buffers)")
     ap.add_argument("--no-extras", action="store_true", help="skip the sustained run, cfg5 and the FP64 microbenchmark")
     ap.add_argument("--variant", type=int, default=None, help="stage-kernel variant index (tuning; default: library's choice)")
     ap.add_argument("--lz", type=int, default=0, help="layers per chunk (tuning; 0 = library default)")

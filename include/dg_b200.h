@@ -166,6 +166,24 @@ int dg_halo_export(dg_ctx *ctx, int face, double *dst_dev);
 int dg_set_halo(dg_ctx *ctx, int face, const double *halo_dev);
 int dg_rk_stage(dg_ctx *ctx, double dt, int stage);
 
+/* "Push" mode of the same decomposition: the face exchange done BY THE STAGE KERNEL, with no export kernel and no message.
+ * Every halo face gets a PAIR of trace buffers, read alternately:
+ *   dg_set_halo_pair(ctx, f, buf0, buf1)  the kernels of a stage read the traces beyond face f from buf[parity], parity =
+ *                            number of stages run since dg_set_state, mod 2 (device buffers of dg_halo_len doubles each)
+ *   dg_set_halo_push(ctx, f, peer0, peer1)  the NEIGHBOUR's pair for ITS opposite face (f ^ 1): while a stage computes,
+ *                            the blocks on face f store the traces of the updated state straight into
+ *                            peer[1 - parity], which is what the neighbour reads in the next stage.  The pointers may be
+ *                            peer-mapped memory of another GPU (CUDA peer access / IPC): the stores then travel over
+ *                            NVLink while the rest of the stage computes -- the paper's computation-communication
+ *                            overlap, tile by tile.
+ * The caller provides the ordering only: every context's stage s must have completed before any neighbour's stage s + 1
+ * starts (same stream, events, or a barrier between processes), and both sides must have run the same number of stages
+ * since dg_set_state.  After dg_set_state the initial traces go to the neighbour's buffer 0 with dg_halo_export.
+ * dg_residual reads buf[parity] and pushes nothing.  Not combined with the per-kernel mode (dg_split_update resets the parity).
+ * Results are bit-identical to the export / import mode and to the single-context run. */
+int dg_set_halo_pair(dg_ctx *ctx, int face, const double *halo0_dev, const double *halo1_dev);
+int dg_set_halo_push(dg_ctx *ctx, int face, double *peer0_dev, double *peer1_dev);
+
 /* Paper-shaped per-kernel mode (Table II): the same spatial residual and stage
  * update as dg_rk_step, run as the paper's three kernels so that their times can be measured one by one (the fused
  * path is the product; this mode exists for the breakdown and is parity-tested against the oracle's terms).

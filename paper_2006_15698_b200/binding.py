@@ -33,6 +33,8 @@ SYMBOLS = {
     "dg_halo_len": (ctypes.c_size_t, [ctypes.c_void_p, ctypes.c_int]),
     "dg_halo_export": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]),
     "dg_set_halo": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]),
+    "dg_set_halo_pair": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]),
+    "dg_set_halo_push": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]),
     "dg_rk_step_cfl": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int, _DP, _DP]),
     "dg_get_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
     "dg_split_volume": (ctypes.c_int, [ctypes.c_void_p]),
@@ -298,6 +300,23 @@ class DG:
         self._halo_keep = getattr(self, "_halo_keep", {})
         self._halo_keep[int(face)] = buf
         self._check(self.lib.dg_set_halo(self._h, int(face), buf.data_ptr()))
+        return self
+
+    def set_halo_pair(self, face, buf0, buf1):
+        """Push mode: the two float64 cuda tensors the kernels read alternately for the traces beyond `face`."""
+        for b in (buf0, buf1):
+            assert b.is_cuda and b.dtype == self._torch.float64 and b.is_contiguous() and b.numel() == self.halo_len(face)
+        self._halo_keep = getattr(self, "_halo_keep", {})
+        self._halo_keep[("pair", int(face))] = (buf0, buf1)
+        self._check(self.lib.dg_set_halo_pair(self._h, int(face), buf0.data_ptr(), buf1.data_ptr()))
+        return self
+
+    def set_halo_push(self, face, peer0, peer1):
+        """Push mode: the neighbour's pair for its opposite face (tensors, or raw device addresses of peer-mapped memory)."""
+        ptr = lambda b: int(b) if isinstance(b, int) else b.data_ptr()
+        self._halo_keep = getattr(self, "_halo_keep", {})
+        self._halo_keep[("push", int(face))] = (peer0, peer1)
+        self._check(self.lib.dg_set_halo_push(self._h, int(face), ptr(peer0), ptr(peer1)))
         return self
 
     # -- paper-shaped per-kernel mode (Table II breakdown) ------------------------------------------

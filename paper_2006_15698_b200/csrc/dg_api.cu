@@ -206,6 +206,8 @@ struct dg_ctx {
     double g[3];        // 2/h_a per axis
     int bc[6];          // boundary condition per domain face (dg_set_boundary), 0 = periodic
     const double *halo[6];   // DG_BC_HALO faces: the caller's device buffer with the neighbour context's traces
+    const double *halo2[6][2];   // ... or a PAIR of buffers read alternately (dg_set_halo_pair; parity = tcur)
+    double *push[6][2];      // push mode: the neighbour context's pair for its opposite face (dg_set_halo_push)
     double qinf[DG_NV];
     bool bound, has_state;
     cudaStream_t stream;
@@ -304,7 +306,9 @@ DgStageArgs stage_args(const dg_ctx *c, int mode) {
     for (int i = 0; i < 3; ++i) a.scale[i] = c->g[i];
     for (int i = 0; i < 6; ++i) {
         a.bc[i] = (c->bc[i] == DG_BC_HALO) ? 0 : c->bc[i];
-        a.halo_ext[i] = (c->bc[i] == DG_BC_HALO) ? c->halo[i] : nullptr;
+        a.halo_ext[i] = (c->bc[i] == DG_BC_HALO) ? (c->halo2[i][0] ? c->halo2[i][c->tcur] : c->halo[i]) : nullptr;
+        // the updated state's traces go where the neighbour reads in the NEXT stage (its parity will be 1 - tcur)
+        a.halo_push[i] = (mode == DG_MODE_STAGE && c->bc[i] == DG_BC_HALO) ? c->push[i][1 - c->tcur] : nullptr;
     }
     for (int i = 0; i < DG_NV; ++i) a.qinf[i] = c->qinf[i];
     return a;
@@ -340,7 +344,7 @@ int export_vector(dg_ctx *c, double *internal, double *out, int on_device, const
 // (a9 fused: no extra sweep over the state, no host round trip).
 int check_halos(dg_ctx *c) {
     for (int f = 0; f < 6; ++f)
-        if (c->bc[f] == DG_BC_HALO && !c->halo[f]) return fail(c, DG_ESTATE, "face %d is a halo face but dg_set_halo was not called", f);
+        if (c->bc[f] == DG_BC_HALO && !c->halo[f] && !c->halo2[f][0]) return fail(c, DG_ESTATE, "face %d is a halo face but dg_set_halo was not called", f);
     return DG_OK;
 }
 
@@ -665,6 +669,22 @@ int dg_set_spacing(dg_ctx *c, const double h[3]) {
 int dg_set_halo(dg_ctx *c, int face, const double *halo_dev) {
     if (!c || face < 0 || face > 5) return c ? fail(c, DG_EINVAL, "face outside 0..5") : DG_EINVAL;
     c->halo[face] = halo_dev;
+    return DG_OK;
+}
+
+int dg_set_halo_pair(dg_ctx *c, int face, const double *halo0_dev, const double *halo1_dev) {
+    if (!c || face < 0 || face > 5) return c ? fail(c, DG_EINVAL, "face outside 0..5") : DG_EINVAL;
+    if ((halo0_dev == nullptr) != (halo1_dev == nullptr)) return fail(c, DG_EINVAL, "both buffers or none");
+    c->halo2[face][0] = halo0_dev;
+    c->halo2[face][1] = halo1_dev;
+    return DG_OK;
+}
+
+int dg_set_halo_push(dg_ctx *c, int face, double *peer0_dev, double *peer1_dev) {
+    if (!c || face < 0 || face > 5) return c ? fail(c, DG_EINVAL, "face outside 0..5") : DG_EINVAL;
+    if ((peer0_dev == nullptr) != (peer1_dev == nullptr)) return fail(c, DG_EINVAL, "both buffers or none");
+    c->push[face][0] = peer0_dev;
+    c->push[face][1] = peer1_dev;
     return DG_OK;
 }
 

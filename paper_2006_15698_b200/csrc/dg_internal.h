@@ -87,6 +87,10 @@ struct DgStageArgs {
     // the elements beyond domain face f come from the caller's buffer halo_ext[f] (null: none), laid out like the
     // neighbour's export (dg_halo_export): x faces [ez][by][5][CX], y faces [ez][bx][5][CY], z faces [by][bx][5][CZ]
     const double *halo_ext[6];
+    // "push" mode: the stage kernel ALSO stores the traces of the UPDATED state on domain face f into halo_push[f] (null:
+    // none), the buffer the neighbour context reads as its halo_ext of the opposite face in the NEXT stage -- possibly in
+    // a peer GPU's memory (NVLink stores from inside the kernel instead of an export kernel and a message)
+    double *halo_push[6];
     int bc[6];            // domain faces x-, x+, y-, y+, z-, z+: 0 periodic, 1 slip wall, 2 far field (R19)
     double qinf[DG_NV];   // far-field state (conserved variables)
 };

@@ -282,11 +282,17 @@ struct BlockInfo {
     int bc[6];                 // boundary condition of this block's x-, x+, y-, y+, z-, z+ side if it lies on a non-periodic
                                // domain face (1 slip wall, 2 far field), else 0
     double qinf[DG_NV];
+    // "push" mode of a block decomposition: where this block ALSO stores the traces of the updated state on the domain
+    // faces it touches (the neighbour context's halo buffer, possibly in a peer GPU's memory), or null
+    double *push[4];           // x low, x high, y low, y high: the [5][Ca] block of layer z0
+    long long pstride[4];      // doubles between consecutive layers
+    double *push_z[2];         // z low (first chunk), z high (last chunk): the [5][CZ] block of this column
 };
 
 // PE for one of the axes x, y: traces of the Q in shared memory on the column boundary -> Tslot.
 template <class C, int AX>
-__device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta, const double *Qs, double *Tslot) {
+__device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta, const double *Qs, double *Tslot,
+                                                double *push_lo = nullptr, double *push_hi = nullptr) {
     using A = Axis<C, AX>;
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE;
     const bool first = g.e == 0, last = g.e == exta - 1;
@@ -309,6 +315,8 @@ __device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta
         for (int n = 0; n < NV; ++n) {
             dst[n * A::Ca] = Tm[n];
             dst[(NV + n) * A::Ca] = Tp[n];
+            if (push_lo) push_lo[n * A::Ca + g.c] = Tm[n];
+            if (push_hi) push_hi[n * A::Ca + g.c] = Tp[n];
         }
     } else if (first) {
         double T[NV];
@@ -319,7 +327,10 @@ __device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta
 #pragma unroll
             for (int n = 0; n < NV; ++n) T[n] = fma(DG_LM(q), Q0[n * PLANE + q * A::S], T[n]);
 #pragma unroll
-        for (int n = 0; n < NV; ++n) dst[n * A::Ca] = T[n];
+        for (int n = 0; n < NV; ++n) {
+            dst[n * A::Ca] = T[n];
+            if (push_lo) push_lo[n * A::Ca + g.c] = T[n];
+        }
     } else {
         double T[NV];
 #pragma unroll
@@ -329,7 +340,10 @@ __device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta
 #pragma unroll
             for (int n = 0; n < NV; ++n) T[n] = fma(DG_LP(q), Q0[n * PLANE + q * A::S], T[n]);
 #pragma unroll
-        for (int n = 0; n < NV; ++n) dst[(NV + n) * A::Ca] = T[n];
+        for (int n = 0; n < NV; ++n) {
+            dst[(NV + n) * A::Ca] = T[n];
+            if (push_hi) push_hi[n * A::Ca + g.c] = T[n];
+        }
     }
 }
 
@@ -691,12 +705,14 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
 #pragma unroll
                     for (int i = 0; i < N; ++i) tm = fma(DG_LM(i), Qn[sq][i], tm);
                     tz_out[n * Ca + g.c] = tm;
+                    if (bi->push_z[0]) bi->push_z[0][n * Ca + g.c] = tm;
                 }
                 if (last_layer) {
                     double tp = 0.0;
 #pragma unroll
                     for (int i = 0; i < N; ++i) tp = fma(DG_LP(i), Qn[sq][i], tp);
                     tz_out[(NV + n) * Ca + g.c] = tp;
+                    if (bi->push_z[1]) bi->push_z[1][n * Ca + g.c] = tp;
                 }
             }
             if (LAM) {
@@ -820,8 +836,12 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
         if (l < 32 && bi->readK && !last_layer) copy_in<C>(KR, bi->kslot + (long long)(it + 1) * bi->kstride, fullk, l);
         double *Tslot = bi->txy_out + toff;
         const Geo gx = make_geo<C, 0>(lx), gy = make_geo<C, 1>(lx);
-        boundary_traces<C, 0>(gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, Qs, Tslot);
-        boundary_traces<C, 1>(gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, Qs, Tslot);
+        boundary_traces<C, 0>(gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, Qs, Tslot,
+                              bi->push[0] ? bi->push[0] + it * bi->pstride[0] : nullptr,
+                              bi->push[1] ? bi->push[1] + it * bi->pstride[1] : nullptr);
+        boundary_traces<C, 1>(gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, Qs, Tslot,
+                              bi->push[2] ? bi->push[2] + it * bi->pstride[2] : nullptr,
+                              bi->push[3] ? bi->push[3] + it * bi->pstride[3] : nullptr);
     }
     fence_proxy_async();
     bar_arrive<C::THREADS>(2);   // hand the layer to the copy warp
@@ -877,6 +897,14 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
         if (a.halo_ext[4] && chunk == 0) bi->tz_lo = a.halo_ext[4] + col * (DG_NV * C::CZ);
         if (a.halo_ext[5] && chunk + 1 == a.nchunks) bi->tz_hi = a.halo_ext[5] + col * (DG_NV * C::CZ);
         bi->tz_out = a.Tz_new + ((size_t)chunk * cstride + col) * C::TZ;
+        // push mode: the same blocks of the neighbour contexts' halo buffers that those contexts read (layout of halo_ext)
+        for (int f = 0; f < 4; ++f) bi->push[f] = nullptr;
+        if (a.halo_push[0] && bxi == 0) { bi->push[0] = a.halo_push[0] + ((size_t)z0 * a.nby + byi) * (DG_NV * C::CX); bi->pstride[0] = (long long)a.nby * (DG_NV * C::CX); }
+        if (a.halo_push[1] && bxi + 1 == a.nbx) { bi->push[1] = a.halo_push[1] + ((size_t)z0 * a.nby + byi) * (DG_NV * C::CX); bi->pstride[1] = (long long)a.nby * (DG_NV * C::CX); }
+        if (a.halo_push[2] && byi == 0) { bi->push[2] = a.halo_push[2] + ((size_t)z0 * a.nbx + bxi) * (DG_NV * C::CY); bi->pstride[2] = (long long)a.nbx * (DG_NV * C::CY); }
+        if (a.halo_push[3] && byi + 1 == a.nby) { bi->push[3] = a.halo_push[3] + ((size_t)z0 * a.nbx + bxi) * (DG_NV * C::CY); bi->pstride[3] = (long long)a.nbx * (DG_NV * C::CY); }
+        bi->push_z[0] = (a.halo_push[4] && chunk == 0) ? a.halo_push[4] + col * (DG_NV * C::CZ) : nullptr;
+        bi->push_z[1] = (a.halo_push[5] && chunk + 1 == a.nchunks) ? a.halo_push[5] + col * (DG_NV * C::CZ) : nullptr;
         bi->tstride = (long long)cstride * C::TXY;
         bi->kslot = a.K + ((size_t)z0 * cstride + col) * C::SLOT;
         bi->kstride = (long long)cstride * C::SLOT;

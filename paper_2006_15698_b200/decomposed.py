@@ -148,7 +148,7 @@ class DistributedDG:
     torch.distributed); `reduce_max(x)` returns the maximum of a float over all ranks (default: all_reduce)."""
 
     def __init__(self, n, p, gamma, extent, procs, rank, bc=(PERIODIC,) * 6, q_inf=None, device="cuda:0", exchange=None,
-                 reduce_max=None, variant=None):
+                 reduce_max=None, variant=None, push=False):
         import torch
         from .binding import DG
         self.dec = Decomposition(n, procs, bc)
@@ -166,18 +166,62 @@ class DistributedDG:
         dev = self.dg.device
         self._send = [(f, nb, torch.empty(self.dg.halo_len(f), dtype=torch.float64, device=dev)) for f, nb in self.dec.sends(self.rank)]
         self._recv = [(f, nb, torch.empty(self.dg.halo_len(f), dtype=torch.float64, device=dev)) for f, nb in self.dec.recvs(self.rank)]
-        for f, _, buf in self._recv:
-            self.dg.set_halo(f, buf)
+        self.push = bool(push)
+        if self.push:
+            # push mode (dg_set_halo_pair / dg_set_halo_push): every halo face reads a PAIR of buffers alternately; the
+            # neighbour's stage kernel stores its traces straight into them.  connect_push() wires the two sides up.
+            self.pairs = {f: (buf, torch.empty_like(buf)) for f, _, buf in self._recv}
+            for f, (b0, b1) in self.pairs.items():
+                self.dg.set_halo_pair(f, b0, b1)
+        else:
+            for f, _, buf in self._recv:
+                self.dg.set_halo(f, buf)
+        self._dist = None
+        if self.push and exchange is None:
+            import torch.distributed as dist
+            self._dist = dist
+            self._wire_push_over_ipc(dist)
         if exchange is None or reduce_max is None:
             import torch.distributed as dist
             if exchange is None:
                 exchange = exchange_torch_distributed(dist)
             if reduce_max is None:
                 def reduce_max(x):
-                    t = torch.tensor([x], dtype=torch.float64, device=dev)
+                    # (a CPU tensor where the process group has no CUDA backend, e.g. gloo in the tests)
+                    on_gpu = dist.get_backend() == "nccl"
+                    t = torch.tensor([x], dtype=torch.float64, device=dev if on_gpu else "cpu")
                     dist.all_reduce(t, op=dist.ReduceOp.MAX)
                     return float(t.item())
         self._exchange, self._reduce_max = exchange, reduce_max
+
+    def connect_push(self, face, peer0, peer1):
+        """Push mode: this rank's stage kernels store the traces of face `face` into the neighbour's pair for its face
+        `face ^ 1` (tensors of this process, or raw addresses of peer-mapped memory opened through CUDA IPC)."""
+        self._push_targets = getattr(self, "_push_targets", {})
+        self._push_targets[face] = (peer0, peer1)
+        self.dg.set_halo_push(face, peer0, peer1)
+
+    def _wire_push_over_ipc(self, dist):
+        """One process per rank: every rank publishes CUDA IPC handles of its halo-buffer pairs (torch's own tensor
+        sharing), opens its neighbours' and hands them to the library as push targets.  The mapped buffers may live on
+        another GPU: the stage kernel's stores then go over NVLink (peer access is enabled when the handle is opened)."""
+        from torch.multiprocessing.reductions import reduce_tensor
+        mine = {f: (reduce_tensor(b0), reduce_tensor(b1)) for f, (b0, b1) in self.pairs.items()}
+        everyone = [None] * dist.get_world_size()
+        dist.all_gather_object(everyone, mine)
+        self._peer_tensors = {}
+        for f, nb in self.dec.sends(self.rank):
+            (fn0, args0), (fn1, args1) = everyone[nb][f ^ 1]
+            t0, t1 = fn0(*args0), fn1(*args1)
+            self._peer_tensors[f] = (t0, t1)             # keeps the mapping alive
+            self.connect_push(f, t0.data_ptr(), t1.data_ptr())
+        dist.barrier()
+
+    def _stage_barrier(self):
+        """Push mode between processes: every rank has finished its stage (its stores have landed in the neighbours'
+        buffers) before anyone starts the next one."""
+        self.dg.stream.synchronize()
+        self._dist.barrier()
 
     # the two halves of an exchange are separate so that a single process can drive several ranks (tests)
     def export_faces(self):
@@ -194,7 +238,12 @@ class DistributedDG:
 
     def set_state(self, q_local):
         self.dg.set_state(q_local)
-        self.exchange()
+        if self.push and self._dist is not None:
+            for f, _ in self.dec.sends(self.rank):     # the initial traces go to the neighbours' buffer 0 (parity 0)
+                self.dg._check(self.dg.lib.dg_halo_export(self.dg._h, f, self._push_targets[f][0]))
+            self._stage_barrier()
+        else:
+            self.exchange()
         return self
 
     def residual(self, out=None):
@@ -207,7 +256,10 @@ class DistributedDG:
         for _ in range(int(nsteps)):
             for stage in range(5):
                 self.dg.rk_stage(dt, stage)
-                self.exchange()
+                if self.push and self._dist is not None:
+                    self._stage_barrier()              # the stage kernel itself has delivered the faces
+                else:
+                    self.exchange()
         return self
 
     def rk_step_cfl(self, cfl, nsteps=1, h_min=None):
@@ -277,3 +329,42 @@ def gather_in_process(ranks, what="state"):
         (x0, x1), (y0, y1), (z0, z1) = r.box
         out[z0:z1, y0:y1, x0:x1] = r.dg.get_state() if what == "state" else r.dg.residual()
     return out
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# push mode (dg_set_halo_pair / dg_set_halo_push): the stage kernels store the boundary traces straight into the
+# neighbour contexts' halo buffers, no export kernel, no message.  Between processes the buffers are opened in the
+# neighbour's address space with CUDA IPC and the stores travel over NVLink; the only communication left is the
+# ordering "every rank has finished stage s before anyone starts stage s + 1" (a barrier) -- written here for contexts
+# of ONE process, where one stream provides that ordering.
+# ------------------------------------------------------------------------------------------------------------------
+def make_in_process_push(n, p, gamma, extent, procs, bc=(PERIODIC,) * 6, q_inf=None, device="cuda:0", variant=None):
+    dec = Decomposition(n, procs, bc)
+    if variant is None:
+        variant = choose_variant(dec, p, variant_shapes(p))
+    nothing = lambda rank, sends, recvs: None
+    ranks = [DistributedDG(n, p, gamma, extent, procs, r, bc, q_inf, device, exchange=nothing, reduce_max=lambda x: x,
+                           variant=variant, push=True) for r in range(dec.size)]
+    for r in ranks:
+        for f, nb in dec.sends(r.rank):
+            r.connect_push(f, *ranks[nb].pairs[f ^ 1])
+    return ranks
+
+
+def set_state_in_process_push(ranks, q_global):
+    """Every rank takes its block; the traces of the initial state go to the neighbours' buffer 0 (parity 0)."""
+    import numpy as np
+    for r in ranks:
+        (x0, x1), (y0, y1), (z0, z1) = r.box
+        r.dg.set_state(np.ascontiguousarray(q_global[z0:z1, y0:y1, x0:x1]))
+    for r in ranks:
+        for f, nb in r.dec.sends(r.rank):
+            r.dg.halo_export(f, ranks[nb].pairs[f ^ 1][0])
+
+
+def rk_step_in_process_push(ranks, dt, nsteps=1):
+    """No exchange step at all: the stage kernels have already put the traces where the neighbours read them."""
+    for _ in range(int(nsteps)):
+        for stage in range(5):
+            for r in ranks:
+                r.dg.rk_stage(dt, stage)

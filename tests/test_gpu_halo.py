@@ -47,6 +47,58 @@ def test_decomposed_run_equals_the_single_context_run_bit_for_bit(procs, p):
     single.close()
 
 
+@pytest.mark.parametrize("procs", [(2, 1, 1), (1, 1, 2), (2, 2, 2), (3, 2, 1)])
+@pytest.mark.parametrize("p", [1, 4, 6])
+def test_push_mode_equals_the_single_context_run_bit_for_bit(procs, p):
+    """dg_set_halo_pair / dg_set_halo_push: the stage kernels store the face traces straight into the neighbour
+    contexts' (double-buffered) halo buffers; no export kernel and no copy between the stages."""
+    n, ext = (7, 6, 5), (1.0, 0.9, 0.8)
+    q = rough_field(*n, p, ext, seed=5)
+    dt = I.cfl_dt(ORC.max_wavespeed(q, p, G), p, ext, n, 0.1)
+    ranks = D.make_in_process_push(n, p, G, ext, procs)
+    single = DG(*n, p, G, ext, variant=ranks[0].dg.kernel_info()["variant"])
+    D.set_state_in_process_push(ranks, q)
+    single.set_state(q)
+    assert np.array_equal(D.gather_in_process(ranks, "residual"), single.residual())
+    launches = sum(r.dg.launch_count for r in ranks)
+    D.rk_step_in_process_push(ranks, dt, 3)
+    assert sum(r.dg.launch_count for r in ranks) - launches == 15 * len(ranks)      # stage kernels only
+    assert np.array_equal(D.gather_in_process(ranks, "residual"), single.rk_step(dt, 3).residual())   # odd parity
+    q_dec, q_one = D.gather_in_process(ranks), single.get_state()
+    assert np.array_equal(q_dec, q_one), relerr(q_dec, q_one)
+    assert relerr(q_dec, ORC.rk_step(q, p, G, ext, dt, 3)) < 1e-12
+    for r in ranks:
+        r.close()
+    single.close()
+
+
+def test_push_mode_between_two_processes():
+    """Two processes, one rank each, the neighbour's halo buffers opened through CUDA IPC and written by the stage kernel
+    (tests/push_ipc_worker.py).  Both ranks share this box's one GPU; on a multi-GPU node the same code stores over NVLink."""
+    import os
+    import socket
+    import subprocess
+    import sys
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    worker = os.path.join(os.path.dirname(os.path.abspath(__file__)), "push_ipc_worker.py")
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, worker], env=env, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True))
+    outs = []
+    try:
+        for pr in procs:
+            outs.append(pr.communicate(timeout=240)[0])
+    finally:
+        for pr in procs:
+            if pr.poll() is None:
+                pr.kill()
+    for rank, (pr, out) in enumerate(zip(procs, outs)):
+        assert pr.returncode == 0 and f"OK rank {rank}" in out, out[-3000:]
+
+
 def test_decomposition_with_walls_and_far_field():
     n, p, ext = (6, 5, 4), 2, (1.0, 1.0, 0.7)
     bc = (D.WALL, D.FARFIELD, D.PERIODIC, D.PERIODIC, D.WALL, D.WALL)
