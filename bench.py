@@ -416,6 +416,62 @@ def navier_stokes_leg(workload, steps, device, mu=1e-3, prandtl=0.72):
     return out
 
 
+def decomposed_one_gpu_leg(workload, steps, device, procs=(2, 2, 2)):
+    """SURVEY.md 8(f)-1 as far as one GPU goes: the workload's mesh cut into blocks, one context per block, ALL on this
+    GPU and one stream (ordinary launches one after another; no kernel waits on another).  Times the export / import
+    mode (six gather kernels per block and stage + device copies) and the push mode (the stage kernels store the faces
+    into the neighbours' buffers; nothing else is launched) against the single-context run of the same mesh."""
+    import torch
+    from paper_2006_15698_b200 import DG
+    from paper_2006_15698_b200 import decomposed as D
+    from paper_2006_15698_b200 import inputs as I
+    c = I.CONFIGS[workload]
+    p, ext, n = c["p"], c["extent"], (c["nx"], c["ny"], c["nz"])
+    dof = n[0] * n[1] * n[2] * (p + 1) ** 3
+    stream = torch.cuda.current_stream(device)
+
+    def timed(step):
+        step(2)
+        torch.cuda.synchronize(device)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        step(steps)
+        e1.record(stream)
+        torch.cuda.synchronize(device)
+        return dof * STAGES * steps / (e0.elapsed_time(e1) * 1e-3)
+
+    out = {"workload": f"{workload}: {list(n)} elements, p={p}, cut into {list(procs)} blocks on ONE GPU", "steps": steps, "unit": UNIT}
+    single = DG(*n, p, GAMMA, ext, device=device)
+    single.set_state(I.make_field(workload, xp=torch, device=device))
+    dt = I.cfl_dt(single.max_wavespeed(), p, ext, n, 0.1)
+    out["single_context"] = timed(lambda k: single.rk_step(dt, k))
+    variant = single.kernel_info()["variant"]
+    single.close()
+    for mode in ("export_import", "push"):
+        make = D.make_in_process_push if mode == "push" else D.make_in_process
+        ranks = make(n, p, GAMMA, ext, procs, device=str(device), variant=variant)
+        for r in ranks:
+            r.dg.set_state(I.make_field(workload, box=r.box, xp=torch, device=device))
+        if mode == "push":
+            for r in ranks:
+                for f, nb in r.dec.sends(r.rank):
+                    r.dg.halo_export(f, ranks[nb].pairs[f ^ 1][0])
+            step = lambda k: D.rk_step_in_process_push(ranks, dt, k)
+        else:
+            D.exchange_in_process(ranks)
+            step = lambda k: D.rk_step_in_process(ranks, dt, k)
+        l0 = sum(r.dg.launch_count for r in ranks)
+        out[mode] = timed(step)
+        out[mode + "_launches_per_stage"] = (sum(r.dg.launch_count for r in ranks) - l0) / ((steps + 2) * STAGES)
+        for r in ranks:
+            r.close()
+        del ranks
+        torch.cuda.empty_cache()
+    out["note"] = ("blocks run one after another on the same GPU, so this measures what the decomposition costs (smaller launches, "
+                   "duplicated shared faces, the exchange), not a speed-up; never run on more than one GPU")
+    return out
+
+
 def reduce_max(x, dist, device):
     """Max over ranks of a per-rank time (replicas: the slowest replica sets the whole-job rate)."""
     if dist is None:
@@ -531,7 +587,7 @@ def run_ours(args, rank, world, local_rank):
 
     ms = reduce_max(main["ms"], dist, device)
     e2e_s = reduce_max(main["e2e"]["seconds"], dist, device)
-    sweep, sustained, big, fp64, per_kernel, ns = [], None, None, None, None, None
+    sweep, sustained, big, fp64, per_kernel, ns, dec1 = [], None, None, None, None, None, None
     # order: the short legs first (burst clocks, like the main leg), then the long ones that heat the board up
     if not args.no_sweep and world == 1:
         for p in range(1, 8):
@@ -545,6 +601,7 @@ def run_ours(args, rank, world, local_rank):
         fp64 = fp64_peak(device)
         per_kernel = per_kernel_breakdown("table2_p6", 10, device)
         ns = navier_stokes_leg("table2_p6", 4, device)
+        dec1 = decomposed_one_gpu_leg(args.workload if args.workload != "cfg5" else "cfg3", 10, device)
         # the same workload for >= 300 steps: the board reaches its power cap after ~0.3 s and holds lower clocks
         sustained = time_workload(args.workload, max(300, K), W, device, None, physical_gpu_index(local_rank), lz=args.lz,
                                   variant=args.variant)
@@ -627,6 +684,8 @@ def run_ours(args, rank, world, local_rank):
         line["per_kernel"] = per_kernel
     if ns is not None:
         line["navier_stokes"] = ns
+    if dec1 is not None:
+        line["decomposed_one_gpu"] = dec1
     if fp64 is not None:
         flops = algo_flops_per_dof(main["p"]) * value
         line["roofline_fp64"] = {"bound": "fp64", "achieved": flops / 1e12, "peak": 2.0 * fp64 / 1e12, "unit": "TFLOP/s",

@@ -705,14 +705,14 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
 #pragma unroll
                     for (int i = 0; i < N; ++i) tm = fma(DG_LM(i), Qn[sq][i], tm);
                     tz_out[n * Ca + g.c] = tm;
-                    if (bi->push_z[0]) bi->push_z[0][n * Ca + g.c] = tm;
+                    if (BC && bi->push_z[0]) bi->push_z[0][n * Ca + g.c] = tm;
                 }
                 if (last_layer) {
                     double tp = 0.0;
 #pragma unroll
                     for (int i = 0; i < N; ++i) tp = fma(DG_LP(i), Qn[sq][i], tp);
                     tz_out[(NV + n) * Ca + g.c] = tp;
-                    if (bi->push_z[1]) bi->push_z[1][n * Ca + g.c] = tp;
+                    if (BC && bi->push_z[1]) bi->push_z[1][n * Ca + g.c] = tp;
                 }
             }
             if (LAM) {
@@ -836,12 +836,13 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
         if (l < 32 && bi->readK && !last_layer) copy_in<C>(KR, bi->kslot + (long long)(it + 1) * bi->kstride, fullk, l);
         double *Tslot = bi->txy_out + toff;
         const Geo gx = make_geo<C, 0>(lx), gy = make_geo<C, 1>(lx);
+        // (push mode runs the BC instances: the periodic, single-context instances carry none of this)
         boundary_traces<C, 0>(gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, Qs, Tslot,
-                              bi->push[0] ? bi->push[0] + it * bi->pstride[0] : nullptr,
-                              bi->push[1] ? bi->push[1] + it * bi->pstride[1] : nullptr);
+                              (BC && bi->push[0]) ? bi->push[0] + it * bi->pstride[0] : nullptr,
+                              (BC && bi->push[1]) ? bi->push[1] + it * bi->pstride[1] : nullptr);
         boundary_traces<C, 1>(gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, Qs, Tslot,
-                              bi->push[2] ? bi->push[2] + it * bi->pstride[2] : nullptr,
-                              bi->push[3] ? bi->push[3] + it * bi->pstride[3] : nullptr);
+                              (BC && bi->push[2]) ? bi->push[2] + it * bi->pstride[2] : nullptr,
+                              (BC && bi->push[3]) ? bi->push[3] + it * bi->pstride[3] : nullptr);
     }
     fence_proxy_async();
     bar_arrive<C::THREADS>(2);   // hand the layer to the copy warp
@@ -1361,7 +1362,9 @@ cudaError_t prepare(const DgRefOps &ref, int *blocks_per_sm) {
 template <class C>
 cudaError_t launch_stage(const DgStageArgs &a, cudaStream_t s) {
     const dim3 grid((unsigned)a.nbx, (unsigned)a.nby, (unsigned)a.nchunks);
-    const bool bc = a.bc[0] || a.bc[1] || a.bc[2] || a.bc[3] || a.bc[4] || a.bc[5];
+    // the instances with boundary code also hold the push-mode stores
+    const bool bc = a.bc[0] || a.bc[1] || a.bc[2] || a.bc[3] || a.bc[4] || a.bc[5] || a.halo_push[0] || a.halo_push[1] ||
+                    a.halo_push[2] || a.halo_push[3] || a.halo_push[4] || a.halo_push[5];
     const size_t sm = Smem<C>::BYTES;
     if (a.mode == DG_MODE_RESIDUAL) {
         if (bc) dg_stage_kernel<C, DG_MODE_RESIDUAL, false, true><<<grid, C::THREADS, sm, s>>>(a);
