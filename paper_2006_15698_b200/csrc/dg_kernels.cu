@@ -1457,7 +1457,7 @@ constexpr DgKernelTable make_table() {
 #define DG_VARIANTS DG_T(5, 2, 3, 2, 0, 154, 4, 0), DG_T(5, 3, 2, 2, 0, 0, 4, 0), DG_T(5, 2, 2, 3, 1, 106, 4, 0), DG_T(5, 5, 1, 2, 0, 0, 4, 0), \
                     DG_T(5, 5, 1, 2, 1, 0, 4, 0), DG_T(5, 1, 5, 2, 0, 138, 0, 1)
 #elif DG_N == 6
-#define DG_VARIANTS DG_T(6, 1, 3, 2, 0, 118, 0, 0), DG_T(6, 3, 1, 2, 0, 114, 2, 0), DG_T(6, 2, 1, 3, 0, 0, 4, 0), DG_T(6, 2, 1, 3, 1, 0, 4, 0), \
+#define DG_VARIANTS DG_T(6, 1, 3, 2, 1, 118, 0, 0), DG_T(6, 1, 3, 2, 0, 118, 0, 0), DG_T(6, 3, 1, 2, 0, 114, 2, 0), DG_T(6, 2, 1, 3, 0, 0, 4, 0), DG_T(6, 2, 1, 3, 1, 0, 4, 0), \
                     DG_T(6, 1, 1, 5, 1, 0, 0, 0), DG_T(6, 1, 1, 4, 0, 0, 0, 0)
 #elif DG_N == 7
 #define DG_VARIANTS DG_T(7, 2, 1, 2, 1, 0, 4, 0, 1), DG_T(7, 2, 1, 2, 1, 0, 4, 0), DG_T(7, 1, 1, 4, 1, 0, 0, 1), DG_T(7, 1, 1, 4, 0, 0, 0, 1), DG_T(7, 1, 1, 3, 0, 0, 0, 1)
