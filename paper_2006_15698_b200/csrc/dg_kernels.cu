@@ -318,7 +318,7 @@ __device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta
             if (push_lo) push_lo[n * A::Ca + g.c] = Tm[n];
             if (push_hi) push_hi[n * A::Ca + g.c] = Tp[n];
         }
-    } else if (first) {
+    } else if (A::ORD < 4 && first) {   // (the lines of the first and of the last element sit in different warps)
         double T[NV];
 #pragma unroll
         for (int n = 0; n < NV; ++n) T[n] = 0.0;
@@ -331,7 +331,7 @@ __device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta
             dst[n * A::Ca] = T[n];
             if (push_lo) push_lo[n * A::Ca + g.c] = T[n];
         }
-    } else {
+    } else if (A::ORD < 4) {
         double T[NV];
 #pragma unroll
         for (int n = 0; n < NV; ++n) T[n] = 0.0;
@@ -343,6 +343,26 @@ __device__ __forceinline__ void boundary_traces(const Geo &g, bool act, int exta
         for (int n = 0; n < NV; ++n) {
             dst[(NV + n) * A::Ca] = T[n];
             if (push_hi) push_hi[n * A::Ca + g.c] = T[n];
+        }
+    } else {
+        // element index fastest in the lane order: lines of the first and of the last element share every warp.  One
+        // trace per line, T- for the former and T+ for the latter, in ONE instruction stream (two divergent branches
+        // would run every load twice with half the lanes, and those lanes' addresses collide in the banks)
+        double T[NV];
+#pragma unroll
+        for (int n = 0; n < NV; ++n) T[n] = 0.0;
+#pragma unroll
+        for (int q = 0; q < N; ++q) {
+            const double w = first ? DG_LM(q) : DG_LP(q);
+#pragma unroll
+            for (int n = 0; n < NV; ++n) T[n] = fma(w, Q0[n * PLANE + q * A::S], T[n]);
+        }
+        double *d1 = dst + (first ? 0 : NV * A::Ca);
+        double *push = first ? push_lo : push_hi;
+#pragma unroll
+        for (int n = 0; n < NV; ++n) {
+            d1[n * A::Ca] = T[n];
+            if (push) push[n * A::Ca + g.c] = T[n];
         }
     }
 }
@@ -458,7 +478,10 @@ __device__ __forceinline__ void xy_pass(const BlockInfo *bi, const Geo &g, bool 
     using A = Axis<C, AX>;
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE, L = C::L, S = A::S, Ca = A::Ca;
     const bool first = g.e == 0, last = g.e == exta - 1;
-    const int lb = g.e * Ca + g.c;   // slot of this line in the hand-over buffers
+    // slot of this line in the hand-over buffers: neighbouring lanes write neighbouring slots (element index fastest
+    // where it is fastest in the lane order); HS = distance to the next element's line
+    constexpr int HS = (A::ORD >= 4) ? 1 : Ca;
+    const int lb = (A::ORD >= 4) ? g.c * A::B + g.e : g.e * Ca + g.c;
     const double gamma = bi->gamma, gm1 = bi->gm1;
     // PH: the neighbour columns' traces this line touches, momentum slots rotated, HBM/L2 -> registers
     double Hlo[NV], Hhi[NV];
@@ -519,7 +542,7 @@ __device__ __forceinline__ void xy_pass(const BlockInfo *bi, const Geo &g, bool 
         }
     } else if (A::MULTI && act && !last) {
 #pragma unroll
-        for (int n = 0; n < NV; ++n) Hhi[n] = Tms[n * L + lb + Ca];   // T- of the next element of this layer
+        for (int n = 0; n < NV; ++n) Hhi[n] = Tms[n * L + lb + HS];   // T- of the next element of this layer
     }
     lax_friedrichs2(Tp, Hhi, 1.0, gamma, gm1, Fp);
     if (SHF) {
@@ -540,7 +563,7 @@ __device__ __forceinline__ void xy_pass(const BlockInfo *bi, const Geo &g, bool 
         bar_sync<C::NCOMP>(1);
         if (!first) {
 #pragma unroll
-            for (int n = 0; n < NV; ++n) Fm[n] = Fss[n * L + lb - Ca];
+            for (int n = 0; n < NV; ++n) Fm[n] = Fss[n * L + lb - HS];
         }
     } else {
         lax_friedrichs2(Tm, Hlo, -1.0, gamma, gm1, Fm);
