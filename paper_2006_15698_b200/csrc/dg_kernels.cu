@@ -206,6 +206,7 @@ struct Geo {
     int c;      // face-node index of the line on the layer side (lane order: this is how the traces are stored)
     int e;      // element along the axis
     int t1, t2; // transverse node indices
+    bool ok;    // the thread has a line of its own (false: it computes on a valid line and stores nothing)
 };
 
 template <class C, int AX>
@@ -213,6 +214,19 @@ __device__ __forceinline__ Geo make_geo(int l) {
     using A = Axis<C, AX>;
     constexpr int N = C::N, T1 = A::T1, T2 = A::T2, B = A::B;
     Geo g;
+    if (A::ORD == 6) {
+        // one (t2) plane of lines per warp, element index fastest: no half-warp straddles two planes, so that the
+        // lanes' addresses stay an arithmetic sequence whatever the plane pitch (needs T1 B <= 32, T2 warps)
+        static_assert(A::ORD != 6 || (T1 * B <= 32 && T2 * 32 <= C::NCOMP), "ORD 6 does not fit this shape");
+        const int r = min(l & 31, T1 * B - 1);
+        g.ok = (l & 31) < T1 * B && (l >> 5) < T2;
+        g.e = r % B;
+        g.t1 = r / B;
+        g.t2 = min(l >> 5, T2 - 1);
+        g.c = g.t2 * T1 + g.t1;
+    } else {
+    g.ok = l < C::L;
+    l = min(l, C::L - 1);
     if (A::ORD == 0) {
         g.t1 = l % T1;
         g.t2 = (l / T1) % T2;
@@ -243,6 +257,7 @@ __device__ __forceinline__ Geo make_geo(int l) {
         g.t2 = (l / B) % T2;
         g.t1 = l / (B * T2);
         g.c = g.t1 * T2 + g.t2;
+    }
     }
     if (AX == 0) g.base = g.t2 * C::PP + g.t1 * C::P + g.e * N;
     else if (AX == 1) g.base = g.t2 * C::PP + g.e * N * C::P + g.t1;
@@ -823,19 +838,18 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
     const double *Qnext = smem + ((it & 1) ? SM::QB0 : SM::QB1);
     double *KR = smem + SM::KR, *Tms = smem + SM::TMS, *Fss = smem + SM::FSS, *FmS = smem + SM::FMS;
     const int l = threadIdx.x, lx = min(l, L - 1);
-    const bool inL = l < L;
     const int ext0 = bi->ext0, ext1 = bi->ext1;
     const long long toff = (long long)it * bi->tstride;
     mbar_wait(&fullq[it & 1], (it >> 1) & 1);
     {
-        const Geo gx = make_geo<C, 0>(lx);
-        xy_pass<C, 0, MODE, BC>(bi, gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, bi->halo[0] + it * bi->hstride[0],
+        const Geo gx = make_geo<C, 0>(l);
+        xy_pass<C, 0, MODE, BC>(bi, gx, gx.ok && line_inside<C, 0>(gx, ext0, ext1), ext0, bi->halo[0] + it * bi->hstride[0],
                                 bi->halo[1] + it * bi->hstride[1], Qs,
                             KR, Tms, Fss, fullk, it & 1);
     }
     {
-        const Geo gy = make_geo<C, 1>(lx);
-        xy_pass<C, 1, MODE, BC>(bi, gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, bi->halo[2] + it * bi->hstride[2],
+        const Geo gy = make_geo<C, 1>(l);
+        xy_pass<C, 1, MODE, BC>(bi, gy, gy.ok && line_inside<C, 1>(gy, ext0, ext1), ext1, bi->halo[2] + it * bi->hstride[2],
                                 bi->halo[3] + it * bi->hstride[3], Qs,
                             KR, Tms, Fss, fullk, it & 1);
     }
@@ -849,8 +863,8 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
     }
     if (!last_layer) mbar_wait(&fullq[(it + 1) & 1], ((it + 1) >> 1) & 1);
     {
-        const Geo gz = make_geo<C, 2>(lx);
-        z_pass<C, MODE, LAM, BC>(bi, gz, lx, inL && line_inside<C, 2>(gz, ext0, ext1), Qs, Qnext, KR, FmS,
+        const Geo gz = make_geo<C, 2>(l);
+        z_pass<C, MODE, LAM, BC>(bi, gz, lx, gz.ok && line_inside<C, 2>(gz, ext0, ext1), Qs, Qnext, KR, FmS,
                              bi->kslot + (long long)it * bi->kstride, it == 0, last_layer, lam_best);
     }
     bar_sync<C::NCOMP>(1);   // the updated Q of the whole layer is in shared memory; every line has read KR
@@ -858,12 +872,12 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
         // the next layer's K can come in now (needed at the end of its x pass)
         if (l < 32 && bi->readK && !last_layer) copy_in<C>(KR, bi->kslot + (long long)(it + 1) * bi->kstride, fullk, l);
         double *Tslot = bi->txy_out + toff;
-        const Geo gx = make_geo<C, 0>(lx), gy = make_geo<C, 1>(lx);
+        const Geo gx = make_geo<C, 0>(l), gy = make_geo<C, 1>(l);
         // (push mode runs the BC instances: the periodic, single-context instances carry none of this)
-        boundary_traces<C, 0>(gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, Qs, Tslot,
+        boundary_traces<C, 0>(gx, gx.ok && line_inside<C, 0>(gx, ext0, ext1), ext0, Qs, Tslot,
                               (BC && bi->push[0]) ? bi->push[0] + it * bi->pstride[0] : nullptr,
                               (BC && bi->push[1]) ? bi->push[1] + it * bi->pstride[1] : nullptr);
-        boundary_traces<C, 1>(gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, Qs, Tslot,
+        boundary_traces<C, 1>(gy, gy.ok && line_inside<C, 1>(gy, ext0, ext1), ext1, Qs, Tslot,
                               (BC && bi->push[2]) ? bi->push[2] + it * bi->pstride[2] : nullptr,
                               (BC && bi->push[3]) ? bi->push[3] + it * bi->pstride[3] : nullptr);
     }
@@ -997,13 +1011,12 @@ __global__ void __launch_bounds__(C::NCOMP) dg_traces_kernel(const __grid_consta
     __syncthreads();
     const Geo gx = make_geo<C, 0>(tid), gy = make_geo<C, 1>(tid), gz = make_geo<C, 2>(tid);
     const int ext0 = min(C::BX, a.nx - bxi * C::BX), ext1 = min(C::BY, a.ny - byi * C::BY);
-    const bool inL = tid < C::L;
     double *Tslot = a.Txy + slot * C::TXY;
-    boundary_traces<C, 0>(gx, inL && line_inside<C, 0>(gx, ext0, ext1), ext0, smem, Tslot);
-    boundary_traces<C, 1>(gy, inL && line_inside<C, 1>(gy, ext0, ext1), ext1, smem, Tslot);
+    boundary_traces<C, 0>(gx, gx.ok && line_inside<C, 0>(gx, ext0, ext1), ext0, smem, Tslot);
+    boundary_traces<C, 1>(gy, gy.ok && line_inside<C, 1>(gy, ext0, ext1), ext1, smem, Tslot);
     const int chunk = ez / a.lz;
     const bool zfirst = ez == chunk * a.lz, zlast = (ez + 1 == a.nz) || (ez + 1 == (chunk + 1) * a.lz);
-    if ((zfirst || zlast) && inL && line_inside<C, 2>(gz, ext0, ext1)) {
+    if ((zfirst || zlast) && gz.ok && line_inside<C, 2>(gz, ext0, ext1)) {
         double *dst = a.Tz + ((size_t)chunk * cstride + col) * C::TZ + gz.c;
 #pragma unroll
         for (int n = 0; n < NV; ++n) {
@@ -1042,13 +1055,11 @@ __global__ void __launch_bounds__(C::NCOMP) dg_split_volume_kernel(const __grid_
     stage_layer_in<C>(Qs, a.Q + slot * C::SLOT, tid);
     __syncthreads();
     const int ext0 = min(C::BX, a.nx - bxi * C::BX), ext1 = min(C::BY, a.ny - byi * C::BY);
-    const int lx = min(tid, C::L - 1);
-    const bool inL = tid < C::L;
     auto axis = [&](auto AXT) {
         constexpr int AX = decltype(AXT)::value;
         using A = Axis<C, AX>;
-        const Geo g = make_geo<C, AX>(lx);
-        const bool act = inL && line_inside<C, AX>(g, ext0, ext1);
+        const Geo g = make_geo<C, AX>(tid);
+        const bool act = g.ok && line_inside<C, AX>(g, ext0, ext1);
         double V[NV][N];
 #pragma unroll
         for (int q = 0; q < N; ++q) {
@@ -1122,13 +1133,11 @@ __global__ void __launch_bounds__(C::NCOMP) dg_split_surface_kernel(const __grid
     stage_layer_in<C>(Rs, a.R + slot * C::SLOT, tid);
     __syncthreads();
     const int ext0 = min(C::BX, a.nx - bxi * C::BX), ext1 = min(C::BY, a.ny - byi * C::BY);
-    const int lx = min(tid, C::L - 1);
-    const bool inL = tid < C::L;
     auto axis = [&](auto AXT) {
         constexpr int AX = decltype(AXT)::value;
         using A = Axis<C, AX>;
-        const Geo g = make_geo<C, AX>(lx);
-        const bool act = inL && line_inside<C, AX>(g, ext0, ext1);
+        const Geo g = make_geo<C, AX>(tid);
+        const bool act = g.ok && line_inside<C, AX>(g, ext0, ext1);
         if (act) {
             double Tp[NV], Tm[NV], Hlo[NV], Hhi[NV], Fp[NV], Fm[NV];
 #pragma unroll
@@ -1188,9 +1197,8 @@ __device__ __forceinline__ void cwd_axis(const DgViscArgs &a, const double *Gs, 
     using A = Axis<C, AX>;
     constexpr int NV = DG_NV, N = C::N, PLANE = C::PLANE;
     const int ext0 = min(C::BX, a.nx - bxi * C::BX), ext1 = min(C::BY, a.ny - byi * C::BY);
-    if (tid >= C::L) return;
     const Geo g = make_geo<C, AX>(tid);
-    if (!line_inside<C, AX>(g, ext0, ext1)) return;
+    if (!g.ok || !line_inside<C, AX>(g, ext0, ext1)) return;
     double Gl[NV][N], Tp[NV], Tm[NV], Hlo[NV], Hhi[NV];
 #pragma unroll
     for (int n = 0; n < NV; ++n) {
@@ -1477,7 +1485,7 @@ constexpr DgKernelTable make_table() {
 #define DG_VARIANTS DG_T(4, 2, 2, 4, 0, 66, 1, 0), DG_T(4, 2, 2, 5, 1, 66, 1, 0), DG_T(4, 4, 2, 2, 0, 130, 3, 0), DG_T(4, 4, 2, 3, 1, 130, 3, 0), \
                     DG_T(4, 2, 2, 3, 0, 66, 1, 0)
 #elif DG_N == 5
-#define DG_VARIANTS DG_T(5, 2, 3, 2, 0, 154, 4, 0), DG_T(5, 3, 2, 2, 0, 0, 4, 0), DG_T(5, 2, 2, 3, 1, 106, 4, 0), DG_T(5, 5, 1, 2, 0, 0, 4, 0), \
+#define DG_VARIANTS DG_T(5, 2, 3, 2, 0, 154, 6, 0), DG_T(5, 2, 3, 2, 0, 154, 4, 0), DG_T(5, 3, 2, 2, 0, 0, 4, 0), DG_T(5, 2, 2, 3, 1, 106, 4, 0), DG_T(5, 5, 1, 2, 0, 0, 4, 0), \
                     DG_T(5, 5, 1, 2, 1, 0, 4, 0), DG_T(5, 1, 5, 2, 0, 138, 0, 1)
 #elif DG_N == 6
 #define DG_VARIANTS DG_T(6, 1, 3, 2, 1, 118, 0, 0), DG_T(6, 1, 3, 2, 0, 118, 0, 0), DG_T(6, 3, 1, 2, 0, 114, 2, 0), DG_T(6, 2, 1, 3, 0, 0, 4, 0), DG_T(6, 2, 1, 3, 1, 0, 4, 0), \
