@@ -215,14 +215,15 @@ __device__ __forceinline__ Geo make_geo(int l) {
     constexpr int N = C::N, T1 = A::T1, T2 = A::T2, B = A::B;
     Geo g;
     if (A::ORD == 6) {
-        // one (t2) plane of lines per warp, element index fastest: no half-warp straddles two planes, so that the
-        // lanes' addresses stay an arithmetic sequence whatever the plane pitch (needs T1 B <= 32, T2 warps)
-        static_assert(A::ORD != 6 || (T1 * B <= 32 && T2 * 32 <= C::NCOMP), "ORD 6 does not fit this shape");
-        const int r = min(l & 31, T1 * B - 1);
-        g.ok = (l & 31) < T1 * B && (l >> 5) < T2;
+        // one (t2) plane of lines per warp -- or per half-warp when it fits --, element index fastest: no half-warp
+        // straddles two planes, so that its lanes' addresses stay an arithmetic sequence whatever the plane pitch
+        constexpr int G = (T1 * B <= 16) ? 16 : 32;
+        static_assert(A::ORD != 6 || (T1 * B <= 32 && T2 * G <= C::NCOMP), "ORD 6 does not fit this shape");
+        const int r = min(l % G, T1 * B - 1);
+        g.ok = (l % G) < T1 * B && (l / G) < T2;
         g.e = r % B;
         g.t1 = r / B;
-        g.t2 = min(l >> 5, T2 - 1);
+        g.t2 = min(l / G, T2 - 1);
         g.c = g.t2 * T1 + g.t1;
     } else {
     g.ok = l < C::L;
@@ -1491,7 +1492,7 @@ constexpr DgKernelTable make_table() {
 #define DG_VARIANTS DG_T(6, 1, 3, 2, 1, 118, 0, 0), DG_T(6, 1, 3, 2, 0, 118, 0, 0), DG_T(6, 3, 1, 2, 0, 114, 2, 0), DG_T(6, 2, 1, 3, 0, 0, 4, 0), DG_T(6, 2, 1, 3, 1, 0, 4, 0), \
                     DG_T(6, 1, 1, 5, 1, 0, 0, 0), DG_T(6, 1, 1, 4, 0, 0, 0, 0)
 #elif DG_N == 7
-#define DG_VARIANTS DG_T(7, 2, 1, 2, 1, 0, 4, 0, 1), DG_T(7, 2, 1, 2, 1, 0, 4, 0), DG_T(7, 1, 1, 4, 1, 0, 0, 1), DG_T(7, 1, 1, 4, 0, 0, 0, 1), DG_T(7, 1, 1, 3, 0, 0, 0, 1)
+#define DG_VARIANTS DG_T(7, 2, 1, 2, 1, 0, 4, 6, 1), DG_T(7, 2, 1, 2, 1, 0, 4, 0, 1), DG_T(7, 2, 1, 2, 1, 0, 4, 0), DG_T(7, 1, 1, 4, 1, 0, 0, 1), DG_T(7, 1, 1, 4, 0, 0, 0, 1), DG_T(7, 1, 1, 3, 0, 0, 0, 1)
 #elif DG_N == 8
 #define DG_VARIANTS DG_T(8, 1, 1, 3, 1, 66, 1, 1), DG_T(8, 1, 1, 3, 0, 66, 1, 1), DG_T(8, 2, 1, 1, 0, 130, 1, 0), DG_T(8, 1, 2, 1, 0, 130, 1, 1)
 #else
