@@ -347,13 +347,13 @@ def per_kernel_breakdown(workload, steps, device):
                                       "source": "derived from PAPER.md:264-269 (3,072 V100, 100 steps); another machine"}}
 
 
-VISC_BYTES_PER_DOF = 800.0   # unfused viscous path, per evaluation: 3 gradients (read Q, write S_a: 240), pointwise flux
-                             # (read Q + S, write Fv: 280), 3 divergences (read Fv_a, read + write R: 360); DESIGN.md 6.6
+VISC_BYTES_PER_DOF = 360.0   # viscous path, per evaluation: gradient + flux sweep (read Q 40, write Fv_x,y,z 120), divergence
+                             # sweep (read Fv 120, read + write R 80); DESIGN.md 6.6
 
 
 def navier_stokes_leg(workload, steps, device, mu=1e-3, prandtl=0.72):
-    """LSERK45 steps of dQ/dt = L(Q) + div Fv (dg_rk_step_ns: per-kernel mode + the seven viscous
-    kernels), timed with CUDA events on the launching stream; the viscous kernels on their own; the oracle's
+    """LSERK45 steps of dQ/dt = L(Q) + div Fv (dg_rk_step_ns: per-kernel mode + the two viscous
+    sweeps), timed with CUDA events on the launching stream; the viscous kernels on their own; the oracle's
     rk_step_ns on a reduced mesh of the same field beside it."""
     import torch
     from paper_2006_15698_b200 import DG
@@ -390,14 +390,14 @@ def navier_stokes_leg(workload, steps, device, mu=1e-3, prandtl=0.72):
     peak, _ = measured_peaks()
     out = {"workload": f"{workload}: {list(n)} periodic elements, p={p}, {dof} nodes, mu={mu}, Pr={prandtl}",
            "steps": steps, "value": dof * evals / total, "unit": UNIT, "seconds": total, "launches": l1 - l0,
-           "viscous_kernels": {"seconds": visc, "dof_per_s": dof * evals / visc, "launches_per_evaluation": 7,
+           "viscous_kernels": {"seconds": visc, "dof_per_s": dof * evals / visc, "launches_per_evaluation": 2,
                                "roofline": {"bound": "hbm", "achieved": VISC_BYTES_PER_DOF * dof * evals / visc / 1e9,
                                             "peak": peak, "unit": "GB/s",
                                             "frac": VISC_BYTES_PER_DOF * dof * evals / visc / 1e9 / peak,
                                             "algorithmic_bytes_per_dof": VISC_BYTES_PER_DOF}},
            "finite": finite,
-           "note": "not fused: per-kernel mode (volume, surface, update-project) + three gradient kernels, the pointwise "
-                   "viscous flux, three divergence kernels per stage; reading R20 (the paper prints no viscous equations)"}
+           "note": "not fused into the stage kernel: per-kernel mode (volume, surface, update-project) + two viscous sweeps per "
+                   "stage (gradients and viscous flux; divergence); reading R20 (the paper prints no viscous equations)"}
     try:
         import numpy as np
         from oracle import Oracle

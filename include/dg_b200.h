@@ -212,7 +212,7 @@ int dg_split_get_r(dg_ctx *ctx, double *r_out, int on_device);
  *   dg_set_viscosity : before dg_bind (three more state-sized vectors in the workspace when mu > 0; DG_ESTATE after);
  *                      mu >= 0, prandtl > 0 (DG_EINVAL otherwise); mu = 0 switches the terms off
  *   dg_split_viscous : R += div Fv of the current state (after dg_split_volume + dg_split_surface R = L(Q) + div Fv);
- *                      seven kernels: three gradients, the pointwise viscous flux, three divergences
+ *                      two sweeps: gradients + pointwise viscous flux (one kernel), divergence (one kernel)
  *   dg_rk_step_ns    : nsteps LSERK45 steps of fixed dt of dQ/dt = L(Q) + div Fv
  *                      (per stage: dg_split_volume, dg_split_surface, dg_split_viscous, dg_split_update)
  * All enqueued on the stream without synchronisation. */

@@ -817,28 +817,15 @@ int dg_split_viscous(dg_ctx *c) {
     a.gm1 = c->gamma - 1.0;
     a.mu = c->mu;
     a.kappa = c->mu * c->gamma / (c->prandtl * (c->gamma - 1.0));
-    for (int d = 0; d < 3; ++d) a.S[d] = c->V[d];
-    cudaError_t e = cudaSuccess;
-    for (int d = 0; d < 3 && e == cudaSuccess; ++d) {   // step v1: S_d = d_d Q
-        a.G = c->Q;
-        a.out = c->V[d];
-        a.axis = d;
-        a.accumulate = 0;
-        a.scale = c->g[d];
-        e = c->kt->launch_cwd(a, c->stream);
-        c->launches++;
+    for (int d = 0; d < 3; ++d) {
+        a.S[d] = c->V[d];
+        a.scale3[d] = c->g[d];
     }
-    if (e == cudaSuccess) {                              // step v2: Fv_d over S_d, pointwise
-        e = c->kt->launch_viscflux(a, c->sms, c->stream);
-        c->launches++;
-    }
-    for (int d = 0; d < 3 && e == cudaSuccess; ++d) {   // step v3: R += d_d Fv_d
-        a.G = c->V[d];
-        a.out = c->S;
-        a.axis = d;
-        a.accumulate = 1;
-        a.scale = c->g[d];
-        e = c->kt->launch_cwd(a, c->stream);
+    a.out = c->S;
+    cudaError_t e = c->kt->launch_visc_gradflux(a, c->stream);   // steps v1 + v2: gradients, then Fv_a at the nodes
+    c->launches++;
+    if (e == cudaSuccess) {
+        e = c->kt->launch_visc_div(a, c->stream);                // step v3: R += div Fv
         c->launches++;
     }
     if (e != cudaSuccess) return cuda_fail(c, e, "viscous kernels");

@@ -113,12 +113,10 @@ struct DgSplitArgs {
 // Arguments of the viscous-term kernels (reading R20).
 struct DgViscArgs {
     const double *Q;      // state, internal layout
-    const double *G;      // dg_cwd_kernel: the nodal field to differentiate (Q, or a viscous flux component vector)
-    double *out;          // dg_cwd_kernel: result, internal layout
-    double *S[3];         // dg_viscflux_kernel: in S_a = d_a Q, out Fv_a (in place)
-    int axis, accumulate; // dg_cwd_kernel: axis of the derivative; out += instead of out =
+    double *S[3];         // dg_visc_gradflux_kernel: out, the nodal viscous fluxes Fv_a; dg_visc_div_kernel: in
+    double *out;          // dg_visc_div_kernel: the residual vector it adds div Fv to, internal layout
     int nx, ny, nz, nbx, nby;
-    double scale;         // 2/h_axis
+    double scale3[3];     // 2/h_a per axis
     double gm1, mu, kappa;   // gamma - 1, dynamic viscosity, mu gamma / (Pr (gamma - 1))
 };
 
@@ -155,8 +153,8 @@ struct DgKernelTable {
     cudaError_t (*launch_split_surface)(const DgSplitArgs &a, cudaStream_t s);
     cudaError_t (*launch_layout)(const DgLayoutArgs &a, int sms, cudaStream_t s);
     cudaError_t (*launch_wavespeed)(const DgWaveArgs &a, int sms, cudaStream_t s);
-    cudaError_t (*launch_cwd)(const DgViscArgs &a, cudaStream_t s);
-    cudaError_t (*launch_viscflux)(const DgViscArgs &a, int sms, cudaStream_t s);
+    cudaError_t (*launch_visc_gradflux)(const DgViscArgs &a, cudaStream_t s);
+    cudaError_t (*launch_visc_div)(const DgViscArgs &a, cudaStream_t s);
 };
 
 // Each kernel TU exports its variants: dg_variants_N<N>(&count) -> array of tables, default first.

@@ -1185,16 +1185,18 @@ __global__ void __launch_bounds__(C::NCOMP) dg_split_surface_kernel(const __grid
 // DESIGN.md reading R20 -- constant viscosity, Stokes hypothesis, Fourier conduction with constant Prandtl number,
 // first Bassi-Rebay scheme in the basis of eq (4)-(7), periodic meshes.  Run as kernels of their own on top of the
 // per-kernel mode (not the fused hot path):
-//   dg_cwd_kernel       out (+)= (2/h_a) [ (l_i(+1) G*_+ - l_i(-1) G*_-)/w_i - sum_q Dhat_iq G_q ] along one axis, with the
-//                       CENTRAL interface value G* = (G_L + G_R)/2: the weak form of eq (5) for d_a G.  Applied to Q it
-//                       gives the gradient S_a, applied to the nodal viscous flux Fv_a it gives div Fv.
-//   dg_viscflux_kernel  pointwise: velocity and p/rho gradients from S by the quotient rule, Fv_a over S_a in place
+//   cwd_axis ("central weak derivative")  (2/h_a) [ (l_i(+1) G*_+ - l_i(-1) G*_-)/w_i - sum_q Dhat_iq G_q ] along one axis
+//                       with the CENTRAL interface value G* = (G_L + G_R)/2: the weak form of eq (5) for d_a G.  Applied to
+//                       Q it gives the gradient S_a, applied to the nodal viscous flux Fv_a it gives div Fv.
+//   dg_visc_gradflux_kernel  S_x, S_y, S_z of a layer slot into shared memory, then pointwise (velocity and p/rho gradients
+//                       from S by the quotient rule) the viscous fluxes Fv_a -> three vectors in HBM
+//   dg_visc_div_kernel  R += d_x Fv_x + d_y Fv_y + d_z Fv_z, the slot of R accumulated in shared memory
 // ------------------------------------------------------------------------------------------------
-template <class C>
-__device__ __forceinline__ size_t internal_offset(size_t node, int nx, int ny, int nbx, int nby);
-
+// One line of the central weak derivative along AX: Gs = the block's own layer slot of the field in shared memory, Gg = the
+// whole field in HBM (the two neighbour elements' traces), o = this slot's output (shared or global memory, slot layout).
 template <class C, int AX>
-__device__ __forceinline__ void cwd_axis(const DgViscArgs &a, const double *Gs, int tid, int bxi, int byi, int ez, size_t slot) {
+__device__ __forceinline__ void cwd_axis(const DgViscArgs &a, const double *Gs, const double *Gg, double *o, bool accumulate,
+                                         double scale, int tid, int bxi, int byi, int ez) {
     using A = Axis<C, AX>;
     constexpr int NV = DG_NV, N = C::N, PLANE = C::PLANE;
     const int ext0 = min(C::BX, a.nx - bxi * C::BX), ext1 = min(C::BY, a.ny - byi * C::BY);
@@ -1222,14 +1224,14 @@ __device__ __forceinline__ void cwd_axis(const DgViscArgs &a, const double *Gs, 
     const int up = (ea + 1 == na) ? 0 : ea + 1, dn = (ea == 0) ? na - 1 : ea - 1;
     // identity slots here (no momentum rotation): global_line_trace_of returns slot s = variable var_of_slot(s)
     double Ru[NV], Rd[NV];
-    global_line_trace_of<C, AX>(a.G, a.nbx, a.nby, AX == 0 ? up : ex, AX == 1 ? up : ey, AX == 2 ? up : ez, n1, n2, false, Ru);
-    global_line_trace_of<C, AX>(a.G, a.nbx, a.nby, AX == 0 ? dn : ex, AX == 1 ? dn : ey, AX == 2 ? dn : ez, n1, n2, true, Rd);
+    global_line_trace_of<C, AX>(Gg, a.nbx, a.nby, AX == 0 ? up : ex, AX == 1 ? up : ey, AX == 2 ? up : ez, n1, n2, false, Ru);
+    global_line_trace_of<C, AX>(Gg, a.nbx, a.nby, AX == 0 ? dn : ex, AX == 1 ? dn : ey, AX == 2 ? dn : ez, n1, n2, true, Rd);
 #pragma unroll
     for (int s = 0; s < NV; ++s) {
         Hhi[var_of_slot<C, AX>(s)] = Ru[s];
         Hlo[var_of_slot<C, AX>(s)] = Rd[s];
     }
-    double *o = a.out + slot * C::SLOT + g.base;
+    o += g.base;
 #pragma unroll
     for (int n = 0; n < NV; ++n) {
         const double sp = Tp[n] + Hhi[n], sm = Hlo[n] + Tm[n];   // 2 G*_+, 2 G*_-; c_ref.lq carries the 1/2 and 1/w
@@ -1239,35 +1241,39 @@ __device__ __forceinline__ void cwd_axis(const DgViscArgs &a, const double *Gs, 
 #pragma unroll
             for (int q = 0; q < N; ++q) v = fma(-c_ref.D[q][i], Gl[n][q], v);
             double *dst = o + n * PLANE + i * A::S;
-            *dst = a.accumulate ? fma(a.scale, v, *dst) : a.scale * v;
+            *dst = accumulate ? fma(scale, v, *dst) : scale * v;
         }
     }
 }
 
+// steps v1 + v2 of reading R20 in one sweep: the three gradients S_a = d_a Q of the block's layer into shared memory, then
+// the viscous fluxes Fv_a at the layer's nodes, written to the three vectors a.S[]
 template <class C>
-__global__ void __launch_bounds__(C::NCOMP) dg_cwd_kernel(const __grid_constant__ DgViscArgs a) {
+__global__ void __launch_bounds__(C::NCOMP) dg_visc_gradflux_kernel(const __grid_constant__ DgViscArgs a) {
+    constexpr int NV = DG_NV, N = C::N, PLANE = C::PLANE;
     extern __shared__ __align__(128) double smem[];
+    double *Qs = smem, *Ss = smem + C::BUF;   // Ss[d * BUF ...]
     const int tid = threadIdx.x, bxi = blockIdx.x, byi = blockIdx.y, ez = blockIdx.z;
     const size_t slot = ((size_t)ez * a.nby + byi) * a.nbx + bxi;
-    stage_layer_in<C>(smem, a.G + slot * C::SLOT, tid);
+    stage_layer_in<C>(Qs, a.Q + slot * C::SLOT, tid);
     __syncthreads();
-    if (a.axis == 0) cwd_axis<C, 0>(a, smem, tid, bxi, byi, ez, slot);
-    else if (a.axis == 1) cwd_axis<C, 1>(a, smem, tid, bxi, byi, ez, slot);
-    else cwd_axis<C, 2>(a, smem, tid, bxi, byi, ez, slot);
-}
-
-template <class C>
-__global__ void __launch_bounds__(256) dg_viscflux_kernel(const DgViscArgs a) {
-    constexpr size_t VS = (size_t)C::N * C::HP;   // doubles per variable inside a slot
-    const size_t total = (size_t)a.nx * a.ny * a.nz * (C::N * C::N * C::N);
-    for (size_t node = (size_t)blockIdx.x * blockDim.x + threadIdx.x; node < total; node += (size_t)gridDim.x * blockDim.x) {
-        const size_t io = internal_offset<C>(node, a.nx, a.ny, a.nbx, a.nby);
-        double Q[DG_NV], S[3][DG_NV];
+    cwd_axis<C, 0>(a, Qs, a.Q, Ss, false, a.scale3[0], tid, bxi, byi, ez);
+    cwd_axis<C, 1>(a, Qs, a.Q, Ss + C::BUF, false, a.scale3[1], tid, bxi, byi, ez);
+    cwd_axis<C, 2>(a, Qs, a.Q, Ss + 2 * C::BUF, false, a.scale3[2], tid, bxi, byi, ez);
+    __syncthreads();
+    // pointwise, one thread per z line of the layer
+    const int ext0 = min(C::BX, a.nx - bxi * C::BX), ext1 = min(C::BY, a.ny - byi * C::BY);
+    const Geo g = make_geo<C, 2>(tid);
+    if (!g.ok || !line_inside<C, 2>(g, ext0, ext1)) return;
+#pragma unroll 1
+    for (int i = 0; i < N; ++i) {
+        const int io = g.base + i * C::PP;
+        double Q[NV], S[3][NV];
 #pragma unroll
-        for (int n = 0; n < DG_NV; ++n) {
-            Q[n] = a.Q[io + n * VS];
+        for (int n = 0; n < NV; ++n) {
+            Q[n] = Qs[io + n * PLANE];
 #pragma unroll
-            for (int d = 0; d < 3; ++d) S[d][n] = a.S[d][io + n * VS];
+            for (int d = 0; d < 3; ++d) S[d][n] = Ss[d * C::BUF + io + n * PLANE];
         }
         const double rinv = 1.0 / Q[0];
         const double u[3] = {Q[1] * rinv, Q[2] * rinv, Q[3] * rinv};
@@ -1287,13 +1293,38 @@ __global__ void __launch_bounds__(256) dg_viscflux_kernel(const DgViscArgs a) {
 #pragma unroll
             for (int b = 0; b < 3; ++b) tau[b] = a.mu * (du[d][b] + du[b][d]);
             tau[d] -= a.mu * (2.0 / 3.0) * divu;
-            a.S[d][io] = 0.0;
-            a.S[d][io + VS] = tau[0];
-            a.S[d][io + 2 * VS] = tau[1];
-            a.S[d][io + 3 * VS] = tau[2];
-            a.S[d][io + 4 * VS] = (u[0] * tau[0] + u[1] * tau[1] + u[2] * tau[2]) + a.kappa * dT[d];
+            double *o = a.S[d] + slot * C::SLOT + io;
+            o[0] = 0.0;
+            o[PLANE] = tau[0];
+            o[2 * PLANE] = tau[1];
+            o[3 * PLANE] = tau[2];
+            o[4 * PLANE] = (u[0] * tau[0] + u[1] * tau[1] + u[2] * tau[2]) + a.kappa * dT[d];
         }
     }
+}
+
+// step v3: R += sum_a d_a Fv_a, the residual's layer slot accumulated in shared memory and written once
+template <class C>
+__global__ void __launch_bounds__(C::NCOMP) dg_visc_div_kernel(const __grid_constant__ DgViscArgs a) {
+    extern __shared__ __align__(128) double smem[];
+    double *Gs = smem, *Rs = smem + C::BUF;
+    const int tid = threadIdx.x, bxi = blockIdx.x, byi = blockIdx.y, ez = blockIdx.z;
+    const size_t slot = ((size_t)ez * a.nby + byi) * a.nbx + bxi;
+    stage_layer_in<C>(Rs, a.out + slot * C::SLOT, tid);
+    stage_layer_in<C>(Gs, a.S[0] + slot * C::SLOT, tid);
+    __syncthreads();
+    cwd_axis<C, 0>(a, Gs, a.S[0], Rs, true, a.scale3[0], tid, bxi, byi, ez);
+    __syncthreads();
+    stage_layer_in<C>(Gs, a.S[1] + slot * C::SLOT, tid);
+    __syncthreads();
+    cwd_axis<C, 1>(a, Gs, a.S[1], Rs, true, a.scale3[1], tid, bxi, byi, ez);
+    __syncthreads();
+    stage_layer_in<C>(Gs, a.S[2] + slot * C::SLOT, tid);
+    __syncthreads();
+    cwd_axis<C, 2>(a, Gs, a.S[2], Rs, true, a.scale3[2], tid, bxi, byi, ez);
+    __syncthreads();
+    double *dst = a.out + slot * C::SLOT;
+    for (int idx = tid; idx < C::NPL * C::HP; idx += C::NCOMP) dst[idx] = Rs[idx];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1385,7 +1416,9 @@ cudaError_t prepare(const DgRefOps &ref, int *blocks_per_sm) {
     if (err == cudaSuccess)
         err = cudaFuncSetAttribute(dg_split_surface_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * C::BUF * 8);
     if (err == cudaSuccess)
-        err = cudaFuncSetAttribute(dg_cwd_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::BUF * 8);
+        err = cudaFuncSetAttribute(dg_visc_gradflux_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * C::BUF * 8);
+    if (err == cudaSuccess)
+        err = cudaFuncSetAttribute(dg_visc_div_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * C::BUF * 8);
     if (err != cudaSuccess) return err;
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, dg_stage_kernel<C, DG_MODE_STAGE, false, false>,
                                                          C::THREADS, Smem<C>::BYTES);
@@ -1433,9 +1466,16 @@ cudaError_t launch_split_surface(const DgSplitArgs &a, cudaStream_t s) {
 }
 
 template <class C>
-cudaError_t launch_cwd(const DgViscArgs &a, cudaStream_t s) {
+cudaError_t launch_visc_gradflux(const DgViscArgs &a, cudaStream_t s) {
     const dim3 grid((unsigned)a.nbx, (unsigned)a.nby, (unsigned)a.nz);
-    dg_cwd_kernel<C><<<grid, C::NCOMP, C::BUF * 8, s>>>(a);
+    dg_visc_gradflux_kernel<C><<<grid, C::NCOMP, 4 * C::BUF * 8, s>>>(a);
+    return cudaGetLastError();
+}
+
+template <class C>
+cudaError_t launch_visc_div(const DgViscArgs &a, cudaStream_t s) {
+    const dim3 grid((unsigned)a.nbx, (unsigned)a.nby, (unsigned)a.nz);
+    dg_visc_div_kernel<C><<<grid, C::NCOMP, 2 * C::BUF * 8, s>>>(a);
     return cudaGetLastError();
 }
 
@@ -1460,17 +1500,10 @@ cudaError_t launch_wavespeed(const DgWaveArgs &a, int sms, cudaStream_t s) {
 }
 
 template <class C>
-cudaError_t launch_viscflux(const DgViscArgs &a, int sms, cudaStream_t s) {
-    const size_t total = (size_t)a.nx * a.ny * a.nz * (C::N * C::N * C::N);
-    dg_viscflux_kernel<C><<<flat_grid(total, sms), 256, 0, s>>>(a);
-    return cudaGetLastError();
-}
-
-template <class C>
 constexpr DgKernelTable make_table() {
     return DgKernelTable{C::N,       C::BX,          C::BY,         C::THREADS,      Smem<C>::BYTES,     C::SLOT,
                          C::TXY,     C::TZ,          C::CX, C::CY, C::CZ, C::RELOAD ? 1 : 0, C::MINB, &prepare<C>, &launch_stage<C>,  &launch_traces<C>, &launch_split_volume<C>, &launch_split_surface<C>,
-                         &launch_layout<C>, &launch_wavespeed<C>, &launch_cwd<C>, &launch_viscflux<C>};
+                         &launch_layout<C>, &launch_wavespeed<C>, &launch_visc_gradflux<C>, &launch_visc_div<C>};
 }
 
 // Variants per N (default first): Cfg<N, BX, BY, min blocks per SM, RELOAD, PP, OX, OY>.
