@@ -47,6 +47,8 @@ namespace {
 //   0: t1 fastest, then t2, then the element e along the axis      1: t2, t1, e
 //   2: t1, e, t2                                                   3: t2, e, t1
 //   4: e, t1, t2                                                   5: e, t2, t1
+//   6: e, t1 inside a group of 32 (or, if t1 x e fits, 16) lanes per t2: every t2 plane of lines has a warp or half-warp
+//      of its own (idle lanes at its end), so that no half-warp straddles two planes
 // (t1,t2) = (gy,k) for x lines, (gx,k) for y lines, (gx,gy) for z lines.  PP (even: planes stay 16-byte
 // aligned for the bulk copies) and the orders are picked per column shape so that the 16 lanes of a
 // half-warp hit different 8-byte bank pairs where such a choice exists.
@@ -70,6 +72,9 @@ struct Cfg {
     // SHFL = 1: an axis with two elements whose element index runs fastest in the lane order (ORD 4) hands its interior
     // face over with warp shuffles instead of shared memory and two block barriers (measured: +1.5 % at N = 7, -4 % at N = 5)
     static constexpr bool SHFL = SHFL_ != 0;
+    // the barrier between the y pass and the z-pass update as a SPLIT barrier (mbarrier: a warp arrives when its y pass ends
+    // and waits only before the update): + 1.5 % at N = 8, + 0.6 % at N = 7, - 1 % at N = 5 and N = 2 (A/B measured)
+    static constexpr bool YSPLIT = N_ >= 7;
     static constexpr int L = GX * GY;                              // node lines per axis = threads that work
     static constexpr int NCOMP = (L + 31) / 32 * 32;               // compute threads
     static constexpr int THREADS = NCOMP + 32;                     // + the copy warp
@@ -638,7 +643,7 @@ __device__ __forceinline__ void xy_pass(const BlockInfo *bi, const Geo &g, bool 
 template <class C, int MODE, bool LAM, bool BC>
 __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l, bool act, double *Qs, const double *Qnext,
                                        const double *KR, double *FmS, double *Kg, bool first_layer, bool last_layer,
-                                       double &lam_best) {
+                                       uint64_t *ydone, unsigned yparity, double &lam_best) {
     constexpr int AX = 2;
     using A = Axis<C, AX>;
     constexpr int N = C::N, NV = DG_NV, PLANE = C::PLANE, S = A::S, Ca = A::Ca, L = C::L;
@@ -705,7 +710,10 @@ __device__ __forceinline__ void z_pass(const BlockInfo *bi, const Geo &g, int l,
                 Qn[s] = C::RELOAD ? Q0[var_of_slot<C, AX>(s) * PLANE + q * S] : QL[C::RELOAD ? 0 : s][C::RELOAD ? 0 : q];
         },
         gm1, Fm, Fp, V);
-    bar_sync<C::NCOMP>(1);   // the y pass of every line is done with K (and, RELOAD, with Q)
+    // every warp's y pass is done with K and with Q (YSPLIT: each warp arrived when its y pass ended, so a warp that is
+    // ahead waits for the others' y passes only, not for their z-pass arithmetic above)
+    if (C::YSPLIT) mbar_wait(ydone, yparity);
+    else bar_sync<C::NCOMP>(1);
     if (act) {
         // PD: the updated K (or R) goes straight to HBM from the z lines (coalesced across the lanes, streaming),
         // so that KR is free for the next layer's K as soon as every line has read it
@@ -854,6 +862,10 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
                                 bi->halo[3] + it * bi->hstride[3], Qs,
                             KR, Tms, Fss, fullk, it & 1);
     }
+    if (C::YSPLIT) {
+        __syncwarp();
+        if ((l & 31) == 0) mbar_arrive(fullk + 1);   // this warp's y pass is done (`ydone`, counted in warps)
+    }
     const bool last_layer = it + 1 == bi->nl;
     // Ask L2 for what the NEXT layer reads with a short lead (about a third of a layer): its K slot, which the
     // copy warp can only fetch once this layer's K has left shared memory, and the neighbour columns' traces.
@@ -866,7 +878,7 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
     {
         const Geo gz = make_geo<C, 2>(l);
         z_pass<C, MODE, LAM, BC>(bi, gz, lx, gz.ok && line_inside<C, 2>(gz, ext0, ext1), Qs, Qnext, KR, FmS,
-                             bi->kslot + (long long)it * bi->kstride, it == 0, last_layer, lam_best);
+                             bi->kslot + (long long)it * bi->kstride, it == 0, last_layer, fullk + 1, it & 1, lam_best);
     }
     bar_sync<C::NCOMP>(1);   // the updated Q of the whole layer is in shared memory; every line has read KR
     if (MODE == DG_MODE_STAGE) {
@@ -907,6 +919,7 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
         mbar_init(&fullq[0], 1);
         mbar_init(&fullq[1], 1);
         mbar_init(fullk, 1);
+        mbar_init(fullk + 1, C::NCOMP / 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         const size_t lstride = (size_t)a.nbx * a.nby;
         const size_t slot0 = (size_t)z0 * lstride + (size_t)byi * a.nbx + bxi;
