@@ -75,6 +75,8 @@ struct Cfg {
     // the barrier between the y pass and the z-pass update as a SPLIT barrier (mbarrier: a warp arrives when its y pass ends
     // and waits only before the update): + 1.5 % at N = 8, + 0.6 % at N = 7, - 1 % at N = 5 and N = 2 (A/B measured)
     static constexpr bool YSPLIT = N_ >= 7;
+    // the x boundary traces of the updated Q computed by the copy warp instead of the compute warps
+    static constexpr bool XPE = N_ <= 4;
     static constexpr int L = GX * GY;                              // node lines per axis = threads that work
     static constexpr int NCOMP = (L + 31) / 32 * 32;               // compute threads
     static constexpr int THREADS = NCOMP + 32;                     // + the copy warp
@@ -798,7 +800,7 @@ __device__ __forceinline__ void copy_out(double *gdst, const double *ssrc, int l
     if (lane == 0) bulk_store(gdst, ssrc, C::NPL * C::HP * 8);
 }
 
-template <class C, int MODE>
+template <class C, int MODE, bool BC>
 __device__ __forceinline__ void copy_warp(const DgStageArgs &a, const BlockInfo *bi, int lane, int bxi, int byi, int z0, int nl,
                                           bool readK, double *Qb0, double *Qb1, double *KR, uint64_t *fullq, uint64_t *fullk) {
     const size_t lstride = (size_t)a.nbx * a.nby;                    // slots per layer
@@ -814,6 +816,18 @@ __device__ __forceinline__ void copy_warp(const DgStageArgs &a, const BlockInfo 
         if (MODE == DG_MODE_STAGE) {
             copy_out<C>(a.Q + slot * C::SLOT, Qcur, lane);
             bulk_commit();
+            if (C::XPE) {
+                // PE of the x axis, done by this otherwise idle warp while the bulk store reads the same buffer: the x
+                // traces of the updated Q on the column boundary (the compute warps have gone on to the next layer)
+                const int ext0 = bi->ext0, ext1 = bi->ext1;
+                double *Tslot = bi->txy_out + (long long)it * bi->tstride;
+                for (int r = lane; r < C::NCOMP; r += 32) {
+                    const Geo gx = make_geo<C, 0>(r);
+                    boundary_traces<C, 0>(gx, gx.ok && line_inside<C, 0>(gx, ext0, ext1), ext0, Qcur, Tslot,
+                                          (BC && bi->push[0]) ? bi->push[0] + it * bi->pstride[0] : nullptr,
+                                          (BC && bi->push[1]) ? bi->push[1] + it * bi->pstride[1] : nullptr);
+                }
+            }
             bulk_wait_read();                                        // shared memory has been read out
             __syncwarp();
         }
@@ -887,9 +901,10 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
         double *Tslot = bi->txy_out + toff;
         const Geo gx = make_geo<C, 0>(l), gy = make_geo<C, 1>(l);
         // (push mode runs the BC instances: the periodic, single-context instances carry none of this)
-        boundary_traces<C, 0>(gx, gx.ok && line_inside<C, 0>(gx, ext0, ext1), ext0, Qs, Tslot,
-                              (BC && bi->push[0]) ? bi->push[0] + it * bi->pstride[0] : nullptr,
-                              (BC && bi->push[1]) ? bi->push[1] + it * bi->pstride[1] : nullptr);
+        if (!C::XPE)
+            boundary_traces<C, 0>(gx, gx.ok && line_inside<C, 0>(gx, ext0, ext1), ext0, Qs, Tslot,
+                                  (BC && bi->push[0]) ? bi->push[0] + it * bi->pstride[0] : nullptr,
+                                  (BC && bi->push[1]) ? bi->push[1] + it * bi->pstride[1] : nullptr);
         boundary_traces<C, 1>(gy, gy.ok && line_inside<C, 1>(gy, ext0, ext1), ext1, Qs, Tslot,
                               (BC && bi->push[2]) ? bi->push[2] + it * bi->pstride[2] : nullptr,
                               (BC && bi->push[3]) ? bi->push[3] + it * bi->pstride[3] : nullptr);
@@ -990,7 +1005,7 @@ __global__ void __launch_bounds__(C::THREADS, C::MINB) dg_stage_kernel(const __g
     }
     __syncthreads();
     if (tid >= C::NCOMP) {
-        copy_warp<C, MODE>(a, reinterpret_cast<const BlockInfo *>(smem + SM::INFO), tid - C::NCOMP, bxi, byi, z0, nl, readK, smem + SM::QB0, smem + SM::QB1, smem + SM::KR, fullq,
+        copy_warp<C, MODE, BC>(a, reinterpret_cast<const BlockInfo *>(smem + SM::INFO), tid - C::NCOMP, bxi, byi, z0, nl, readK, smem + SM::QB0, smem + SM::QB1, smem + SM::KR, fullq,
                            fullk);
         return;
     }
