@@ -826,6 +826,10 @@ __device__ __forceinline__ void copy_warp(const DgStageArgs &a, const BlockInfo 
                     boundary_traces<C, 0>(gx, gx.ok && line_inside<C, 0>(gx, ext0, ext1), ext0, Qcur, Tslot,
                                           (BC && bi->push[0]) ? bi->push[0] + it * bi->pstride[0] : nullptr,
                                           (BC && bi->push[1]) ? bi->push[1] + it * bi->pstride[1] : nullptr);
+                    const Geo gy = make_geo<C, 1>(r);
+                    boundary_traces<C, 1>(gy, gy.ok && line_inside<C, 1>(gy, ext0, ext1), ext1, Qcur, Tslot,
+                                          (BC && bi->push[2]) ? bi->push[2] + it * bi->pstride[2] : nullptr,
+                                          (BC && bi->push[3]) ? bi->push[3] + it * bi->pstride[3] : nullptr);
                 }
             }
             bulk_wait_read();                                        // shared memory has been read out
@@ -905,9 +909,10 @@ __device__ __noinline__ double layer_body(int it, double lam_best) {
             boundary_traces<C, 0>(gx, gx.ok && line_inside<C, 0>(gx, ext0, ext1), ext0, Qs, Tslot,
                                   (BC && bi->push[0]) ? bi->push[0] + it * bi->pstride[0] : nullptr,
                                   (BC && bi->push[1]) ? bi->push[1] + it * bi->pstride[1] : nullptr);
-        boundary_traces<C, 1>(gy, gy.ok && line_inside<C, 1>(gy, ext0, ext1), ext1, Qs, Tslot,
-                              (BC && bi->push[2]) ? bi->push[2] + it * bi->pstride[2] : nullptr,
-                              (BC && bi->push[3]) ? bi->push[3] + it * bi->pstride[3] : nullptr);
+        if (!C::XPE)
+            boundary_traces<C, 1>(gy, gy.ok && line_inside<C, 1>(gy, ext0, ext1), ext1, Qs, Tslot,
+                                  (BC && bi->push[2]) ? bi->push[2] + it * bi->pstride[2] : nullptr,
+                                  (BC && bi->push[3]) ? bi->push[3] + it * bi->pstride[3] : nullptr);
     }
     fence_proxy_async();
     bar_arrive<C::THREADS>(2);   // hand the layer to the copy warp
