@@ -75,8 +75,9 @@ struct Cfg {
     // the barrier between the y pass and the z-pass update as a SPLIT barrier (mbarrier: a warp arrives when its y pass ends
     // and waits only before the update): + 1.5 % at N = 8, + 0.6 % at N = 7, - 1 % at N = 5 and N = 2 (A/B measured)
     static constexpr bool YSPLIT = N_ >= 7;
-    // the x boundary traces of the updated Q computed by the copy warp instead of the compute warps
-    static constexpr bool XPE = N_ <= 4;
+    // the x and y boundary traces of the updated Q (phase PE) computed by the copy warp instead of the compute warps
+    // (A/B measured: p = 1 +2.6 %, p = 2 +0.8 %, p = 3 +1.8 %, p = 7 +3.8 %, cfg5 +3 %; none at N = 5, 6, -1 % at N = 7)
+    static constexpr bool XPE = N_ <= 4 || N_ == 8;
     static constexpr int L = GX * GY;                              // node lines per axis = threads that work
     static constexpr int NCOMP = (L + 31) / 32 * 32;               // compute threads
     static constexpr int THREADS = NCOMP + 32;                     // + the copy warp
