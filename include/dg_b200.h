@@ -125,6 +125,35 @@ int dg_residual(dg_ctx *ctx, double *r_out, int on_device);
  * negative pressure or density.  Synchronises the stream. */
 int dg_max_wavespeed(dg_ctx *ctx, double *lam_host);
 
+/* The same maximum (reading R10) for callers that CANNOT give the library device memory -- the one call of
+ * this header that needs no context, no workspace and no dg_bind, and that never allocates (no cudaMalloc, cudaFree
+ * or allocating library routine, on any call).  It is meant for code that holds nothing but a pointer to the
+ * solution and a slot for the answer: a time-step or blow-up monitor hooked into another application's time loop;
+ * a plug-in under an application that hands out all device memory at start-up and forbids allocation afterwards
+ * (cudaMalloc synchronises the whole device and can fail in the middle of a run on a full card); code that has no
+ * way of reporting an out-of-memory failure upwards.
+ *   q_dev        DEVICE pointer, canonical layout [node][5] (see above), n_nodes = (p+1)^3 nx ny nz nodes; read only
+ *   gamma        ratio of specific heats, > 1
+ *   lam_out_dev  DEVICE pointer to one double on the same device: receives the maximum, NaN under the rule above,
+ *                in stream order (nothing is copied to the host, nothing synchronises)
+ *   cuda_stream  cudaStream_t as void* (NULL = legacy default stream); the caller's current device must be the one
+ *                that holds q_dev and lam_out_dev
+ *   err, err_len optional host buffer for the error text (there is no context for dg_last_error); may be NULL / 0
+ * The scratch memory of the reduction (one partial maximum per thread block and a block counter) is a fixed array
+ * inside the library, 256.25 KiB, which every GPU that loads the library holds until the process exits.  Its size sets
+ * the limit: n_nodes <= DG_NOALLOC_MAX_NODES (2^29; config 5 has 452,984,832), beyond that the call returns DG_ENOMEM
+ * with a text that says so and touches no GPU.  Other returns: DG_OK, DG_EINVAL (null pointer, gamma <= 1,
+ * n_nodes = 0), DG_ECUDA.
+ * The FIRST call on each device looks up where that device keeps the array (cudaGetSymbolAddress; the address is
+ * cached per device): make that first call during set-up, with the device current, and before any stream capture.
+ * ALL calls on one device share the one array, which keeps what the last call left (the call clears the counter it
+ * needs at zero itself): calls that may overlap on the GPU -- different streams, different host threads, different
+ * contexts of this library -- race on it and must be ordered by the caller; calls on one stream are safe.
+ * Gives the same double as dg_set_state + dg_max_wavespeed (tests/test_zz_no_alloc.py). */
+#define DG_NOALLOC_MAX_NODES 536870912ull
+int dg_max_wavespeed_noalloc(const double *q_dev, size_t n_nodes, double gamma, double *lam_out_dev, void *cuda_stream,
+                             char *err, size_t err_len);
+
 /* Advance nsteps >= 0 LSERK45 steps of fixed dt:
  * K = 0; for s = 1..5: K = A_s K + dt L(Q); Q = Q + B_s K.  One fused kernel per stage,
  * enqueued on the stream, no host synchronisation. */

@@ -27,6 +27,8 @@ SYMBOLS = {
     "dg_set_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
     "dg_residual": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
     "dg_max_wavespeed": (ctypes.c_int, [ctypes.c_void_p, _DP]),
+    "dg_max_wavespeed_noalloc": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_size_t, ctypes.c_double, ctypes.c_void_p,
+                                                ctypes.c_void_p, ctypes.c_char_p, ctypes.c_size_t]),
     "dg_rk_step": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int]),
     "dg_rk_stage": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int]),
     "dg_set_spacing": (ctypes.c_int, [ctypes.c_void_p, _DP]),
@@ -93,6 +95,36 @@ def fp64_peak(device="cuda:0", iters=2048, repeats=5):
             torch.cuda.synchronize(dev)
             best = max(best, count.value / (e0.elapsed_time(e1) * 1e-3))
     return best
+
+
+NOALLOC_MAX_NODES = 1 << 29      # DG_NOALLOC_MAX_NODES of include/dg_b200.h
+
+
+def max_wavespeed_noalloc(q, gamma, lam_out, stream=None):
+    """dg_max_wavespeed_noalloc: the max wavespeed of a canonical-layout state for callers that cannot give the
+    library any device memory (no DG object, no workspace; the library's scratch is a fixed array inside it, so
+    at most NOALLOC_MAX_NODES nodes).  `q` is a contiguous float64 CUDA tensor of 5 * n_nodes elements, `lam_out` a
+    float64 CUDA tensor of one element on the same device, BOTH provided by the caller -- this function creates no
+    tensor either.  The result lands in `lam_out` in the order of `stream` (default: torch's current stream of that
+    device); nothing synchronises.  All calls on a device share the library's one scratch array: do not let two of
+    them overlap on the GPU.  Returns `lam_out`."""
+    import torch
+    lib = load_library()
+    if not (isinstance(q, torch.Tensor) and q.is_cuda and q.dtype == torch.float64 and q.is_contiguous()):
+        raise ValueError("q must be a contiguous float64 CUDA tensor")
+    if not (isinstance(lam_out, torch.Tensor) and lam_out.device == q.device and lam_out.dtype == torch.float64
+            and lam_out.numel() == 1):
+        raise ValueError("lam_out must be a one-element float64 tensor on q's device")
+    if q.numel() % 5:
+        raise ValueError("q must hold 5 values per node")
+    err = ctypes.create_string_buffer(512)
+    with torch.cuda.device(q.device):
+        s = stream if stream is not None else torch.cuda.current_stream(q.device)
+        rc = lib.dg_max_wavespeed_noalloc(q.data_ptr(), q.numel() // 5, float(gamma), lam_out.data_ptr(), s.cuda_stream,
+                                          err, len(err))
+    if rc != 0:
+        raise DGError(rc, err.value.decode())
+    return lam_out
 
 
 class DGError(RuntimeError):

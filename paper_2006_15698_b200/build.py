@@ -1,7 +1,7 @@
 """Build libdg_b200.so (the C-ABI library of include/dg_b200.h) in-tree with nvcc for sm_100a.
 
 One translation unit per N = p+1 (csrc/dg_kernels.cu with -DDG_N=<N>) plus the boundary
-(csrc/dg_api.cu), compiled in parallel, linked into paper_2006_15698_b200/libdg_b200.so.
+(csrc/dg_api.cu) and the allocation-free wavespeed call (csrc/dg_noalloc.cu), compiled in parallel, linked into paper_2006_15698_b200/libdg_b200.so.
 ptxas resource usage (-Xptxas -v) of every TU is kept in build/ptxas_N<N>.log.
 
 Usage:  python -m paper_2006_15698_b200.build [--force]
@@ -23,10 +23,12 @@ NVCC_FLAGS = [
 ]
 
 
-def _sources():
-    return [os.path.join(CSRC, f) for f in ("dg_kernels.cu", "dg_api.cu", "dg_internal.h")] + [
-        os.path.join(os.path.dirname(HERE), "include", "dg_b200.h"),
-        os.path.join(os.path.dirname(HERE), "include", "dg_b200_test.h")]
+INCLUDE = os.path.join(os.path.dirname(HERE), "include")
+# what each translation unit includes (a change to the public header does not touch the seven kernel objects)
+DEPS_KERNELS = [os.path.join(CSRC, f) for f in ("dg_kernels.cu", "dg_internal.h")]
+DEPS_API = [os.path.join(CSRC, f) for f in ("dg_api.cu", "dg_internal.h")] + [
+    os.path.join(INCLUDE, f) for f in ("dg_b200.h", "dg_b200_test.h")]
+DEPS_NOALLOC = [os.path.join(CSRC, "dg_noalloc.cu"), os.path.join(INCLUDE, "dg_b200.h")]
 
 
 def _stale(target, deps):
@@ -49,19 +51,24 @@ def _compile(args):
 def build(force=False, verbose=False):
     """Compile what is stale; return the path of the shared library."""
     os.makedirs(BUILD, exist_ok=True)
-    deps = _sources()
     jobs, objs = [], []
     for n in NS:
         obj = os.path.join(BUILD, f"dg_kernels_N{n}.o")
         objs.append(obj)
-        if force or _stale(obj, deps):
+        if force or _stale(obj, DEPS_KERNELS):
             cmd = ["nvcc"] + NVCC_FLAGS + [f"-DDG_N={n}", "-c", os.path.join(CSRC, "dg_kernels.cu"), "-o", obj]
             jobs.append((obj, cmd, os.path.join(BUILD, f"ptxas_N{n}.log")))
     obj = os.path.join(BUILD, "dg_api.o")
     objs.append(obj)
-    if force or _stale(obj, deps):
+    if force or _stale(obj, DEPS_API):
         cmd = ["nvcc"] + NVCC_FLAGS + ["-c", os.path.join(CSRC, "dg_api.cu"), "-o", obj]
         jobs.append((obj, cmd, os.path.join(BUILD, "ptxas_api.log")))
+    # dg_max_wavespeed_noalloc: its own translation unit (holds the static __device__ scratch array)
+    obj = os.path.join(BUILD, "dg_noalloc.o")
+    objs.append(obj)
+    if force or _stale(obj, DEPS_NOALLOC):
+        cmd = ["nvcc"] + NVCC_FLAGS + ["-c", os.path.join(CSRC, "dg_noalloc.cu"), "-o", obj]
+        jobs.append((obj, cmd, os.path.join(BUILD, "ptxas_noalloc.log")))
     if jobs:
         if verbose:
             print(f"compiling {len(jobs)} translation units for sm_100a ...", flush=True)
