@@ -168,6 +168,13 @@ int dg_rk_step(dg_ctx *ctx, double dt, int nsteps);
  * one (host pointers, either may be NULL; DG_ESTATE if the state went non-physical on the way).  cfl > 0. */
 int dg_rk_step_cfl(dg_ctx *ctx, double cfl, int nsteps, double *t_advanced, double *dt_last);
 
+/* The time step of the same rule (reading R10) as a plain host computation, for callers that reduce the wavespeed
+ * themselves -- a block decomposition takes the maximum of dg_max_wavespeed over all contexts (below):
+ *     *dt = (cfl * min(hx,hy,hz) / (2p+1)) / lam_max,
+ * the operations dg_rk_step_cfl performs on the device, in the same order.  Touches no GPU and does not change the
+ * context.  cfl, lam_max positive and finite and dt non-null, else DG_EINVAL (no text: the context is const). */
+int dg_cfl_dt(const dg_ctx *ctx, double cfl, double lam_max, double *dt);
+
 /* Block decomposition over several contexts / GPUs (one exchange of face
  * data per Runge-Kutta stage).  The library does no communication itself: it exports and imports face traces, the
  * caller moves them (NCCL / peer copies between GPUs, plain copies between contexts of one GPU).  All contexts of a
@@ -184,8 +191,9 @@ int dg_rk_step_cfl(dg_ctx *ctx, double cfl, int nsteps, double *t_advanced, doub
  *   dg_rk_stage(ctx, dt, s)  ONE stage s = 0..4 of the LSERK45 step (dg_rk_step = stages 0..4 in a row), so that the
  *                            caller can exchange the faces between stages: export -> move -> next stage.
  * The interface flux of a shared face is evaluated by both contexts, bit-identically, so a decomposed run reproduces
- * the single-context run bit for bit (tests/test_gpu_halo.py).  dg_rk_step_cfl is refused with halo faces (the CFL
- * wavespeed is a maximum over all contexts: reduce dg_max_wavespeed across them and use dg_rk_stage). */
+ * the single-context run bit for bit (tests/test_gpu_halo.py).  With halo faces dg_rk_step is refused (DG_EUNSUPPORTED:
+ * five stages back to back would read stale neighbour traces) and so is dg_rk_step_cfl (the CFL wavespeed is a maximum
+ * over all contexts: reduce dg_max_wavespeed across them, form dt with dg_cfl_dt and use dg_rk_stage). */
 /* Before dg_bind: element sizes h = {hx, hy, hz} given directly instead of extent / n (a block of a decomposed mesh
  * must use the SAME doubles as its neighbours; extent * n_local / n_global divided by n_local again can differ in
  * the last bit).  DG_ESTATE after dg_bind. */
@@ -204,7 +212,10 @@ int dg_rk_stage(dg_ctx *ctx, double dt, int stage);
  *                            peer[1 - parity], which is what the neighbour reads in the next stage.  The pointers may be
  *                            peer-mapped memory of another GPU (CUDA peer access / IPC): the stores then travel over
  *                            NVLink while the rest of the stage computes -- the paper's computation-communication
- *                            overlap, tile by tile.
+ *                            overlap, tile by tile.  The call looks up the device that holds the buffers
+ *                            and, if it is not the current one, enables peer access to it (DG_EUNSUPPORTED if the two
+ *                            GPUs have none).  UNVERIFIED across GPUs: this code has only ever run with both
+ *                            contexts on ONE GPU (the tests' CUDA-IPC case included).
  * The caller provides the ordering only: every context's stage s must have completed before any neighbour's stage s + 1
  * starts (same stream, events, or a barrier between processes), and both sides must have run the same number of stages
  * since dg_set_state.  After dg_set_state the initial traces go to the neighbour's buffer 0 with dg_halo_export.

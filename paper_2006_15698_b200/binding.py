@@ -37,6 +37,7 @@ SYMBOLS = {
     "dg_set_halo": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]),
     "dg_set_halo_pair": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]),
     "dg_set_halo_push": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]),
+    "dg_cfl_dt": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_double, _DP]),
     "dg_rk_step_cfl": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_double, ctypes.c_int, _DP, _DP]),
     "dg_get_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
     "dg_split_volume": (ctypes.c_int, [ctypes.c_void_p]),
@@ -304,6 +305,14 @@ class DG:
         with self._torch.cuda.device(self.device):
             self._check(self.lib.dg_rk_step_cfl(self._h, float(cfl), int(nsteps), ctypes.byref(t), ctypes.byref(dt)))
         return t.value, dt.value
+
+    def cfl_dt(self, cfl, lam_max):
+        """dg_cfl_dt: cfl * min(h) / ((2p+1) * lam_max), formed by the library (host arithmetic, no GPU work)."""
+        dt = ctypes.c_double(0.0)
+        rc = self.lib.dg_cfl_dt(self._h, float(cfl), float(lam_max), ctypes.byref(dt))
+        if rc != 0:
+            raise DGError(rc, f"dg_cfl_dt(cfl={cfl}, lam_max={lam_max}): both must be positive and finite")
+        return dt.value
 
     # -- block decomposition over several contexts / GPUs: face export / import, stage by stage ----------
     def rk_stage(self, dt, stage):

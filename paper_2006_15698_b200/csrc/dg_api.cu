@@ -414,6 +414,29 @@ DgSplitArgs split_args(const dg_ctx *c) {
     return a;
 }
 
+// Push mode: make sure kernels of the current device can store to `ptr`.  Memory of the current device, host-registered
+// memory and pointers the runtime does not know (no GPU in this process: the CPU-side tests) pass unchanged.
+int enable_peer_access_to(dg_ctx *c, const void *ptr) {
+    cudaPointerAttributes attr;
+    int cur = -1;
+    if (cudaPointerGetAttributes(&attr, ptr) != cudaSuccess || cudaGetDevice(&cur) != cudaSuccess) {
+        (void)cudaGetLastError();   // not fatal: nothing known about the pointer
+        return DG_OK;
+    }
+    if (attr.type != cudaMemoryTypeDevice || attr.device == cur) return DG_OK;
+    int can = 0;
+    cudaError_t e = cudaDeviceCanAccessPeer(&can, cur, attr.device);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaDeviceCanAccessPeer");
+    if (!can) return fail(c, DG_EUNSUPPORTED, "device %d cannot access the memory of device %d: push mode needs peer access, use dg_halo_export + a copy", cur, attr.device);
+    e = cudaDeviceEnablePeerAccess(attr.device, 0);
+    if (e == cudaErrorPeerAccessAlreadyEnabled) {
+        (void)cudaGetLastError();
+        e = cudaSuccess;
+    }
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaDeviceEnablePeerAccess");
+    return DG_OK;
+}
+
 // the max wavespeed of the current state is in scal[lcur] (enqueued; reduction kernel only if no stage left it there)
 int ensure_lam(dg_ctx *c) {
     if (c->lam_valid) return DG_OK;
@@ -636,6 +659,11 @@ int dg_rk_step(dg_ctx *c, double dt, int nsteps) {
     if (!c) return DG_EINVAL;
     if (nsteps < 0 || !std::isfinite(dt)) return fail(c, DG_EINVAL, "nsteps < 0 or dt not finite");
     if (!c->bound || !c->has_state) return fail(c, DG_ESTATE, "dg_rk_step needs dg_bind and dg_set_state first");
+    // five stages back to back would read the neighbours' traces of the FIRST stage in all five (and, in push mode, store
+    // into their buffers out of step): with halo faces the caller exchanges between stages
+    for (int f = 0; f < 6; ++f)
+        if (c->bc[f] == DG_BC_HALO)
+            return fail(c, DG_EUNSUPPORTED, "face %d is a halo face: the faces must be exchanged after every stage, use dg_rk_stage", f);
     for (int step = 0; step < nsteps; ++step) {
         const int rc = enqueue_step(c, dt, 0.0);
         if (rc != DG_OK) return rc;
@@ -683,6 +711,14 @@ int dg_set_halo_pair(dg_ctx *c, int face, const double *halo0_dev, const double 
 int dg_set_halo_push(dg_ctx *c, int face, double *peer0_dev, double *peer1_dev) {
     if (!c || face < 0 || face > 5) return c ? fail(c, DG_EINVAL, "face outside 0..5") : DG_EINVAL;
     if ((peer0_dev == nullptr) != (peer1_dev == nullptr)) return fail(c, DG_EINVAL, "both buffers or none");
+    // The stage kernel of THIS context's device stores into these buffers.  When they live on another GPU (peer
+    // allocation or CUDA IPC mapping) the current device needs peer access to that GPU; opening an IPC handle enables
+    // it only for the device that was current at the time, which need not be this one.
+    double *const peers[2] = {peer0_dev, peer1_dev};
+    for (int i = 0; i < 2 && peers[i]; ++i) {
+        int rc = enable_peer_access_to(c, peers[i]);
+        if (rc != DG_OK) return rc;
+    }
     c->push[face][0] = peer0_dev;
     c->push[face][1] = peer1_dev;
     return DG_OK;
@@ -755,6 +791,16 @@ int dg_rk_step_cfl(dg_ctx *c, double cfl, int nsteps, double *t_advanced, double
     if (t_advanced) *t_advanced = out[0];
     if (dt_last) *dt_last = out[1];
     if (!std::isfinite(out[0])) return fail(c, DG_ESTATE, "the state became non-physical during the steps (time advanced %g)", out[0]);
+    return DG_OK;
+}
+
+int dg_cfl_dt(const dg_ctx *c, double cfl, double lam_max, double *dt) {
+    if (!c || !dt) return DG_EINVAL;
+    if (!(cfl > 0.0) || !std::isfinite(cfl) || !(lam_max > 0.0) || !std::isfinite(lam_max)) return DG_EINVAL;
+    double hmin = c->h[0];
+    if (c->h[1] < hmin) hmin = c->h[1];
+    if (c->h[2] < hmin) hmin = c->h[2];
+    *dt = (cfl * hmin / (2.0 * c->p + 1.0)) / lam_max;   // the same operations, in the same order, as dg_rk_step_cfl's device-side dt
     return DG_OK;
 }
 

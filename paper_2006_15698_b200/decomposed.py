@@ -204,7 +204,8 @@ class DistributedDG:
     def _wire_push_over_ipc(self, dist):
         """One process per rank: every rank publishes CUDA IPC handles of its halo-buffer pairs (torch's own tensor
         sharing), opens its neighbours' and hands them to the library as push targets.  The mapped buffers may live on
-        another GPU: the stage kernel's stores then go over NVLink (peer access is enabled when the handle is opened)."""
+        another GPU: the stage kernel's stores then go over NVLink (dg_set_halo_push enables peer access from this rank's
+        device to the buffers' device; never run on more than one GPU so far)."""
         from torch.multiprocessing.reductions import reduce_tensor
         mine = {f: (reduce_tensor(b0), reduce_tensor(b1)) for f, (b0, b1) in self.pairs.items()}
         everyone = [None] * dist.get_world_size()
@@ -262,11 +263,12 @@ class DistributedDG:
                     self.exchange()
         return self
 
-    def rk_step_cfl(self, cfl, nsteps=1, h_min=None):
-        """dt = cfl h_min / ((2p+1) lam) with lam the maximum wavespeed over ALL ranks, before every step."""
+    def rk_step_cfl(self, cfl, nsteps=1):
+        """nsteps steps, each with the CFL time step of reading R10 from the maximum wavespeed over ALL ranks; the
+        library forms dt (dg_cfl_dt; every block was given the global element sizes).  Returns the time advanced."""
         t = 0.0
         for _ in range(int(nsteps)):
-            dt = cfl * h_min / ((2 * self.p + 1) * self.max_wavespeed())
+            dt = self.dg.cfl_dt(cfl, self.max_wavespeed())
             self.rk_step(dt, 1)
             t += dt
         return t
@@ -317,6 +319,16 @@ def rk_step_in_process(ranks, dt, nsteps=1):
             for r in ranks:
                 r.dg.rk_stage(dt, stage)
             exchange_in_process(ranks)
+
+
+def rk_step_cfl_in_process(ranks, cfl, nsteps=1):
+    """The CFL-stepped run of all ranks: the wavespeed is the maximum over the ranks, the library forms dt (dg_cfl_dt)."""
+    t = 0.0
+    for _ in range(int(nsteps)):
+        dt = ranks[0].dg.cfl_dt(cfl, max(r.dg.max_wavespeed() for r in ranks))
+        rk_step_in_process(ranks, dt, 1)
+        t += dt
+    return t
 
 
 def gather_in_process(ranks, what="state"):

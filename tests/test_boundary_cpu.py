@@ -95,6 +95,22 @@ def test_calls_before_bind_are_refused_and_brick_knob():
     lib.dg_destroy(h)
 
 
+def test_cfl_dt_is_the_rule_of_reading_r10():
+    """dg_cfl_dt: cfl min(h) / ((2p+1) lam), host arithmetic of the library (no GPU)."""
+    lib, h, rc = _create(8, 4, 5, 3, extent=(1.0, 0.9, 0.8))        # h = 0.125, 0.225, 0.16
+    dt = ctypes.c_double(-1.0)
+    assert lib.dg_cfl_dt(h, 0.1, 2.7, ctypes.byref(dt)) == 0
+    want = 0.1 * 0.125 / (7 * 2.7)
+    assert abs(dt.value - want) <= 4 * np.spacing(want)
+    for cfl, lam in ((0.0, 2.7), (0.1, 0.0), (0.1, float("nan")), (float("inf"), 1.0), (-0.1, 1.0)):
+        assert lib.dg_cfl_dt(h, cfl, lam, ctypes.byref(dt)) == 1
+    assert lib.dg_cfl_dt(h, 0.1, 2.7, None) == 1 and lib.dg_cfl_dt(None, 0.1, 2.7, ctypes.byref(dt)) == 1
+    hs = (ctypes.c_double * 3)(0.3, 0.05, 0.2)                       # dg_set_spacing overrides extent / n
+    assert lib.dg_set_spacing(h, hs) == 0
+    assert lib.dg_cfl_dt(h, 0.5, 1.0, ctypes.byref(dt)) == 0 and abs(dt.value - 0.5 * 0.05 / 7) <= 1e-17
+    lib.dg_destroy(h)
+
+
 def test_set_boundary_validates_its_arguments():
     lib, h, rc = _create(4, 4, 4, 2)
     IA, DA = ctypes.c_int * 6, ctypes.c_double * 5

@@ -118,9 +118,46 @@ def test_decomposition_with_walls_and_far_field():
 def test_halo_faces_need_their_buffers_and_refuse_the_device_side_cfl_step():
     from paper_2006_15698_b200 import DGError
     dg = DG(4, 4, 4, 1).set_boundary((D.HALO, D.HALO, 0, 0, 0, 0))
-    dg.set_state(rough_field(4, 4, 4, 1, (1.0,) * 3))
+    q = rough_field(4, 4, 4, 1, (1.0,) * 3)
+    dg.set_state(q)
     with pytest.raises(DGError):
-        dg.rk_step(1e-3, 1)                                    # dg_set_halo not called
+        dg.rk_stage(1e-3, 0)                                   # dg_set_halo not called
     with pytest.raises(DGError):
         dg.rk_step_cfl(0.1, 1)                                 # the wavespeed would be this context's only
+    # with the buffers in place a single stage runs, but five stages back to back (dg_rk_step) are refused: stages
+    # 2..5 would read the neighbours' traces of the first stage.  The state is left alone by the refused call.
+    for f in (0, 1):
+        dg.set_halo(f, torch.zeros(dg.halo_len(f), dtype=torch.float64, device="cuda"))
+    with pytest.raises(DGError) as e:
+        dg.rk_step(1e-3, 1)
+    assert e.value.code == 2 and "dg_rk_stage" in str(e.value)  # DG_EUNSUPPORTED
+    assert np.array_equal(dg.get_state(), q)
     dg.close()
+
+
+@pytest.mark.parametrize("procs", [(1, 1, 1), (2, 1, 2)])
+def test_decomposed_cfl_steps_use_the_global_wavespeed_and_the_librarys_dt(procs):
+    """dg_cfl_dt + the maximum of dg_max_wavespeed over the blocks against dg_rk_step_cfl of the single context (whose
+    dt comes from the wavespeed fused into the last stage: the kernels' own reciprocal / square root, a few ulp from
+    the reduction kernel's, so the two runs agree to rounding, not bit for bit) and against the oracle-driven loop."""
+    n, p, ext = (6, 5, 4), 3, (1.0, 0.9, 0.8)
+    q = rough_field(*n, p, ext, seed=4)
+    ranks = D.make_in_process(n, p, G, ext, procs)
+    single = DG(*n, p, G, ext, variant=ranks[0].dg.kernel_info()["variant"])
+    D.set_state_in_process(ranks, q)
+    if len(ranks) == 1:
+        t_dec = ranks[0].rk_step_cfl(0.1, 3)                   # DistributedDG's own method (one rank: no exchange)
+    else:
+        t_dec = D.rk_step_cfl_in_process(ranks, 0.1, 3)
+    t_one, _ = single.set_state(q).rk_step_cfl(0.1, 3)
+    q_dec = D.gather_in_process(ranks)
+    assert abs(t_dec - t_one) <= 1e-13 * t_one
+    assert relerr(q_dec, single.get_state()) < 1e-13
+    qo, to = q, 0.0
+    for _ in range(3):
+        dt = I.cfl_dt(ORC.max_wavespeed(qo, p, G), p, ext, n, 0.1)
+        qo, to = ORC.rk_step(qo, p, G, ext, dt, 1), to + dt
+    assert abs(t_dec - to) <= 1e-13 * to and relerr(q_dec, qo) < 1e-12
+    for r in ranks:
+        r.close()
+    single.close()
