@@ -342,10 +342,8 @@ def per_kernel_breakdown(workload, steps, device):
             "split_total_seconds": total, "split_dof_updates_per_s": dof * evals / total,
             "fused_seconds": fused, "fused_dof_updates_per_s": dof * evals / fused, "launches": launches, "finite": finite,
             "note": "update_project = K, Q update over the whole vectors + the face-trace kernel; the surface kernel evaluates "
-                    "every face from both sides; flop rates use the algorithmic counts of PAPER.md:135 / SURVEY.md 8(d)",
-            "paper_table2_per_v100": {"volume_dof_per_s": 6.35e9, "surface_dof_per_s": 5.23e9,
-                                      "update_project_dof_per_s": 1.87e9,
-                                      "source": "derived from PAPER.md:264-269 (3,072 V100, 100 steps); another machine"}}
+                    "every face from both sides; flop rates use the algorithmic counts of PAPER.md:135 / SURVEY.md 8(d); "
+                    "the paper's own per-V100 rates (Table II) are in BASELINE.md"}
 
 
 VISC_BYTES_PER_DOF = 360.0   # viscous path, per evaluation: gradient + flux sweep (read Q 40, write Fv_x,y,z 120), divergence
@@ -723,9 +721,22 @@ def run_ours(args, rank, world, local_rank):
         one = oracle_sample(args.workload, fixed_steps=1, build="fp64", nodes=2.0e5)
         line["cpu_baseline"]["single_thread"] = {"value": one["value"], "sample": one["sample"]}
         line["cpu_baseline"]["per_p"] = oracle_per_p()
-    print(json.dumps(line), flush=True)
+    # a shorter line: nested floats to 6 significant digits (top-level scalars stay exact), and `roofline` moved to the
+    # end, where a truncated tail of the line still shows it
+    line["roofline"] = line.pop("roofline")
+    print(json.dumps({k: _compact(v) if isinstance(v, (dict, list)) else v for k, v in line.items()}), flush=True)
     if dist is not None:
         dist.destroy_process_group()
+
+
+def _compact(x):
+    if isinstance(x, float):
+        return float(f"{x:.6g}") if x == x and abs(x) != float("inf") else x
+    if isinstance(x, dict):
+        return {k: _compact(v) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_compact(v) for v in x]
+    return x
 
 
 def main():

@@ -234,7 +234,9 @@ int dg_set_halo_push(dg_ctx *ctx, int face, double *peer0_dev, double *peer1_dev
  * After volume + surface R = dQ/dt = L(Q) as dg_residual returns it.  R lives in the library's staging vector: do
  * not interleave host-pointer dg_set_state / dg_get_state / dg_residual calls between volume and update.  All three
  * are enqueued on the stream without synchronisation.  dg_split_get_r copies R out in canonical layout (host or
- * device pointer; the host variant overwrites the Runge-Kutta register, which is dead between steps). */
+ * device pointer).  The HOST variant stages the copy through the Runge-Kutta register K and destroys its contents: K is
+ * dead only BETWEEN steps (after stage 4 and before the next stage 0), so call it there -- between dg_split_update
+ * stages 0..3 of one step it would corrupt the step.  The device variant touches nothing but R and r_out. */
 int dg_split_volume(dg_ctx *ctx);
 int dg_split_surface(dg_ctx *ctx);
 int dg_split_update(dg_ctx *ctx, double dt, int stage);
