@@ -96,6 +96,35 @@ def test_far_field_free_stream_and_far_field_as_wall_ghost(p):
 
 
 @pytest.mark.parametrize("p", [1, 3])
+@pytest.mark.parametrize("axis", [0, 1, 2])
+@pytest.mark.parametrize("side", [0, 1])
+def test_far_field_equal_to_the_wall_ghost_reproduces_the_wall(p, axis, side):
+    """The far-field branch with an exterior state that DIFFERS from the interior, pinned by the wall branch: for a
+    state that varies along one axis only, the trace on a face of that axis is one and the same state at every face
+    node, so its wall ghost (normal momentum negated) can be handed over as q_inf.  Far field on that face (low and
+    high in turn), wall on the opposite one, must then give the residual of walls on both."""
+    n, ext = [3, 2, 4], [1.0, 0.7, 1.3]
+    q3 = field(*n, p, ext, seed=7)
+    elem_ax, node_ax = {0: (2, 5), 1: (1, 4), 2: (0, 3)}[axis]
+    keep = [slice(0, 1)] * 6 + [slice(None)]
+    keep[elem_ax] = keep[node_ax] = slice(None)
+    q = np.ascontiguousarray(np.broadcast_to(q3[tuple(keep)], q3.shape))       # varies along `axis` only
+    _, _, _, lp, lm = bf.basis_1d(p + 1)                                          # l_i(+1), l_i(-1): numpy, not the oracle's
+    line = np.moveaxis(q, (elem_ax, node_ax), (0, 1))[:, :, 0, 0, 0, 0, :]       # (element, node, variable) along the axis
+    trace = lp @ line[-1] if side else lm @ line[0]
+    ghost = trace.copy()
+    ghost[1 + axis] *= -1.0
+    bc_far, bc_wall = [PER] * 6, [PER] * 6
+    bc_wall[2 * axis] = bc_wall[2 * axis + 1] = WALL
+    bc_far[2 * axis + side], bc_far[2 * axis + 1 - side] = FAR, WALL
+    r_far = ORC.residual_bc(q, p, G, ext, bc_far, ghost)
+    r_wall = ORC.residual_bc(q, p, G, ext, bc_wall)
+    assert relerr(r_far, r_wall) < 1e-13, (p, axis, side, relerr(r_far, r_wall))
+    # and the pin bites: the un-negated trace as exterior state (a transparent face) gives another residual
+    assert relerr(ORC.residual_bc(q, p, G, ext, bc_far, trace), r_wall) > 1e-3
+
+
+@pytest.mark.parametrize("p", [1, 3])
 def test_walls_conserve_mass_and_energy(p):
     n, ext = [3, 2, 3], [1.0, 0.8, 1.1]
     q = field(*n, p, ext, seed=2)
