@@ -16,7 +16,7 @@ torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
 
 from oracle import Oracle                                    # noqa: E402
-from oracle.parity import assert_parity                      # noqa: E402
+from oracle.parity import add_term_scale, assert_parity, assert_term_scale   # noqa: E402
 from paper_2006_15698_b200 import DG                         # noqa: E402
 from paper_2006_15698_b200 import inputs as I                # noqa: E402
 
@@ -65,9 +65,14 @@ def sampled_parity(cfg, boxes_res, boxes_rk, tol_res=1e-11, tol_rk=1e-11, cfl=0.
         inner = (slice(1, -1),) * 3
         rep = assert_parity(r_gpu[inner], r_orc[inner], lambda: ARB.residual(qb, p, G, sub_ext)[inner], tol_res,
                             (cfg, "residual", lo), allowed=allowed_res, always_arbiter=always_arbiter)
+        # the number that needs no arbiter: the difference against the size of the volume and surface terms that
+        # cancel in the residual (every variable, strict, 1e-13)
+        add_term_scale(rep, [ORC.volume_term(qb, p, G, sub_ext)[inner], ORC.surface_term(qb, p, G, sub_ext)[inner]])
+        assert_term_scale(rep, (cfg, "residual", lo))
         if reports is not None:
             reports.append((cfg, "residual", lo, size, rep))
         worst["residual"] = max(worst.get("residual", 0.0), rep["strict_rel_max"])
+        worst["residual_rel_to_terms"] = max(worst.get("residual_rel_to_terms", 0.0), rep["rel_to_terms_max"])
         worst.setdefault("residual_arbiter_vars", set()).update(rep["arbiter_vars"])
     del r
     q_boxes = [take_box(q, lo, size) for lo, size in boxes_rk]
@@ -94,8 +99,9 @@ def sampled_parity(cfg, boxes_res, boxes_rk, tol_res=1e-11, tol_rk=1e-11, cfl=0.
 # Which variables may pass through the arbiter clause (oracle/parity.py).  At full size the residual of every
 # variable is a cancellation residue of terms 1e4-1e5 times larger (2/h is 100-700 and the fields are smooth), so
 # the fp64 ORACLE's own error against its long-double build is 1e-11..1e-9 of the result there (eta/s column of
-# profiles/r02_parity_report.md): no fp64 evaluation can meet 1e-11 of the result, and the GPU is held to
-# g <= 4 eta instead (measured: g/eta <= 1.3).  After a Runge-Kutta step only rho w of the Taylor-Green fields
+# profiles/r03_parity_report.md): no fp64 evaluation can meet 1e-11 of the result, and the GPU is held to
+# g <= ARBITER_FACTOR eta instead (measured: g/eta <= 1.3) AND, with no arbiter involved, to 1e-13 of the volume and
+# surface terms that cancel (d/terms column of the report).  After a Runge-Kutta step only rho w of the Taylor-Green fields
 # (identically zero initially) is such a residue.
 RES_ALLOWED = ("rho", "rho u", "rho v", "rho w", "rho E")
 RK_ALLOWED_TGV = ("rho w",)

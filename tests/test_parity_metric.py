@@ -64,3 +64,29 @@ def test_strict_metric_without_arbiter():
     b[..., 2] = 0.0
     a[..., 2] = 1e-30                                         # zero variable: absolute comparison, no arbiter given
     assert not compare(a, b, None, 1e-11)[0]
+
+
+def test_term_scale_metric_needs_no_arbiter_and_rejects_real_errors():
+    """d / max(|V|, |S|): the same vortex, whose rho w residual is pure rounding residue.  The independent strong-form
+    evaluation is within 1e-13 of the oracle in EVERY variable once the difference is measured against the volume and
+    surface terms that cancel (no arbiter, no allowed list); a perturbation of 1e-11 of those terms is rejected."""
+    import pytest
+    from oracle.parity import TERM_TOL, add_term_scale, assert_term_scale
+    c = dict(nx=4, ny=4, nz=2, p=3, extent=(10.0, 10.0, 2.5), field="isentropic_vortex")
+    p, ext = c["p"], c["extent"]
+    q = I.make_field(c)
+    orc = Oracle("fp64")
+    r, V, S = orc.residual(q, p, G, ext), orc.volume_term(q, p, G, ext), orc.surface_term(q, p, G, ext)
+    assert relerr(V - S, r) < 1e-12 or np.abs((V - S) - r).max() < 1e-13 * np.abs(V).max()   # residual = V - S
+    other = bf.residual(q, p, G, ext, "strong")
+    _, rep = compare(other, r, None, 1e-11)
+    assert rep["rows"][3]["passed_by"] == "FAILED"            # rho w: hopeless relative to its own size ...
+    add_term_scale(rep, [V, S])
+    assert_term_scale(rep)                                    # ... and plain roundoff relative to the terms
+    assert 0 < rep["rel_to_terms_max"] < TERM_TOL and all(row["term_scale"] > 0 for row in rep["rows"])
+    for n in range(5):
+        bad = other.copy()
+        bad[1, 2, 3, 1, 2, 0, n] += 1e-11 * max(np.abs(V[..., n]).max(), np.abs(S[..., n]).max())
+        _, rep = compare(bad, r, None, 1e-11)
+        with pytest.raises(AssertionError):
+            assert_term_scale(add_term_scale(rep, [V, S]))
