@@ -55,7 +55,9 @@ enum {
     DG_EUNSUPPORTED = 2, /* p outside 1..7 */
     DG_ENOMEM = 3,       /* workspace too small / host allocation failed */
     DG_ECUDA = 4,        /* CUDA runtime error (text in dg_last_error) */
-    DG_ESTATE = 5        /* call out of order: not bound, or no state set */
+    DG_ESTATE = 5,       /* call out of order: not bound, or no state set */
+    DG_ENONPHYSICAL = 6  /* dg_rk_step_cfl only: the state has a node with rho <= 0, p <= 0 or a non-finite value, so its
+                            wavespeed gives no time step (the call itself was in order; the paper has no limiter) */
 };
 
 /* Create a context for nx*ny*nz periodic elements on [0,Lx]x[0,Ly]x[0,Lz], extent = {Lx,Ly,Lz},
@@ -163,9 +165,9 @@ int dg_rk_step(dg_ctx *ctx, double dt, int nsteps);
  *     dt = cfl * min(hx,hy,hz) / ((2p+1) * lam_max(Q at the start of the step)),
  * formed ON THE DEVICE: lam_max is reduced by the last stage of the previous step (no extra sweep over the state)
  * and the next step's kernels read it from device memory, so the steps are enqueued without a host round trip.
- * One read-back at the start checks the wavespeed of the current state (DG_ESTATE if not positive and finite,
- * nothing stepped) and one at the end returns *t_advanced = sum of the time steps taken and *dt_last = the last
- * one (host pointers, either may be NULL; DG_ESTATE if the state went non-physical on the way).  cfl > 0. */
+ * One read-back at the start checks the wavespeed of the current state (DG_ENONPHYSICAL if not positive and
+ * finite, nothing stepped) and one at the end returns *t_advanced = sum of the time steps taken and *dt_last = the last
+ * one (host pointers, either may be NULL; DG_ENONPHYSICAL if the state went non-physical on the way).  cfl > 0. */
 int dg_rk_step_cfl(dg_ctx *ctx, double cfl, int nsteps, double *t_advanced, double *dt_last);
 
 /* The time step of the same rule (reading R10) as a plain host computation, for callers that reduce the wavespeed

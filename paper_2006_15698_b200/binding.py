@@ -57,7 +57,7 @@ SYMBOLS = {
     "dg_destroy": (ctypes.c_int, [ctypes.c_void_p]),
     "dg_last_error": (ctypes.c_char_p, [ctypes.c_void_p]),
 }
-ERRORS = {1: "DG_EINVAL", 2: "DG_EUNSUPPORTED", 3: "DG_ENOMEM", 4: "DG_ECUDA", 5: "DG_ESTATE"}
+ERRORS = {1: "DG_EINVAL", 2: "DG_EUNSUPPORTED", 3: "DG_ENOMEM", 4: "DG_ECUDA", 5: "DG_ESTATE", 6: "DG_ENONPHYSICAL"}
 
 
 def selftest_fastmath(x):

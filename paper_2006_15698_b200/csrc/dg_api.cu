@@ -773,7 +773,7 @@ int dg_rk_step_cfl(dg_ctx *c, double cfl, int nsteps, double *t_advanced, double
     double lam = 0.0;
     int rc = read_lam(c, &lam);
     if (rc != DG_OK) return rc;
-    if (!(lam > 0.0) || !std::isfinite(lam)) return fail(c, DG_ESTATE, "max wavespeed %g is not positive and finite", lam);
+    if (!(lam > 0.0) || !std::isfinite(lam)) return fail(c, DG_ENONPHYSICAL, "max wavespeed %g is not positive and finite: the state is non-physical, nothing stepped", lam);
     double out[2] = {0.0, 0.0};
     if (nsteps > 0) {
         // ... every step then forms its dt on the device from the wavespeed the step before reduced
@@ -790,7 +790,7 @@ int dg_rk_step_cfl(dg_ctx *c, double cfl, int nsteps, double *t_advanced, double
     }
     if (t_advanced) *t_advanced = out[0];
     if (dt_last) *dt_last = out[1];
-    if (!std::isfinite(out[0])) return fail(c, DG_ESTATE, "the state became non-physical during the steps (time advanced %g)", out[0]);
+    if (!std::isfinite(out[0])) return fail(c, DG_ENONPHYSICAL, "the state became non-physical during the steps (time advanced %g)", out[0]);
     return DG_OK;
 }
 

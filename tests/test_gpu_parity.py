@@ -260,15 +260,27 @@ def test_fused_wavespeed_of_a_fluid_at_rest():
 
 def test_max_wavespeed_propagates_nan():
     """A node with negative pressure: the wavespeed is NaN (no limiter, reading R15), in the stand-alone
-    reduction and in the one fused into the last stage; dg_rk_step_cfl then refuses to step (DG_ESTATE)."""
+    reduction and in the one fused into the last stage; dg_rk_step_cfl then refuses to step (DG_ENONPHYSICAL, a code
+    of its own: the call was in order, the state is not)."""
     p, shape, ext = 2, (4, 3, 2), (1.0, 1.0, 1.0)
     q = rough_field(*shape, p, ext, seed=9)
     q[1, 2, 3, 0, 1, 2, 4] = 1e-3                              # rho E far below the kinetic energy
     dg = DG(*shape, p, G, ext)
     assert np.isnan(dg.set_state(q).max_wavespeed())
     assert np.isnan(ORC.max_wavespeed(q, p, G))
-    with pytest.raises(DGError):
+    with pytest.raises(DGError) as e:
         dg.rk_step_cfl(0.1, 1)
+    assert e.value.code == 6 and "non-physical" in str(e.value)
+    assert np.array_equal(dg.get_state(), q)                   # nothing stepped
+    # a state that turns non-physical DURING the steps: the same code after the fact (the steps are enqueued without
+    # a host round trip, so this is found at the read-back at the end)
+    q2 = rough_field(*shape, p, ext, seed=9)
+    q2[1, 2, 3, 0, 1, 2, 4] = 0.56 * q2[1, 2, 3, 0, 1, 2, 4]   # pressure just above zero at one node, far from its neighbours
+    dg.set_state(q2)
+    assert np.isfinite(dg.max_wavespeed())                    # p = 0.51 there: still a physical state
+    with pytest.raises(DGError) as e:
+        dg.rk_step_cfl(20.0, 60)                               # far beyond the stable CFL number: blows up on the way
+    assert e.value.code == 6
     dg.close()
 
 
