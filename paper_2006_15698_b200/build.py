@@ -4,7 +4,7 @@ One translation unit per N = p+1 (csrc/dg_kernels.cu with -DDG_N=<N>) plus the b
 (csrc/dg_api.cu) and the allocation-free wavespeed call (csrc/dg_noalloc.cu), compiled in parallel, linked into paper_2006_15698_b200/libdg_b200.so.
 ptxas resource usage (-Xptxas -v) of every TU is kept in build/ptxas_N<N>.log.
 
-Usage:  python -m paper_2006_15698_b200.build [--force]
+Usage:  python -m paper_2006_15698_b200.build [--force] [--all-variants]
 """
 import os
 import subprocess
@@ -48,15 +48,17 @@ def _compile(args):
     return obj
 
 
-def build(force=False, verbose=False):
-    """Compile what is stale; return the path of the shared library."""
+def build(force=False, verbose=False, all_variants=False):
+    """Compile what is stale; return the path of the shared library.  all_variants=True also compiles the stage-kernel
+    variants that only dg_set_variant can reach (-DDG_ALL_VARIANTS; for bench.py --sweep-variants): 48 instead of 30
+    variants, a 41 MB instead of a 25 MB library.  Switching between the two needs force=True."""
     os.makedirs(BUILD, exist_ok=True)
     jobs, objs = [], []
     for n in NS:
         obj = os.path.join(BUILD, f"dg_kernels_N{n}.o")
         objs.append(obj)
         if force or _stale(obj, DEPS_KERNELS):
-            cmd = ["nvcc"] + NVCC_FLAGS + [f"-DDG_N={n}", "-c", os.path.join(CSRC, "dg_kernels.cu"), "-o", obj]
+            cmd = ["nvcc"] + NVCC_FLAGS + (["-DDG_ALL_VARIANTS"] if all_variants else []) + [f"-DDG_N={n}", "-c", os.path.join(CSRC, "dg_kernels.cu"), "-o", obj]
             jobs.append((obj, cmd, os.path.join(BUILD, f"ptxas_N{n}.log")))
     obj = os.path.join(BUILD, "dg_api.o")
     objs.append(obj)
@@ -83,4 +85,5 @@ def build(force=False, verbose=False):
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose=True))
+    print(build(force="--force" in sys.argv or "--all-variants" in sys.argv, verbose=True,
+                all_variants="--all-variants" in sys.argv))

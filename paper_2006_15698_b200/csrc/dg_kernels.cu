@@ -1542,32 +1542,46 @@ constexpr DgKernelTable make_table() {
 
 // Variants per N (default first): Cfg<N, BX, BY, min blocks per SM, RELOAD, PP, OX, OY>.
 // DESIGN.md "column shapes" and "shared-memory layout" explain the choices.
-#define DG_T(...) make_table<Cfg<__VA_ARGS__>>()
+// dg_create and dg_set_brick select by column SHAPE and take the first variant of a shape, so a later variant with the
+// same (BX, BY) can only be reached through dg_set_variant: those (other residency / reload / offset settings of a shape,
+// all measured slower than the first) are compiled only with -DDG_ALL_VARIANTS (python -m
+// paper_2006_15698_b200.build --all-variants, for bench.py --sweep-variants); DG_X(...) marks them.
+#define DG_T(...) make_table<Cfg<__VA_ARGS__>>(),
+#ifdef DG_ALL_VARIANTS
+#define DG_X(...) DG_T(__VA_ARGS__)
+#else
+#define DG_X(...)
+#endif
 #if DG_N == 2
-#define DG_VARIANTS DG_T(2, 9, 8, 2, 1, 290, 0, 0), DG_T(2, 8, 4, 3, 0, 0, 3, 0), DG_T(2, 4, 4, 6, 0, 0, 3, 0), DG_T(2, 8, 8, 2, 0, 0, 3, 0), \
-                    DG_T(2, 9, 7, 2, 1, 258, 3, 0), DG_T(2, 9, 7, 3, 1, 258, 3, 0)
+#define DG_VARIANTS DG_T(2, 9, 8, 2, 1, 290, 0, 0) DG_T(2, 8, 4, 3, 0, 0, 3, 0) DG_T(2, 4, 4, 6, 0, 0, 3, 0) DG_T(2, 8, 8, 2, 0, 0, 3, 0) \
+                    DG_T(2, 9, 7, 2, 1, 258, 3, 0) DG_X(2, 9, 7, 3, 1, 258, 3, 0)
 #elif DG_N == 3
-#define DG_VARIANTS DG_T(3, 6, 4, 2, 0, 0, 4, 0), DG_T(3, 4, 4, 2, 0, 0, 4, 4), DG_T(3, 2, 7, 3, 0, 134, 4, 0), DG_T(3, 6, 3, 2, 0, 0, 4, 0), \
-                    DG_T(3, 4, 4, 3, 1, 0, 4, 4), DG_T(3, 4, 2, 4, 1, 0, 4, 0)
+#define DG_VARIANTS DG_T(3, 6, 4, 2, 0, 0, 4, 0) DG_T(3, 4, 4, 2, 0, 0, 4, 4) DG_T(3, 2, 7, 3, 0, 134, 4, 0) DG_T(3, 6, 3, 2, 0, 0, 4, 0) \
+                    DG_X(3, 4, 4, 3, 1, 0, 4, 4) DG_T(3, 4, 2, 4, 1, 0, 4, 0)
 #elif DG_N == 4
-#define DG_VARIANTS DG_T(4, 2, 2, 4, 0, 66, 1, 0), DG_T(4, 2, 2, 5, 1, 66, 1, 0), DG_T(4, 4, 2, 2, 0, 130, 3, 0), DG_T(4, 4, 2, 3, 1, 130, 3, 0), \
-                    DG_T(4, 2, 2, 3, 0, 66, 1, 0)
+#define DG_VARIANTS DG_T(4, 2, 2, 4, 0, 66, 1, 0) DG_X(4, 2, 2, 5, 1, 66, 1, 0) DG_T(4, 4, 2, 2, 0, 130, 3, 0) DG_X(4, 4, 2, 3, 1, 130, 3, 0) \
+                    DG_X(4, 2, 2, 3, 0, 66, 1, 0)
 #elif DG_N == 5
-#define DG_VARIANTS DG_T(5, 2, 3, 2, 0, 154, 6, 0), DG_T(5, 2, 3, 2, 0, 154, 4, 0), DG_T(5, 3, 2, 2, 0, 0, 4, 0), DG_T(5, 2, 2, 3, 1, 106, 4, 0), DG_T(5, 5, 1, 2, 0, 0, 4, 0), \
-                    DG_T(5, 5, 1, 2, 1, 0, 4, 0), DG_T(5, 1, 5, 2, 0, 138, 0, 1)
+#define DG_VARIANTS DG_T(5, 2, 3, 2, 0, 154, 6, 0) DG_X(5, 2, 3, 2, 0, 154, 4, 0) DG_T(5, 3, 2, 2, 0, 0, 4, 0) DG_T(5, 2, 2, 3, 1, 106, 4, 0) DG_T(5, 5, 1, 2, 0, 0, 4, 0) \
+                    DG_X(5, 5, 1, 2, 1, 0, 4, 0) DG_T(5, 1, 5, 2, 0, 138, 0, 1)
 #elif DG_N == 6
-#define DG_VARIANTS DG_T(6, 1, 3, 2, 1, 118, 0, 0), DG_T(6, 1, 3, 2, 0, 118, 0, 0), DG_T(6, 3, 1, 2, 0, 114, 2, 0), DG_T(6, 2, 1, 3, 0, 0, 4, 0), DG_T(6, 2, 1, 3, 1, 0, 4, 0), \
-                    DG_T(6, 1, 1, 5, 1, 0, 0, 0), DG_T(6, 1, 1, 4, 0, 0, 0, 0)
+#define DG_VARIANTS DG_T(6, 1, 3, 2, 1, 118, 0, 0) DG_X(6, 1, 3, 2, 0, 118, 0, 0) DG_T(6, 3, 1, 2, 0, 114, 2, 0) DG_T(6, 2, 1, 3, 0, 0, 4, 0) DG_X(6, 2, 1, 3, 1, 0, 4, 0) \
+                    DG_T(6, 1, 1, 5, 1, 0, 0, 0) DG_X(6, 1, 1, 4, 0, 0, 0, 0)
 #elif DG_N == 7
-#define DG_VARIANTS DG_T(7, 2, 1, 2, 1, 0, 4, 6, 1), DG_T(7, 2, 1, 2, 1, 0, 4, 0, 1), DG_T(7, 2, 1, 2, 1, 0, 4, 0), DG_T(7, 1, 1, 4, 1, 0, 0, 1), DG_T(7, 1, 1, 4, 0, 0, 0, 1), DG_T(7, 1, 1, 3, 0, 0, 0, 1)
+#define DG_VARIANTS DG_T(7, 2, 1, 2, 1, 0, 4, 6, 1) DG_X(7, 2, 1, 2, 1, 0, 4, 0, 1) DG_X(7, 2, 1, 2, 1, 0, 4, 0) DG_T(7, 1, 1, 4, 1, 0, 0, 1) DG_X(7, 1, 1, 4, 0, 0, 0, 1) DG_X(7, 1, 1, 3, 0, 0, 0, 1)
 #elif DG_N == 8
-#define DG_VARIANTS DG_T(8, 1, 1, 3, 1, 66, 1, 1), DG_T(8, 1, 1, 3, 0, 66, 1, 1), DG_T(8, 2, 1, 1, 0, 130, 1, 0), DG_T(8, 1, 2, 1, 0, 130, 1, 1)
+#define DG_VARIANTS DG_T(8, 1, 1, 3, 1, 66, 1, 1) DG_X(8, 1, 1, 3, 0, 66, 1, 1) DG_T(8, 2, 1, 1, 0, 130, 1, 0) DG_T(8, 1, 2, 1, 0, 130, 1, 1)
 #else
 #error "DG_N must be 2..8"
 #endif
 
-// last: one element per layer, always there (tiny and ragged meshes, tests)
-const DgKernelTable k_tables[] = {DG_VARIANTS, DG_T(DG_N, 1, 1, 2, 1)};
+// last: one element per layer, always there (tiny and ragged meshes, tests); for N >= 6 the list above already has a
+// 1 x 1 shape in front of it, so this one is unreachable there and is kept for DG_ALL_VARIANTS only
+#if DG_N <= 5 || defined(DG_ALL_VARIANTS)
+const DgKernelTable k_tables[] = {DG_VARIANTS DG_T(DG_N, 1, 1, 2, 1)};
+#else
+const DgKernelTable k_tables[] = {DG_VARIANTS};
+#endif
 
 }  // namespace
 
